@@ -1,0 +1,213 @@
+// rt_oracle.cpp — fp64 CPU ORACLE for the Ray-trax ray march.  TEST INFRASTRUCTURE ONLY.
+//
+// This file is the plain, slow, obviously-correct restatement of what the hot path computes, written
+// from the paper (/root/reference/PAPER.md, cited below as P:<line>) and from nothing else.  It shares
+// no code, header, table or constant with the CUDA path under paper_2511_09389_b200/csrc/, and neither
+// side includes or links the other.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+// `--impl reference` legs may build, load or call it.  The product path never routes through it.
+//
+// What it computes (eq. (2) at P:23; readings D1..D16 are listed in DESIGN.md §4):
+//
+//   N_s   = substeps(step_size, c, dt)                                   P:25   (reading D6)
+//   acc[nx][ny][nz][B] = 0
+//   for m in 0 .. n_steps-1:                                             P:56, P:35 (reading D7: rays continue)
+//     for every source s and every Fibonacci direction i (any order; state I[b], tau[b] kept per (s,i)):
+//       nhat = fib(i, N_Omega)                                           P:27   (reading D1)
+//       for k in m*N_s .. (m+1)*N_s - 1:
+//         p   = x0[s] + (k*ds) * nhat                                    P:23   (x_{k+1} = x_k + nhat ds, closed form, D3)
+//         i0  = floor(p) per axis;  f = p - i0 in [0,1)
+//         lo  = clamp(i0, 0, N-1);  hi = clamp(i0+1, 0, N-1)             P:29   "Indexing is clamped" (D5)
+//         for every bin b:                                               P:39   bins are a batch axis
+//           kap = kappa[lo0][lo1][lo2][b]                                P:29   nearest-neighbour at the cell of x_k (D4)
+//           jv  = sum over the 8 corners of w_c * j[corner_c][b]         P:29   trilinear read of j at x_k
+//           I[b]   = I[b]*exp(-kap*ds) + jv*exp(-tau[b])*ds              P:23   eq. (2), uses tau_k
+//           tau[b] = tau[b] + kap*ds
+//           acc[corner_c][b] += w_c * I[b]   for the same 8 corners      P:29   deposit I_{k+1}, same weights (D2)
+//     out[m] = (4 pi / N_Omega) * acc                                    P:27   (cumulative snapshot, D7/D8)
+//
+// Pins (tests/test_oracle_pins.py, all `-m "not gpu"`): closed form in a uniform medium, deposit-mass
+// conservation, N_Omega invariance, the analytic point source of P:45 (eq. 3), the light-front horizon,
+// hand-unrolled traces on 4^3 grids, the prefix property, the optically thin limit, linearity /
+// additivity / bin independence, trilinear consistency, and the direction lattice against 50-digit
+// arithmetic.  Reading D4 (floor vs round for "nearest neighbour") and the exact lattice D1 are pinned
+// only by those hand traces and by DESIGN.md's decision: the paper itself does not fix them.
+//
+// All arithmetic is double (long double only to reduce the golden-angle phase accurately).  No SIMD, no
+// blocking, no reordering beyond "rays are independent": rays are split over threads, each thread
+// owns a private grid, and the private grids are added in thread order, so a run is bit-reproducible for a
+// given thread count.
+#include <algorithm>
+#include <cmath>
+#include <cstddef>
+#include <cstdint>
+#include <thread>
+#include <vector>
+
+namespace {
+
+constexpr long double kPiL = 3.14159265358979323846264338327950288L;
+
+struct Medium {
+    const float* j;
+    const float* kappa;
+    long nx, ny, nz, nb;
+    size_t cell(long a, long b, long c) const { return ((size_t(a) * ny + b) * nz + c) * nb; }
+};
+
+// P:25 / reading D6: N_s = ceil(c dt / ds); a ratio within 1e-6 (relative) of an integer is that integer
+// (step_size, c, dt arrive as fp32, so e.g. 0.3f/0.1f = 3.00000007 must give 3, not 4).
+long substeps(double ds, double c, double dt) {
+    double r = c * dt / ds;
+    double rr = std::round(r);
+    if (rr >= 1.0 && std::fabs(r - rr) <= 1e-6 * r) return long(rr);
+    return long(std::ceil(r));
+}
+
+// P:27 / reading D1: golden-angle lattice, i = 0..n-1, z_i = 1 - (2i+1)/n, phi_i = i * pi * (3 - sqrt 5).
+void fib_direction(long i, long n, double nhat[3]) {
+    long double z = 1.0L - (2.0L * (long double)i + 1.0L) / (long double)n;
+    long double turn = (long double)i * ((3.0L - sqrtl(5.0L)) / 2.0L);   // phi / (2 pi)
+    turn -= floorl(turn);
+    long double phi = 2.0L * kPiL * turn;
+    long double s = sqrtl((1.0L - z) * (1.0L + z));
+    nhat[0] = double(s * cosl(phi));
+    nhat[1] = double(s * sinl(phi));
+    nhat[2] = double(z);
+}
+
+inline long clampl(long v, long lo, long hi) { return v < lo ? lo : (v > hi ? hi : v); }
+
+// Substeps k_begin .. k_end-1 of one ray, eq. (2) + deposit.  I/tau: per-bin state (in/out).
+// trace_* (optional, may be null): per-substep records for the pin tests.
+void march_ray(const Medium& M, const double x0[3], const double nhat[3], double ds, long k_begin, long k_end,
+               double* I, double* tau, double* acc, double* trace_I, double* trace_tau, double* trace_pos) {
+    const long N[3] = {M.nx, M.ny, M.nz};
+    for (long k = k_begin; k < k_end; ++k) {
+        long lo[3], hi[3];
+        double f[3];
+        for (int a = 0; a < 3; ++a) {
+            double p = x0[a] + (double(k) * ds) * nhat[a];
+            double fl = std::floor(p);
+            f[a] = p - fl;
+            long i0 = long(fl);
+            lo[a] = clampl(i0, 0, N[a] - 1);
+            hi[a] = clampl(i0 + 1, 0, N[a] - 1);
+            if (trace_pos) trace_pos[(k - k_begin) * 3 + a] = p;
+        }
+        size_t corner[8];
+        double w[8];
+        for (int c = 0; c < 8; ++c) {
+            int dx = (c >> 2) & 1, dy = (c >> 1) & 1, dz = c & 1;
+            corner[c] = M.cell(dx ? hi[0] : lo[0], dy ? hi[1] : lo[1], dz ? hi[2] : lo[2]);
+            w[c] = (dx ? f[0] : 1.0 - f[0]) * (dy ? f[1] : 1.0 - f[1]) * (dz ? f[2] : 1.0 - f[2]);
+        }
+        const size_t base = M.cell(lo[0], lo[1], lo[2]);
+        for (long b = 0; b < M.nb; ++b) {
+            double kap = double(M.kappa[base + b]);
+            double jv = 0.0;
+            for (int c = 0; c < 8; ++c) jv += w[c] * double(M.j[corner[c] + b]);
+            I[b] = I[b] * std::exp(-kap * ds) + jv * std::exp(-tau[b]) * ds;
+            tau[b] = tau[b] + kap * ds;
+            for (int c = 0; c < 8; ++c) acc[corner[c] + b] += w[c] * I[b];
+            if (trace_I) trace_I[(k - k_begin) * M.nb + b] = I[b];
+            if (trace_tau) trace_tau[(k - k_begin) * M.nb + b] = tau[b];
+        }
+    }
+}
+
+bool bad(double v) { return !(std::isfinite(v) && v > 0.0); }
+
+}  // namespace
+
+extern "C" {
+
+// N_s as the oracle computes it (D6).  Returns -1 on invalid arguments.
+long rt_oracle_substeps(float step_size, float c, float dt) {
+    if (bad(step_size) || bad(c) || bad(dt)) return -1;
+    return substeps(double(step_size), double(c), double(dt));
+}
+
+// Direction i of an n-point lattice (D1) -> nhat[3] (array axes 0,1,2).
+int rt_oracle_direction(long i, long n, double* nhat) {
+    if (n < 1 || i < 0 || i >= n || !nhat) return -1;
+    fib_direction(i, n, nhat);
+    return 0;
+}
+
+// One ray, n_sub substeps from k = 0 (I_0 = tau_0 = 0, D11).  Records I_{k+1}, tau_{k+1} and x_k for every
+// substep and adds the UNNORMALISED deposits into acc (double [nx][ny][nz][B], caller-zeroed; may be null).
+int rt_oracle_trace_ray(const float* j, const float* kappa, int nx, int ny, int nz, int n_bins,
+                        const float* source_pos, long ray_index, long n_rays, float step_size, long n_sub,
+                        double* trace_I, double* trace_tau, double* trace_pos, double* acc) {
+    if (!j || !kappa || !source_pos || nx < 1 || ny < 1 || nz < 1 || n_bins < 1 || n_sub < 0 || bad(step_size))
+        return -1;
+    Medium M{j, kappa, nx, ny, nz, n_bins};
+    double nhat[3];
+    if (rt_oracle_direction(ray_index, n_rays, nhat)) return -1;
+    double x0[3] = {double(source_pos[0]), double(source_pos[1]), double(source_pos[2])};
+    std::vector<double> I(n_bins, 0.0), tau(n_bins, 0.0), scratch;
+    if (!acc) { scratch.assign(size_t(nx) * ny * nz * n_bins, 0.0); acc = scratch.data(); }
+    march_ray(M, x0, nhat, double(step_size), 0, n_sub, I.data(), tau.data(), acc, trace_I, trace_tau, trace_pos);
+    return 0;
+}
+
+// The multi-source march.  Host pointers.  out: double [n_steps][nx][ny][nz][n_bins],
+// overwritten; snapshot m is cumulative (D7) and scaled once by 4 pi / N_Omega (D8).
+// n_threads < 1 means 1.  Returns 0, or -1 on invalid arguments.
+int rt_march_oracle(const float* j, const float* kappa, int nx, int ny, int nz, const float* sources, int n_src,
+                    int n_rays, int n_bins, float step_size, float c, float dt, int n_steps, double* out,
+                    int n_threads) {
+    if (!j || !kappa || !sources || !out) return -1;
+    if (nx < 1 || ny < 1 || nz < 1 || n_src < 1 || n_rays < 1 || n_bins < 1 || n_steps < 1) return -1;
+    if (bad(step_size) || bad(c) || bad(dt)) return -1;
+    const long Ns = substeps(double(step_size), double(c), double(dt));
+    const double ds = double(step_size);
+    const Medium M{j, kappa, nx, ny, nz, n_bins};
+    const size_t grid = size_t(nx) * ny * nz * n_bins;
+    const long total_rays = long(n_src) * n_rays;
+    long T = std::max(1, n_threads);
+    T = std::min<long>(T, total_rays);
+
+    std::vector<std::vector<double>> acc(T);                           // one private cumulative grid per thread
+    std::vector<double> state(size_t(total_rays) * n_bins * 2, 0.0);   // (I[b], tau[b]) per ray; I_0 = tau_0 = 0
+    for (auto& a : acc) a.assign(grid, 0.0);
+    const double scale = double(4.0L * kPiL / (long double)n_rays);
+
+    for (long m = 0; m < n_steps; ++m) {
+        auto work = [&](long t) {
+            long r0 = total_rays * t / T, r1 = total_rays * (t + 1) / T;   // contiguous chunk of (s, i) pairs
+            for (long r = r0; r < r1; ++r) {
+                long s = r / n_rays, i = r % n_rays;
+                double nhat[3];
+                fib_direction(i, n_rays, nhat);
+                double x0[3] = {double(sources[3 * s]), double(sources[3 * s + 1]), double(sources[3 * s + 2])};
+                double* I = &state[size_t(r) * n_bins * 2];
+                march_ray(M, x0, nhat, ds, m * Ns, (m + 1) * Ns, I, I + n_bins, acc[t].data(), nullptr, nullptr,
+                          nullptr);
+            }
+        };
+        std::vector<std::thread> pool;
+        for (long t = 1; t < T; ++t) pool.emplace_back(work, t);
+        work(0);
+        for (auto& th : pool) th.join();
+
+        double* snap = out + size_t(m) * grid;
+        auto reduce = [&](long t) {                                    // fixed order over the private grids
+            size_t v0 = grid * size_t(t) / T, v1 = grid * size_t(t + 1) / T;
+            for (size_t v = v0; v < v1; ++v) {
+                double sum = 0.0;
+                for (long u = 0; u < T; ++u) sum += acc[u][v];
+                snap[v] = scale * sum;
+            }
+        };
+        pool.clear();
+        for (long t = 1; t < T; ++t) pool.emplace_back(reduce, t);
+        reduce(0);
+        for (auto& th : pool) th.join();
+    }
+    return 0;
+}
+
+const char* rt_oracle_version(void) { return "rt_oracle 1 (fp64, PAPER.md eq. 2)"; }
+
+}  // extern "C"
