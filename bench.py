@@ -1,0 +1,349 @@
+#!/usr/bin/env python
+"""bench.py — ray-substep-bin updates/s of the Ray-trax march (BASELINE.json metric) on N B200s.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config C2] [--impl reference]
+
+A "step" is one pass of the whole hot path: one rt_march call (zero-fill, ray-order, march, snapshot
+prefix) over the full workload.  Default workload = BASELINE.json configs[2] ("C2": 128^3, 4,096 rays,
+2,097 sources at the density peaks, 444 substeps), the configuration the metric is quoted on.
+One JSON line is printed by rank 0; see DESIGN.md §8 for every field.
+
+N > 1 (under torchrun): weak scaling — rank r marches sources [r*n_src, (r+1)*n_src) of the N*n_src
+highest-density cells, then one NCCL sum all-reduce of the field (sharding.py).
+
+--impl reference times the fp64 CPU oracle (oracle/, as it stands) on this box's host cores on a bounded
+sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "ray-substep-bin updates/s"
+UNIT = "updates/s"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="C2", choices=["C0", "C1", "C2", "C3", "C4"])
+    ap.add_argument("--impl", default="native", choices=["native", "reference"])
+    ap.add_argument("--variant", type=int, default=0, help="RT_VARIANT_* (0 = the product path)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target host time of the oracle sample")
+    return ap.parse_args()
+
+
+def make_workload(name, world_size=1):
+    """Config `name`; for world_size > 1 the source list is extended to world_size * n_src sources by the
+    config's own placement rule (weak scaling: per-GPU work fixed)."""
+    from paper_2511_09389_b200 import workloads
+    w = workloads.make_config(name)
+    if world_size > 1:
+        n = w.n_src * world_size
+        if name in ("C2", "C3"):
+            rho = workloads.lognormal_density(128, 938902, 1.5)
+            order = np.argsort(-rho.ravel(), kind="stable")[:n]
+            w.sources = np.stack(np.unravel_index(order, rho.shape), axis=1).astype(np.float32)
+        else:
+            seed = {"C0": 939900, "C1": 939901, "C4": 939904}[name]
+            hi = w.shape[0] - 1.0
+            w.sources = np.random.default_rng(seed).uniform(0.0, hi, (n, 3)).astype(np.float32)
+    return w
+
+
+def describe(w, world_size):
+    nx, ny, nz = w.shape
+    return {"workload": f"{w.name}: {nx}x{ny}x{nz} fp32 grid x {w.n_bins} bin(s), {w.n_src} sources/GPU, "
+                        f"N_Omega={w.n_rays}, ds={w.step_size}, {w.n_steps} step(s) x N_s={w.substeps_per_step}",
+            "medium": w.meta.get("medium", ""), "baseline_config_index": int(w.name[1]),
+            "ray_substeps_per_gpu": w.ray_substeps, "updates_per_gpu": w.updates,
+            "parallelism": f"sources sharded over {world_size} GPU(s)" + (", 1 all-reduce" if world_size > 1 else "")}
+
+
+# ----------------------------------------------------------------------------------------------------
+# the oracle on host cores: cpu_baseline leg and --impl reference
+# ----------------------------------------------------------------------------------------------------
+def oracle_sample(w, seconds, repeats=1):
+    """Time the oracle (as it stands) on a stratified subset of the sources sized for ~`seconds` of host
+    time.  Returns (updates/s, cores, description, [seconds per repeat])."""
+    import oracle
+    cores = oracle.host_threads()
+    per_src = w.n_rays * w.n_steps * w.substeps_per_step * w.n_bins
+    probe_n = min(w.n_src, cores)
+    idx = np.unique(np.linspace(0, w.n_src - 1, probe_n).round().astype(int))
+    t0 = time.perf_counter()
+    oracle.march(w.j, w.kappa, w.sources[idx], w.n_rays, w.step_size, w.c, w.dt, w.n_steps)
+    rate = len(idx) * per_src / (time.perf_counter() - t0)
+    n = int(min(w.n_src, max(cores, seconds * rate / per_src)))
+    idx = np.unique(np.linspace(0, w.n_src - 1, n).round().astype(int))
+    src = np.ascontiguousarray(w.sources[idx])
+    times = []
+    for _ in range(repeats):
+        t0 = time.perf_counter()
+        oracle.march(w.j, w.kappa, src, w.n_rays, w.step_size, w.c, w.dt, w.n_steps)
+        times.append(time.perf_counter() - t0)
+    ups = len(idx) * per_src / min(times)
+    what = (f"{len(idx)} of {w.n_src} sources of {w.name} (stratified), all {w.n_rays} rays x "
+            f"{w.n_steps * w.substeps_per_step} substeps x {w.n_bins} bin(s); fp64 oracle, {cores} threads")
+    return ups, cores, what, times, len(idx) * per_src
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    w = make_workload(args.config)
+    steps = max(1, args.steps)
+    for _ in range(min(args.warmup, 1)):
+        oracle_sample(w, 1.0)
+    budget = max(2.0, min(args.cpu_seconds, 120.0 / steps))
+    ups, cores, what, times, units = oracle_sample(w, budget, repeats=steps)
+    value = units * len(times) / sum(times)
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * sum(times) / len(times), "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": describe(w, 1),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": what},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0,
+            "note": "each step = the fp64 CPU oracle on the bounded sample described in cpu_baseline.sample"}
+    print(json.dumps(line))
+    return 0
+
+
+# ----------------------------------------------------------------------------------------------------
+# clocks during the timed region
+# ----------------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.perf_counter(), [c.strip() for c in line.split(",")]))
+
+    def stop(self):
+        if self.proc:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=5)
+            except subprocess.TimeoutExpired:
+                self.proc.kill()
+
+    def summary(self, t0, t1):
+        rows = [r for t, r in self.rows if t0 <= t <= t1 and len(r) >= 7] or [r for _, r in self.rows if len(r) >= 7]
+        if not rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        sm = sorted(float(r[0]) for r in rows)
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(r[3 + i].lower().startswith("active") for r in rows)]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(rows[0][1]), "reasons": reasons,
+                "power_w_max": max(float(r[2]) for r in rows), "samples": len(rows)}
+
+
+# ----------------------------------------------------------------------------------------------------
+# the CUDA path
+# ----------------------------------------------------------------------------------------------------
+def measure_ceilings(rt, torch, shape, n_bins):
+    """Reduction-throughput ceilings on a grid of the workload's size, in this process, back to back with
+    the march: best of 5 launches of >= 2^28 reductions each, CUDA events.  Greds/s."""
+    grid = torch.zeros(shape + (n_bins,), dtype=torch.float32, device="cuda")
+    res = {}
+    for name, mode in (("M1_scalar_random", 0), ("M2_v4_random", 1), ("M3_stencil", 2), ("M4_one_address", 3),
+                       ("M5_coalesced", 4), ("M6_stencil_walk", 5)):
+        if mode == 1 and grid.numel() % 4:
+            continue
+        n_red = (1 << 24) if mode == 3 else (1 << 28)
+        best = None
+        for rep in range(6):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            issued = rt.rt_bench_red_ceiling(mode, grid, n_red, seed=rep + 1)
+            e1.record()
+            e1.synchronize()
+            ms = e0.elapsed_time(e1)
+            if rep and (best is None or ms < best):
+                best = ms
+        res[name] = issued / (best * 1e-3) / 1e9
+    del grid
+    return res
+
+
+def run_native(args):
+    import torch
+    import torch.distributed as dist
+
+    import paper_2511_09389_b200 as rt          # raises if librtmarch.so is missing: no fallback
+    from paper_2511_09389_b200 import sharding
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device (use --impl reference for the CPU oracle)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if world != args.gpus and rank == 0:
+        print(f"warning: --gpus {args.gpus} but WORLD_SIZE={world}", file=sys.stderr)
+
+    w = make_workload(args.config, world)
+    n_src_per_gpu = w.n_src // world
+    sl = sharding.source_slice(w.n_src, rank, world)
+    nx, ny, nz = w.shape
+    nb = w.n_bins
+    j, kappa = torch.from_numpy(w.j).cuda(), torch.from_numpy(w.kappa).cuda()
+    src = torch.from_numpy(np.ascontiguousarray(w.sources[sl])).cuda()
+    out = torch.empty((w.n_steps, nx, ny, nz, nb), dtype=torch.float32, device="cuda")
+    ws = rt.alloc_workspace(nx, ny, nz, src.shape[0], w.n_rays, nb, w.n_steps)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB L2
+    units_per_gpu = src.shape[0] * w.n_rays * w.n_steps * w.substeps_per_step * nb
+
+    def step():
+        rt.rt_march_ex(j, kappa, src, w.n_rays, w.step_size, w.c, w.dt, w.n_steps, out=out, workspace=ws,
+                       variant=args.variant)
+        if world > 1:
+            sharding.allreduce_field(out)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 0)):
+        flush.zero_()
+        step()
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.3)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    barrier()
+    t0 = time.perf_counter()
+    for e0, e1 in ev:
+        flush.zero_()                 # L2 flush between timed iterations (outside the event pair)
+        e0.record()
+        step()
+        e1.record()
+    barrier()
+    t1 = time.perf_counter()
+    step_ms = [e0.elapsed_time(e1) for e0, e1 in ev]
+    total_ms = torch.tensor([sum(step_ms)], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(total_ms, op=dist.ReduceOp.MAX)
+    total_s = float(total_ms.item()) * 1e-3
+    if rank == 0:
+        time.sleep(0.2)
+        sampler.stop()
+    clocks = sampler.summary(t0, t1) if rank == 0 else None
+    value = units_per_gpu * world * args.steps / total_s
+
+    line = None
+    if rank == 0:
+        field_sum = float(out.double().sum().item())
+        launches = rt.rt_launch_count(nb, w.n_steps)
+        cfg = describe(w, world)
+        cfg["workload"] = cfg["workload"].replace(f"{w.n_src} sources/GPU", f"{n_src_per_gpu} sources/GPU")
+        cfg.update({"timing": "CUDA events per step on the launch stream; 256 MiB L2 flush (memset) between "
+                              "timed steps, outside the event pairs; inputs resident in HBM",
+                    "kernel_variant": args.variant, "field_checksum": field_sum})
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": 1e3 * total_s / args.steps, "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": cfg,
+                "ray_substeps_per_s": value / nb, "step_ms_each": step_ms, "clocks": clocks,
+                "gpu_launches": launches * args.steps, "impl": "native", "library": rt.rt_version()}
+
+    # ---- end to end through the host-pointer entry point: pinned host buffers, H2D + D2H inside the call
+    if not args.no_e2e:
+        hj, hk = torch.from_numpy(w.j).pin_memory(), torch.from_numpy(w.kappa).pin_memory()
+        hs = torch.from_numpy(np.ascontiguousarray(w.sources[sl])).pin_memory()
+        hout = torch.empty((w.n_steps, nx, ny, nz, nb), dtype=torch.float32).pin_memory()
+        n_e2e = max(1, min(args.steps, 3))
+        rt.rt_march_host(hj.numpy(), hk.numpy(), hs.numpy(), w.n_rays, w.step_size, w.c, w.dt, w.n_steps,
+                         out=hout.numpy())
+        barrier()
+        te = time.perf_counter()
+        for _ in range(n_e2e):
+            rt.rt_march_host(hj.numpy(), hk.numpy(), hs.numpy(), w.n_rays, w.step_size, w.c, w.dt, w.n_steps,
+                             out=hout.numpy())
+            if world > 1:          # the field leaves the call on the host: reduce it there
+                dist.all_reduce(hout.cuda(), op=dist.ReduceOp.SUM)
+        barrier()
+        e2e_s = torch.tensor([time.perf_counter() - te], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(e2e_s, op=dist.ReduceOp.MAX)
+        if rank == 0:
+            line["e2e"] = {"value": units_per_gpu * world * n_e2e / float(e2e_s.item()), "unit": UNIT,
+                           "h2d_bytes_per_step": int(hj.numel() * 4 + hk.numel() * 4 + hs.numel() * 4),
+                           "d2h_bytes_per_step": int(hout.numel() * 4), "steps": n_e2e,
+                           "api": "rt_march_host (cudaMalloc + H2D + march + D2H + free inside the call), "
+                                  "wall clock around the synchronous call, pinned host buffers"}
+
+    # ---- roofline of the dominant kernel (the march kernel) against the measured L2-reduction ceiling
+    if rank == 0:
+        ceil = measure_ceilings(rt, torch, (nx, ny, nz), nb)
+        reds_per_substep = 8 * ((nb + 3) // 4 if nb % 4 == 0 else nb)     # algorithmic: 8 corners x bin groups
+        alg_reds = reds_per_substep * src.shape[0] * w.n_rays * w.n_steps * w.substeps_per_step
+        kernel_s = min(step_ms) * 1e-3 if world == 1 else total_s / args.steps
+        achieved = alg_reds / (total_s / args.steps) / 1e9
+        peak = ceil["M3_stencil"]
+        line["roofline"] = {
+            "bound": "l2_red", "achieved": achieved, "peak": peak, "unit": "Gred/s", "frac": achieved / peak,
+            "traffic": None, "kernel": "march_sliding_kernel",
+            "how": "achieved = ALGORITHMIC reductions (8 corners x bin-groups x ray-substeps) / mean CUDA-event "
+                   "time of the whole rt_march call (the march kernel is >99.9% of it, profiles/); peak = "
+                   "M3 stencil-pattern red.global.add ceiling measured in this process on a grid of the same "
+                   "size (DESIGN.md §8); frac > 1 means register/warp aggregation removed reductions",
+            "best_step_frac": alg_reds / kernel_s / 1e9 / peak, "ceilings_Gred_per_s": ceil,
+            "hbm": {"algorithmic_bytes": int((2 + 2 * w.n_steps) * nx * ny * nz * nb * 4),
+                    "achieved_GBps": (2 + 2 * w.n_steps) * nx * ny * nz * nb * 4 / (total_s / args.steps) / 1e9,
+                    "peak_GBps": _measured_hbm()}}
+        if not args.no_cpu_baseline and world == 1:
+            ups, cores, what, _, _ = oracle_sample(make_workload(args.config), args.cpu_seconds)
+            line["cpu_baseline"] = {"value": ups, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": what}
+        print(json.dumps(line))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+def _measured_hbm():
+    try:
+        return json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
+    except (OSError, KeyError, ValueError):
+        return 6650.0      # fallback of B200_PROFILING.md
+
+
+if __name__ == "__main__":
+    a = parse()
+    sys.exit(run_reference(a) if a.impl == "reference" else run_native(a))

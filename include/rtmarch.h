@@ -1,0 +1,125 @@
+/* rtmarch.h — C ABI of librtmarch.so: the time-dependent emission-absorption ray march of
+ * Ray-trax (arXiv 2511.09389), hand-written CUDA for sm_100a (NVIDIA B200).
+ *
+ * Citations: P:<n> = line n of the paper text; D<n> = reading n in DESIGN.md §4.
+ *
+ * WHAT rt_march COMPUTES (eq. (2) at P:23).  For every source s, every direction i of an
+ * N_Omega-point Fibonacci (golden-angle) lattice (D1) and every frequency bin b, a ray starts
+ * at x_0 = sources[s] with I_0 = tau_0 = 0 (D11) and takes n_steps * N_s substeps, N_s = ceil(c dt / ds)
+ * (D6).  Substep k, at x_k = x_0 + k ds n_i (D3):
+ *     kappa_b = kappa at the base cell floor(x_k), nearest neighbour, clamped            (D4, D5)
+ *     j_b     = trilinear read of j at x_k, indices clamped to the domain                (D5)
+ *     I_b   <- I_b exp(-kappa_b ds) + j_b exp(-tau_b) ds ;  tau_b <- tau_b + kappa_b ds  (eq. 2)
+ *     field[corner_c][b] += w_c I_b  for the 8 corners, with the SAME trilinear weights  (D2)
+ * out[m] is the field after (m+1) N_s substeps (cumulative snapshots, D7), summed over sources
+ * and scaled once by 4 pi / N_Omega (D8).
+ *
+ * LAYOUT.  j, kappa: [nx][ny][nz][n_bins] float32, C order, bin innermost; kappa in 1/cell-length.
+ * sources: [n_src][3] float32 grid coordinates (axis 0, 1, 2); voxel (a,b,c) sits at coordinate (a,b,c).
+ * out: [n_steps][nx][ny][nz][n_bins] float32, OVERWRITTEN.  Directions map to axes (0,1,2) as
+ * (sqrt(1-z^2) cos phi, sqrt(1-z^2) sin phi, z).
+ *
+ * POINTERS AND OWNERSHIP.  Unless a function says "host", every pointer is a DEVICE pointer on the current
+ * CUDA device, owned by the caller (e.g. a torch tensor's data_ptr()); the library never frees or keeps
+ * it.  rt_march* are ASYNCHRONOUS: all work is enqueued on `stream` (a cudaStream_t passed as void*; NULL =
+ * the legacy default stream) and the caller synchronises.  j, kappa, sources, out and workspace must not
+ * overlap.  No global state; re-entrant per stream (each concurrent call needs its own workspace and out).
+ *
+ * ERRORS.  Functions returning int give RT_OK (0) or a negative RT_E* code; rt_strerror() names it.
+ * Argument errors are detected on the host BEFORE any CUDA call, so they can be exercised without a GPU.
+ * Source positions may be any finite value (a source outside the box is legal: clamping defines the
+ * result); they are saturated to +-2^29 cells.  Non-finite positions give an unspecified field.
+ *
+ * LIMITS (RT_EINVAL otherwise): nx*ny*nz*n_bins < 2^31; n_steps*N_s < 2^31; n_steps*N_s*step_size <= 2^28
+ * cells; n_rays <= 2^30.
+ */
+#ifndef RTMARCH_H
+#define RTMARCH_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define RT_OK 0
+#define RT_EINVAL (-1)     /* null pointer, non-positive size, non-finite / non-positive step_size, c or dt, limit exceeded */
+#define RT_EWORKSPACE (-2) /* workspace is NULL or smaller than rt_workspace_bytes() */
+#define RT_ECUDA (-3)      /* a CUDA runtime call or kernel launch failed; rt_strerror(RT_ECUDA) holds the CUDA message */
+#define RT_EALIGN (-4)     /* j, kappa or out not 4-byte aligned */
+
+/* Kernel variants for rt_march_ex (tests and bench only; rt_march always uses RT_VARIANT_DEFAULT).
+ * All variants compute the same field; they differ in how the deposit of P:29 is issued. */
+#define RT_VARIANT_DEFAULT 0 /* sliding-stencil register accumulation + coherent ray order */
+#define RT_VARIANT_DIRECT 1  /* textbook form: 8 reductions per ray-substep-bin-group, lattice order */
+#define RT_VARIANT_DIRECT_COHERENT 2 /* 8 reductions per ray-substep, coherent ray order */
+#define RT_VARIANT_SLIDING_LATTICE 3 /* sliding stencil, rays in lattice-index order */
+
+/* The multi-source march ("loop-and-sum wrapper").  See the header comment for semantics. */
+int rt_march(const float* j, const float* kappa, int nx, int ny, int nz,
+             const float* sources, int n_src, int n_rays /* N_Omega */, int n_bins,
+             float step_size /* ds, cells */, float c /* radiation velocity */, float dt /* time step */,
+             int n_steps, float* out,
+             void* workspace, size_t workspace_bytes, /* device scratch, >= rt_workspace_bytes(), 16-byte aligned */
+             void* stream);
+
+/* The paper's single-source kernel: rt_march with n_src = 1; source_pos = 3 floats (device). */
+int rt_march_single(const float* j, const float* kappa, int nx, int ny, int nz,
+                    const float* source_pos, int n_rays, int n_bins,
+                    float step_size, float c, float dt, int n_steps, float* out,
+                    void* workspace, size_t workspace_bytes, void* stream);
+
+/* rt_march with an explicit kernel variant (RT_VARIANT_*).  Unknown variant -> RT_EINVAL. */
+int rt_march_ex(const float* j, const float* kappa, int nx, int ny, int nz,
+                const float* sources, int n_src, int n_rays, int n_bins,
+                float step_size, float c, float dt, int n_steps, float* out,
+                void* workspace, size_t workspace_bytes, void* stream, int variant);
+
+/* End-to-end form with HOST pointers (j, kappa, sources, out are host memory, pinned or pageable).
+ * Allocates device buffers, copies the inputs in, marches, copies out[] back, frees, and returns after the
+ * copy has completed (SYNCHRONOUS).  Same semantics, limits and error codes as rt_march. */
+int rt_march_host(const float* j, const float* kappa, int nx, int ny, int nz,
+                  const float* sources, int n_src, int n_rays, int n_bins,
+                  float step_size, float c, float dt, int n_steps, float* out);
+
+/* Bytes of device scratch one rt_march call needs (the ray-order table).  0 on invalid arguments. */
+size_t rt_workspace_bytes(int nx, int ny, int nz, int n_src, int n_rays, int n_bins, int n_steps);
+
+/* N_s as the library computes it (D6): ceil(c dt / step_size), a ratio within 1e-6 (relative) of an
+ * integer counts as that integer.  Host only.  Returns RT_EINVAL on non-finite or non-positive input, or if
+ * N_s >= 2^31. */
+int rt_substeps_per_step(float step_size, float c, float dt);
+
+/* Number of kernels of this library that one rt_march call with these arguments enqueues (memsets excluded). */
+int rt_launch_count(int n_bins, int n_steps);
+
+/* TEST HOOK.  Writes the library's direction lattice (D1) for i = 0..n_rays-1 into
+ * nhat[n_rays][3] (float64, device), computed exactly as the march kernel does. */
+int rt_directions(int n_rays, double* nhat, void* stream);
+
+/* TEST HOOK.  Writes the coherent ray order into order[rt_ray_slots(n_rays)] (uint32, device): slot ->
+ * lattice index, 0xFFFFFFFF for padding slots.  Every index 0..n_rays-1 appears exactly once. */
+int rt_ray_order(int n_rays, unsigned int* order, void* stream);
+int rt_ray_slots(int n_rays);
+
+/* BENCH ONLY: reduction-throughput ceilings ("measured L2-atomic roofline").  Issues
+ * `n_red` (rounded up to a whole number per thread; the exact count issued is returned through
+ * *n_issued, host pointer, may be NULL) fp32 reductions into grid[nx][ny][nz][n_bins] on `stream`:
+ *   mode 0  scalar red.global.add.f32, uniformly random addresses                         (M1)
+ *   mode 1  red.global.add.v4.f32, uniformly random 16-byte-aligned addresses             (M2)
+ *   mode 2  trilinear-stencil pattern: random base voxel, its 8 corners; scalar reds when
+ *           n_bins % 4 != 0, else n_bins/4 v4 reds per corner                             (M3 = R*)
+ *   mode 3  every reduction to one address                                                (M4)
+ *   mode 4  warp-coalesced: 32 consecutive floats per warp instruction, random line       (M5)
+ *   mode 5  M3 issued along a random walk of half a cell per step (ray-like locality)     (M6)
+ * The grid is only accumulated into (caller zero-fills if the content matters). */
+int rt_bench_red_ceiling(int mode, float* grid, int nx, int ny, int nz, int n_bins,
+                         long long n_red, unsigned int seed, long long* n_issued, void* stream);
+
+const char* rt_strerror(int code);
+const char* rt_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RTMARCH_H */

@@ -1,0 +1,233 @@
+"""Thin ctypes binding of ``librtmarch.so`` (``include/rtmarch.h``): argument marshalling only.
+
+Every function has the name of the C entry point it calls.  Device-pointer functions take torch CUDA
+tensors (PyTorch is used for device memory and streams, nothing else) and enqueue on torch's current
+stream unless ``stream`` is given; ``rt_march_host`` takes numpy arrays.  There is no CPU or PyTorch
+fallback: if the library cannot be loaded the import of this module raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+from . import build as _build
+
+RT_OK, RT_EINVAL, RT_EWORKSPACE, RT_ECUDA, RT_EALIGN = 0, -1, -2, -3, -4
+RT_VARIANT_DEFAULT, RT_VARIANT_DIRECT, RT_VARIANT_DIRECT_COHERENT, RT_VARIANT_SLIDING_LATTICE = 0, 1, 2, 3
+RED_MODES = {"M1_scalar_random": 0, "M2_v4_random": 1, "M3_stencil": 2, "M4_one_address": 3,
+             "M5_coalesced": 4, "M6_stencil_walk": 5}
+
+EXPORTS = ("rt_march", "rt_march_single", "rt_march_ex", "rt_march_host", "rt_workspace_bytes",
+           "rt_substeps_per_step", "rt_launch_count", "rt_directions", "rt_ray_order", "rt_ray_slots",
+           "rt_bench_red_ceiling", "rt_strerror", "rt_version")
+
+
+class RtError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        super().__init__(f"{where}: {rt_strerror(code)} (code {code})")
+
+
+def _load() -> ctypes.CDLL:
+    path = _build.LIB_PATH
+    if not os.path.exists(path):
+        path = _build.build_library()          # raises if nvcc is missing: no fallback
+    L = ctypes.CDLL(path)
+    vp, i, f, sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_float, ctypes.c_size_t
+    march_args = [vp, vp, i, i, i, vp, i, i, i, f, f, f, i, vp]
+    L.rt_march.argtypes = march_args + [vp, sz, vp]
+    L.rt_march_single.argtypes = [vp, vp, i, i, i, vp, i, i, f, f, f, i, vp, vp, sz, vp]
+    L.rt_march_ex.argtypes = march_args + [vp, sz, vp, i]
+    L.rt_march_host.argtypes = march_args
+    L.rt_workspace_bytes.argtypes = [i] * 7
+    L.rt_workspace_bytes.restype = sz
+    L.rt_substeps_per_step.argtypes = [f, f, f]
+    L.rt_launch_count.argtypes = [i, i]
+    L.rt_directions.argtypes = [i, vp, vp]
+    L.rt_ray_order.argtypes = [i, vp, vp]
+    L.rt_ray_slots.argtypes = [i]
+    L.rt_bench_red_ceiling.argtypes = [i, vp, i, i, i, i, ctypes.c_longlong, ctypes.c_uint,
+                                       ctypes.POINTER(ctypes.c_longlong), vp]
+    L.rt_strerror.argtypes = [i]
+    L.rt_strerror.restype = ctypes.c_char_p
+    L.rt_version.restype = ctypes.c_char_p
+    for name in EXPORTS:
+        getattr(L, name)                       # AttributeError if the library lacks a declared symbol
+    return L
+
+
+_lib = _load()
+
+
+def library_path() -> str:
+    return _build.LIB_PATH
+
+
+def rt_strerror(code: int) -> str:
+    return _lib.rt_strerror(int(code)).decode()
+
+
+def rt_version() -> str:
+    return _lib.rt_version().decode()
+
+
+def rt_substeps_per_step(step_size: float, c: float, dt: float) -> int:
+    return int(_lib.rt_substeps_per_step(step_size, c, dt))
+
+
+def rt_workspace_bytes(nx, ny, nz, n_src, n_rays, n_bins, n_steps) -> int:
+    return int(_lib.rt_workspace_bytes(nx, ny, nz, n_src, n_rays, n_bins, n_steps))
+
+
+def rt_launch_count(n_bins: int, n_steps: int) -> int:
+    return int(_lib.rt_launch_count(n_bins, n_steps))
+
+
+def rt_ray_slots(n_rays: int) -> int:
+    return int(_lib.rt_ray_slots(n_rays))
+
+
+# ---------------------------------------------------------------------------------------------------
+# device-pointer entry points (torch tensors carry the memory)
+# ---------------------------------------------------------------------------------------------------
+def _torch():
+    import torch
+    return torch
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        return _torch().cuda.current_stream().cuda_stream
+    return getattr(stream, "cuda_stream", stream)
+
+
+def _check_dev(t, name, dtype, ndim=None):
+    torch = _torch()
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise TypeError(f"{name}: expected a CUDA torch tensor (there is no CPU path)")
+    if t.dtype != dtype or not t.is_contiguous():
+        raise TypeError(f"{name}: expected contiguous {dtype}")
+    if ndim is not None and t.dim() != ndim:
+        raise ValueError(f"{name}: expected {ndim} dimensions, got {tuple(t.shape)}")
+    return t
+
+
+def alloc_workspace(nx, ny, nz, n_src, n_rays, n_bins, n_steps, device=None):
+    torch = _torch()
+    n = max(16, rt_workspace_bytes(nx, ny, nz, n_src, n_rays, n_bins, n_steps))
+    return torch.empty(n, dtype=torch.uint8, device=device or "cuda")
+
+
+def rt_march_ex(j, kappa, sources, n_rays, step_size, c, dt, n_steps, out=None, workspace=None, stream=None,
+                variant=RT_VARIANT_DEFAULT):
+    """out[n_steps,nx,ny,nz,n_bins] = the march of include/rtmarch.h; asynchronous on the stream."""
+    torch = _torch()
+    _check_dev(j, "j", torch.float32, 4)
+    _check_dev(kappa, "kappa", torch.float32, 4)
+    _check_dev(sources, "sources", torch.float32, 2)
+    if kappa.shape != j.shape or sources.shape[1] != 3:
+        raise ValueError("kappa must have j's shape and sources must be [n_src, 3]")
+    nx, ny, nz, nb = j.shape
+    n_src = sources.shape[0]
+    if out is None:
+        out = torch.empty((n_steps, nx, ny, nz, nb), dtype=torch.float32, device=j.device)
+    else:
+        _check_dev(out, "out", torch.float32)
+        if out.numel() != n_steps * j.numel():
+            raise ValueError("out has the wrong size")
+    if workspace is None:
+        workspace = alloc_workspace(nx, ny, nz, n_src, n_rays, nb, n_steps, j.device)
+    rc = _lib.rt_march_ex(j.data_ptr(), kappa.data_ptr(), nx, ny, nz, sources.data_ptr(), n_src, n_rays, nb,
+                          step_size, c, dt, n_steps, out.data_ptr(), workspace.data_ptr(), workspace.numel(),
+                          _stream_ptr(stream), variant)
+    if rc != RT_OK:
+        raise RtError(rc, "rt_march")
+    return out
+
+
+def rt_march(j, kappa, sources, n_rays, step_size, c, dt, n_steps, out=None, workspace=None, stream=None):
+    return rt_march_ex(j, kappa, sources, n_rays, step_size, c, dt, n_steps, out, workspace, stream,
+                       RT_VARIANT_DEFAULT)
+
+
+def rt_march_single(j, kappa, source_pos, n_rays, step_size, c, dt, n_steps, out=None, workspace=None,
+                    stream=None):
+    torch = _torch()
+    _check_dev(j, "j", torch.float32, 4)
+    _check_dev(kappa, "kappa", torch.float32, 4)
+    _check_dev(source_pos, "source_pos", torch.float32)
+    if source_pos.numel() != 3 or kappa.shape != j.shape:
+        raise ValueError("source_pos must hold 3 floats and kappa must have j's shape")
+    nx, ny, nz, nb = j.shape
+    if out is None:
+        out = torch.empty((n_steps, nx, ny, nz, nb), dtype=torch.float32, device=j.device)
+    if workspace is None:
+        workspace = alloc_workspace(nx, ny, nz, 1, n_rays, nb, n_steps, j.device)
+    rc = _lib.rt_march_single(j.data_ptr(), kappa.data_ptr(), nx, ny, nz, source_pos.data_ptr(), n_rays, nb,
+                              step_size, c, dt, n_steps, out.data_ptr(), workspace.data_ptr(),
+                              workspace.numel(), _stream_ptr(stream))
+    if rc != RT_OK:
+        raise RtError(rc, "rt_march_single")
+    return out
+
+
+def rt_directions(n_rays: int, stream=None):
+    torch = _torch()
+    nhat = torch.empty((n_rays, 3), dtype=torch.float64, device="cuda")
+    rc = _lib.rt_directions(n_rays, nhat.data_ptr(), _stream_ptr(stream))
+    if rc != RT_OK:
+        raise RtError(rc, "rt_directions")
+    return nhat
+
+
+def rt_ray_order(n_rays: int, stream=None):
+    torch = _torch()
+    order = torch.empty(rt_ray_slots(n_rays), dtype=torch.int32, device="cuda")
+    rc = _lib.rt_ray_order(n_rays, order.data_ptr(), _stream_ptr(stream))
+    if rc != RT_OK:
+        raise RtError(rc, "rt_ray_order")
+    return order
+
+
+def rt_bench_red_ceiling(mode: int, grid, n_red: int, seed: int = 1, stream=None) -> int:
+    """Enqueue one ceiling microbenchmark on ``grid`` [nx,ny,nz,nb]; returns the reductions issued."""
+    torch = _torch()
+    _check_dev(grid, "grid", torch.float32, 4)
+    nx, ny, nz, nb = grid.shape
+    issued = ctypes.c_longlong(0)
+    rc = _lib.rt_bench_red_ceiling(mode, grid.data_ptr(), nx, ny, nz, nb, n_red, seed, ctypes.byref(issued),
+                                   _stream_ptr(stream))
+    if rc != RT_OK:
+        raise RtError(rc, "rt_bench_red_ceiling")
+    return int(issued.value)
+
+
+# ---------------------------------------------------------------------------------------------------
+# host-pointer entry point (end to end: H2D, march, D2H inside the call)
+# ---------------------------------------------------------------------------------------------------
+def rt_march_host(j, kappa, sources, n_rays, step_size, c, dt, n_steps, out=None):
+    def f32(a, nd):
+        a = np.asarray(a)
+        if a.dtype != np.float32 or not a.flags.c_contiguous or a.ndim != nd:
+            raise TypeError(f"expected a C-contiguous float32 array with {nd} dimensions")
+        return a
+    j, kappa, sources = f32(j, 4), f32(kappa, 4), f32(sources, 2)
+    if kappa.shape != j.shape or sources.shape[1] != 3:
+        raise ValueError("kappa must have j's shape and sources must be [n_src, 3]")
+    nx, ny, nz, nb = j.shape
+    if out is None:
+        out = np.empty((n_steps, nx, ny, nz, nb), dtype=np.float32)
+    elif out.dtype != np.float32 or not out.flags.c_contiguous or out.size != n_steps * j.size:
+        raise TypeError("out: expected C-contiguous float32 of n_steps * j.size elements")
+    rc = _lib.rt_march_host(j.ctypes.data, kappa.ctypes.data, nx, ny, nz, sources.ctypes.data, sources.shape[0],
+                            n_rays, nb, step_size, c, dt, n_steps, out.ctypes.data)
+    if rc != RT_OK:
+        raise RtError(rc, "rt_march_host")
+    return out
+
+
+def raw():
+    """The ctypes library handle (tests exercise error paths with raw pointers through it)."""
+    return _lib

@@ -1,0 +1,56 @@
+"""Build ``librtmarch.so`` (the C-ABI CUDA library, ``include/rtmarch.h``) in-tree with nvcc for sm_100a.
+
+``python -m paper_2511_09389_b200.build`` or ``build_library()``.  nvcc cross-compiles without a GPU.
+The library links cudart statically, so it loads (and its host-side argument checks run) on a box
+with no driver; any call that reaches CUDA there returns ``RT_ECUDA``.
+"""
+from __future__ import annotations
+
+import os
+import shutil
+import subprocess
+import sys
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+_ROOT = os.path.dirname(_PKG)
+CSRC = os.path.join(_PKG, "csrc")
+LIB_PATH = os.path.join(_PKG, "librtmarch.so")
+SOURCES = [os.path.join(CSRC, "rt_api.cu")]
+HEADERS = [os.path.join(CSRC, f) for f in ("rt_march_kernels.cuh", "rt_ceiling_kernels.cuh")] + \
+          [os.path.join(_ROOT, "include", "rtmarch.h")]
+
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
+              "-Xptxas=-v", "-Xcompiler", "-fPIC", "-shared"]
+
+
+def _nvcc() -> str:
+    for cand in (os.environ.get("NVCC"), shutil.which("nvcc"), "/usr/local/cuda/bin/nvcc"):
+        if cand and os.path.exists(cand):
+            return cand
+    raise RuntimeError("nvcc not found: librtmarch.so cannot be built (there is no fallback path)")
+
+
+def is_stale() -> bool:
+    if not os.path.exists(LIB_PATH):
+        return True
+    t = os.path.getmtime(LIB_PATH)
+    return any(os.path.getmtime(p) > t for p in SOURCES + HEADERS if os.path.exists(p))
+
+
+def build_library(force: bool = False, verbose: bool = False) -> str:
+    """Compile csrc/rt_api.cu -> librtmarch.so.  Returns the path.  Raises on failure."""
+    if not force and not is_stale():
+        return LIB_PATH
+    tmp = LIB_PATH + f".tmp{os.getpid()}"
+    cmd = [_nvcc()] + NVCC_FLAGS + ["-I", os.path.join(_ROOT, "include"), "-o", tmp] + SOURCES
+    r = subprocess.run(cmd, capture_output=True, text=True)
+    if verbose or r.returncode:
+        sys.stderr.write(r.stdout + r.stderr)
+    if r.returncode:
+        raise RuntimeError("nvcc failed building librtmarch.so")
+    os.replace(tmp, LIB_PATH)
+    return LIB_PATH
+
+
+if __name__ == "__main__":
+    print(build_library(force="--force" in sys.argv, verbose=True))

@@ -1,0 +1,265 @@
+"""GPU-vs-oracle parity (tier T2/T3): every test calls the CUDA path through the C ABI (ctypes binding) and
+compares with the fp64 oracle on the same seeded inputs, element by element, at BASELINE.json's tolerances
+(relative L2 <= 1e-4; per-voxel relative error <= 1e-3 on voxels above 1e-6 of the field maximum).
+
+Sizes: C0 and C1 in full; C2/C3/C4 against the oracle on stratified SOURCE SUBSETS (the field is a plain sum
+over sources, so a subset is the same computation with fewer terms; every other argument is the
+config's own), and at FULL size — the launch configuration bench.py times — through properties that hold at
+any size: agreement of the sliding-stencil kernel with the textbook 8-reductions-per-substep kernel,
+additivity over source chunks, exact darkness beyond the light front, run-to-run agreement.
+Set RT_FULL_PARITY=1 to also run the oracle on the full C2/C3/C4 (minutes of host time).
+"""
+import os
+
+import numpy as np
+import pytest
+
+import parity
+from paper_2511_09389_b200 import workloads
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def rt():
+    if not torch.cuda.is_available():
+        pytest.fail("-m gpu tests need a CUDA device")
+    import paper_2511_09389_b200 as rt
+    return rt
+
+
+def _dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def gpu_march(rt, w, variant=0, sources=None, n_steps=None, dt=None):
+    src = w.sources if sources is None else sources
+    out = rt.rt_march_ex(_dev(w.j), _dev(w.kappa), _dev(src), w.n_rays, w.step_size, w.c,
+                         w.dt if dt is None else dt, w.n_steps if n_steps is None else n_steps, variant=variant)
+    torch.cuda.synchronize()
+    return out.cpu().numpy()
+
+
+def oracle_march(oracle_mod, w, sources=None):
+    src = w.sources if sources is None else sources
+    return oracle_mod.march(w.j, w.kappa, src, w.n_rays, w.step_size, w.c, w.dt, w.n_steps)
+
+
+_cache = {}
+
+
+def config(name):
+    if name not in _cache:
+        _cache.clear()              # one large config in memory at a time
+        _cache[name] = workloads.make_config(name)
+    return _cache[name]
+
+
+VARIANTS = [0, 1, 2, 3]
+
+
+# ------------------------------------------------------------------------------------------------
+# building blocks
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n", [1, 2, 64, 1000, 4096, 16384])
+def test_directions_match_oracle(rt, oracle_mod, n):
+    got = rt.rt_directions(n).cpu().numpy()
+    want = np.stack([oracle_mod.direction(i, n) for i in range(n)])
+    assert np.abs(got - want).max() <= 4e-16
+    if n == 1:
+        assert got[0].tolist() == [1.0, 0.0, 0.0]          # the hand-traceable axis ray (pin P6)
+
+
+@pytest.mark.parametrize("n", [1, 31, 64, 1000, 4096, 16384, 100003])
+def test_ray_order_is_a_permutation(rt, n):
+    order = rt.rt_ray_order(n).cpu().numpy().astype(np.int64) & 0xFFFFFFFF
+    real = order[order != 0xFFFFFFFF]
+    assert len(order) == rt.rt_ray_slots(n)
+    assert np.array_equal(np.sort(real), np.arange(n))
+
+
+def test_substeps_rule_matches_oracle(rt, oracle_mod):
+    rng = np.random.default_rng(5)
+    cases = [(0.5, 1.0, 12.0), (0.5, 1.0, 222.0), (0.1, 1.0, 0.3), (0.3, 2.0, 1.0), (1.0, 1.0, 1e-3), (0.7, 3.0, 9.1)]
+    cases += [tuple(np.float32(rng.uniform(0.05, 3.0, 3))) for _ in range(200)]
+    for ds, c, dt in cases:
+        assert rt.rt_substeps_per_step(ds, c, dt) == oracle_mod.substeps(ds, c, dt), (ds, c, dt)
+
+
+# ------------------------------------------------------------------------------------------------
+# C0, C1: full configs, every kernel variant, every snapshot
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("name", ["C0", "C1"])
+def test_small_configs_full_parity(rt, oracle_mod, name, variant):
+    w = config(name)
+    ref = oracle_march(oracle_mod, w)
+    got = gpu_march(rt, w, variant)
+    parity.assert_parity(got, ref, f"{name} variant {variant}")
+
+
+def test_single_source_entry_point(rt, oracle_mod):
+    w = config("C0")
+    out = rt.rt_march_single(_dev(w.j), _dev(w.kappa), _dev(w.sources[0]), w.n_rays, w.step_size, w.c, w.dt,
+                             w.n_steps)
+    torch.cuda.synchronize()
+    parity.assert_parity(out.cpu().numpy(), oracle_march(oracle_mod, w), "rt_march_single C0")
+
+
+def test_host_entry_point(rt, oracle_mod):
+    w = config("C1")
+    out = rt.rt_march_host(w.j, w.kappa, w.sources, w.n_rays, w.step_size, w.c, w.dt, w.n_steps)
+    parity.assert_parity(out, oracle_march(oracle_mod, w), "rt_march_host C1")
+
+
+# ------------------------------------------------------------------------------------------------
+# hand-traceable and degenerate cases
+# ------------------------------------------------------------------------------------------------
+def _random_medium(shape, nb, seed):
+    rng = np.random.default_rng(seed)
+    j = rng.uniform(0.1, 1.0, shape + (nb,)).astype(np.float32)
+    k = rng.uniform(0.0, 0.6, shape + (nb,)).astype(np.float32)
+    return j, k
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("shape,nb,src,n_rays,ds,dt", [
+    ((4, 4, 4), 1, [(1.0, 2.0, 1.0)], 1, 0.5, 4.0),            # axis ray through and out of a 4-cube (pin P6)
+    ((4, 4, 4), 1, [(2.0, 1.0, 2.0)], 2, 0.5, 4.0),            # N_Omega = 2
+    ((5, 4, 3), 3, [(2.3, 1.6, 0.8), (0.0, 3.0, 2.0)], 7, 0.5, 5.0),   # ragged shape, 3 bins (scalar path)
+    ((3, 6, 4), 4, [(0.0, 5.0, 1.5)], 33, 0.25, 3.0),          # 4 bins (v4 path), source on a face
+    ((6, 5, 7), 8, [(-3.0, 9.0, 2.5)], 40, 0.5, 8.0),          # 8 bins, source OUTSIDE the box (clamped)
+    ((1, 1, 1), 1, [(0.0, 0.0, 0.0)], 5, 0.5, 2.0),            # one-voxel grid: everything clamps to it
+    ((2, 9, 1), 5, [(0.5, 4.0, 0.0)], 19, 0.5, 6.0),           # flat grid, 5 bins
+    ((8, 8, 8), 1, [(3.5, 3.5, 3.5)], 50, 1.7, 13.6),          # steps longer than a cell (stencil jumps)
+    ((8, 8, 8), 4, [(3.0, 4.0, 5.0)], 50, 0.05, 1.0),          # many substeps per cell
+    ((8, 8, 8), 1, [(3.5, 3.5, 3.5)], 17, 0.5, 0.4),           # N_s = 1
+])
+def test_small_cases(rt, oracle_mod, shape, nb, src, n_rays, ds, dt, variant):
+    j, k = _random_medium(shape, nb, seed=sum(shape) + nb)
+    src = np.array(src, dtype=np.float32)
+    for n_steps in (1, 3):
+        ref = oracle_mod.march(j, k, src, n_rays, ds, 1.0, dt, n_steps)
+        out = rt.rt_march_ex(_dev(j), _dev(k), _dev(src), n_rays, ds, 1.0, dt, n_steps, variant=variant)
+        torch.cuda.synchronize()
+        parity.assert_parity(out.cpu().numpy(), ref, f"{shape} nb={nb} variant={variant} steps={n_steps}")
+
+
+def test_out_is_overwritten_and_call_is_repeatable(rt, oracle_mod):
+    w = config("C0")
+    j, k, s = _dev(w.j), _dev(w.kappa), _dev(w.sources)
+    out = torch.full((1,) + w.j.shape, 7.0, device="cuda")
+    ws = rt.alloc_workspace(16, 16, 16, 1, w.n_rays, 1, 1)
+    for _ in range(3):
+        rt.rt_march(j, k, s, w.n_rays, w.step_size, w.c, w.dt, 1, out=out, workspace=ws)
+    torch.cuda.synchronize()
+    parity.assert_parity(out.cpu().numpy(), oracle_march(oracle_mod, w), "repeat")
+
+
+def test_runs_on_a_side_stream(rt, oracle_mod):
+    w = config("C0")
+    st = torch.cuda.Stream()
+    j, k, s = _dev(w.j), _dev(w.kappa), _dev(w.sources)
+    torch.cuda.synchronize()
+    with torch.cuda.stream(st):
+        out = rt.rt_march(j, k, s, w.n_rays, w.step_size, w.c, w.dt, 1)
+    st.synchronize()
+    parity.assert_parity(out.cpu().numpy(), oracle_march(oracle_mod, w), "side stream")
+
+
+def test_error_codes_on_device(rt):
+    w = config("C0")
+    j, k, s = _dev(w.j), _dev(w.kappa), _dev(w.sources)
+    with pytest.raises(rt.RtError) as e:
+        rt.rt_march(j, k, s, w.n_rays, w.step_size, w.c, w.dt, 1, workspace=torch.empty(16, dtype=torch.uint8, device="cuda"))
+    assert e.value.code == rt.RT_EWORKSPACE
+    with pytest.raises(rt.RtError) as e:
+        rt.rt_march(j, k, s, 0, w.step_size, w.c, w.dt, 1)
+    assert e.value.code == rt.RT_EINVAL
+    with pytest.raises(rt.RtError) as e:
+        rt.rt_march(j, k, s, w.n_rays, -1.0, w.c, w.dt, 1)
+    assert e.value.code == rt.RT_EINVAL
+
+
+# ------------------------------------------------------------------------------------------------
+# C2, C3, C4: oracle parity on stratified source subsets (all other arguments are the config's)
+# ------------------------------------------------------------------------------------------------
+def _stratified(n_src, count):
+    return np.unique(np.linspace(0, n_src - 1, count).round().astype(int))
+
+
+SUBSETS = {"C2": 48, "C3": 6, "C4": 3}
+
+
+@pytest.mark.parametrize("name", ["C2", "C3", "C4"])
+def test_large_configs_subset_parity(rt, oracle_mod, name):
+    w = config(name)
+    idx = _stratified(w.n_src, SUBSETS[name])
+    src = np.ascontiguousarray(w.sources[idx])
+    ref = oracle_march(oracle_mod, w, src)
+    for variant in (0, 1):
+        got = gpu_march(rt, w, variant, sources=src)
+        rows = parity.assert_parity(got, ref, f"{name} subset variant {variant}")
+    print(name, "subset parity:", rows[-1])
+
+
+# ------------------------------------------------------------------------------------------------
+# full size, the launch configuration bench.py times: properties that hold at any size
+# ------------------------------------------------------------------------------------------------
+def _close(a, b, what):
+    """Two fp32 GPU fields of the same quantity: each is within tolerance of the exact field, so they are
+    within twice the tolerance of one another."""
+    rows = parity.compare(a, b.astype(np.float64))
+    for r in rows:
+        assert r["nonfinite"] == 0, (what, r)
+        assert r["rel_l2"] <= 2 * parity.REL_L2_TOL and r["max_voxel_rel"] <= 2 * parity.PER_VOXEL_TOL, (what, r)
+    return rows
+
+
+@pytest.mark.parametrize("name", ["C2", "C3", "C4"])
+def test_full_size_properties(rt, name):
+    w = config(name)
+    full = gpu_march(rt, w, 0)
+    assert np.isfinite(full).all() and full.min() >= 0.0
+    # (1) run-to-run: only the order of the fp32 reductions differs
+    _close(gpu_march(rt, w, 0), full, f"{name} rerun")
+    # (2) additivity over sources: the sum of chunk fields is the field
+    chunks = np.array_split(np.arange(w.n_src), 4)
+    parts = sum(gpu_march(rt, w, 0, sources=np.ascontiguousarray(w.sources[c])).astype(np.float64) for c in chunks)
+    _close(full, parts, f"{name} additivity")
+    # (3) snapshots are cumulative and non-decreasing (D7): deposits are non-negative
+    for m in range(1, w.n_steps):
+        assert (full[m] >= full[m - 1] * (1 - 1e-6)).all()
+    # (4) prefix property (pin P7): the last snapshot's predecessor equals a shorter run's last snapshot
+    if w.n_steps > 1:
+        short = gpu_march(rt, w, 0, n_steps=w.n_steps - 1)
+        _close(short, full[:-1], f"{name} prefix")
+    # (5) beyond the light front the field is exactly zero (pin P5): last deposit position + stencil reach
+    ax = [np.arange(n, dtype=np.float32) for n in w.shape]
+    d2min = np.full(w.shape, np.inf, dtype=np.float32)
+    for s in w.sources:
+        d2 = ((ax[0] - s[0]) ** 2)[:, None, None] + ((ax[1] - s[1]) ** 2)[None, :, None] + \
+             ((ax[2] - s[2]) ** 2)[None, None, :]
+        np.minimum(d2min, d2, out=d2min)
+    for m in range(w.n_steps):
+        reach = ((m + 1) * w.substeps_per_step - 1) * w.step_size + np.sqrt(3.0)
+        dark = d2min > np.float32(reach * reach * 1.0001)
+        assert np.count_nonzero(full[m][dark]) == 0, (name, m, int(dark.sum()))
+
+
+@pytest.mark.parametrize("name", ["C2"])
+def test_full_size_textbook_kernel_agrees(rt, name):
+    """The sliding-stencil kernel (default) and the 8-reductions-per-substep kernel give the same field."""
+    w = config(name)
+    _close(gpu_march(rt, w, 0), gpu_march(rt, w, 1), f"{name} sliding vs direct")
+
+
+@pytest.mark.skipif(os.environ.get("RT_FULL_PARITY") != "1", reason="set RT_FULL_PARITY=1 (minutes of host time)")
+@pytest.mark.parametrize("name", ["C2", "C3", "C4"])
+def test_full_size_oracle_parity(rt, oracle_mod, name):
+    w = config(name)
+    ref = oracle_march(oracle_mod, w)
+    rows = parity.assert_parity(gpu_march(rt, w, 0), ref, f"{name} full")
+    print(name, "full parity:", rows)
