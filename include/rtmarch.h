@@ -97,6 +97,14 @@ int rt_launch_count(int n_bins, int n_steps);
  * nhat[n_rays][3] (float64, device), computed exactly as the march kernel does. */
 int rt_directions(int n_rays, double* nhat, void* stream);
 
+/* TEST HOOK.  Marches ONE ray (source_pos[3], lattice index ray_index of n_rays) for n_sub substeps from k = 0
+ * with the arithmetic of the march kernels (fixed-point position, fp32 weights, gather, eq. (2)) and records,
+ * per substep k: pos[k][3] = x_k (float64), trace_I[k][b] = I_{k+1} (NOT scaled by 4 pi/N_Omega) and
+ * trace_T[k][b] = exp(-tau_{k+1}).  All pointers device; nothing is deposited. */
+int rt_trace_ray(const float* j, const float* kappa, int nx, int ny, int nz, int n_bins,
+                 const float* source_pos, int ray_index, int n_rays, float step_size, int n_sub,
+                 double* pos, float* trace_I, float* trace_T, void* stream);
+
 /* TEST HOOK.  Writes the coherent ray order into order[rt_ray_slots(n_rays)] (uint32, device): slot ->
  * lattice index, 0xFFFFFFFF for padding slots.  Every index 0..n_rays-1 appears exactly once. */
 int rt_ray_order(int n_rays, unsigned int* order, void* stream);

@@ -14,7 +14,7 @@
 //     for every source s and every Fibonacci direction i (any order; state I[b], tau[b] kept per (s,i)):
 //       nhat = fib(i, N_Omega)                                           P:27   (reading D1)
 //       for k in m*N_s .. (m+1)*N_s - 1:
-//         p   = x0[s] + (k*ds) * nhat                                    P:23   (x_{k+1} = x_k + nhat ds, closed form, D3)
+//         p   = x0[s] + k * (ds * nhat)   on the 2^-64 cell grid         P:23   (x_{k+1} = x_k + nhat ds, closed form, D3)
 //         i0  = floor(p) per axis;  f = p - i0 in [0,1)
 //         lo  = clamp(i0, 0, N-1);  hi = clamp(i0+1, 0, N-1)             P:29   "Indexing is clamped" (D5)
 //         for every bin b:                                               P:39   bins are a batch axis
@@ -32,7 +32,9 @@
 // arithmetic.  Reading D4 (floor vs round for "nearest neighbour") and the exact lattice D1 are pinned
 // only by those hand traces and by DESIGN.md's decision: the paper itself does not fix them.
 //
-// All arithmetic is double (long double only to reduce the golden-angle phase accurately).  No SIMD, no
+// All arithmetic is double, except: long double to reduce the golden-angle phase accurately, and the position
+// x_k, which is evaluated EXACTLY on a 2^-64 cell grid in 128-bit integers (reading D3) so that floor(x_k) is the
+// same decision for every implementation of that reading.  No SIMD, no
 // blocking, no reordering beyond "rays are independent": rays are split over threads, each thread
 // owns a private grid, and the private grids are added in thread order, so a run is bit-reproducible for a
 // given thread count.
@@ -63,16 +65,46 @@ long substeps(double ds, double c, double dt) {
     return long(std::ceil(r));
 }
 
-// P:27 / reading D1: golden-angle lattice, i = 0..n-1, z_i = 1 - (2i+1)/n, phi_i = i * pi * (3 - sqrt 5).
+// P:27 / reading D1: golden-angle lattice, i = 0..n-1, z_i = 1 - (2i+1)/n = (n-2i-1)/n, phi_i = i * pi * (3 - sqrt 5).
+// z and the radius sqrt((1-z)(1+z)) are formed from exact integers with correctly rounded IEEE double operations
+// only (one division for z; two divisions, one product, one square root for the radius), so that any
+// implementation stating the same operations gets the same bits: z decides floor() ties of rational positions
+// (reading D3).  The azimuth is reduced in long double with a two-term golden-angle constant.
 void fib_direction(long i, long n, double nhat[3]) {
-    long double z = 1.0L - (2.0L * (long double)i + 1.0L) / (long double)n;
-    long double turn = (long double)i * ((3.0L - sqrtl(5.0L)) / 2.0L);   // phi / (2 pi)
-    turn -= floorl(turn);
+    const double dn = double(n), di = double(i);
+    volatile double one_minus_z = (2.0 * di + 1.0) / dn;
+    volatile double one_plus_z = (2.0 * double(n - i) - 1.0) / dn;
+    volatile double prod = one_minus_z * one_plus_z;
+    const double r = std::sqrt(prod);
+    // phi / (2 pi) mod 1 = frac(i g), g = (3 - sqrt 5)/2 = 0x0.61C8864680B583EA0C633F9FA31237CB... split into two
+    // exactly representable long doubles; the product i*g_hi is taken with its exact residual (fmal), so the
+    // reduced turn is good to ~1e-19 for every i < 2^30 (a plain long double product loses i * 2^-64 turn).
+    const long double g_hi = 0x61C8864680B583EAp-64L, g_lo = 0x0C633F9FA31237CBp-128L, li = (long double)i;
+    const long double p = li * g_hi;
+    const long double resid = fmal(li, g_hi, -p);
+    long double turn = (p - floorl(p)) + (resid + li * g_lo);
     long double phi = 2.0L * kPiL * turn;
-    long double s = sqrtl((1.0L - z) * (1.0L + z));
-    nhat[0] = double(s * cosl(phi));
-    nhat[1] = double(s * sinl(phi));
-    nhat[2] = double(z);
+    volatile double c = double(cosl(phi)), s = double(sinl(phi));
+    nhat[0] = r * c;
+    nhat[1] = r * s;
+    nhat[2] = (dn - 2.0 * di - 1.0) / dn;
+}
+
+// Reading D3: positions live on the 2^-64 cell grid.  fx(v) = floor(v * 2^64) EXACTLY (the double's significand is
+// shifted, nothing is rounded), and x_k := (fx(x_0) + k * fx(ds * nhat)) / 2^64 in exact integer arithmetic, so
+// floor(x_k) -- the one discontinuous decision of the method (nearest-neighbour kappa) -- does not depend on
+// floating-point rounding order.  |x_k - (x_0 + k ds nhat)| < (k+1) 2^-64 cell.
+typedef __int128 fx_t;
+
+fx_t fx(double v) {
+    if (v == 0.0) return 0;
+    int e;
+    const double m = std::frexp(v, &e);                   // v = m 2^e, 0.5 <= |m| < 1
+    const long long M = (long long)std::ldexp(m, 53);     // exact 53-bit signed integer: v = M 2^(e-53)
+    const int sh = e + 11;                                // v 2^64 = M 2^sh
+    if (sh >= 0) return fx_t(M) << sh;                    // |v| < 2^30 in every caller: no overflow
+    if (sh > -64) return fx_t(M >> (-sh));                // arithmetic shift of a negative value = floor
+    return M < 0 ? -1 : 0;
 }
 
 inline long clampl(long v, long lo, long hi) { return v < lo ? lo : (v > hi ? hi : v); }
@@ -82,17 +114,23 @@ inline long clampl(long v, long lo, long hi) { return v < lo ? lo : (v > hi ? hi
 void march_ray(const Medium& M, const double x0[3], const double nhat[3], double ds, long k_begin, long k_end,
                double* I, double* tau, double* acc, double* trace_I, double* trace_tau, double* trace_pos) {
     const long N[3] = {M.nx, M.ny, M.nz};
+    fx_t X0[3], D[3];
+    for (int a = 0; a < 3; ++a) {
+        X0[a] = fx(x0[a]);
+        volatile double step = ds * nhat[a];              // one rounding, no contraction
+        D[a] = fx(step);
+    }
     for (long k = k_begin; k < k_end; ++k) {
         long lo[3], hi[3];
         double f[3];
         for (int a = 0; a < 3; ++a) {
-            double p = x0[a] + (double(k) * ds) * nhat[a];
-            double fl = std::floor(p);
-            f[a] = p - fl;
-            long i0 = long(fl);
+            const fx_t X = X0[a] + fx_t(k) * D[a];        // x_k on the 2^-64 grid (reading D3)
+            const long i0 = long((long long)(X >> 64));   // floor(x_k)
+            const unsigned long long frac = (unsigned long long)X;
+            f[a] = double(frac) * 5.42101086242752217e-20;   // (x_k - floor x_k), frac * 2^-64
             lo[a] = clampl(i0, 0, N[a] - 1);
             hi[a] = clampl(i0 + 1, 0, N[a] - 1);
-            if (trace_pos) trace_pos[(k - k_begin) * 3 + a] = p;
+            if (trace_pos) trace_pos[(k - k_begin) * 3 + a] = double(i0) + f[a];
         }
         size_t corner[8];
         double w[8];

@@ -20,7 +20,7 @@ RED_MODES = {"M1_scalar_random": 0, "M2_v4_random": 1, "M3_stencil": 2, "M4_one_
              "M5_coalesced": 4, "M6_stencil_walk": 5}
 
 EXPORTS = ("rt_march", "rt_march_single", "rt_march_ex", "rt_march_host", "rt_workspace_bytes",
-           "rt_substeps_per_step", "rt_launch_count", "rt_directions", "rt_ray_order", "rt_ray_slots",
+           "rt_substeps_per_step", "rt_launch_count", "rt_directions", "rt_ray_order", "rt_ray_slots", "rt_trace_ray",
            "rt_bench_red_ceiling", "rt_strerror", "rt_version")
 
 
@@ -34,6 +34,12 @@ def _load() -> ctypes.CDLL:
     path = _build.LIB_PATH
     if not os.path.exists(path):
         path = _build.build_library()          # raises if nvcc is missing: no fallback
+    elif _build.is_stale():                    # sources newer than the library: rebuild if a compiler is here
+        try:
+            path = _build.build_library()
+        except RuntimeError:
+            if os.environ.get("RT_REQUIRE_FRESH_LIB"):
+                raise
     L = ctypes.CDLL(path)
     vp, i, f, sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_float, ctypes.c_size_t
     march_args = [vp, vp, i, i, i, vp, i, i, i, f, f, f, i, vp]
@@ -48,6 +54,7 @@ def _load() -> ctypes.CDLL:
     L.rt_directions.argtypes = [i, vp, vp]
     L.rt_ray_order.argtypes = [i, vp, vp]
     L.rt_ray_slots.argtypes = [i]
+    L.rt_trace_ray.argtypes = [vp, vp, i, i, i, i, vp, i, i, f, i, vp, vp, vp, vp]
     L.rt_bench_red_ceiling.argtypes = [i, vp, i, i, i, i, ctypes.c_longlong, ctypes.c_uint,
                                        ctypes.POINTER(ctypes.c_longlong), vp]
     L.rt_strerror.argtypes = [i]
@@ -189,6 +196,23 @@ def rt_ray_order(n_rays: int, stream=None):
     if rc != RT_OK:
         raise RtError(rc, "rt_ray_order")
     return order
+
+
+def rt_trace_ray(j, kappa, source_pos, ray_index: int, n_rays: int, step_size: float, n_sub: int, stream=None):
+    """One ray on the GPU, per-substep records: dict(pos=[n_sub,3] f64, I=[n_sub,B] f32, T=[n_sub,B] f32)."""
+    torch = _torch()
+    _check_dev(j, "j", torch.float32, 4)
+    _check_dev(kappa, "kappa", torch.float32, 4)
+    _check_dev(source_pos, "source_pos", torch.float32)
+    nx, ny, nz, nb = j.shape
+    pos = torch.empty((n_sub, 3), dtype=torch.float64, device=j.device)
+    tr_i = torch.empty((n_sub, nb), dtype=torch.float32, device=j.device)
+    tr_t = torch.empty((n_sub, nb), dtype=torch.float32, device=j.device)
+    rc = _lib.rt_trace_ray(j.data_ptr(), kappa.data_ptr(), nx, ny, nz, nb, source_pos.data_ptr(), ray_index, n_rays,
+                           step_size, n_sub, pos.data_ptr(), tr_i.data_ptr(), tr_t.data_ptr(), _stream_ptr(stream))
+    if rc != RT_OK:
+        raise RtError(rc, "rt_trace_ray")
+    return {"pos": pos, "I": tr_i, "T": tr_t}
 
 
 def rt_bench_red_ceiling(mode: int, grid, n_red: int, seed: int = 1, stream=None) -> int:

@@ -232,6 +232,25 @@ int rt_directions(int n_rays, double* nhat, void* stream) {
     return RT_OK;
 }
 
+int rt_trace_ray(const float* j, const float* kappa, int nx, int ny, int nz, int n_bins, const float* source_pos,
+                 int ray_index, int n_rays, float step_size, int n_sub, double* pos, float* trace_I, float* trace_T,
+                 void* stream) {
+    if (!j || !kappa || !source_pos || !pos || !trace_I || !trace_T) return RT_EINVAL;
+    if (nx < 1 || ny < 1 || nz < 1 || n_bins < 1 || n_rays < 1 || n_rays > (1 << 30) || ray_index < 0 ||
+        ray_index >= n_rays || n_sub < 1 || !positive_finite(step_size))
+        return RT_EINVAL;
+    if ((long long)nx * ny * nz * n_bins > 2147483647LL) return RT_EINVAL;
+    rt::MarchParams P{};
+    P.j = j; P.kappa = kappa; P.sources = source_pos; P.out = nullptr; P.ray_order = nullptr;
+    P.nx = nx; P.ny = ny; P.nz = nz; P.nb = n_bins;
+    P.n_src = 1; P.n_rays = n_rays; P.n_slots = n_rays; P.n_groups = 1; P.n_steps = 1; P.n_sub = n_sub;
+    P.ds = double(step_size); P.ds_f = step_size; P.emis = step_size; P.snap_stride = 0;
+    rt::trace_ray_kernel<<<1, 32, 0, static_cast<cudaStream_t>(stream)>>>(P, uint32_t(ray_index), n_sub, pos, trace_I,
+                                                                         trace_T);
+    RT_CUDA(cudaGetLastError());
+    return RT_OK;
+}
+
 int rt_ray_slots(int n_rays) {
     if (n_rays < 1 || n_rays > (1 << 30)) return RT_EINVAL;
     return ray_slots(n_rays);

@@ -40,40 +40,59 @@ struct MarchParams {
 };
 
 constexpr uint32_t kPad = 0xFFFFFFFFu;
-// (3 - sqrt 5)/2 * 2^64: the golden angle as a fraction of a turn, exact to 2^-65 turn
-constexpr uint64_t kGoldenTurn64 = 0x61C8864680B583EBull;
+// (3 - sqrt 5)/2 * 2^128, floored: the golden angle as a fraction of a turn in 0.128 fixed point
+constexpr uint64_t kGoldenTurnHi = 0x61C8864680B583EAull;
+constexpr uint64_t kGoldenTurnLo = 0x0C633F9FA31237CBull;
+
+// i * golden turn mod 1 as a 0.64 fraction (error < 2^-64 + i 2^-128 turn)
+__device__ __forceinline__ uint64_t golden_turn64(uint32_t i) {
+    return uint64_t(i) * kGoldenTurnHi + __umul64hi(uint64_t(i), kGoldenTurnLo);
+}
 
 // ---------------------------------------------------------------------------------------------------
-// direction lattice (D1): z_i = 1 - (2i+1)/N, phi_i = i * pi (3 - sqrt 5)
+// direction lattice (D1): z_i = 1 - (2i+1)/N = (N-2i-1)/N, phi_i = i * pi (3 - sqrt 5).
+// z and sqrt(1-z^2) use only correctly rounded IEEE double operations on exact integers (one division for z;
+// (2i+1)/N, (2(N-i)-1)/N, their product and its square root for the radius), so the oracle, which states
+// the same operations, gets bit-identical values; the azimuth is reduced exactly in integer arithmetic.
 // ---------------------------------------------------------------------------------------------------
 __device__ __forceinline__ void fib_direction(uint32_t i, uint32_t n, double nh[3]) {
     const double q = (2.0 * double(i) + 1.0) / double(n);          // 1 - z
-    const double z = 1.0 - q;
-    const int64_t t = int64_t(uint64_t(i) * kGoldenTurn64);        // phi/(2 pi) mod 1 as a signed 0.64 fraction
+    const double q2 = (2.0 * double(n - i) - 1.0) / double(n);     // 1 + z
+    const double z = (double(n) - 2.0 * double(i) - 1.0) / double(n);
+    const int64_t t = int64_t(golden_turn64(i));                   // phi/(2 pi) mod 1 as a signed 0.64 fraction
     const double turn = double(t) * 5.42101086242752217e-20;       // * 2^-64  -> [-0.5, 0.5)
     double s, c;
     sincospi(2.0 * turn, &s, &c);
-    const double r = sqrt(q * (2.0 - q));                          // sqrt((1-z)(1+z))
-    nh[0] = r * c;
-    nh[1] = r * s;
+    const double r = sqrt(__dmul_rn(q, q2));                       // sqrt((1-z)(1+z))
+    nh[0] = __dmul_rn(r, c);
+    nh[1] = __dmul_rn(r, s);
     nh[2] = z;
 }
 
 // ---------------------------------------------------------------------------------------------------
-// 96-bit fixed point: value = c + fh 2^-32 + fl 2^-64
+// 96-bit fixed point: value = c + fh 2^-32 + fl 2^-64 (D3: positions live on the 2^-64 cell grid)
 // ---------------------------------------------------------------------------------------------------
 struct Fx96 {
     int32_t c;
     uint32_t fh, fl;
 };
 
-__device__ __forceinline__ Fx96 fx_from_double(double v) {   // |v| < 2^30
+// floor(v * 2^64) EXACTLY, for |v| < 2^30 (no floating-point rounding: the double's significand is shifted)
+__device__ __forceinline__ Fx96 fx_from_double(double v) {
+    const long long bits = __double_as_longlong(v);
+    const int e = int((bits >> 52) & 0x7FF);
+    long long m = bits & 0xFFFFFFFFFFFFFll;
+    if (e) m |= 1ll << 52;                                   // v = +-m 2^(e' - 1075), e' = max(e, 1)
+    if (bits < 0) m = -m;
+    const int sh = (e ? e : 1) - 1011;                       // v 2^64 = m 2^sh; sh <= 41 since |v| < 2^30
+    __int128 n;
+    if (sh >= 0) n = __int128(m) << sh;
+    else if (sh > -64) n = __int128(m >> (-sh));             // arithmetic shift = floor
+    else n = (m < 0) ? -1 : 0;
     Fx96 r;
-    const double fl = floor(v);
-    r.c = int32_t(fl);
-    const double t = (v - fl) * 4294967296.0;                // exact
-    r.fh = uint32_t(t);
-    r.fl = uint32_t((t - double(r.fh)) * 4294967296.0);
+    r.c = int32_t(int64_t(n >> 64));
+    r.fh = uint32_t(uint64_t(n) >> 32);
+    r.fl = uint32_t(uint64_t(n));
     return r;
 }
 
@@ -193,7 +212,7 @@ __device__ __forceinline__ RaySetup ray_setup(const MarchParams& P, const RayId&
         float x0 = __ldg(P.sources + 3 * size_t(id.src) + a);
         x0 = fminf(fmaxf(x0, -536870912.0f), 536870912.0f);       // saturate to +-2^29 cells (rtmarch.h)
         r.p[a] = fx_from_double(double(x0));
-        r.d[a] = fx_from_double(P.ds * nh[a]);
+        r.d[a] = fx_from_double(__dmul_rn(P.ds, nh[a]));
         r.neg[a] = nh[a] < 0.0;
     }
     return r;
@@ -253,6 +272,44 @@ __global__ void __launch_bounds__(128) march_direct_kernel(const MarchParams P) 
             for (int a = 0; a < 3; ++a) fx_add(R.p[a], R.d[a]);
         }
         og += P.snap_stride;
+    }
+}
+
+// ===================================================================================================
+// trace kernel (TEST HOOK): one thread marches one ray with the direct kernel's arithmetic and records, per
+// substep, the position x_k (as double: cell + 64-bit fraction), I_{k+1} (UNscaled by 4 pi/N_Omega: emis = ds)
+// and T_{k+1} = exp(-tau_{k+1}) for every bin.  No deposits.
+// ===================================================================================================
+__global__ void trace_ray_kernel(const MarchParams P, uint32_t ray_index, int n_sub, double* pos, float* trI, float* trT) {
+    if (blockIdx.x || threadIdx.x) return;
+    RayId id;
+    id.src = 0; id.group = 0; id.index = ray_index;
+    RaySetup R = ray_setup(P, id);
+    const int sx = P.ny * P.nz * P.nb, sy = P.nz * P.nb, sz = P.nb;
+    for (int b = 0; b < P.nb; ++b) {
+        Fx96 p[3] = {R.p[0], R.p[1], R.p[2]};
+        float I = 0.0f, T = 1.0f;
+        for (int k = 0; k < n_sub; ++k) {
+            const AxisLoHi ax = axis_lohi(p[0], P.nx - 1), ay = axis_lohi(p[1], P.ny - 1), az = axis_lohi(p[2], P.nz - 1);
+            const int ox[2] = {ax.lo * sx, ax.hi * sx}, oy[2] = {ay.lo * sy, ay.hi * sy}, oz[2] = {az.lo * sz, az.hi * sz};
+            const float wx[2] = {ax.g, ax.f}, wy[2] = {ay.g, ay.f}, wz[2] = {az.g, az.f};
+            const float kap = __ldg(P.kappa + ox[0] + oy[0] + oz[0] + b);
+            float jv = 0.0f;
+            for (int c = 0; c < 8; ++c) {
+                const float w = wx[c >> 2] * wy[(c >> 1) & 1] * wz[c & 1];
+                jv = fmaf(w, __ldg(P.j + ox[c >> 2] + oy[(c >> 1) & 1] + oz[c & 1] + b), jv);
+            }
+            const float a = expf(-kap * P.ds_f);
+            I = fmaf(I, a, jv * T * P.ds_f);
+            T *= a;
+            if (b == 0)
+                for (int q = 0; q < 3; ++q)
+                    pos[3 * size_t(k) + q] = double(p[q].c) + double(p[q].fh) * 2.3283064365386963e-10 +
+                                             double(p[q].fl) * 5.42101086242752217e-20;
+            trI[size_t(k) * P.nb + b] = I;
+            trT[size_t(k) * P.nb + b] = T;
+            for (int q = 0; q < 3; ++q) fx_add(p[q], R.d[q]);
+        }
     }
 }
 
@@ -403,7 +460,7 @@ __global__ void __launch_bounds__(128) march_sliding_kernel(const MarchParams P)
 __global__ void ray_order_kernel(uint32_t* order, int n_rays, int band) {
     extern __shared__ unsigned long long keys[];
     const uint32_t i = blockIdx.x * uint32_t(band) + threadIdx.x;
-    const uint64_t turn = uint64_t(i) * kGoldenTurn64;
+    const uint64_t turn = golden_turn64(i);
     keys[threadIdx.x] = (i < uint32_t(n_rays)) ? ((turn & 0xFFFFFFFF00000000ull) | i) : ~0ull;
     __syncthreads();
     for (int size = 2; size <= band; size <<= 1)

@@ -36,6 +36,16 @@ def test_p0_directions_match_50_digit_arithmetic(oracle_mod):
             ref = [float(s * mp.cos(phi)), float(s * mp.sin(phi)), float(z)]
             got = oracle_mod.direction(i, n)
             assert np.max(np.abs(got - ref)) < 3e-16, (n, i, got, ref)
+    # every index of the largest lattice the configs use: the azimuth reduction must not lose i * eps
+    n = 16384
+    worst = 0.0
+    for i in range(0, n, 7):
+        z = 1 - mp.mpf(2 * i + 1) / n
+        s = mp.sqrt(1 - z * z)
+        phi = i * golden_angle
+        ref = [float(s * mp.cos(phi)), float(s * mp.sin(phi)), float(z)]
+        worst = max(worst, float(np.max(np.abs(oracle_mod.direction(i, n) - ref))))
+    assert worst < 3.5e-16, worst
 
 
 def test_p0_lattice_is_unit_and_nearly_uniform(oracle_mod):
@@ -231,6 +241,57 @@ def test_p5_horizon_is_exactly_dark(oracle_mod):
         assert np.all(out[m, ..., 0][d < min(reach - 2.5, 5.0)] > 0.0)      # and lit inside (512 rays: gap-free to r = 5)
         assert np.mean(out[m, ..., 0][d < reach - 2.5] > 0.0) > 0.9
     assert np.all(out[1] >= out[0]) and np.all(out[2] >= out[1])  # cumulative snapshots (D7)
+
+
+# ------------------------------------------------------------------------------------------------------
+# D3  positions on the 2^-64 cell grid (DESIGN.md §4 D3): x_k = (floor(x_0 2^64) + k floor(ds nhat 2^64)) / 2^64.
+#     Independent arithmetic: Python exact rationals (fractions.Fraction of the very doubles).  The cases
+#     include rays whose exact position lands on an integer plane (z_i rational, N_Omega not a power of two),
+#     where floor() -- hence the nearest-neighbour kappa cell -- would otherwise hinge on
+#     floating-point rounding order.
+# ------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n_rays,ray,src,ds,n_sub", [
+    (7, 4, (0.0, 3.0, 2.0), 0.5, 10),          # z = -2/7: exact z-position 1.0 at k = 7
+    (33, 7, (0.0, 5.0, 1.5), 0.25, 12),
+    (40, 18, (-3.0, 9.0, 2.5), 0.5, 48),
+    (5, 0, (1.0, 2.0, 0.0), 0.5, 12),          # nhat = (0.6, 0, 0.8) up to rounding: x hits 4.0 at k = 10
+    (64, 11, (7.5, 7.5, 7.5), 0.5, 24),
+    (1, 0, (1.0, 1.25, 2.5), 0.5, 8),
+])
+def test_d3_positions_live_on_the_2_64_grid(oracle_mod, n_rays, ray, src, ds, n_sub):
+    from fractions import Fraction
+    shape = (6, 5, 4)
+    rng = np.random.default_rng(11)
+    j = rng.uniform(0.1, 1.0, shape + (1,)).astype(np.float32)
+    kap = rng.uniform(0.0, 0.6, shape + (1,)).astype(np.float32)
+    tr = oracle_mod.trace_ray(j, kap, src, ray, n_rays, ds, n_sub)
+    nh = oracle_mod.direction(ray, n_rays)
+    two64 = 1 << 64
+    X0 = [math.floor(Fraction(f32(v)) * two64) for v in src]
+    D = [math.floor(Fraction(float(f32(ds)) * float(nh[a])) * two64) for a in range(3)]   # ONE double rounding of ds*nhat
+    I = tau = 0.0
+    dsd = float(f32(ds))
+    for k in range(n_sub):
+        lo, hi, f = [], [], []
+        for a in range(3):
+            X = X0[a] + k * D[a]
+            i0, frac = X >> 64, X & (two64 - 1)                 # Python's >> floors
+            f.append(float(frac) * 2.0 ** -64)
+            lo.append(min(max(i0, 0), shape[a] - 1))
+            hi.append(min(max(i0 + 1, 0), shape[a] - 1))
+            assert abs(tr["pos"][k, a] - (i0 + f[a])) <= 1e-15 * max(1.0, abs(i0))
+            assert abs((i0 + f[a]) - (float(f32(src[a])) + k * dsd * nh[a])) < 1e-13
+        jv = 0.0
+        for c in range(8):
+            d = ((c >> 2) & 1, (c >> 1) & 1, c & 1)
+            w = 1.0
+            for a in range(3):
+                w *= f[a] if d[a] else 1.0 - f[a]
+            jv += w * float(j[tuple(hi[a] if d[a] else lo[a] for a in range(3))][0])
+        kk = float(kap[lo[0], lo[1], lo[2], 0])
+        I = I * math.exp(-kk * dsd) + jv * math.exp(-tau) * dsd
+        tau += kk * dsd
+        assert abs(tr["I"][k, 0] - I) <= 1e-13 * I and abs(tr["tau"][k, 0] - tau) <= 1e-13 * max(tau, 1e-30)
 
 
 # ------------------------------------------------------------------------------------------------------
