@@ -175,9 +175,10 @@ def measure_ceilings(rt, torch, shape, n_bins):
     """Reduction-throughput ceilings on a grid of the workload's size, in this process, back to back with
     the march: best of 5 launches of >= 2^28 reductions each, CUDA events.  Greds/s."""
     grid = torch.zeros(shape + (n_bins,), dtype=torch.float32, device="cuda")
+    grid64 = torch.zeros(shape + (n_bins,), dtype=torch.float64, device="cuda")
     res = {}
-    for name, mode in (("M1_scalar_random", 0), ("M2_v4_random", 1), ("M3_stencil", 2), ("M4_one_address", 3),
-                       ("M5_coalesced", 4), ("M6_stencil_walk", 5)):
+    for name, mode in rt.binding.RED_MODES.items():
+        g = grid64 if mode in (6, 7) else grid
         if mode == 1 and grid.numel() % 4:
             continue
         n_red = (1 << 24) if mode == 3 else (1 << 28)
@@ -185,13 +186,14 @@ def measure_ceilings(rt, torch, shape, n_bins):
         for rep in range(6):
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             e0.record()
-            issued = rt.rt_bench_red_ceiling(mode, grid, n_red, seed=rep + 1)
+            issued = rt.rt_bench_red_ceiling(mode, g, n_red, seed=rep + 1)
             e1.record()
             e1.synchronize()
             ms = e0.elapsed_time(e1)
             if rep and (best is None or ms < best):
                 best = ms
         res[name] = issued / (best * 1e-3) / 1e9
+    del grid64
     del grid
     return res
 
@@ -270,7 +272,7 @@ def run_native(args):
     line = None
     if rank == 0:
         field_sum = float(out.double().sum().item())
-        launches = rt.rt_launch_count(nb, w.n_steps)
+        launches = rt.rt_launch_count(int(src.shape[0]), nb, w.n_steps)
         cfg = describe(w, world)
         cfg["workload"] = cfg["workload"].replace(f"{w.n_src} sources/GPU", f"{n_src_per_gpu} sources/GPU")
         cfg.update({"timing": "CUDA events per step on the launch stream; 256 MiB L2 flush (memset) between "

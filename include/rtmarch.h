@@ -16,7 +16,7 @@
  *
  * LAYOUT.  j, kappa: [nx][ny][nz][n_bins] float32, C order, bin innermost; kappa in 1/cell-length.
  * sources: [n_src][3] float32 grid coordinates (axis 0, 1, 2); voxel (a,b,c) sits at coordinate (a,b,c).
- * out: [n_steps][nx][ny][nz][n_bins] float32, OVERWRITTEN.  Directions map to axes (0,1,2) as
+ * out: [n_steps][nx][ny][nz][n_bins] float32, OVERWRITTEN.  j must be finite (a weight-0 corner is still read).  Directions map to axes (0,1,2) as
  * (sqrt(1-z^2) cos phi, sqrt(1-z^2) sin phi, z).
  *
  * POINTERS AND OWNERSHIP.  Unless a function says "host", every pointer is a DEVICE pointer on the current
@@ -49,11 +49,16 @@ extern "C" {
 #define RT_EALIGN (-4)     /* j, kappa or out not 4-byte aligned */
 
 /* Kernel variants for rt_march_ex (tests and bench only; rt_march always uses RT_VARIANT_DEFAULT).
- * All variants compute the same field; they differ in how the deposit of P:29 is issued. */
-#define RT_VARIANT_DEFAULT 0 /* sliding-stencil register accumulation + coherent ray order */
+ * All variants compute the same field; they differ in how the deposit of P:29 is issued and in which rays
+ * share a warp.  A variant code is one kind (0..5), optionally OR-ed with one flag. */
+#define RT_VARIANT_DEFAULT 0 /* sliding-stencil register accumulation, coherent ray order; warp = 32 sources x 1
+                                direction when n_src >= 32, else 32 directions of one source */
 #define RT_VARIANT_DIRECT 1  /* textbook form: 8 reductions per ray-substep-bin-group, lattice order */
 #define RT_VARIANT_DIRECT_COHERENT 2 /* 8 reductions per ray-substep, coherent ray order */
-#define RT_VARIANT_SLIDING_LATTICE 3 /* sliding stencil, rays in lattice-index order */
+#define RT_VARIANT_SLIDING_LATTICE 3 /* sliding stencil, rays in lattice-index order, warp = 32 directions */
+#define RT_VARIANT_SLIDING_BY_DIRECTION 4 /* sliding stencil, coherent ray order, warp = 32 directions of one source */
+#define RT_VARIANT_SLIDING_BY_SOURCE 5 /* sliding stencil, coherent ray order, warp = 32 sorted sources x 1 direction */
+#define RT_VARIANT_FLAG_ACC_F32 16 /* accumulate straight into `out` in fp32 instead of the fp64 workspace grid */
 
 /* The multi-source march ("loop-and-sum wrapper").  See the header comment for semantics. */
 int rt_march(const float* j, const float* kappa, int nx, int ny, int nz,
@@ -82,7 +87,9 @@ int rt_march_host(const float* j, const float* kappa, int nx, int ny, int nz,
                   const float* sources, int n_src, int n_rays, int n_bins,
                   float step_size, float c, float dt, int n_steps, float* out);
 
-/* Bytes of device scratch one rt_march call needs (the ray-order table).  0 on invalid arguments. */
+/* Bytes of device scratch one rt_march call needs: the ray-order and source-order tables and the fp64
+ * accumulation grid (n_steps * nx*ny*nz*n_bins doubles: deposits are summed in fp64 and rounded to fp32 once,
+ * DESIGN.md §7).  0 on invalid arguments. */
 size_t rt_workspace_bytes(int nx, int ny, int nz, int n_src, int n_rays, int n_bins, int n_steps);
 
 /* N_s as the library computes it (D6): ceil(c dt / step_size), a ratio within 1e-6 (relative) of an
@@ -91,7 +98,7 @@ size_t rt_workspace_bytes(int nx, int ny, int nz, int n_src, int n_rays, int n_b
 int rt_substeps_per_step(float step_size, float c, float dt);
 
 /* Number of kernels of this library that one rt_march call with these arguments enqueues (memsets excluded). */
-int rt_launch_count(int n_bins, int n_steps);
+int rt_launch_count(int n_src, int n_bins, int n_steps);
 
 /* TEST HOOK.  Writes the library's direction lattice (D1) for i = 0..n_rays-1 into
  * nhat[n_rays][3] (float64, device), computed exactly as the march kernel does. */
@@ -120,8 +127,11 @@ int rt_ray_slots(int n_rays);
  *   mode 3  every reduction to one address                                                (M4)
  *   mode 4  warp-coalesced: 32 consecutive floats per warp instruction, random line       (M5)
  *   mode 5  M3 issued along a random walk of half a cell per step (ray-like locality)     (M6)
+ *   mode 6  scalar red.global.add.f64, uniformly random addresses                         (M1 in fp64)
+ *   mode 7  the stencil pattern of mode 2 with n_bins scalar red.global.add.f64 per corner (M3 in fp64)
+ * `grid` holds nx*ny*nz*n_bins floats (modes 0-5) or doubles (modes 6, 7).
  * The grid is only accumulated into (caller zero-fills if the content matters). */
-int rt_bench_red_ceiling(int mode, float* grid, int nx, int ny, int nz, int n_bins,
+int rt_bench_red_ceiling(int mode, void* grid, int nx, int ny, int nz, int n_bins,
                          long long n_red, unsigned int seed, long long* n_issued, void* stream);
 
 const char* rt_strerror(int code);

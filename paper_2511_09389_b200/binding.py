@@ -16,8 +16,9 @@ from . import build as _build
 
 RT_OK, RT_EINVAL, RT_EWORKSPACE, RT_ECUDA, RT_EALIGN = 0, -1, -2, -3, -4
 RT_VARIANT_DEFAULT, RT_VARIANT_DIRECT, RT_VARIANT_DIRECT_COHERENT, RT_VARIANT_SLIDING_LATTICE = 0, 1, 2, 3
+RT_VARIANT_SLIDING_BY_DIRECTION, RT_VARIANT_SLIDING_BY_SOURCE, RT_VARIANT_FLAG_ACC_F32 = 4, 5, 16
 RED_MODES = {"M1_scalar_random": 0, "M2_v4_random": 1, "M3_stencil": 2, "M4_one_address": 3,
-             "M5_coalesced": 4, "M6_stencil_walk": 5}
+             "M5_coalesced": 4, "M6_stencil_walk": 5, "M1_f64_scalar_random": 6, "M3_f64_stencil": 7}
 
 EXPORTS = ("rt_march", "rt_march_single", "rt_march_ex", "rt_march_host", "rt_workspace_bytes",
            "rt_substeps_per_step", "rt_launch_count", "rt_directions", "rt_ray_order", "rt_ray_slots", "rt_trace_ray",
@@ -50,7 +51,7 @@ def _load() -> ctypes.CDLL:
     L.rt_workspace_bytes.argtypes = [i] * 7
     L.rt_workspace_bytes.restype = sz
     L.rt_substeps_per_step.argtypes = [f, f, f]
-    L.rt_launch_count.argtypes = [i, i]
+    L.rt_launch_count.argtypes = [i, i, i]
     L.rt_directions.argtypes = [i, vp, vp]
     L.rt_ray_order.argtypes = [i, vp, vp]
     L.rt_ray_slots.argtypes = [i]
@@ -88,8 +89,8 @@ def rt_workspace_bytes(nx, ny, nz, n_src, n_rays, n_bins, n_steps) -> int:
     return int(_lib.rt_workspace_bytes(nx, ny, nz, n_src, n_rays, n_bins, n_steps))
 
 
-def rt_launch_count(n_bins: int, n_steps: int) -> int:
-    return int(_lib.rt_launch_count(n_bins, n_steps))
+def rt_launch_count(n_src: int, n_bins: int, n_steps: int) -> int:
+    return int(_lib.rt_launch_count(n_src, n_bins, n_steps))
 
 
 def rt_ray_slots(n_rays: int) -> int:
@@ -216,9 +217,10 @@ def rt_trace_ray(j, kappa, source_pos, ray_index: int, n_rays: int, step_size: f
 
 
 def rt_bench_red_ceiling(mode: int, grid, n_red: int, seed: int = 1, stream=None) -> int:
-    """Enqueue one ceiling microbenchmark on ``grid`` [nx,ny,nz,nb]; returns the reductions issued."""
+    """Enqueue one ceiling microbenchmark on ``grid`` [nx,ny,nz,nb] (float32; float64 for modes 6, 7);
+    returns the reductions issued."""
     torch = _torch()
-    _check_dev(grid, "grid", torch.float32, 4)
+    _check_dev(grid, "grid", torch.float64 if mode in (6, 7) else torch.float32, 4)
     nx, ny, nz, nb = grid.shape
     issued = ctypes.c_longlong(0)
     rc = _lib.rt_bench_red_ceiling(mode, grid.data_ptr(), nx, ny, nz, nb, n_red, seed, ctypes.byref(issued),

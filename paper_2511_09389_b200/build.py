@@ -16,7 +16,7 @@ _ROOT = os.path.dirname(_PKG)
 CSRC = os.path.join(_PKG, "csrc")
 LIB_PATH = os.path.join(_PKG, "librtmarch.so")
 SOURCES = [os.path.join(CSRC, "rt_api.cu")]
-HEADERS = [os.path.join(CSRC, f) for f in ("rt_march_kernels.cuh", "rt_ceiling_kernels.cuh")] + \
+HEADERS = sorted(os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith(".cuh")) + \
           [os.path.join(_ROOT, "include", "rtmarch.h")]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

@@ -8,7 +8,9 @@
 #include <cstring>
 
 #include "rt_ceiling_kernels.cuh"
-#include "rt_march_kernels.cuh"
+#include "rt_march_direct.cuh"
+#include "rt_march_sliding.cuh"
+#include "rt_setup_kernels.cuh"
 
 namespace {
 
@@ -70,17 +72,28 @@ int check_args(const void* j, const void* kappa, int nx, int ny, int nz, const v
     return RT_OK;
 }
 
-template <int NB>
-int launch_march(const rt::MarchParams& P, int variant, cudaStream_t st) {
-    const int threads = 128;
-    const long long chunks = (P.n_slots + threads - 1) / threads;
-    const long long blocks = chunks * P.n_groups * P.n_src;
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+// workspace layout: [ray order: slots u32][source order: n_src u32][fp64 accumulation grid]
+struct Workspace {
+    size_t src_order_at, acc_at, total;
+};
+Workspace workspace_layout(long long cells, int n_src, int n_rays, int n_steps) {
+    Workspace w;
+    w.src_order_at = align_up(size_t(ray_slots(n_rays)) * sizeof(uint32_t), 16);
+    w.acc_at = align_up(w.src_order_at + size_t(n_src) * sizeof(uint32_t), 256);
+    w.total = w.acc_at + size_t(cells) * size_t(n_steps) * sizeof(double);
+    return w;
+}
+
+template <int NB, typename ACC>
+int launch_march(const rt::MarchParams& P, bool sliding, cudaStream_t st) {
+    const long long blocks = rt::march_blocks(P.n_src, P.n_slots, P.n_groups, P.map_src);
     if (blocks > 2147483647LL) return RT_EINVAL;
-    const bool sliding = (variant == RT_VARIANT_DEFAULT || variant == RT_VARIANT_SLIDING_LATTICE);
     if (sliding)
-        rt::march_sliding_kernel<NB><<<unsigned(blocks), threads, 0, st>>>(P);
+        rt::march_sliding_kernel<NB, ACC><<<unsigned(blocks), rt::kThreads, 0, st>>>(P);
     else
-        rt::march_direct_kernel<NB><<<unsigned(blocks), threads, 0, st>>>(P);
+        rt::march_direct_kernel<NB, ACC><<<unsigned(blocks), rt::kThreads, 0, st>>>(P);
     RT_CUDA(cudaGetLastError());
     return RT_OK;
 }
@@ -93,53 +106,83 @@ int build_ray_order(int n_rays, uint32_t* order, cudaStream_t st) {
     return RT_OK;
 }
 
+constexpr int kMaxSortedSources = 65536;   // above this the O(n^2) source sort is skipped (identity order)
+
+// what a variant code means (rtmarch.h RT_VARIANT_*)
+struct Plan {
+    bool sliding, coherent, map_src, acc64;
+};
+bool make_plan(int variant, int n_src, Plan* pl) {
+    const int kind = variant & 15;
+    if (variant < 0 || (variant & ~31) || kind > RT_VARIANT_SLIDING_BY_SOURCE) return false;
+    pl->acc64 = !(variant & RT_VARIANT_FLAG_ACC_F32);
+    pl->sliding = !(kind == RT_VARIANT_DIRECT || kind == RT_VARIANT_DIRECT_COHERENT);
+    pl->coherent = !(kind == RT_VARIANT_DIRECT || kind == RT_VARIANT_SLIDING_LATTICE);
+    pl->map_src = (kind == RT_VARIANT_SLIDING_BY_SOURCE) || (kind == RT_VARIANT_DEFAULT && n_src >= 32);
+    return true;
+}
+
 int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const float* sources, int n_src, int n_rays,
                int n_bins, float step_size, float c, float dt, int n_steps, float* out, void* workspace,
                size_t workspace_bytes, void* stream, int variant) {
     Checked ck;
     const int rc = check_args(j, kappa, nx, ny, nz, sources, n_src, n_rays, n_bins, step_size, c, dt, n_steps, out, &ck);
     if (rc != RT_OK) return rc;
-    if (variant < RT_VARIANT_DEFAULT || variant > RT_VARIANT_SLIDING_LATTICE) return RT_EINVAL;
-    const bool coherent = (variant == RT_VARIANT_DEFAULT || variant == RT_VARIANT_DIRECT_COHERENT);
-    const size_t need = rt_workspace_bytes(nx, ny, nz, n_src, n_rays, n_bins, n_steps);
-    if (coherent && (!workspace || workspace_bytes < need || (uintptr_t(workspace) & 15u))) return RT_EWORKSPACE;
+    Plan pl;
+    if (!make_plan(variant, n_src, &pl)) return RT_EINVAL;
+    const Workspace wl = workspace_layout(ck.cells, n_src, n_rays, n_steps);
+    if (!workspace || workspace_bytes < wl.total || (uintptr_t(workspace) & 15u)) return RT_EWORKSPACE;
+    char* ws = static_cast<char*>(workspace);
 
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     rt::MarchParams P;
-    P.j = j; P.kappa = kappa; P.sources = sources; P.out = out;
+    P.j = j; P.kappa = kappa; P.sources = sources;
     P.nx = nx; P.ny = ny; P.nz = nz; P.nb = n_bins;
     P.n_src = n_src; P.n_rays = n_rays;
     P.n_steps = n_steps; P.n_sub = int(ck.n_sub);
     P.ds = double(step_size); P.ds_f = step_size;
     P.emis = float(double(step_size) * 4.0 * 3.14159265358979323846 / double(n_rays));
     P.snap_stride = ck.cells;
-    if (coherent) {
-        P.ray_order = static_cast<const uint32_t*>(workspace);
+    P.map_src = pl.map_src ? 1 : 0;
+    if (pl.coherent) {
+        P.ray_order = reinterpret_cast<const uint32_t*>(ws);
         P.n_slots = ray_slots(n_rays);
-        const int rc2 = build_ray_order(n_rays, static_cast<uint32_t*>(workspace), st);
+        const int rc2 = build_ray_order(n_rays, reinterpret_cast<uint32_t*>(ws), st);
         if (rc2 != RT_OK) return rc2;
     } else {
         P.ray_order = nullptr;
         P.n_slots = n_rays;
     }
-    RT_CUDA(cudaMemsetAsync(out, 0, size_t(ck.cells) * size_t(n_steps) * sizeof(float), st));   // D14: overwrite
-
-    // 4 bins per thread with 16-byte reductions when the layout allows it, else one bin per thread
-    const bool vec4 = (n_bins % 4 == 0) && !((uintptr_t(j) | uintptr_t(kappa) | uintptr_t(out)) & 15u);
-    int rc3;
-    if (vec4) {
-        P.n_groups = n_bins / 4;
-        rc3 = launch_march<4>(P, variant, st);
+    if (pl.map_src && n_src <= kMaxSortedSources) {
+        uint32_t* so = reinterpret_cast<uint32_t*>(ws + wl.src_order_at);
+        rt::src_order_kernel<<<(n_src + 127) / 128, 128, 0, st>>>(so, sources, n_src, nx, ny, nz);
+        RT_CUDA(cudaGetLastError());
+        P.src_order = so;
     } else {
-        P.n_groups = n_bins;
-        rc3 = launch_march<1>(P, variant, st);
+        P.src_order = nullptr;
     }
+    // the accumulation grid: fp64 in the workspace (default), or `out` itself (RT_VARIANT_FLAG_ACC_F32)
+    const size_t n_acc = size_t(ck.cells) * size_t(n_steps);
+    P.acc = pl.acc64 ? static_cast<void*>(ws + wl.acc_at) : static_cast<void*>(out);
+    RT_CUDA(cudaMemsetAsync(P.acc, 0, n_acc * (pl.acc64 ? sizeof(double) : sizeof(float)), st));   // D14: overwrite
+
+    // 4 bins per thread with 16-byte loads (and 16-byte reductions into an fp32 grid) when the layout allows it
+    const bool vec4 = (n_bins % 4 == 0) && !((uintptr_t(j) | uintptr_t(kappa) | uintptr_t(out)) & 15u);
+    P.n_groups = vec4 ? n_bins / 4 : n_bins;
+    int rc3;
+    if (vec4) rc3 = pl.acc64 ? launch_march<4, double>(P, pl.sliding, st) : launch_march<4, float>(P, pl.sliding, st);
+    else rc3 = pl.acc64 ? launch_march<1, double>(P, pl.sliding, st) : launch_march<1, float>(P, pl.sliding, st);
     if (rc3 != RT_OK) return rc3;
-    if (n_steps > 1) {
-        const int threads = 256;
-        long long blocks = (ck.cells + threads - 1) / threads;
-        if (blocks > 148 * 16) blocks = 148 * 16;
-        rt::snapshot_prefix_kernel<<<unsigned(blocks), threads, 0, st>>>(out, ck.cells, n_steps);
+
+    const int threads = 256;
+    long long blocks = (ck.cells + threads - 1) / threads;
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    if (pl.acc64) {
+        rt::snapshot_finalize_kernel<double><<<unsigned(blocks), threads, 0, st>>>(
+            static_cast<const double*>(P.acc), out, ck.cells, n_steps);
+        RT_CUDA(cudaGetLastError());
+    } else if (n_steps > 1) {
+        rt::snapshot_finalize_kernel<float><<<unsigned(blocks), threads, 0, st>>>(out, out, ck.cells, n_steps);
         RT_CUDA(cudaGetLastError());
     }
     return RT_OK;
@@ -211,7 +254,9 @@ int rt_march_host(const float* j, const float* kappa, int nx, int ny, int nz, co
 size_t rt_workspace_bytes(int nx, int ny, int nz, int n_src, int n_rays, int n_bins, int n_steps) {
     if (nx < 1 || ny < 1 || nz < 1 || n_src < 1 || n_rays < 1 || n_bins < 1 || n_steps < 1 || n_rays > (1 << 30))
         return 0;
-    return size_t(ray_slots(n_rays)) * sizeof(uint32_t);
+    const long long cells = (long long)nx * ny;
+    if (cells > 2147483647LL || cells * nz > 2147483647LL || cells * nz * n_bins > 2147483647LL) return 0;
+    return workspace_layout(cells * nz * n_bins, n_src, n_rays, n_steps).total;
 }
 
 int rt_substeps_per_step(float step_size, float c, float dt) {
@@ -220,9 +265,12 @@ int rt_substeps_per_step(float step_size, float c, float dt) {
     return ns < 1 ? RT_EINVAL : int(ns);
 }
 
-int rt_launch_count(int n_bins, int n_steps) {
-    if (n_bins < 1 || n_steps < 1) return RT_EINVAL;
-    return 2 + (n_steps > 1 ? 1 : 0);   // ray order, march, (snapshot prefix)
+int rt_launch_count(int n_src, int n_bins, int n_steps) {
+    if (n_src < 1 || n_bins < 1 || n_steps < 1) return RT_EINVAL;
+    Plan pl;
+    make_plan(RT_VARIANT_DEFAULT, n_src, &pl);
+    // ray order, (source order), march, snapshot finalisation
+    return 3 + ((pl.map_src && n_src <= kMaxSortedSources) ? 1 : 0);
 }
 
 int rt_directions(int n_rays, double* nhat, void* stream) {
@@ -241,7 +289,7 @@ int rt_trace_ray(const float* j, const float* kappa, int nx, int ny, int nz, int
         return RT_EINVAL;
     if ((long long)nx * ny * nz * n_bins > 2147483647LL) return RT_EINVAL;
     rt::MarchParams P{};
-    P.j = j; P.kappa = kappa; P.sources = source_pos; P.out = nullptr; P.ray_order = nullptr;
+    P.j = j; P.kappa = kappa; P.sources = source_pos; P.acc = nullptr; P.ray_order = nullptr; P.src_order = nullptr; P.map_src = 0;
     P.nx = nx; P.ny = ny; P.nz = nz; P.nb = n_bins;
     P.n_src = 1; P.n_rays = n_rays; P.n_slots = n_rays; P.n_groups = 1; P.n_steps = 1; P.n_sub = n_sub;
     P.ds = double(step_size); P.ds_f = step_size; P.emis = step_size; P.snap_stride = 0;
@@ -261,20 +309,23 @@ int rt_ray_order(int n_rays, unsigned int* order, void* stream) {
     return build_ray_order(n_rays, order, static_cast<cudaStream_t>(stream));
 }
 
-int rt_bench_red_ceiling(int mode, float* grid, int nx, int ny, int nz, int n_bins, long long n_red, unsigned int seed,
+int rt_bench_red_ceiling(int mode, void* grid, int nx, int ny, int nz, int n_bins, long long n_red, unsigned int seed,
                          long long* n_issued, void* stream) {
-    if (!grid || mode < 0 || mode > 5 || nx < 2 || ny < 2 || nz < 2 || n_bins < 1 || n_red < 1) return RT_EINVAL;
+    if (!grid || mode < 0 || mode > 7 || nx < 2 || ny < 2 || nz < 2 || n_bins < 1 || n_red < 1) return RT_EINVAL;
     const long long elems = (long long)nx * ny * nz * n_bins;
     if (elems > 2147483647LL || elems < 32) return RT_EINVAL;
     const bool vec = (n_bins % 4 == 0) && !(uintptr_t(grid) & 15u);
     if (mode == 1 && (elems % 4 || (uintptr_t(grid) & 15u))) return RT_EALIGN;
+    if (mode >= 6 && (uintptr_t(grid) & 7u)) return RT_EALIGN;
     const int threads = 256, blocks = 148 * 8;
     // reductions (red instructions x lanes) one thread issues per iteration
-    const long long per_iter = (mode == 2 || mode == 5) ? 8LL * (vec ? n_bins / 4 : n_bins) : 8LL;
+    long long per_iter = 8LL;
+    if (mode == 2 || mode == 5) per_iter = 8LL * (vec ? n_bins / 4 : n_bins);
+    if (mode == 7) per_iter = 8LL * n_bins;
     const long long lanes = (long long)threads * blocks;
     long long iters = (n_red + lanes * per_iter - 1) / (lanes * per_iter);
     if (iters > 2147483647LL) return RT_EINVAL;
-    rt::CeilingParams P{grid, nx, ny, nz, n_bins, int(iters), seed};
+    rt::CeilingParams P{static_cast<float*>(grid), nx, ny, nz, n_bins, int(iters), seed};
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     switch (mode) {
         case 0: rt::red_ceiling_kernel<0, 1><<<blocks, threads, 0, st>>>(P); break;
@@ -285,6 +336,8 @@ int rt_bench_red_ceiling(int mode, float* grid, int nx, int ny, int nz, int n_bi
             break;
         case 3: rt::red_ceiling_kernel<3, 1><<<blocks, threads, 0, st>>>(P); break;
         case 4: rt::red_ceiling_kernel<4, 1><<<blocks, threads, 0, st>>>(P); break;
+        case 6: rt::red_ceiling_kernel<6, 1><<<blocks, threads, 0, st>>>(P); break;
+        case 7: rt::red_ceiling_kernel<7, 1><<<blocks, threads, 0, st>>>(P); break;
         default:
             if (vec) rt::red_ceiling_kernel<5, 4><<<blocks, threads, 0, st>>>(P);
             else rt::red_ceiling_kernel<5, 1><<<blocks, threads, 0, st>>>(P);
@@ -305,6 +358,6 @@ const char* rt_strerror(int code) {
     }
 }
 
-const char* rt_version(void) { return "rtmarch 0.1 (sm_100a; sliding-stencil RED march)"; }
+const char* rt_version(void) { return "rtmarch 0.2 (sm_100a; sliding-stencil RED march, fp64 accumulation grid)"; }
 
 }  // extern "C"

@@ -26,8 +26,12 @@ __device__ __forceinline__ void red4(float* p, float v) {
     asm volatile("red.global.add.v4.f32 [%0], {%1, %1, %1, %1};" ::"l"(p), "f"(v) : "memory");
 }
 
+__device__ __forceinline__ void red1d(double* p, double v) {
+    asm volatile("red.global.add.f64 [%0], %1;" ::"l"(p), "d"(v) : "memory");
+}
+
 struct CeilingParams {
-    float* grid;
+    float* grid;                 // doubles for the fp64 modes
     int nx, ny, nz, nb;
     int iters;
     uint32_t seed;
@@ -77,6 +81,23 @@ __global__ void __launch_bounds__(256) red_ceiling_kernel(const CeilingParams P)
         for (int it = 0; it < P.iters; ++it)
 #pragma unroll
             for (int u = 0; u < 8; ++u) red1(P.grid + 32 * size_t(below(xorshift32(ws), n_elem / 32)) + (tid & 31), v);
+    } else if (MODE == 6) {     // M1 in fp64: scalar, uniformly random
+        double* g = reinterpret_cast<double*>(P.grid);
+        for (int it = 0; it < P.iters; ++it)
+#pragma unroll
+            for (int u = 0; u < 8; ++u) red1d(g + below(xorshift32(s), n_elem), 1.0);
+    } else if (MODE == 7) {     // M3 in fp64: trilinear stencil at a random base voxel, nb scalar reds per corner
+        double* g = reinterpret_cast<double*>(P.grid);
+        const size_t sy = size_t(P.nz) * P.nb, sx = sy * P.ny;
+        for (int it = 0; it < P.iters; ++it) {
+            const int x = below(xorshift32(s), P.nx - 1), y = below(xorshift32(s), P.ny - 1),
+                      z = below(xorshift32(s), P.nz - 1);
+#pragma unroll
+            for (int c = 0; c < 8; ++c) {
+                double* p = g + (x + (c >> 2)) * sx + (y + ((c >> 1) & 1)) * sy + size_t(z + (c & 1)) * P.nb;
+                for (int b = 0; b < P.nb; ++b) red1d(p + b, 1.0);
+            }
+        }
     } else {                    // M6: stencil along a random walk of half a cell per step
         float px = float(below(xorshift32(s), P.nx - 1)), py = float(below(xorshift32(s), P.ny - 1)),
               pz = float(below(xorshift32(s), P.nz - 1));

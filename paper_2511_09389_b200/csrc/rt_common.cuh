@@ -1,0 +1,185 @@
+// rt_common.cuh — shared device code of the ray-march kernels (sm_100a): launch parameters, the direction
+// lattice, the 96-bit fixed-point position, bin-vector loads / reductions, and the thread -> ray mapping.
+//
+// Geometry is exact integer arithmetic (DESIGN.md §4 D3): a position is a 96-bit fixed-point number per axis
+// (int32 cell, 64 fractional bits), x_k = (floor(x_0 2^64) + k floor(fl(ds n) 2^64)) / 2^64, advanced with an
+// add-with-carry chain; floor(x_k) is the top word and the trilinear fraction is the next 32 bits.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace rt {
+
+struct MarchParams {
+    const float* j;
+    const float* kappa;
+    const float* sources;        // [n_src][3]
+    void* acc;                   // accumulation grid [n_steps][nx][ny][nz][nb], float or double: per-step INCREMENTS
+    const uint32_t* ray_order;   // [n_slots] slot -> lattice index (0xFFFFFFFF = padding) or nullptr = identity
+    const uint32_t* src_order;   // [n_src] rank -> source index (spatially sorted) or nullptr = identity
+    int nx, ny, nz, nb;
+    int n_src, n_rays, n_slots;
+    int n_groups;                // bin groups per ray (nb / NB)
+    int n_steps, n_sub;          // time steps, substeps per step (N_s)
+    int map_src;                 // 0: the lanes of a warp are 32 directions of one source; 1: 32 sources, one direction
+    double ds;                   // step_size as double
+    float ds_f;                  // step_size
+    float emis;                  // ds * 4 pi / N_Omega: emission quadrature weight times solid-angle weight (D8)
+    long long snap_stride;       // elements per snapshot
+};
+
+constexpr uint32_t kPad = 0xFFFFFFFFu;
+constexpr int kThreads = 128;    // threads per march block (4 warps)
+
+// (3 - sqrt 5)/2 * 2^128, floored: the golden angle as a fraction of a turn in 0.128 fixed point
+constexpr uint64_t kGoldenTurnHi = 0x61C8864680B583EAull;
+constexpr uint64_t kGoldenTurnLo = 0x0C633F9FA31237CBull;
+
+// i * golden turn mod 1 as a 0.64 fraction (error < 2^-64 + i 2^-128 turn)
+__device__ __forceinline__ uint64_t golden_turn64(uint32_t i) {
+    return uint64_t(i) * kGoldenTurnHi + __umul64hi(uint64_t(i), kGoldenTurnLo);
+}
+
+// ---------------------------------------------------------------------------------------------------
+// direction lattice (D1): z_i = 1 - (2i+1)/N = (N-2i-1)/N, phi_i = i * pi (3 - sqrt 5).
+// z and sqrt(1-z^2) use only correctly rounded IEEE double operations on exact integers (one division for z;
+// (2i+1)/N, (2(N-i)-1)/N, their product and its square root for the radius), so the oracle, which states
+// the same operations, gets bit-identical values; the azimuth is reduced exactly in integer arithmetic.
+// ---------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void fib_direction(uint32_t i, uint32_t n, double nh[3]) {
+    const double q = (2.0 * double(i) + 1.0) / double(n);          // 1 - z
+    const double q2 = (2.0 * double(n - i) - 1.0) / double(n);     // 1 + z
+    const double z = (double(n) - 2.0 * double(i) - 1.0) / double(n);
+    const int64_t t = int64_t(golden_turn64(i));                   // phi/(2 pi) mod 1 as a signed 0.64 fraction
+    const double turn = double(t) * 5.42101086242752217e-20;       // * 2^-64  -> [-0.5, 0.5)
+    double s, c;
+    sincospi(2.0 * turn, &s, &c);
+    const double r = sqrt(__dmul_rn(q, q2));                       // sqrt((1-z)(1+z))
+    nh[0] = __dmul_rn(r, c);
+    nh[1] = __dmul_rn(r, s);
+    nh[2] = z;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// 96-bit fixed point: value = c + fh 2^-32 + fl 2^-64
+// ---------------------------------------------------------------------------------------------------
+struct Fx96 {
+    int32_t c;
+    uint32_t fh, fl;
+};
+
+// floor(v * 2^64) EXACTLY, for |v| < 2^30 (no floating-point rounding: the double's significand is shifted);
+// with `negate` the result is -floor(v * 2^64), also exact (the mirrored coordinate of a descending axis)
+__device__ __forceinline__ Fx96 fx_from_double(double v, bool negate = false) {
+    const long long bits = __double_as_longlong(v);
+    const int e = int((bits >> 52) & 0x7FF);
+    long long m = bits & 0xFFFFFFFFFFFFFll;
+    if (e) m |= 1ll << 52;                                   // v = +-m 2^(e' - 1075), e' = max(e, 1)
+    if (bits < 0) m = -m;
+    const int sh = (e ? e : 1) - 1011;                       // v 2^64 = m 2^sh; sh <= 41 since |v| < 2^30
+    __int128 n;
+    if (sh >= 0) n = __int128(m) << sh;
+    else if (sh > -64) n = __int128(m >> (-sh));             // arithmetic shift = floor
+    else n = (m < 0) ? -1 : 0;
+    if (negate) n = -n;
+    Fx96 r;
+    r.c = int32_t(int64_t(n >> 64));
+    r.fh = uint32_t(uint64_t(n) >> 32);
+    r.fl = uint32_t(uint64_t(n));
+    return r;
+}
+
+__device__ __forceinline__ void fx_add(Fx96& p, const Fx96& d) {
+    asm("add.cc.u32 %0, %0, %3;\n\t"
+        "addc.cc.u32 %1, %1, %4;\n\t"
+        "addc.s32 %2, %2, %5;"
+        : "+r"(p.fl), "+r"(p.fh), "+r"(p.c)
+        : "r"(d.fl), "r"(d.fh), "r"(d.c));
+}
+
+// source coordinate a of source s, saturated to +-2^29 cells (rtmarch.h)
+__device__ __forceinline__ double source_coord(const MarchParams& P, int s, int a) {
+    const float x0 = __ldg(P.sources + 3 * size_t(s) + a);
+    return double(fminf(fmaxf(x0, -536870912.0f), 536870912.0f));
+}
+
+// ---------------------------------------------------------------------------------------------------
+// NB-wide (1 or 4 bins) loads and reductions into a float or a double accumulation grid
+// ---------------------------------------------------------------------------------------------------
+template <int NB> struct BinVec { float v[NB]; };
+
+template <int NB> __device__ __forceinline__ BinVec<NB> ld_bins(const float* p);
+template <> __device__ __forceinline__ BinVec<1> ld_bins<1>(const float* p) {
+    BinVec<1> r;
+    r.v[0] = __ldg(p);
+    return r;
+}
+template <> __device__ __forceinline__ BinVec<4> ld_bins<4>(const float* p) {
+    const float4 t = __ldg(reinterpret_cast<const float4*>(p));
+    BinVec<4> r;
+    r.v[0] = t.x; r.v[1] = t.y; r.v[2] = t.z; r.v[3] = t.w;
+    return r;
+}
+
+__device__ __forceinline__ void red_bins(float* p, const BinVec<1>& a) {
+    asm volatile("red.global.add.f32 [%0], %1;" ::"l"(p), "f"(a.v[0]) : "memory");
+}
+__device__ __forceinline__ void red_bins(float* p, const BinVec<4>& a) {
+    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(a.v[0]), "f"(a.v[1]), "f"(a.v[2]),
+                 "f"(a.v[3])
+                 : "memory");
+}
+template <int NB> __device__ __forceinline__ void red_bins(double* p, const BinVec<NB>& a) {
+#pragma unroll
+    for (int b = 0; b < NB; ++b)
+        asm volatile("red.global.add.f64 [%0], %1;" ::"l"(p + b), "d"(double(a.v[b])) : "memory");
+}
+
+template <int NB> __device__ __forceinline__ bool any_nonzero(const BinVec<NB>& a) {
+    bool nz = false;
+#pragma unroll
+    for (int b = 0; b < NB; ++b) nz |= (a.v[b] != 0.0f);
+    return nz;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// thread -> (source, lattice index, bin group).  Two mappings:
+//   map_src = 0  block = 128 consecutive direction slots of one source (lanes of a warp: a patch of the sphere);
+//   map_src = 1  block = 4 consecutive direction slots x 32 consecutive sources of the spatially sorted source
+//                list (lanes of a warp: 32 sources, ONE direction).  Rays of a warp are parallel; when the
+//                sources share their fractional cell offsets (cell-centred sources) the lanes cross
+//                cell faces in the same substep, so the stencil-slide branches are warp-uniform.
+// Block order: direction chunk fastest, then bin group, then source (group).
+// ---------------------------------------------------------------------------------------------------
+struct RayId {
+    int src, group;
+    uint32_t index;   // lattice index
+};
+
+__host__ __device__ inline long long march_blocks(int n_src, int n_slots, int n_groups, int map_src) {
+    if (map_src) return (long long)((n_slots + 3) / 4) * n_groups * ((n_src + 31) / 32);
+    return (long long)((n_slots + kThreads - 1) / kThreads) * n_groups * n_src;
+}
+
+__device__ __forceinline__ bool ray_id(const MarchParams& P, RayId& id) {
+    uint32_t b = blockIdx.x, slot, s;
+    if (P.map_src) {
+        const uint32_t chunks = (uint32_t(P.n_slots) + 3u) / 4u;
+        slot = (b % chunks) * 4u + (threadIdx.x >> 5);
+        b /= chunks;
+        id.group = int(b % uint32_t(P.n_groups));
+        s = (b / uint32_t(P.n_groups)) * 32u + (threadIdx.x & 31u);
+    } else {
+        const uint32_t chunks = (uint32_t(P.n_slots) + kThreads - 1) / kThreads;
+        slot = (b % chunks) * kThreads + threadIdx.x;
+        b /= chunks;
+        id.group = int(b % uint32_t(P.n_groups));
+        s = b / uint32_t(P.n_groups);
+    }
+    if (slot >= uint32_t(P.n_slots) || s >= uint32_t(P.n_src)) return false;
+    id.src = int(P.src_order ? P.src_order[s] : s);
+    id.index = P.ray_order ? P.ray_order[slot] : slot;
+    return id.index != kPad && id.index < uint32_t(P.n_rays);
+}
+
+}  // namespace rt

@@ -1,0 +1,79 @@
+// rt_setup_kernels.cuh — the small kernels around the march: ray order, source order, direction dump (test
+// hook), and the finalisation of the accumulation grid into cumulative fp32 snapshots.
+#pragma once
+#include "rt_common.cuh"
+
+namespace rt {
+
+// Coherent ray order.  Consecutive lattice indices share a latitude band but sit a golden angle apart in
+// azimuth; sorting each band of M consecutive indices by azimuth makes every 32 consecutive slots (a warp)
+// a compact patch of the sphere.  One block per band, bitonic sort of (azimuth fraction, index) keys.
+__global__ void ray_order_kernel(uint32_t* order, int n_rays, int band) {
+    extern __shared__ unsigned long long keys[];
+    const uint32_t i = blockIdx.x * uint32_t(band) + threadIdx.x;
+    const uint64_t turn = golden_turn64(i);
+    keys[threadIdx.x] = (i < uint32_t(n_rays)) ? ((turn & 0xFFFFFFFF00000000ull) | i) : ~0ull;
+    __syncthreads();
+    for (int size = 2; size <= band; size <<= 1)
+        for (int stride = size >> 1; stride > 0; stride >>= 1) {
+            const int t = threadIdx.x, partner = t ^ stride;
+            if (partner > t) {
+                const unsigned long long a = keys[t], b = keys[partner];
+                const bool up = (t & size) == 0;
+                if ((a > b) == up) { keys[t] = b; keys[partner] = a; }
+            }
+            __syncthreads();
+        }
+    const unsigned long long kq = keys[threadIdx.x];
+    order[i] = (kq == ~0ull) ? kPad : uint32_t(kq & 0xFFFFFFFFull);
+}
+
+// Spatial source order: rank of every source by the linear index of the (clamped) cell it sits in, ties by
+// source index.  Consecutive ranks are then neighbours along z, then y, then x, so the 32 parallel rays of a
+// map_src warp touch adjacent voxels.  O(n_src^2) comparisons, one thread per source (n_src <= 65536).
+__device__ __forceinline__ unsigned long long source_cell_key(const float* sources, int s, int nx, int ny, int nz) {
+    const float x = __ldg(sources + 3 * size_t(s)), y = __ldg(sources + 3 * size_t(s) + 1),
+                z = __ldg(sources + 3 * size_t(s) + 2);
+    const long long ix = (long long)fminf(fmaxf(floorf(x), 0.0f), float(nx - 1));
+    const long long iy = (long long)fminf(fmaxf(floorf(y), 0.0f), float(ny - 1));
+    const long long iz = (long long)fminf(fmaxf(floorf(z), 0.0f), float(nz - 1));
+    return (unsigned long long)((ix * ny + iy) * nz + iz);
+}
+
+__global__ void src_order_kernel(uint32_t* order, const float* sources, int n_src, int nx, int ny, int nz) {
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= n_src) return;
+    const unsigned long long key = source_cell_key(sources, s, nx, ny, nz);
+    uint32_t rank = 0;
+    for (int t = 0; t < n_src; ++t) {
+        const unsigned long long kt = source_cell_key(sources, t, nx, ny, nz);
+        rank += (kt < key) | ((kt == key) & (t < s));
+    }
+    order[rank] = uint32_t(s);
+}
+
+__global__ void directions_kernel(double* nhat, int n_rays) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_rays) return;
+    double nh[3];
+    fib_direction(uint32_t(i), uint32_t(n_rays), nh);
+    nhat[3 * size_t(i)] = nh[0];
+    nhat[3 * size_t(i) + 1] = nh[1];
+    nhat[3 * size_t(i) + 2] = nh[2];
+}
+
+// out[m] <- acc[0] + ... + acc[m]: per-step increments become the cumulative snapshots (D7).
+// ACC = float with acc == out: in place; ACC = double: the fp64 accumulation grid is summed in fp64 and rounded once.
+template <typename ACC>
+__global__ void snapshot_finalize_kernel(const ACC* acc, float* out, long long stride, int n_steps) {
+    for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < stride;
+         e += (long long)gridDim.x * blockDim.x) {
+        ACC run = ACC(0);
+        for (int m = 0; m < n_steps; ++m) {
+            run += acc[m * stride + e];
+            out[m * stride + e] = float(run);
+        }
+    }
+}
+
+}  // namespace rt

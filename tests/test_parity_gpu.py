@@ -57,7 +57,7 @@ def config(name):
     return _cache[name]
 
 
-VARIANTS = [0, 1, 2, 3]
+VARIANTS = [0, 1, 2, 3, 4, 5, 16, 17, 21]     # kinds 0..5, and fp32 accumulation (flag 16) on kinds 0, 1, 5
 
 
 # ------------------------------------------------------------------------------------------------
@@ -228,7 +228,7 @@ def test_large_configs_subset_parity(rt, oracle_mod, name):
     idx = _stratified(w.n_src, SUBSETS[name])
     src = np.ascontiguousarray(w.sources[idx])
     ref = oracle_march(oracle_mod, w, src)
-    for variant in (0, 3):
+    for variant in (0, 4, 5):
         got = gpu_march(rt, w, variant, sources=src)
         rows = parity.assert_parity(got, ref, f"{name} subset variant {variant}")
     print(name, "subset parity:", rows[-1])
