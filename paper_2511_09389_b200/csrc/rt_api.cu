@@ -142,6 +142,7 @@ int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const
     P.n_steps = n_steps; P.n_sub = int(ck.n_sub);
     P.ds = double(step_size); P.ds_f = step_size;
     P.emis = float(double(step_size) * 4.0 * 3.14159265358979323846 / double(n_rays));
+    P.att_scale = float(-double(step_size) * 1.4426950408889634074);
     P.snap_stride = ck.cells;
     P.map_src = pl.map_src ? 1 : 0;
     if (pl.coherent) {
@@ -225,7 +226,6 @@ int rt_march_host(const float* j, const float* kappa, int nx, int ny, int nz, co
     void* dws = nullptr;
     cudaStream_t st = nullptr;
     int result = RT_OK;
-    cudaError_t e = cudaSuccess;
     auto ok = [&](cudaError_t err, const char* where) {
         if (err != cudaSuccess && result == RT_OK) result = cuda_fail(err, where);
         return err == cudaSuccess;
@@ -244,7 +244,6 @@ int rt_march_host(const float* j, const float* kappa, int nx, int ny, int nz, co
             ok(cudaStreamSynchronize(st), "cudaStreamSynchronize");
         }
     }
-    (void)e;
     if (st) cudaStreamSynchronize(st);
     cudaFree(dj); cudaFree(dk); cudaFree(ds); cudaFree(dout); cudaFree(dws);
     if (st) cudaStreamDestroy(st);
@@ -292,7 +291,7 @@ int rt_trace_ray(const float* j, const float* kappa, int nx, int ny, int nz, int
     P.j = j; P.kappa = kappa; P.sources = source_pos; P.acc = nullptr; P.ray_order = nullptr; P.src_order = nullptr; P.map_src = 0;
     P.nx = nx; P.ny = ny; P.nz = nz; P.nb = n_bins;
     P.n_src = 1; P.n_rays = n_rays; P.n_slots = n_rays; P.n_groups = 1; P.n_steps = 1; P.n_sub = n_sub;
-    P.ds = double(step_size); P.ds_f = step_size; P.emis = step_size; P.snap_stride = 0;
+    P.ds = double(step_size); P.ds_f = step_size; P.emis = step_size; P.att_scale = 0.0f; P.snap_stride = 0;
     rt::trace_ray_kernel<<<1, 32, 0, static_cast<cudaStream_t>(stream)>>>(P, uint32_t(ray_index), n_sub, pos, trace_I,
                                                                          trace_T);
     RT_CUDA(cudaGetLastError());

@@ -25,6 +25,7 @@ struct MarchParams {
     double ds;                   // step_size as double
     float ds_f;                  // step_size
     float emis;                  // ds * 4 pi / N_Omega: emission quadrature weight times solid-angle weight (D8)
+    float att_scale;             // -ds * log2(e): exp(-kappa ds) = 2^(kappa * att_scale)
     long long snap_stride;       // elements per snapshot
 };
 
@@ -68,9 +69,12 @@ struct Fx96 {
     uint32_t fh, fl;
 };
 
-// floor(v * 2^64) EXACTLY, for |v| < 2^30 (no floating-point rounding: the double's significand is shifted);
-// with `negate` the result is -floor(v * 2^64), also exact (the mirrored coordinate of a descending axis)
-__device__ __forceinline__ Fx96 fx_from_double(double v, bool negate = false) {
+// floor(v * 2^64) EXACTLY, for |v| < 2^30 (no floating-point rounding: the double's significand is shifted).
+// mode kFxNegate returns -floor(v 2^64), mode kFxComplement returns -floor(v 2^64) - 1 (both exact): the
+// increment and the position of a descending axis in travel coordinates (rt_march_sliding.cuh)
+constexpr int kFxPlain = 0, kFxNegate = 1, kFxComplement = 2;
+
+__device__ __forceinline__ Fx96 fx_from_double(double v, int mode = kFxPlain) {
     const long long bits = __double_as_longlong(v);
     const int e = int((bits >> 52) & 0x7FF);
     long long m = bits & 0xFFFFFFFFFFFFFll;
@@ -81,7 +85,8 @@ __device__ __forceinline__ Fx96 fx_from_double(double v, bool negate = false) {
     if (sh >= 0) n = __int128(m) << sh;
     else if (sh > -64) n = __int128(m >> (-sh));             // arithmetic shift = floor
     else n = (m < 0) ? -1 : 0;
-    if (negate) n = -n;
+    if (mode == kFxNegate) n = -n;
+    if (mode == kFxComplement) n = ~n;
     Fx96 r;
     r.c = int32_t(int64_t(n >> 64));
     r.fh = uint32_t(uint64_t(n) >> 32);

@@ -7,16 +7,21 @@
 // and a ray that has left the box on all three axes issues one reduction for the rest of its path.  The sums are
 // the same sums (each voxel still receives every w_c I_{k+1}); only their association changes.
 //
-// Each axis is handled in TRAVEL coordinates u = +x or u = -x (exact negation of the fixed-point position), so
-// every axis ascends: the stencil's slots are (trailing, leading) per axis, a cell crossing is the carry out of
-// the fraction, and a slide flushes the 4 trailing slots, moves 4, loads 4.  For a descending axis the array
-// index of u-cell c is -c, the weight pair (trailing, leading) = (1 - frac u, frac u) is the oracle's
-// (weight of hi, weight of lo), and floor(x) -- the nearest-neighbour kappa cell, PAPER.md:29 / D4 -- is the
-// LEADING index unless frac u = 0 exactly, when it is the trailing one (and the leading slot has weight 0 where
-// the array-coordinate stencil has its weight-0 hi corner: the same field).
+// TRAVEL COORDINATES.  Each axis is marched in a coordinate u that ascends: u = x on an ascending axis and, on a
+// descending one, the bitwise complement of the fixed-point position, U = ~X = -X - 1, i.e. u = -x - 2^-64 (the
+// increment is -D, exact).  A cell crossing is then always "the cell word of u went up", the stencil's slots are
+// (trailing, leading) per axis, and a slide flushes the 4 trailing slots, moves 4, loads 4.  The grid point of
+// u-cell c is array index c (ascending) or -c (descending).  With the complement (rather than the negation):
+//   * floor(x) -- the nearest-neighbour kappa cell, PAPER.md:29 / D4 -- is ALWAYS the leading index of a
+//     descending axis (and the trailing index of an ascending one), also when x sits exactly on a cell plane;
+//   * on a plane x = m the u-fraction is all ones, so the leading weight rounds to exactly 1 and the trailing
+//     one (~fraction = 0) to exactly 0: the same corners and weights as the array-coordinate stencil (m, m+1).
 //
-// Clamping (D5): where both indices of an axis clamp to the same voxel the two slots are merged
-// (weights (1, 0)); nothing slides while the ray moves on outside the box.
+// WEIGHTS.  Leading weight f = top 32 fraction bits, trailing weight = their complement (each truncated to the
+// 2^-32 grid, so tiny weights keep their relative accuracy); conversions stay unscaled (values up to 2^32) and
+// the 2^-96 of the triple product is folded into the z pair.  CLAMPING (D5): where both indices of
+// an axis clamp to the same voxel the two slots are merged -- the fraction is masked to 0, which makes the pair
+// exactly (trailing 1, leading 0) -- and nothing slides while the ray moves on outside the box.
 #pragma once
 #include "rt_common.cuh"
 
@@ -27,17 +32,23 @@ template <int AX> __device__ __forceinline__ constexpr int slot(int p, int u, in
     return AX == 0 ? (p * 4 + u * 2 + v) : (AX == 1 ? (u * 4 + p * 2 + v) : (u * 4 + v * 2 + p));
 }
 
+__device__ __forceinline__ float ex2_approx(float x) {
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
 struct TravelAxis {
     Fx96 p, d;          // position and per-substep increment in travel coordinates (d >= 0)
     int t, dl;          // element offset of the trailing index; leading minus trailing offset (0 = merged)
-    int stride, nmax;   // element stride of this axis, N - 1
-    bool neg;           // the ray descends this axis (u = -x)
+    int stride, lim;    // element stride of this axis, N - 1
+    int sg;             // +1 ascending, -1 descending
+    uint32_t fmask;     // 0 while merged (dl == 0), else all ones
+    int kmask;          // all ones on a descending axis: the kappa cell is the LEADING index there
 
     __device__ __forceinline__ int eoff(int c) const {          // element offset of u-cell c, index clamped
-        const int idx = neg ? -c : c;
-        return min(max(idx, 0), nmax) * stride;
+        return min(max(c * sg, 0), lim) * stride;
     }
-    __device__ __forceinline__ bool on_a_plane() const { return (p.fh | p.fl) == 0u; }
 };
 
 template <int NB, typename ACC> struct Stencil {
@@ -65,6 +76,7 @@ template <int NB, typename ACC> struct Stencil {
         for (int a = 0; a < 3; ++a) {
             A[a].t = A[a].eoff(A[a].p.c);
             A[a].dl = A[a].eoff(A[a].p.c + 1) - A[a].t;
+            A[a].fmask = A[a].dl ? 0xFFFFFFFFu : 0u;
         }
 #pragma unroll
         for (int s = 0; s < 8; ++s) {
@@ -73,32 +85,32 @@ template <int NB, typename ACC> struct Stencil {
             jc[s] = ld_bins<NB>(jg + off[s]);
         }
     }
-    // axis AX advanced by one cell.  move: the trailing index changed (the old leading plane is the new trailing
-    // plane); load: the leading plane holds new voxels; dl: new leading-minus-trailing offset
-    template <int AX> __device__ __forceinline__ void slide(ACC* og, const float* jg, bool move, bool load, int dl) {
-#pragma unroll
-        for (int u = 0; u < 2; ++u)
-#pragma unroll
-            for (int v = 0; v < 2; ++v) {
-                const int s0 = slot<AX>(0, u, v), s1 = slot<AX>(1, u, v);
-                if (move) {
-                    flush_slot(og, s0);
-                    acc[s0] = acc[s1];
-                    jc[s0] = jc[s1];
-                    off[s0] = off[s1];
-                    zero_slot(s1);
-                }
-                off[s1] = off[s0] + dl;
-                if (load) jc[s1] = ld_bins<NB>(jg + off[s1]);
-            }
-    }
+    // Axis AX advanced by one cell.  The old leading plane is the new trailing plane (also under clamping: both
+    // are clamp(c+1)), so the trailing index moves iff the axis was not merged; the new leading index is looked up.
     template <int AX> __device__ __forceinline__ void axis_step(TravelAxis& A, ACC* og, const float* jg) {
-        const int tn = A.eoff(A.p.c), dln = A.eoff(A.p.c + 1) - tn;
-        const bool move = (tn != A.t);
-        const bool load = (dln != 0) & (move | (dln != A.dl));
-        if (move | load) slide<AX>(og, jg, move, load, dln);
+        const int tn = A.t + A.dl;
+        const int dln = A.eoff(A.p.c + 1) - tn;
+        const bool move = (A.dl != 0), load = (dln != 0);
+        if (move | load) {
+#pragma unroll
+            for (int u = 0; u < 2; ++u)
+#pragma unroll
+                for (int v = 0; v < 2; ++v) {
+                    const int s0 = slot<AX>(0, u, v), s1 = slot<AX>(1, u, v);
+                    if (move) {
+                        flush_slot(og, s0);
+                        acc[s0] = acc[s1];
+                        jc[s0] = jc[s1];
+                        off[s0] = off[s1];
+                        zero_slot(s1);
+                    }
+                    off[s1] = off[s0] + dln;
+                    if (load) jc[s1] = ld_bins<NB>(jg + off[s1]);
+                }
+        }
         A.t = tn;
         A.dl = dln;
+        A.fmask = dln ? 0xFFFFFFFFu : 0u;
     }
 };
 
@@ -114,14 +126,16 @@ __global__ void __launch_bounds__(kThreads) march_sliding_kernel(const MarchPara
     {
         double nh[3];
         fib_direction(id.index, uint32_t(P.n_rays), nh);
-        const int strides[3] = {P.ny * P.nz * P.nb, P.nz * P.nb, P.nb}, nmaxs[3] = {P.nx - 1, P.ny - 1, P.nz - 1};
+        const int strides[3] = {P.ny * P.nz * P.nb, P.nz * P.nb, P.nb}, lims[3] = {P.nx - 1, P.ny - 1, P.nz - 1};
 #pragma unroll
         for (int a = 0; a < 3; ++a) {
-            A[a].neg = nh[a] < 0.0;
-            A[a].p = fx_from_double(source_coord(P, id.src, a), A[a].neg);
-            A[a].d = fx_from_double(__dmul_rn(P.ds, nh[a]), A[a].neg);
+            const bool neg = nh[a] < 0.0;
+            A[a].p = fx_from_double(source_coord(P, id.src, a), neg ? kFxComplement : kFxPlain);
+            A[a].d = fx_from_double(__dmul_rn(P.ds, nh[a]), neg ? kFxNegate : kFxPlain);
+            A[a].sg = neg ? -1 : 1;
             A[a].stride = strides[a];
-            A[a].nmax = nmaxs[a];
+            A[a].lim = lims[a];
+            A[a].kmask = neg ? -1 : 0;
         }
     }
     Stencil<NB, ACC> S;
@@ -131,50 +145,33 @@ __global__ void __launch_bounds__(kThreads) march_sliding_kernel(const MarchPara
 
     float I[NB], T[NB], att[NB];     // I scaled by 4 pi/N_Omega; T = exp(-tau); att = exp(-kappa ds) of the kappa cell
 #pragma unroll
-    for (int b = 0; b < NB; ++b) { I[b] = 0.0f; T[b] = 1.0f; att[b] = 1.0f; }
-    int kof = -1;                    // element offset of the kappa cell att[] belongs to
-    bool refresh = true;             // re-derive the kappa cell before the next substep
+    for (int b = 0; b < NB; ++b) { I[b] = 0.0f; T[b] = 1.0f; }
+    // kappa: nearest neighbour at clamp(floor(x_k)) (D4) = trailing index, leading on descending axes
+    auto load_att = [&]() {
+        const int ko = S.off[0] + (A[0].dl & A[0].kmask) + (A[1].dl & A[1].kmask) + (A[2].dl & A[2].kmask);
+        const BinVec<NB> kap = ld_bins<NB>(kg + ko);
+#pragma unroll
+        for (int b = 0; b < NB; ++b) att[b] = ex2_approx(kap.v[b] * P.att_scale);
+    };
+    load_att();
+    const bool long_steps = !(P.ds_f < 1.0f);      // only then can one substep cross more than one cell plane
 
     for (int m = 0; m < P.n_steps; ++m) {
         for (int k = 0; k < P.n_sub; ++k) {
-            if (refresh) {
-                // kappa: nearest neighbour at clamp(floor(x_k)) (D4): the trailing index, or the
-                // leading one on an axis the ray descends unless it sits exactly on a cell plane -- then the
-                // cell changes at the next substep with no slide, so look again
-                int ko = S.off[0];
-                refresh = false;
-#pragma unroll
-                for (int a = 0; a < 3; ++a)
-                    if (A[a].neg) {
-                        if (A[a].on_a_plane()) refresh = true;
-                        else ko += A[a].dl;
-                    }
-                if (ko != kof) {
-                    kof = ko;
-                    const BinVec<NB> kap = ld_bins<NB>(kg + ko);
-#pragma unroll
-                    for (int b = 0; b < NB; ++b) att[b] = expf(-kap.v[b] * P.ds_f);
-                }
-            }
-            // trilinear weights from the top 32 fraction bits: leading f, trailing 1 - f (each truncated to the
-            // 2^-32 grid, so tiny weights keep their relative accuracy); merged axes carry (1, 0)
-            float wt[3], wl[3];
-#pragma unroll
-            for (int a = 0; a < 3; ++a) {
-                const float f = __uint2float_rn(A[a].p.fh) * 2.3283064365386963e-10f;      // 2^-32
-                const float g = __uint2float_rn(~A[a].p.fh) * 2.3283064365386963e-10f;
-                const bool merged = (A[a].dl == 0);
-                wl[a] = merged ? 0.0f : f;
-                wt[a] = merged ? 1.0f : g;
-            }
-            const float wxy[4] = {wt[0] * wt[1], wt[0] * wl[1], wl[0] * wt[1], wl[0] * wl[1]};
+            // unscaled weights in [0, 2^32]; 2^-96 rides on the z pair
+            const uint32_t hx = A[0].p.fh & A[0].fmask, hy = A[1].p.fh & A[1].fmask, hz = A[2].p.fh & A[2].fmask;
+            const float lx = __uint2float_rn(hx), tx = __uint2float_rn(~hx);
+            const float ly = __uint2float_rn(hy), ty = __uint2float_rn(~hy);
+            const float wz[2] = {__uint2float_rn(~hz) * 1.2621774483536189e-29f,      // 2^-96
+                                 __uint2float_rn(hz) * 1.2621774483536189e-29f};
+            const float wxy[4] = {tx * ty, tx * ly, lx * ty, lx * ly};
             float w[8];
             float jv[NB];
 #pragma unroll
             for (int b = 0; b < NB; ++b) jv[b] = 0.0f;
 #pragma unroll
             for (int s = 0; s < 8; ++s) {
-                w[s] = wxy[s >> 1] * ((s & 1) ? wl[2] : wt[2]);
+                w[s] = wxy[s >> 1] * wz[s & 1];
 #pragma unroll
                 for (int b = 0; b < NB; ++b) jv[b] = fmaf(w[s], S.jc[s].v[b], jv[b]);
             }
@@ -192,17 +189,16 @@ __global__ void __launch_bounds__(kThreads) march_sliding_kernel(const MarchPara
             const int c0 = A[0].p.c, c1 = A[1].p.c, c2 = A[2].p.c;
 #pragma unroll
             for (int a = 0; a < 3; ++a) fx_add(A[a].p, A[a].d);
-            const int d0 = A[0].p.c - c0, d1 = A[1].p.c - c1, d2 = A[2].p.c - c2;
-            if (d0 | d1 | d2) {
-                if ((d0 | d1 | d2) > 1) {          // a step longer than a cell: restart the stencil
-                    S.flush_all(og);
+            if ((c0 ^ A[0].p.c) | (c1 ^ A[1].p.c) | (c2 ^ A[2].p.c)) {
+                if (long_steps && (((A[0].p.c - c0) | (A[1].p.c - c1) | (A[2].p.c - c2)) > 1)) {
+                    S.flush_all(og);               // a step longer than a cell: restart the stencil
                     S.restart(A, jg);
                 } else {
-                    if (d0) S.template axis_step<0>(A[0], og, jg);
-                    if (d1) S.template axis_step<1>(A[1], og, jg);
-                    if (d2) S.template axis_step<2>(A[2], og, jg);
+                    if (c0 != A[0].p.c) S.template axis_step<0>(A[0], og, jg);
+                    if (c1 != A[1].p.c) S.template axis_step<1>(A[1], og, jg);
+                    if (c2 != A[2].p.c) S.template axis_step<2>(A[2], og, jg);
                 }
-                refresh = true;
+                load_att();
             }
         }
         S.flush_all(og);       // time-step boundary: the increments of step m are complete (rays continue, D7)
