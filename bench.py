@@ -313,22 +313,39 @@ def run_native(args):
     # ---- roofline of the dominant kernel (the march kernel) against the measured L2-reduction ceiling
     if rank == 0:
         ceil = measure_ceilings(rt, torch, (nx, ny, nz), nb)
-        reds_per_substep = 8 * ((nb + 3) // 4 if nb % 4 == 0 else nb)     # algorithmic: 8 corners x bin groups
+        step_s = total_s / args.steps
+        reds_per_substep = 8 * (nb // 4 if nb % 4 == 0 else nb)           # algorithmic: 8 corners x bin groups
         alg_reds = reds_per_substep * src.shape[0] * w.n_rays * w.n_steps * w.substeps_per_step
-        kernel_s = min(step_ms) * 1e-3 if world == 1 else total_s / args.steps
-        achieved = alg_reds / (total_s / args.steps) / 1e9
+        achieved = alg_reds / step_s / 1e9
         peak = ceil["M3_stencil"]
-        line["roofline"] = {
+        hbm_bytes = int((2 + 3 * w.n_steps) * nx * ny * nz * nb * 4)      # j, kappa read; fp64 grid zeroed+read; out written
+        roof = {
             "bound": "l2_red", "achieved": achieved, "peak": peak, "unit": "Gred/s", "frac": achieved / peak,
             "traffic": None, "kernel": "march_sliding_kernel",
             "how": "achieved = ALGORITHMIC reductions (8 corners x bin-groups x ray-substeps) / mean CUDA-event "
                    "time of the whole rt_march call (the march kernel is >99.9% of it, profiles/); peak = "
                    "M3 stencil-pattern red.global.add ceiling measured in this process on a grid of the same "
-                   "size (DESIGN.md §8); frac > 1 means register/warp aggregation removed reductions",
-            "best_step_frac": alg_reds / kernel_s / 1e9 / peak, "ceilings_Gred_per_s": ceil,
-            "hbm": {"algorithmic_bytes": int((2 + 2 * w.n_steps) * nx * ny * nz * nb * 4),
-                    "achieved_GBps": (2 + 2 * w.n_steps) * nx * ny * nz * nb * 4 / (total_s / args.steps) / 1e9,
-                    "peak_GBps": _measured_hbm()}}
+                   "size (DESIGN.md §8), of measured; frac > 1: the sliding stencil sums a voxel's deposits in "
+                   "registers, so fewer reductions are issued than the method states (see `issued`)",
+            "best_step_frac": alg_reds / (min(step_ms) * 1e-3) / 1e9 / peak if world == 1 else None,
+            "ceilings_Gred_per_s": ceil,
+            "hbm": {"algorithmic_bytes": hbm_bytes, "achieved_GBps": hbm_bytes / step_s / 1e9,
+                    "peak_GBps": _measured_hbm(), "note": "grids are L2 resident at C0-C2: HBM is not the bound"}}
+        cnt = _ncu_counters(args.config, args.variant)
+        if cnt and world == 1:
+            sm_hz = (clocks.get("sm_mhz") or 1965.0) * 1e6
+            roof["traffic"] = cnt["dram_bytes"]
+            roof["issued"] = {"red_sectors_per_launch": cnt["red_sectors"],
+                              "red_sectors_per_ray_substep": cnt["red_sectors"] / (alg_reds / reds_per_substep),
+                              "achieved_Gsectors_per_s": cnt["red_sectors"] / step_s / 1e9,
+                              "frac_of_M3": cnt["red_sectors"] / step_s / 1e9 / ceil["M3_f64_stencil"]}
+            roof["alu"] = {"warp_instructions_per_launch": cnt["warp_instructions"],
+                           "achieved_Ginst_per_s": cnt["warp_instructions"] / step_s / 1e9,
+                           "peak_Ginst_per_s": 148 * 4 * sm_hz / 1e9,
+                           "frac": cnt["warp_instructions"] / step_s / (148 * 4 * sm_hz),
+                           "peak_how": "148 SMs x 4 schedulers x 1 warp-instruction/clk x SM clock sampled in the run"}
+            roof["counters_from"] = cnt["source"]
+        line["roofline"] = roof
         if not args.no_cpu_baseline and world == 1:
             ups, cores, what, _, _ = oracle_sample(make_workload(args.config), args.cpu_seconds)
             line["cpu_baseline"] = {"value": ups, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": what}
@@ -337,6 +354,22 @@ def run_native(args):
         dist.barrier()
         dist.destroy_process_group()
     return 0
+
+
+def _ncu_counters(config, variant):
+    """Per-launch ncu counters of the march kernel (committed text under profiles/, one capture per kernel
+    revision): instruction count, L2 reduction sectors, DRAM bytes.  None if there is no capture for this case."""
+    try:
+        table = json.load(open(os.path.join(ROOT, "profiles", "march_counters.json")))
+        row = table.get(f"{config}:v{variant}")
+        return row if row and row.get("library") == _lib_version() else None
+    except (OSError, ValueError):
+        return None
+
+
+def _lib_version():
+    import paper_2511_09389_b200 as rt
+    return rt.rt_version()
 
 
 def _measured_hbm():

@@ -90,10 +90,14 @@ template <int NB, typename ACC>
 int launch_march(const rt::MarchParams& P, bool sliding, cudaStream_t st) {
     const long long blocks = rt::march_blocks(P.n_src, P.n_slots, P.n_groups, P.map_src);
     if (blocks > 2147483647LL) return RT_EINVAL;
-    if (sliding)
-        rt::march_sliding_kernel<NB, ACC><<<unsigned(blocks), rt::kThreads, 0, st>>>(P);
-    else
-        rt::march_direct_kernel<NB, ACC><<<unsigned(blocks), rt::kThreads, 0, st>>>(P);
+    const unsigned g = unsigned(blocks);
+    if (sliding) {
+        // registers: 1 bin per thread fits 6 blocks/SM (80 registers) without spilling; 4 bins need ~155
+        constexpr int kMinBlocks = (NB == 1) ? 6 : 1;
+        rt::march_sliding_kernel<NB, ACC, kMinBlocks><<<g, rt::kThreads, 0, st>>>(P);
+    } else {
+        rt::march_direct_kernel<NB, ACC><<<g, rt::kThreads, 0, st>>>(P);
+    }
     RT_CUDA(cudaGetLastError());
     return RT_OK;
 }

@@ -41,15 +41,16 @@ __device__ __forceinline__ float ex2_approx(float x) {
 struct TravelAxis {
     Fx96 p, d;          // position and per-substep increment in travel coordinates (d >= 0)
     int t, dl;          // element offset of the trailing index; leading minus trailing offset (0 = merged)
-    int stride, lim;    // element stride of this axis, N - 1
     int sg;             // +1 ascending, -1 descending
     uint32_t fmask;     // 0 while merged (dl == 0), else all ones
-    int kmask;          // all ones on a descending axis: the kappa cell is the LEADING index there
-
-    __device__ __forceinline__ int eoff(int c) const {          // element offset of u-cell c, index clamped
-        return min(max(c * sg, 0), lim) * stride;
-    }
 };
+
+// element offset of u-cell c of axis AX (array index c or -c, clamped to the domain: PAPER.md:29)
+template <int AX> __device__ __forceinline__ int eoff(const MarchParams& P, int c, int sg) {
+    const int lim = (AX == 0 ? P.nx : (AX == 1 ? P.ny : P.nz)) - 1;
+    const int stride = AX == 0 ? P.ny * P.nz * P.nb : (AX == 1 ? P.nz * P.nb : P.nb);
+    return min(max(c * sg, 0), lim) * stride;
+}
 
 template <int NB, typename ACC> struct Stencil {
     BinVec<NB> acc[8];   // pending deposits for the 8 stencil voxels
@@ -70,14 +71,16 @@ template <int NB, typename ACC> struct Stencil {
             zero_slot(s);
         }
     }
+    template <int AX> __device__ __forceinline__ void place(const MarchParams& P, TravelAxis& A) {
+        A.t = eoff<AX>(P, A.p.c, A.sg);
+        A.dl = eoff<AX>(P, A.p.c + 1, A.sg) - A.t;
+        A.fmask = A.dl ? 0xFFFFFFFFu : 0u;
+    }
     // (re)build the stencil at the axes' current cells; pending deposits must have been flushed
-    __device__ __forceinline__ void restart(TravelAxis (&A)[3], const float* jg) {
-#pragma unroll
-        for (int a = 0; a < 3; ++a) {
-            A[a].t = A[a].eoff(A[a].p.c);
-            A[a].dl = A[a].eoff(A[a].p.c + 1) - A[a].t;
-            A[a].fmask = A[a].dl ? 0xFFFFFFFFu : 0u;
-        }
+    __device__ __forceinline__ void restart(const MarchParams& P, TravelAxis (&A)[3], const float* jg) {
+        place<0>(P, A[0]);
+        place<1>(P, A[1]);
+        place<2>(P, A[2]);
 #pragma unroll
         for (int s = 0; s < 8; ++s) {
             off[s] = A[0].t + A[1].t + A[2].t + ((s & 4) ? A[0].dl : 0) + ((s & 2) ? A[1].dl : 0) +
@@ -87,9 +90,10 @@ template <int NB, typename ACC> struct Stencil {
     }
     // Axis AX advanced by one cell.  The old leading plane is the new trailing plane (also under clamping: both
     // are clamp(c+1)), so the trailing index moves iff the axis was not merged; the new leading index is looked up.
-    template <int AX> __device__ __forceinline__ void axis_step(TravelAxis& A, ACC* og, const float* jg) {
+    template <int AX>
+    __device__ __forceinline__ void axis_step(const MarchParams& P, TravelAxis& A, ACC* og, const float* jg) {
         const int tn = A.t + A.dl;
-        const int dln = A.eoff(A.p.c + 1) - tn;
+        const int dln = eoff<AX>(P, A.p.c + 1, A.sg) - tn;
         const bool move = (A.dl != 0), load = (dln != 0);
         if (move | load) {
 #pragma unroll
@@ -114,8 +118,8 @@ template <int NB, typename ACC> struct Stencil {
     }
 };
 
-template <int NB, typename ACC>
-__global__ void __launch_bounds__(kThreads) march_sliding_kernel(const MarchParams P) {
+template <int NB, typename ACC, int MINB>
+__global__ void __launch_bounds__(kThreads, MINB) march_sliding_kernel(const MarchParams P) {
     RayId id;
     if (!ray_id(P, id)) return;
     const float* jg = P.j + id.group * NB;
@@ -126,29 +130,25 @@ __global__ void __launch_bounds__(kThreads) march_sliding_kernel(const MarchPara
     {
         double nh[3];
         fib_direction(id.index, uint32_t(P.n_rays), nh);
-        const int strides[3] = {P.ny * P.nz * P.nb, P.nz * P.nb, P.nb}, lims[3] = {P.nx - 1, P.ny - 1, P.nz - 1};
 #pragma unroll
         for (int a = 0; a < 3; ++a) {
             const bool neg = nh[a] < 0.0;
             A[a].p = fx_from_double(source_coord(P, id.src, a), neg ? kFxComplement : kFxPlain);
             A[a].d = fx_from_double(__dmul_rn(P.ds, nh[a]), neg ? kFxNegate : kFxPlain);
             A[a].sg = neg ? -1 : 1;
-            A[a].stride = strides[a];
-            A[a].lim = lims[a];
-            A[a].kmask = neg ? -1 : 0;
         }
     }
     Stencil<NB, ACC> S;
 #pragma unroll
     for (int s = 0; s < 8; ++s) S.zero_slot(s);
-    S.restart(A, jg);
+    S.restart(P, A, jg);
 
     float I[NB], T[NB], att[NB];     // I scaled by 4 pi/N_Omega; T = exp(-tau); att = exp(-kappa ds) of the kappa cell
 #pragma unroll
     for (int b = 0; b < NB; ++b) { I[b] = 0.0f; T[b] = 1.0f; }
     // kappa: nearest neighbour at clamp(floor(x_k)) (D4) = trailing index, leading on descending axes
     auto load_att = [&]() {
-        const int ko = S.off[0] + (A[0].dl & A[0].kmask) + (A[1].dl & A[1].kmask) + (A[2].dl & A[2].kmask);
+        const int ko = S.off[0] + (A[0].dl & (A[0].sg >> 1)) + (A[1].dl & (A[1].sg >> 1)) + (A[2].dl & (A[2].sg >> 1));
         const BinVec<NB> kap = ld_bins<NB>(kg + ko);
 #pragma unroll
         for (int b = 0; b < NB; ++b) att[b] = ex2_approx(kap.v[b] * P.att_scale);
@@ -166,15 +166,23 @@ __global__ void __launch_bounds__(kThreads) march_sliding_kernel(const MarchPara
                                  __uint2float_rn(hz) * 1.2621774483536189e-29f};
             const float wxy[4] = {tx * ty, tx * ly, lx * ty, lx * ly};
             float w[8];
-            float jv[NB];
+            float jv[NB], ju[NB];          // two partial sums: half the dependent-FMA chain length
 #pragma unroll
-            for (int b = 0; b < NB; ++b) jv[b] = 0.0f;
+            for (int s = 0; s < 8; ++s) w[s] = wxy[s >> 1] * wz[s & 1];
 #pragma unroll
-            for (int s = 0; s < 8; ++s) {
-                w[s] = wxy[s >> 1] * wz[s & 1];
-#pragma unroll
-                for (int b = 0; b < NB; ++b) jv[b] = fmaf(w[s], S.jc[s].v[b], jv[b]);
+            for (int b = 0; b < NB; ++b) {
+                jv[b] = w[0] * S.jc[0].v[b];
+                ju[b] = w[1] * S.jc[1].v[b];
             }
+#pragma unroll
+            for (int s = 2; s < 8; s += 2)
+#pragma unroll
+                for (int b = 0; b < NB; ++b) {
+                    jv[b] = fmaf(w[s], S.jc[s].v[b], jv[b]);
+                    ju[b] = fmaf(w[s + 1], S.jc[s + 1].v[b], ju[b]);
+                }
+#pragma unroll
+            for (int b = 0; b < NB; ++b) jv[b] += ju[b];
 #pragma unroll
             for (int b = 0; b < NB; ++b) {                       // eq. (2)
                 I[b] = fmaf(I[b], att[b], jv[b] * T[b] * P.emis);
@@ -192,11 +200,11 @@ __global__ void __launch_bounds__(kThreads) march_sliding_kernel(const MarchPara
             if ((c0 ^ A[0].p.c) | (c1 ^ A[1].p.c) | (c2 ^ A[2].p.c)) {
                 if (long_steps && (((A[0].p.c - c0) | (A[1].p.c - c1) | (A[2].p.c - c2)) > 1)) {
                     S.flush_all(og);               // a step longer than a cell: restart the stencil
-                    S.restart(A, jg);
+                    S.restart(P, A, jg);
                 } else {
-                    if (c0 != A[0].p.c) S.template axis_step<0>(A[0], og, jg);
-                    if (c1 != A[1].p.c) S.template axis_step<1>(A[1], og, jg);
-                    if (c2 != A[2].p.c) S.template axis_step<2>(A[2], og, jg);
+                    if (c0 != A[0].p.c) S.template axis_step<0>(P, A[0], og, jg);
+                    if (c1 != A[1].p.c) S.template axis_step<1>(P, A[1], og, jg);
+                    if (c2 != A[2].p.c) S.template axis_step<2>(P, A[2], og, jg);
                 }
                 load_att();
             }

@@ -176,6 +176,37 @@ def test_small_cases(rt, oracle_mod, shape, nb, src, n_rays, ds, dt, variant):
         parity.assert_parity(out.cpu().numpy(), ref, f"{shape} nb={nb} variant={variant} steps={n_steps}")
 
 
+@pytest.mark.parametrize("variant", [0, 4, 5, 21])
+@pytest.mark.parametrize("n_src,integer", [(32, True), (33, False), (70, True), (100, False)])
+def test_many_sources_fill_warps_raggedly(rt, oracle_mod, n_src, integer, variant):
+    """n_src >= 32 selects the warp = 32 sorted sources x 1 direction mapping: ragged last source group,
+    duplicate sources, sources on faces and outside the box (clamped), cell-centred and not."""
+    shape, nb, n_rays = (7, 6, 9), 1, 11
+    j, k = _random_medium(shape, nb, seed=n_src)
+    rng = np.random.default_rng(1000 + n_src)
+    src = rng.uniform(-2.0, 10.0, (n_src, 3))
+    if integer:
+        src = np.round(src)
+    src[1] = src[0]                                   # a duplicate
+    src[2] = (0.0, 5.0, 8.0)                          # on three faces
+    src = src.astype(np.float32)
+    ref = oracle_mod.march(j, k, src, n_rays, 0.5, 1.0, 4.0, 2)
+    out = rt.rt_march_ex(_dev(j), _dev(k), _dev(src), n_rays, 0.5, 1.0, 4.0, 2, variant=variant)
+    torch.cuda.synchronize()
+    parity.assert_parity(out.cpu().numpy(), ref, f"n_src={n_src} variant={variant}")
+
+
+def test_more_sources_than_the_sort_handles(rt, oracle_mod):
+    """Above 65,536 sources the spatial source sort is skipped (identity order); same field."""
+    shape, n_src = (4, 4, 4), 66000
+    j, k = _random_medium(shape, 1, seed=3)
+    src = np.random.default_rng(4).uniform(-1.0, 4.0, (n_src, 3)).astype(np.float32)
+    ref = oracle_mod.march(j, k, src, 1, 0.5, 1.0, 3.0, 1)
+    out = rt.rt_march(_dev(j), _dev(k), _dev(src), 1, 0.5, 1.0, 3.0, 1)
+    torch.cuda.synchronize()
+    parity.assert_parity(out.cpu().numpy(), ref, "66000 sources")
+
+
 def test_out_is_overwritten_and_call_is_repeatable(rt, oracle_mod):
     w = config("C0")
     j, k, s = _dev(w.j), _dev(w.kappa), _dev(w.sources)
