@@ -50,7 +50,7 @@ extern "C" {
 
 /* Kernel variants for rt_march_ex (tests and bench only; rt_march always uses RT_VARIANT_DEFAULT).
  * All variants compute the same field; they differ in how the deposit of P:29 is issued and in which rays
- * share a warp.  A variant code is one kind (0..5), optionally OR-ed with one flag. */
+ * share a warp.  A variant code is one kind (0..5), optionally OR-ed with flags. */
 #define RT_VARIANT_DEFAULT 0 /* sliding-stencil register accumulation, coherent ray order; warp = 32 sources x 1
                                 direction when n_src >= 32, else 32 directions of one source */
 #define RT_VARIANT_DIRECT 1  /* textbook form: 8 reductions per ray-substep-bin-group, lattice order */
@@ -59,6 +59,7 @@ extern "C" {
 #define RT_VARIANT_SLIDING_BY_DIRECTION 4 /* sliding stencil, coherent ray order, warp = 32 directions of one source */
 #define RT_VARIANT_SLIDING_BY_SOURCE 5 /* sliding stencil, coherent ray order, warp = 32 sorted sources x 1 direction */
 #define RT_VARIANT_FLAG_ACC_F32 16 /* accumulate straight into `out` in fp32 instead of the fp64 workspace grid */
+#define RT_VARIANT_FLAG_ONE_BIN 32 /* one bin per thread even when n_bins % 4 == 0 (bins in adjacent lanes) */
 
 /* The multi-source march ("loop-and-sum wrapper").  See the header comment for semantics. */
 int rt_march(const float* j, const float* kappa, int nx, int ny, int nz,
@@ -98,7 +99,7 @@ size_t rt_workspace_bytes(int nx, int ny, int nz, int n_src, int n_rays, int n_b
 int rt_substeps_per_step(float step_size, float c, float dt);
 
 /* Number of kernels of this library that one rt_march call with these arguments enqueues (memsets excluded). */
-int rt_launch_count(int n_src, int n_bins, int n_steps);
+int rt_launch_count(int n_src, int n_rays, int n_bins, int n_steps);
 
 /* TEST HOOK.  Writes the library's direction lattice (D1) for i = 0..n_rays-1 into
  * nhat[n_rays][3] (float64, device), computed exactly as the march kernel does. */

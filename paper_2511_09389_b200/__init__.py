@@ -5,7 +5,8 @@ synthetic inputs (shared with the oracle's tests; no method arithmetic).  Import
 ``librtmarch.so`` and raises if it is missing and cannot be built: there is no CPU fallback.
 """
 from .binding import (RT_EALIGN, RT_ECUDA, RT_EINVAL, RT_EWORKSPACE, RT_OK, RT_VARIANT_DEFAULT,  # noqa: F401
-                      RT_VARIANT_DIRECT, RT_VARIANT_DIRECT_COHERENT, RT_VARIANT_FLAG_ACC_F32, RT_VARIANT_SLIDING_BY_DIRECTION,
+                      RT_VARIANT_DIRECT, RT_VARIANT_DIRECT_COHERENT, RT_VARIANT_FLAG_ACC_F32, RT_VARIANT_FLAG_ONE_BIN,
+                      RT_VARIANT_SLIDING_BY_DIRECTION,
                       RT_VARIANT_SLIDING_BY_SOURCE, RT_VARIANT_SLIDING_LATTICE, RtError,
                       alloc_workspace, library_path, rt_bench_red_ceiling, rt_directions, rt_launch_count,
                       rt_march, rt_march_ex, rt_march_host, rt_march_single, rt_ray_order, rt_ray_slots,

@@ -17,6 +17,7 @@ from . import build as _build
 RT_OK, RT_EINVAL, RT_EWORKSPACE, RT_ECUDA, RT_EALIGN = 0, -1, -2, -3, -4
 RT_VARIANT_DEFAULT, RT_VARIANT_DIRECT, RT_VARIANT_DIRECT_COHERENT, RT_VARIANT_SLIDING_LATTICE = 0, 1, 2, 3
 RT_VARIANT_SLIDING_BY_DIRECTION, RT_VARIANT_SLIDING_BY_SOURCE, RT_VARIANT_FLAG_ACC_F32 = 4, 5, 16
+RT_VARIANT_FLAG_ONE_BIN = 32
 RED_MODES = {"M1_scalar_random": 0, "M2_v4_random": 1, "M3_stencil": 2, "M4_one_address": 3,
              "M5_coalesced": 4, "M6_stencil_walk": 5, "M1_f64_scalar_random": 6, "M3_f64_stencil": 7}
 
@@ -51,7 +52,7 @@ def _load() -> ctypes.CDLL:
     L.rt_workspace_bytes.argtypes = [i] * 7
     L.rt_workspace_bytes.restype = sz
     L.rt_substeps_per_step.argtypes = [f, f, f]
-    L.rt_launch_count.argtypes = [i, i, i]
+    L.rt_launch_count.argtypes = [i, i, i, i]
     L.rt_directions.argtypes = [i, vp, vp]
     L.rt_ray_order.argtypes = [i, vp, vp]
     L.rt_ray_slots.argtypes = [i]
@@ -89,8 +90,8 @@ def rt_workspace_bytes(nx, ny, nz, n_src, n_rays, n_bins, n_steps) -> int:
     return int(_lib.rt_workspace_bytes(nx, ny, nz, n_src, n_rays, n_bins, n_steps))
 
 
-def rt_launch_count(n_src: int, n_bins: int, n_steps: int) -> int:
-    return int(_lib.rt_launch_count(n_src, n_bins, n_steps))
+def rt_launch_count(n_src: int, n_rays: int, n_bins: int, n_steps: int) -> int:
+    return int(_lib.rt_launch_count(n_src, n_rays, n_bins, n_steps))
 
 
 def rt_ray_slots(n_rays: int) -> int:

@@ -2,6 +2,7 @@
 // launches on the caller's stream.  No torch types, no global state besides a thread-local error string.
 #include "../../include/rtmarch.h"
 
+#include <algorithm>
 #include <cmath>
 #include <cstdint>
 #include <cstdio>
@@ -114,12 +115,13 @@ constexpr int kMaxSortedSources = 65536;   // above this the O(n^2) source sort 
 
 // what a variant code means (rtmarch.h RT_VARIANT_*)
 struct Plan {
-    bool sliding, coherent, map_src, acc64;
+    bool sliding, coherent, map_src, acc64, one_bin;
 };
 bool make_plan(int variant, int n_src, Plan* pl) {
     const int kind = variant & 15;
-    if (variant < 0 || (variant & ~31) || kind > RT_VARIANT_SLIDING_BY_SOURCE) return false;
+    if (variant < 0 || (variant & ~63) || kind > RT_VARIANT_SLIDING_BY_SOURCE) return false;
     pl->acc64 = !(variant & RT_VARIANT_FLAG_ACC_F32);
+    pl->one_bin = (variant & RT_VARIANT_FLAG_ONE_BIN) != 0;
     pl->sliding = !(kind == RT_VARIANT_DIRECT || kind == RT_VARIANT_DIRECT_COHERENT);
     pl->coherent = !(kind == RT_VARIANT_DIRECT || kind == RT_VARIANT_SLIDING_LATTICE);
     pl->map_src = (kind == RT_VARIANT_SLIDING_BY_SOURCE) || (kind == RT_VARIANT_DEFAULT && n_src >= 32);
@@ -142,7 +144,7 @@ int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const
     rt::MarchParams P;
     P.j = j; P.kappa = kappa; P.sources = sources;
     P.nx = nx; P.ny = ny; P.nz = nz; P.nb = n_bins;
-    P.n_src = n_src; P.n_rays = n_rays;
+    P.n_src = n_src; P.src_begin = 0; P.n_rays = n_rays;
     P.n_steps = n_steps; P.n_sub = int(ck.n_sub);
     P.ds = double(step_size); P.ds_f = step_size;
     P.emis = float(double(step_size) * 4.0 * 3.14159265358979323846 / double(n_rays));
@@ -166,28 +168,53 @@ int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const
     } else {
         P.src_order = nullptr;
     }
-    // the accumulation grid: fp64 in the workspace (default), or `out` itself (RT_VARIANT_FLAG_ACC_F32)
     const size_t n_acc = size_t(ck.cells) * size_t(n_steps);
-    P.acc = pl.acc64 ? static_cast<void*>(ws + wl.acc_at) : static_cast<void*>(out);
-    RT_CUDA(cudaMemsetAsync(P.acc, 0, n_acc * (pl.acc64 ? sizeof(double) : sizeof(float)), st));   // D14: overwrite
+    double* master = reinterpret_cast<double*>(ws + wl.acc_at);
+    const int fin_threads = 256;
+    long long fin_blocks = (ck.cells + fin_threads - 1) / fin_threads;
+    if (fin_blocks > 148 * 16) fin_blocks = 148 * 16;
 
-    // 4 bins per thread with 16-byte loads (and 16-byte reductions into an fp32 grid) when the layout allows it
-    const bool vec4 = (n_bins % 4 == 0) && !((uintptr_t(j) | uintptr_t(kappa) | uintptr_t(out)) & 15u);
+    // 4 bins per thread with 16-byte loads and 16-byte fp32 reductions when the layout allows it
+    const bool vec4 = (n_bins % 4 == 0) && !pl.one_bin && !((uintptr_t(j) | uintptr_t(kappa) | uintptr_t(out)) & 15u);
     P.n_groups = vec4 ? n_bins / 4 : n_bins;
+
+    if (vec4 && pl.acc64 && pl.sliding) {
+        // Batched fp32: there is no 16-byte fp64 reduction, and four scalar fp64 reductions per voxel make the
+        // 4-bin kernel reduction bound.  So `out` is the fp32 scratch grid of ONE batch of sources (<= 2^18 rays:
+        // no fp32 sum grows past a batch, which bounds the stagnation error), reduced into with
+        // red.v4.f32 and folded into the fp64 grid after every batch.
+        RT_CUDA(cudaMemsetAsync(master, 0, n_acc * sizeof(double), st));
+        RT_CUDA(cudaMemsetAsync(out, 0, n_acc * sizeof(float), st));                 // D14: overwrite
+        int per_batch = int(std::max(1LL, (1LL << 18) / (long long)n_rays));
+        if (pl.map_src) per_batch = (per_batch + 31) / 32 * 32;
+        P.acc = out;
+        for (int s0 = 0; s0 < n_src; s0 += per_batch) {
+            P.src_begin = s0;
+            P.n_src = std::min(per_batch, n_src - s0);
+            const int rcb = launch_march<4, float>(P, true, st);
+            if (rcb != RT_OK) return rcb;
+            long long db = ((long long)(n_acc / 4) + fin_threads - 1) / fin_threads;
+            if (db > 148 * 16) db = 148 * 16;
+            rt::drain_kernel<<<unsigned(db), fin_threads, 0, st>>>(master, out, (long long)n_acc);
+            RT_CUDA(cudaGetLastError());
+        }
+        rt::snapshot_finalize_kernel<double><<<unsigned(fin_blocks), fin_threads, 0, st>>>(master, out, ck.cells, n_steps);
+        RT_CUDA(cudaGetLastError());
+        return RT_OK;
+    }
+
+    // the accumulation grid: fp64 in the workspace (default), or `out` itself (RT_VARIANT_FLAG_ACC_F32)
+    P.acc = pl.acc64 ? static_cast<void*>(master) : static_cast<void*>(out);
+    RT_CUDA(cudaMemsetAsync(P.acc, 0, n_acc * (pl.acc64 ? sizeof(double) : sizeof(float)), st));   // D14: overwrite
     int rc3;
     if (vec4) rc3 = pl.acc64 ? launch_march<4, double>(P, pl.sliding, st) : launch_march<4, float>(P, pl.sliding, st);
     else rc3 = pl.acc64 ? launch_march<1, double>(P, pl.sliding, st) : launch_march<1, float>(P, pl.sliding, st);
     if (rc3 != RT_OK) return rc3;
-
-    const int threads = 256;
-    long long blocks = (ck.cells + threads - 1) / threads;
-    if (blocks > 148 * 16) blocks = 148 * 16;
     if (pl.acc64) {
-        rt::snapshot_finalize_kernel<double><<<unsigned(blocks), threads, 0, st>>>(
-            static_cast<const double*>(P.acc), out, ck.cells, n_steps);
+        rt::snapshot_finalize_kernel<double><<<unsigned(fin_blocks), fin_threads, 0, st>>>(master, out, ck.cells, n_steps);
         RT_CUDA(cudaGetLastError());
     } else if (n_steps > 1) {
-        rt::snapshot_finalize_kernel<float><<<unsigned(blocks), threads, 0, st>>>(out, out, ck.cells, n_steps);
+        rt::snapshot_finalize_kernel<float><<<unsigned(fin_blocks), fin_threads, 0, st>>>(out, out, ck.cells, n_steps);
         RT_CUDA(cudaGetLastError());
     }
     return RT_OK;
@@ -268,12 +295,17 @@ int rt_substeps_per_step(float step_size, float c, float dt) {
     return ns < 1 ? RT_EINVAL : int(ns);
 }
 
-int rt_launch_count(int n_src, int n_bins, int n_steps) {
-    if (n_src < 1 || n_bins < 1 || n_steps < 1) return RT_EINVAL;
+int rt_launch_count(int n_src, int n_rays, int n_bins, int n_steps) {
+    if (n_src < 1 || n_rays < 1 || n_bins < 1 || n_steps < 1) return RT_EINVAL;
     Plan pl;
     make_plan(RT_VARIANT_DEFAULT, n_src, &pl);
-    // ray order, (source order), march, snapshot finalisation
-    return 3 + ((pl.map_src && n_src <= kMaxSortedSources) ? 1 : 0);
+    const int setup = 1 + ((pl.map_src && n_src <= kMaxSortedSources) ? 1 : 0);     // ray order, (source order)
+    if (n_bins % 4 == 0) {                                                          // batched: (march, drain) per batch
+        int per_batch = int(std::max(1LL, (1LL << 18) / (long long)n_rays));
+        if (pl.map_src) per_batch = (per_batch + 31) / 32 * 32;
+        return setup + 2 * ((n_src + per_batch - 1) / per_batch) + 1;
+    }
+    return setup + 2;                                                               // march, snapshot finalisation
 }
 
 int rt_directions(int n_rays, double* nhat, void* stream) {
@@ -294,7 +326,7 @@ int rt_trace_ray(const float* j, const float* kappa, int nx, int ny, int nz, int
     rt::MarchParams P{};
     P.j = j; P.kappa = kappa; P.sources = source_pos; P.acc = nullptr; P.ray_order = nullptr; P.src_order = nullptr; P.map_src = 0;
     P.nx = nx; P.ny = ny; P.nz = nz; P.nb = n_bins;
-    P.n_src = 1; P.n_rays = n_rays; P.n_slots = n_rays; P.n_groups = 1; P.n_steps = 1; P.n_sub = n_sub;
+    P.n_src = 1; P.src_begin = 0; P.n_rays = n_rays; P.n_slots = n_rays; P.n_groups = 1; P.n_steps = 1; P.n_sub = n_sub;
     P.ds = double(step_size); P.ds_f = step_size; P.emis = step_size; P.att_scale = 0.0f; P.snap_stride = 0;
     rt::trace_ray_kernel<<<1, 32, 0, static_cast<cudaStream_t>(stream)>>>(P, uint32_t(ray_index), n_sub, pos, trace_I,
                                                                          trace_T);

@@ -18,7 +18,8 @@ struct MarchParams {
     const uint32_t* ray_order;   // [n_slots] slot -> lattice index (0xFFFFFFFF = padding) or nullptr = identity
     const uint32_t* src_order;   // [n_src] rank -> source index (spatially sorted) or nullptr = identity
     int nx, ny, nz, nb;
-    int n_src, n_rays, n_slots;
+    int n_src, n_rays, n_slots;  // n_src: sources of THIS launch, ranks src_begin .. src_begin + n_src - 1
+    int src_begin;
     int n_groups;                // bin groups per ray (nb / NB)
     int n_steps, n_sub;          // time steps, substeps per step (N_s)
     int map_src;                 // 0: the lanes of a warp are 32 directions of one source; 1: 32 sources, one direction
@@ -148,13 +149,16 @@ template <int NB> __device__ __forceinline__ bool any_nonzero(const BinVec<NB>& 
 }
 
 // ---------------------------------------------------------------------------------------------------
-// thread -> (source, lattice index, bin group).  Two mappings:
-//   map_src = 0  block = 128 consecutive direction slots of one source (lanes of a warp: a patch of the sphere);
-//   map_src = 1  block = 4 consecutive direction slots x 32 consecutive sources of the spatially sorted source
-//                list (lanes of a warp: 32 sources, ONE direction).  Rays of a warp are parallel; when the
-//                sources share their fractional cell offsets (cell-centred sources) the lanes cross
-//                cell faces in the same substep, so the stencil-slide branches are warp-uniform.
-// Block order: direction chunk fastest, then bin group, then source (group).
+// thread -> (source, lattice index, bin group).  The bin group is the FASTEST lane index: the G = n_bins / NB
+// threads that march the same ray for different bins sit in adjacent lanes, so their loads and reductions hit
+// adjacent words of the bin-innermost grids (one 32-byte sector for 4 fp64 or 8 fp32 bins).  Two mappings of
+// the rays:
+//   map_src = 0  block = 128 consecutive (direction slot, group) pairs of one source (a patch of the sphere);
+//   map_src = 1  block = 4 consecutive direction slots; each warp 32 consecutive (source, group) pairs of the
+//                spatially sorted source list, ONE direction.  Rays of a warp are parallel; when the sources
+//                share their fractional cell offsets (cell-centred sources) the lanes cross cell
+//                faces in the same substep, so the stencil-slide branches are warp-uniform.
+// Block order: direction chunk fastest, then source (chunk).
 // ---------------------------------------------------------------------------------------------------
 struct RayId {
     int src, group;
@@ -162,26 +166,28 @@ struct RayId {
 };
 
 __host__ __device__ inline long long march_blocks(int n_src, int n_slots, int n_groups, int map_src) {
-    if (map_src) return (long long)((n_slots + 3) / 4) * n_groups * ((n_src + 31) / 32);
-    return (long long)((n_slots + kThreads - 1) / kThreads) * n_groups * n_src;
+    if (map_src) return (long long)((n_slots + 3) / 4) * (((long long)n_src * n_groups + 31) / 32);
+    return (((long long)n_slots * n_groups + kThreads - 1) / kThreads) * n_src;
 }
 
 __device__ __forceinline__ bool ray_id(const MarchParams& P, RayId& id) {
+    const uint32_t G = uint32_t(P.n_groups);
     uint32_t b = blockIdx.x, slot, s;
     if (P.map_src) {
         const uint32_t chunks = (uint32_t(P.n_slots) + 3u) / 4u;
         slot = (b % chunks) * 4u + (threadIdx.x >> 5);
-        b /= chunks;
-        id.group = int(b % uint32_t(P.n_groups));
-        s = (b / uint32_t(P.n_groups)) * 32u + (threadIdx.x & 31u);
+        const uint32_t f = (b / chunks) * 32u + (threadIdx.x & 31u);      // (source rank, group), group fastest
+        s = f / G;
+        id.group = int(f - s * G);
     } else {
-        const uint32_t chunks = (uint32_t(P.n_slots) + kThreads - 1) / kThreads;
-        slot = (b % chunks) * kThreads + threadIdx.x;
-        b /= chunks;
-        id.group = int(b % uint32_t(P.n_groups));
-        s = b / uint32_t(P.n_groups);
+        const uint32_t chunks = (uint32_t(P.n_slots) * G + kThreads - 1) / kThreads;
+        const uint32_t f = (b % chunks) * kThreads + threadIdx.x;         // (direction slot, group), group fastest
+        slot = f / G;
+        id.group = int(f - slot * G);
+        s = b / chunks;
     }
     if (slot >= uint32_t(P.n_slots) || s >= uint32_t(P.n_src)) return false;
+    s += uint32_t(P.src_begin);
     id.src = int(P.src_order ? P.src_order[s] : s);
     id.index = P.ray_order ? P.ray_order[slot] : slot;
     return id.index != kPad && id.index < uint32_t(P.n_rays);

@@ -68,7 +68,8 @@ def test_host_side_helpers(rt):
     assert rt.rt_workspace_bytes(16, 16, 16, 1, 64, 1, 1) >= 64 * 4
     assert rt.rt_workspace_bytes(16, 16, 16, 1, 0, 1, 1) == 0
     assert rt.rt_ray_slots(4096) >= 4096 and rt.rt_ray_slots(0) == rt.RT_EINVAL
-    assert rt.rt_launch_count(1, 1, 1) >= 1 and rt.rt_launch_count(64, 1, 4) >= rt.rt_launch_count(1, 1, 1)
+    assert rt.rt_launch_count(1, 64, 1, 1) == 3 and rt.rt_launch_count(64, 64, 1, 4) == 4
+    assert rt.rt_launch_count(256, 4096, 8, 2) == 2 + 2 * 4 + 1
     for code in (0, -1, -2, -3, -4, -99):
         assert isinstance(rt.rt_strerror(code), str) and rt.rt_strerror(code)
 
@@ -97,7 +98,7 @@ def test_argument_errors_are_caught_before_cuda(rt):
     assert call(workspace=p + 4) == rt.RT_EWORKSPACE
     assert L.rt_march_host(None, p, 8, 8, 8, p, 1, 16, 1, 0.5, 1.0, 2.0, 1, p) == rt.RT_EINVAL
     assert L.rt_march_ex(p, p, 8, 8, 8, p, 1, 16, 1, 0.5, 1.0, 2.0, 1, p, p, 1 << 20, None, 7) == rt.RT_EINVAL
-    assert L.rt_march_ex(p, p, 8, 8, 8, p, 1, 16, 1, 0.5, 1.0, 2.0, 1, p, p, 1 << 20, None, 64) == rt.RT_EINVAL
+    assert L.rt_march_ex(p, p, 8, 8, 8, p, 1, 16, 1, 0.5, 1.0, 2.0, 1, p, p, 1 << 20, None, 128) == rt.RT_EINVAL
     assert L.rt_bench_red_ceiling(9, p, 8, 8, 8, 1, 100, 1, None, None) == rt.RT_EINVAL
     assert L.rt_directions(0, p, None) == rt.RT_EINVAL
     assert L.rt_ray_order(16, None, None) == rt.RT_EINVAL

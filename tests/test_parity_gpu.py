@@ -57,7 +57,7 @@ def config(name):
     return _cache[name]
 
 
-VARIANTS = [0, 1, 2, 3, 4, 5, 16, 17, 21]     # kinds 0..5, and fp32 accumulation (flag 16) on kinds 0, 1, 5
+VARIANTS = [0, 1, 2, 3, 4, 5, 16, 17, 21, 32, 36, 53]   # kinds 0..5; flags: 16 fp32 accumulation, 32 one bin per thread
 
 
 # ------------------------------------------------------------------------------------------------
