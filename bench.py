@@ -359,12 +359,16 @@ def run_native(args):
 def _ncu_counters(config, variant):
     """Per-launch ncu counters of the march kernel (committed text under profiles/, one capture per kernel
     revision): instruction count, L2 reduction sectors, DRAM bytes.  None if there is no capture for this case."""
+    import csv
     try:
-        table = json.load(open(os.path.join(ROOT, "profiles", "march_counters.json")))
-        row = table.get(f"{config}:v{variant}")
-        return row if row and row.get("library") == _lib_version() else None
-    except (OSError, ValueError):
-        return None
+        with open(os.path.join(ROOT, "profiles", "march_counters.csv"), newline="") as f:
+            for row in csv.DictReader(f):
+                if row["case"] == f"{config}:v{variant}" and row["library"] == _lib_version():
+                    return {"warp_instructions": float(row["warp_instructions"]), "red_sectors": float(row["red_sectors"]),
+                            "dram_bytes": float(row["dram_bytes"]), "source": row["source"]}
+    except (OSError, KeyError, ValueError):
+        pass
+    return None
 
 
 def _lib_version():
