@@ -36,7 +36,7 @@ UNIT = "updates/s"
 def parse():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", default="C2", choices=["C0", "C1", "C2", "C3", "C4"])
     ap.add_argument("--impl", default="native", choices=["native", "reference"])
@@ -138,7 +138,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "20"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
@@ -323,7 +323,7 @@ def run_native(args):
             "bound": "l2_red", "achieved": achieved, "peak": peak, "unit": "Gred/s", "frac": achieved / peak,
             "traffic": None, "kernel": "march_sliding_kernel",
             "how": "achieved = ALGORITHMIC reductions (8 corners x bin-groups x ray-substeps) / mean CUDA-event "
-                   "time of the whole rt_march call (the march kernel is >99.9% of it, profiles/); peak = "
+                   "time of the whole rt_march call (the march kernel is 99% of it at C2, profiles/r01b); peak = "
                    "M3 stencil-pattern red.global.add ceiling measured in this process on a grid of the same "
                    "size (DESIGN.md §8), of measured; frac > 1: the sliding stencil sums a voxel's deposits in "
                    "registers, so fewer reductions are issued than the method states (see `issued`)",
