@@ -51,6 +51,10 @@ def lib() -> ctypes.CDLL:
             L.rt_march_oracle.argtypes = [fp, fp, ctypes.c_int, ctypes.c_int, ctypes.c_int, fp, ctypes.c_int,
                                           ctypes.c_int, ctypes.c_int, ctypes.c_float, ctypes.c_float,
                                           ctypes.c_float, ctypes.c_int, dp, ctypes.c_int]
+            L.rt_oracle_step.restype = ctypes.c_int
+            L.rt_oracle_step.argtypes = [fp, fp, ctypes.c_int, ctypes.c_int, ctypes.c_int, fp, ctypes.c_int,
+                                         ctypes.c_int, ctypes.c_int, ctypes.c_float, ctypes.c_float, ctypes.c_float,
+                                         ctypes.c_long, dp, dp, ctypes.c_int]
             L.rt_oracle_version.restype = ctypes.c_char_p
             _lib = L
     return _lib
@@ -109,6 +113,32 @@ def march(j, kappa, sources, n_rays, step_size, c, dt, n_steps, n_threads: int |
     if rc:
         raise ValueError("rt_march_oracle: invalid arguments")
     return out
+
+
+def new_state(n_src: int, n_rays: int, n_bins: int) -> np.ndarray:
+    """Fresh ray state for ``step``: float64 [n_src, n_rays, 2, n_bins] = (I, tau), all zero (I_0 = tau_0 = 0)."""
+    return np.zeros((n_src, n_rays, 2, n_bins), dtype=np.float64)
+
+
+def step(j, kappa, sources, n_rays, step_size, c, dt, k_begin: int, state: np.ndarray,
+         n_threads: int | None = None) -> np.ndarray:
+    """One time step in the given medium from substep ``k_begin``; updates ``state`` in place and returns the
+    increment of the field, float64 [nx, ny, nz, n_bins] (scaled by 4π/N_Ω)."""
+    j = _f32(j, 4)
+    kappa = _f32(kappa, 4)
+    sources = _f32(sources, 2)
+    nx, ny, nz, nb = j.shape
+    if state.dtype != np.float64 or not state.flags.c_contiguous or state.shape != (sources.shape[0], n_rays, 2, nb):
+        raise ValueError("state must be the C-contiguous float64 array of new_state()")
+    if n_threads is None:
+        n_threads = host_threads()
+    n_threads = max(1, min(n_threads, (24 << 30) // max(1, j.size * 8)))
+    inc = np.empty((nx, ny, nz, nb), dtype=np.float64)
+    rc = lib().rt_oracle_step(_fp(j), _fp(kappa), nx, ny, nz, _fp(sources), sources.shape[0], n_rays, nb, step_size,
+                              c, dt, k_begin, _dp(state), _dp(inc), n_threads)
+    if rc:
+        raise ValueError("rt_oracle_step: invalid arguments")
+    return inc
 
 
 def trace_ray(j, kappa, source_pos, ray_index, n_rays, step_size, n_sub, deposit: bool = False):

@@ -246,6 +246,51 @@ int rt_march_oracle(const float* j, const float* kappa, int nx, int ny, int nz, 
     return 0;
 }
 
+// One time step with EXPLICIT ray state ("for strict time integration we fix dt and iterate"; P:58 RT substeps
+// between hydro updates; reading D17): substeps k_begin .. k_begin + N_s - 1 of every ray, in the medium
+// (j, kappa) passed to THIS call -- the caller may change it between calls.  Positions continue the same straight
+// line, x_k = x_0 + k ds nhat; (I, tau) carry over in `state`.
+//   state: double [n_src][n_rays][2][n_bins] = I[b] then tau[b] per ray; all zeros for a fresh start (D11); updated.
+//   inc:   double [nx][ny][nz][n_bins], OVERWRITTEN with (4 pi / N_Omega) * the deposits of this step alone.
+// With an unchanged medium the increments of successive calls add up to the cumulative snapshots of rt_march_oracle.
+int rt_oracle_step(const float* j, const float* kappa, int nx, int ny, int nz, const float* sources, int n_src,
+                   int n_rays, int n_bins, float step_size, float c, float dt, long k_begin, double* state,
+                   double* inc, int n_threads) {
+    if (!j || !kappa || !sources || !state || !inc) return -1;
+    if (nx < 1 || ny < 1 || nz < 1 || n_src < 1 || n_rays < 1 || n_bins < 1 || k_begin < 0) return -1;
+    if (bad(step_size) || bad(c) || bad(dt)) return -1;
+    const long Ns = substeps(double(step_size), double(c), double(dt));
+    const double ds = double(step_size);
+    const Medium M{j, kappa, nx, ny, nz, n_bins};
+    const size_t grid = size_t(nx) * ny * nz * n_bins;
+    const long total_rays = long(n_src) * n_rays;
+    long T = std::min<long>(std::max(1, n_threads), total_rays);
+    std::vector<std::vector<double>> acc(T);
+    for (auto& a : acc) a.assign(grid, 0.0);
+    auto work = [&](long t) {
+        long r0 = total_rays * t / T, r1 = total_rays * (t + 1) / T;
+        for (long r = r0; r < r1; ++r) {
+            long s = r / n_rays, i = r % n_rays;
+            double nhat[3];
+            fib_direction(i, n_rays, nhat);
+            double x0[3] = {double(sources[3 * s]), double(sources[3 * s + 1]), double(sources[3 * s + 2])};
+            double* I = state + size_t(r) * n_bins * 2;
+            march_ray(M, x0, nhat, ds, k_begin, k_begin + Ns, I, I + n_bins, acc[t].data(), nullptr, nullptr, nullptr);
+        }
+    };
+    std::vector<std::thread> pool;
+    for (long t = 1; t < T; ++t) pool.emplace_back(work, t);
+    work(0);
+    for (auto& th : pool) th.join();
+    const double scale = double(4.0L * kPiL / (long double)n_rays);
+    for (size_t v = 0; v < grid; ++v) {
+        double sum = 0.0;
+        for (long u = 0; u < T; ++u) sum += acc[u][v];
+        inc[v] = scale * sum;
+    }
+    return 0;
+}
+
 const char* rt_oracle_version(void) { return "rt_oracle 1 (fp64, PAPER.md eq. 2)"; }
 
 }  // extern "C"

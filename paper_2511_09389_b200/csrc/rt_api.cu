@@ -162,7 +162,7 @@ int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const
     }
     if (pl.map_src && n_src <= kMaxSortedSources) {
         uint32_t* so = reinterpret_cast<uint32_t*>(ws + wl.src_order_at);
-        rt::src_order_kernel<<<(n_src + 127) / 128, 128, 0, st>>>(so, sources, n_src, nx, ny, nz);
+        rt::src_order_kernel<<<(n_src + 3) / 4, 128, 0, st>>>(so, sources, n_src, nx, ny, nz);
         RT_CUDA(cudaGetLastError());
         P.src_order = so;
     } else {

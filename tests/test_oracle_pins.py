@@ -571,3 +571,68 @@ def test_config_c0_matches_its_recipe(oracle_mod):
                for i in range(w.n_rays))
     assert out.sum() == pytest.approx(FOUR_PI / w.n_rays * mass, rel=1e-12)
     assert oracle_mod.substeps(w.step_size, w.c, w.dt) == w.substeps_per_step == 24
+
+
+# ------------------------------------------------------------------------------------------------------
+# D17  stepping with explicit ray state (oracle.step; "fix dt and iterate")
+# ------------------------------------------------------------------------------------------------------
+def test_d17_steps_in_a_static_medium_add_up_to_the_snapshots(oracle_mod):
+    rho = W.lognormal_density(12, 5, 1.0)
+    ks, js = W.bin_scalings(3)
+    j = np.ascontiguousarray((1e-2 * rho ** 2)[..., None] * js, dtype=np.float32)
+    kap = np.ascontiguousarray((0.1 * rho)[..., None] * ks, dtype=np.float32)
+    src = np.array([[5.5, 6.0, 3.25], [-1.0, 4.0, 13.5]], dtype=np.float32)
+    n_rays, ds, dt, n_steps = 37, 0.5, 3.0, 4
+    snaps = oracle_mod.march(j, kap, src, n_rays, ds, 1.0, dt, n_steps)
+    state = oracle_mod.new_state(2, n_rays, 3)
+    ns = oracle_mod.substeps(ds, 1.0, dt)
+    run = np.zeros_like(snaps[0])
+    for m in range(n_steps):
+        run += oracle_mod.step(j, kap, src, n_rays, ds, 1.0, dt, m * ns, state)
+        assert np.abs(run - snaps[m]).max() <= 1e-12 * snaps[m].max()
+    assert (state[:, :, 1, :] > 0).all()          # tau grew on every ray
+
+
+def test_d17_medium_changed_between_steps_closed_form(oracle_mod):
+    """Uniform (j1, k1) during step 1, uniform (j2, k2) during step 2: by induction on eq. (2)
+    I_{N+i} = I_N a2^i + i j2 ds e^{-tau_N} a2^{i-1}, with I_N = N j1 ds a1^{N-1}, tau_N = N k1 ds."""
+    n, n_rays, ds, dt = 10, 24, 0.5, 3.0
+    N = oracle_mod.substeps(ds, 1.0, dt)
+    j1, k1, j2, k2 = f32(0.3), f32(0.2), f32(0.7), f32(0.05)
+    src = np.array([[4.5, 4.5, 4.5], [8.0, 1.0, 2.0]], dtype=np.float32)
+    state = oracle_mod.new_state(2, n_rays, 1)
+    ja, ka = W.uniform_medium(n, j1, k1)
+    jb, kb = W.uniform_medium(n, j2, k2)
+    oracle_mod.step(ja, ka, src, n_rays, ds, 1.0, dt, 0, state)
+    a1, a2 = math.exp(-k1 * ds), math.exp(-k2 * ds)
+    I_N, tau_N = N * j1 * ds * a1 ** (N - 1), N * k1 * ds
+    assert np.allclose(state[:, :, 0, 0], I_N, rtol=1e-13) and np.allclose(state[:, :, 1, 0], tau_N, rtol=1e-13)
+    inc = oracle_mod.step(jb, kb, src, n_rays, ds, 1.0, dt, N, state)
+    I_end = I_N * a2 ** N + N * j2 * ds * math.exp(-tau_N) * a2 ** (N - 1)
+    assert np.allclose(state[:, :, 0, 0], I_end, rtol=1e-13)
+    assert np.allclose(state[:, :, 1, 0], tau_N + N * k2 * ds, rtol=1e-13)
+    mass = sum(I_N * a2 ** i + i * j2 * ds * math.exp(-tau_N) * a2 ** (i - 1) for i in range(1, N + 1))
+    assert abs(inc.sum() - FOUR_PI * 2 * mass) <= 1e-12 * inc.sum()      # every substep deposits total weight 1
+
+
+def test_d17_a_step_sees_only_its_own_medium(oracle_mod):
+    """j = 0 in step 2 with kappa = 0: the intensity of step 1 is carried unchanged and keeps being deposited;
+    positions continue the same straight line (the increment equals a static-medium run's, scaled)."""
+    n, n_rays, ds, dt = 8, 16, 0.5, 2.0
+    N = oracle_mod.substeps(ds, 1.0, dt)
+    ja, ka = W.uniform_medium(n, 0.4, 0.0)
+    jz, kz = W.uniform_medium(n, 0.0, 0.0)
+    src = np.array([[3.5, 3.5, 3.5]], dtype=np.float32)
+    state = oracle_mod.new_state(1, n_rays, 1)
+    oracle_mod.step(ja, ka, src, n_rays, ds, 1.0, dt, 0, state)
+    I_N = N * f32(0.4) * ds
+    inc = oracle_mod.step(jz, kz, src, n_rays, ds, 1.0, dt, N, state)
+    assert np.allclose(state[:, :, 0, 0], I_N, rtol=1e-14)
+    # the same geometry deposited with unit intensity: a static run with I forced to 1 does not exist, but the
+    # deposit pattern of substeps N..2N-1 is that of (snapshot 2 - snapshot 1) of a run whose I is constant:
+    # j = 0, kappa = 0 after an initial state of I = 1 <=> linearity in the carried intensity
+    state1 = oracle_mod.new_state(1, n_rays, 1)
+    state1[:, :, 0, 0] = 1.0
+    unit = oracle_mod.step(jz, kz, src, n_rays, ds, 1.0, dt, N, state1)
+    assert np.abs(inc - I_N * unit).max() <= 1e-13 * inc.max()
+    assert abs(unit.sum() - FOUR_PI * N) <= 1e-12 * unit.sum()
