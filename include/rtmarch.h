@@ -81,6 +81,25 @@ int rt_march_ex(const float* j, const float* kappa, int nx, int ny, int nz,
                 float step_size, float c, float dt, int n_steps, float* out,
                 void* workspace, size_t workspace_bytes, void* stream, int variant);
 
+/* STEPPING WITH PERSISTENT RAY STATE ("for strict time integration we fix dt and iterate"; P:58 RT substeps
+ * between hydro updates; reading D17).  rt_march_step advances every ray by ONE time step -- substeps
+ * k_begin .. k_begin + N_s - 1 -- in the medium (j, kappa) passed to THIS call, which the caller may change
+ * between calls.  Rays continue their straight lines (x_k = x_0 + k ds n: pass k_begin = m * N_s for step m, with
+ * the same sources, n_rays, step_size, c, dt); (I, exp(-tau)) of every (source, direction, bin) carry over in
+ * `state`.  out[nx][ny][nz][n_bins] receives the field deposited during this step, scaled by 4 pi / N_Omega:
+ * overwritten (accumulate = 0) or added to (accumulate != 0; summed in fp64, rounded once per call).  With an
+ * unchanged medium, steps 0..m accumulated reproduce snapshot m of rt_march.
+ *   state: device, rt_state_bytes() bytes, 16-byte aligned, float32 [2][n_src][n_rays][n_bins] = I then exp(-tau);
+ *          rt_state_reset() gives the fresh state I = 0, tau = 0 (D11).  Indexed by source and lattice index.
+ *   workspace: rt_step_workspace_bytes() bytes.  Errors and limits as rt_march, with n_steps*N_s -> k_begin + N_s. */
+size_t rt_state_bytes(int n_src, int n_rays, int n_bins);
+int rt_state_reset(float* state, int n_src, int n_rays, int n_bins, void* stream);
+size_t rt_step_workspace_bytes(int nx, int ny, int nz, int n_src, int n_rays, int n_bins);
+int rt_march_step(const float* j, const float* kappa, int nx, int ny, int nz,
+                  const float* sources, int n_src, int n_rays, int n_bins,
+                  float step_size, float c, float dt, long long k_begin, float* state,
+                  float* out, int accumulate, void* workspace, size_t workspace_bytes, void* stream);
+
 /* End-to-end form with HOST pointers (j, kappa, sources, out are host memory, pinned or pageable).
  * Allocates device buffers, copies the inputs in, marches, copies out[] back, frees, and returns after the
  * copy has completed (SYNCHRONOUS).  Same semantics, limits and error codes as rt_march. */

@@ -23,7 +23,8 @@ RED_MODES = {"M1_scalar_random": 0, "M2_v4_random": 1, "M3_stencil": 2, "M4_one_
 
 EXPORTS = ("rt_march", "rt_march_single", "rt_march_ex", "rt_march_host", "rt_workspace_bytes",
            "rt_substeps_per_step", "rt_launch_count", "rt_directions", "rt_ray_order", "rt_ray_slots", "rt_trace_ray",
-           "rt_bench_red_ceiling", "rt_strerror", "rt_version")
+           "rt_bench_red_ceiling", "rt_strerror", "rt_version", "rt_state_bytes", "rt_state_reset",
+           "rt_step_workspace_bytes", "rt_march_step")
 
 
 class RtError(RuntimeError):
@@ -59,6 +60,12 @@ def _load() -> ctypes.CDLL:
     L.rt_trace_ray.argtypes = [vp, vp, i, i, i, i, vp, i, i, f, i, vp, vp, vp, vp]
     L.rt_bench_red_ceiling.argtypes = [i, vp, i, i, i, i, ctypes.c_longlong, ctypes.c_uint,
                                        ctypes.POINTER(ctypes.c_longlong), vp]
+    L.rt_state_bytes.argtypes = [i, i, i]
+    L.rt_state_bytes.restype = sz
+    L.rt_state_reset.argtypes = [vp, i, i, i, vp]
+    L.rt_step_workspace_bytes.argtypes = [i] * 6
+    L.rt_step_workspace_bytes.restype = sz
+    L.rt_march_step.argtypes = [vp, vp, i, i, i, vp, i, i, i, f, f, f, ctypes.c_longlong, vp, vp, i, vp, sz, vp]
     L.rt_strerror.argtypes = [i]
     L.rt_strerror.restype = ctypes.c_char_p
     L.rt_version.restype = ctypes.c_char_p
@@ -179,6 +186,62 @@ def rt_march_single(j, kappa, source_pos, n_rays, step_size, c, dt, n_steps, out
                               workspace.numel(), _stream_ptr(stream))
     if rc != RT_OK:
         raise RtError(rc, "rt_march_single")
+    return out
+
+
+def rt_state_bytes(n_src: int, n_rays: int, n_bins: int) -> int:
+    return int(_lib.rt_state_bytes(n_src, n_rays, n_bins))
+
+
+def rt_step_workspace_bytes(nx, ny, nz, n_src, n_rays, n_bins) -> int:
+    return int(_lib.rt_step_workspace_bytes(nx, ny, nz, n_src, n_rays, n_bins))
+
+
+def rt_state_reset(n_src: int, n_rays: int, n_bins: int, state=None, stream=None):
+    """Fresh ray state (I = 0, exp(-tau) = 1): float32 [2, n_src, n_rays, n_bins] on the current device."""
+    torch = _torch()
+    if state is None:
+        state = torch.empty((2, n_src, n_rays, n_bins), dtype=torch.float32, device="cuda")
+    _check_dev(state, "state", torch.float32)
+    if state.numel() * 4 != rt_state_bytes(n_src, n_rays, n_bins):
+        raise ValueError("state has the wrong size")
+    rc = _lib.rt_state_reset(state.data_ptr(), n_src, n_rays, n_bins, _stream_ptr(stream))
+    if rc != RT_OK:
+        raise RtError(rc, "rt_state_reset")
+    return state
+
+
+def rt_march_step(j, kappa, sources, n_rays, step_size, c, dt, k_begin: int, state, out=None, accumulate=False,
+                  workspace=None, stream=None):
+    """One time step from substep ``k_begin`` in the medium (j, kappa); ``state`` is updated in place.  Returns
+    ``out`` [nx,ny,nz,n_bins]: the field deposited during the step (added to ``out`` when ``accumulate``)."""
+    torch = _torch()
+    _check_dev(j, "j", torch.float32, 4)
+    _check_dev(kappa, "kappa", torch.float32, 4)
+    _check_dev(sources, "sources", torch.float32, 2)
+    _check_dev(state, "state", torch.float32)
+    if kappa.shape != j.shape or sources.shape[1] != 3:
+        raise ValueError("kappa must have j's shape and sources must be [n_src, 3]")
+    nx, ny, nz, nb = j.shape
+    n_src = sources.shape[0]
+    if state.numel() * 4 != rt_state_bytes(n_src, n_rays, nb):
+        raise ValueError("state has the wrong size")
+    if out is None:
+        if accumulate:
+            raise ValueError("accumulate needs the running field in `out`")
+        out = torch.empty((nx, ny, nz, nb), dtype=torch.float32, device=j.device)
+    else:
+        _check_dev(out, "out", torch.float32)
+        if out.numel() != j.numel():
+            raise ValueError("out has the wrong size")
+    if workspace is None:
+        workspace = torch.empty(max(16, rt_step_workspace_bytes(nx, ny, nz, n_src, n_rays, nb)), dtype=torch.uint8,
+                                device=j.device)
+    rc = _lib.rt_march_step(j.data_ptr(), kappa.data_ptr(), nx, ny, nz, sources.data_ptr(), n_src, n_rays, nb,
+                            step_size, c, dt, int(k_begin), state.data_ptr(), out.data_ptr(), int(bool(accumulate)),
+                            workspace.data_ptr(), workspace.numel(), _stream_ptr(stream))
+    if rc != RT_OK:
+        raise RtError(rc, "rt_march_step")
     return out
 
 

@@ -95,7 +95,8 @@ int launch_march(const rt::MarchParams& P, bool sliding, cudaStream_t st) {
     if (sliding) {
         // registers: 1 bin per thread fits 6 blocks/SM (80 registers) without spilling; 4 bins need ~155
         constexpr int kMinBlocks = (NB == 1) ? 6 : 1;
-        rt::march_sliding_kernel<NB, ACC, kMinBlocks><<<g, rt::kThreads, 0, st>>>(P);
+        if (P.state_I) rt::march_sliding_kernel<NB, ACC, kMinBlocks, true><<<g, rt::kThreads, 0, st>>>(P);
+        else rt::march_sliding_kernel<NB, ACC, kMinBlocks, false><<<g, rt::kThreads, 0, st>>>(P);
     } else {
         rt::march_direct_kernel<NB, ACC><<<g, rt::kThreads, 0, st>>>(P);
     }
@@ -128,17 +129,32 @@ bool make_plan(int variant, int n_src, Plan* pl) {
     return true;
 }
 
+// rt_march_step: one time step from substep k0 with the ray state carried in `state`
+struct StepArgs {
+    float* state;
+    long long k0;
+    int accumulate;
+};
+
+size_t step_scratch_bytes(long long cells, int n_bins) { return (n_bins % 4 == 0) ? size_t(cells) * sizeof(float) : 0; }
+
 int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const float* sources, int n_src, int n_rays,
                int n_bins, float step_size, float c, float dt, int n_steps, float* out, void* workspace,
-               size_t workspace_bytes, void* stream, int variant) {
+               size_t workspace_bytes, void* stream, int variant, const StepArgs* step = nullptr) {
     Checked ck;
     const int rc = check_args(j, kappa, nx, ny, nz, sources, n_src, n_rays, n_bins, step_size, c, dt, n_steps, out, &ck);
     if (rc != RT_OK) return rc;
     Plan pl;
     if (!make_plan(variant, n_src, &pl)) return RT_EINVAL;
     const Workspace wl = workspace_layout(ck.cells, n_src, n_rays, n_steps);
-    if (!workspace || workspace_bytes < wl.total || (uintptr_t(workspace) & 15u)) return RT_EWORKSPACE;
+    const size_t need = wl.total + (step ? step_scratch_bytes(ck.cells, n_bins) : 0);
+    if (!workspace || workspace_bytes < need || (uintptr_t(workspace) & 15u)) return RT_EWORKSPACE;
     char* ws = static_cast<char*>(workspace);
+    if (step) {
+        if (!step->state || (uintptr_t(step->state) & 15u)) return RT_EINVAL;
+        const double last = double(step->k0) + double(ck.n_sub);
+        if (step->k0 < 0 || last > 2147483647.0 || last * double(step_size) > 268435456.0) return RT_EINVAL;
+    }
 
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     rt::MarchParams P;
@@ -151,6 +167,9 @@ int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const
     P.att_scale = float(-double(step_size) * 1.4426950408889634074);
     P.snap_stride = ck.cells;
     P.map_src = pl.map_src ? 1 : 0;
+    P.state_I = step ? step->state : nullptr;
+    P.state_T = step ? step->state + size_t(n_src) * size_t(n_rays) * size_t(n_bins) : nullptr;
+    P.k0 = step ? step->k0 : 0;
     if (pl.coherent) {
         P.ray_order = reinterpret_cast<const uint32_t*>(ws);
         P.n_slots = ray_slots(n_rays);
@@ -183,11 +202,13 @@ int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const
         // 4-bin kernel reduction bound.  So `out` is the fp32 scratch grid of ONE batch of sources (<= 2^18 rays:
         // no fp32 sum grows past a batch, which bounds the stagnation error), reduced into with
         // red.v4.f32 and folded into the fp64 grid after every batch.
+        // (rt_march_step may be accumulating into `out`: its scratch grid lives behind the fp64 grid instead)
+        float* scratch = step ? reinterpret_cast<float*>(ws + wl.total) : out;
         RT_CUDA(cudaMemsetAsync(master, 0, n_acc * sizeof(double), st));
-        RT_CUDA(cudaMemsetAsync(out, 0, n_acc * sizeof(float), st));                 // D14: overwrite
+        RT_CUDA(cudaMemsetAsync(scratch, 0, n_acc * sizeof(float), st));             // D14: overwrite
         int per_batch = int(std::max(1LL, (1LL << 18) / (long long)n_rays));
         if (pl.map_src) per_batch = (per_batch + 31) / 32 * 32;
-        P.acc = out;
+        P.acc = scratch;
         for (int s0 = 0; s0 < n_src; s0 += per_batch) {
             P.src_begin = s0;
             P.n_src = std::min(per_batch, n_src - s0);
@@ -195,10 +216,22 @@ int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const
             if (rcb != RT_OK) return rcb;
             long long db = ((long long)(n_acc / 4) + fin_threads - 1) / fin_threads;
             if (db > 148 * 16) db = 148 * 16;
-            rt::drain_kernel<<<unsigned(db), fin_threads, 0, st>>>(master, out, (long long)n_acc);
+            rt::drain_kernel<<<unsigned(db), fin_threads, 0, st>>>(master, scratch, (long long)n_acc);
             RT_CUDA(cudaGetLastError());
         }
-        rt::snapshot_finalize_kernel<double><<<unsigned(fin_blocks), fin_threads, 0, st>>>(master, out, ck.cells, n_steps);
+        if (step)
+            rt::step_finalize_kernel<<<unsigned(fin_blocks), fin_threads, 0, st>>>(master, out, ck.cells, step->accumulate);
+        else
+            rt::snapshot_finalize_kernel<double><<<unsigned(fin_blocks), fin_threads, 0, st>>>(master, out, ck.cells, n_steps);
+        RT_CUDA(cudaGetLastError());
+        return RT_OK;
+    }
+    if (step) {                        // 1 bin per thread: fp64 reductions into the workspace grid, then the update of out
+        P.acc = master;
+        RT_CUDA(cudaMemsetAsync(master, 0, n_acc * sizeof(double), st));
+        const int rcs = vec4 ? launch_march<4, double>(P, true, st) : launch_march<1, double>(P, true, st);
+        if (rcs != RT_OK) return rcs;
+        rt::step_finalize_kernel<<<unsigned(fin_blocks), fin_threads, 0, st>>>(master, out, ck.cells, step->accumulate);
         RT_CUDA(cudaGetLastError());
         return RT_OK;
     }
@@ -243,6 +276,34 @@ int rt_march_ex(const float* j, const float* kappa, int nx, int ny, int nz, cons
                 size_t workspace_bytes, void* stream, int variant) {
     return march_impl(j, kappa, nx, ny, nz, sources, n_src, n_rays, n_bins, step_size, c, dt, n_steps, out, workspace,
                       workspace_bytes, stream, variant);
+}
+
+size_t rt_state_bytes(int n_src, int n_rays, int n_bins) {
+    if (n_src < 1 || n_rays < 1 || n_bins < 1) return 0;
+    return size_t(2) * size_t(n_src) * size_t(n_rays) * size_t(n_bins) * sizeof(float);
+}
+
+int rt_state_reset(float* state, int n_src, int n_rays, int n_bins, void* stream) {
+    if (!state || n_src < 1 || n_rays < 1 || n_bins < 1) return RT_EINVAL;
+    const long long n = (long long)n_src * n_rays * n_bins;
+    long long blocks = (n + 255) / 256;
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    rt::state_reset_kernel<<<unsigned(blocks), 256, 0, static_cast<cudaStream_t>(stream)>>>(state, state + n, n);
+    RT_CUDA(cudaGetLastError());
+    return RT_OK;
+}
+
+size_t rt_step_workspace_bytes(int nx, int ny, int nz, int n_src, int n_rays, int n_bins) {
+    const size_t base = rt_workspace_bytes(nx, ny, nz, n_src, n_rays, n_bins, 1);
+    return base ? base + step_scratch_bytes((long long)nx * ny * nz * n_bins, n_bins) : 0;
+}
+
+int rt_march_step(const float* j, const float* kappa, int nx, int ny, int nz, const float* sources, int n_src,
+                  int n_rays, int n_bins, float step_size, float c, float dt, long long k_begin, float* state,
+                  float* out, int accumulate, void* workspace, size_t workspace_bytes, void* stream) {
+    const StepArgs sa{state, k_begin, accumulate};
+    return march_impl(j, kappa, nx, ny, nz, sources, n_src, n_rays, n_bins, step_size, c, dt, 1, out, workspace,
+                      workspace_bytes, stream, RT_VARIANT_DEFAULT, &sa);
 }
 
 int rt_march_host(const float* j, const float* kappa, int nx, int ny, int nz, const float* sources, int n_src,
@@ -328,6 +389,7 @@ int rt_trace_ray(const float* j, const float* kappa, int nx, int ny, int nz, int
     P.nx = nx; P.ny = ny; P.nz = nz; P.nb = n_bins;
     P.n_src = 1; P.src_begin = 0; P.n_rays = n_rays; P.n_slots = n_rays; P.n_groups = 1; P.n_steps = 1; P.n_sub = n_sub;
     P.ds = double(step_size); P.ds_f = step_size; P.emis = step_size; P.att_scale = 0.0f; P.snap_stride = 0;
+    P.state_I = nullptr; P.state_T = nullptr; P.k0 = 0;
     rt::trace_ray_kernel<<<1, 32, 0, static_cast<cudaStream_t>(stream)>>>(P, uint32_t(ray_index), n_sub, pos, trace_I,
                                                                          trace_T);
     RT_CUDA(cudaGetLastError());

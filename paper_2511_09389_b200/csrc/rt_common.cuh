@@ -28,6 +28,9 @@ struct MarchParams {
     float emis;                  // ds * 4 pi / N_Omega: emission quadrature weight times solid-angle weight (D8)
     float att_scale;             // -ds * log2(e): exp(-kappa ds) = 2^(kappa * att_scale)
     long long snap_stride;       // elements per snapshot
+    float* state_I;              // rt_march_step: carried I per (source, lattice index, bin), else nullptr
+    float* state_T;              //                carried exp(-tau), same layout
+    long long k0;                // substep index of the first substep of this launch (0 for rt_march)
 };
 
 constexpr uint32_t kPad = 0xFFFFFFFFu;
@@ -101,6 +104,16 @@ __device__ __forceinline__ void fx_add(Fx96& p, const Fx96& d) {
         "addc.s32 %2, %2, %5;"
         : "+r"(p.fl), "+r"(p.fh), "+r"(p.c)
         : "r"(d.fl), "r"(d.fh), "r"(d.c));
+}
+
+// p += k d, exact (k >= 0, the product stays far below 2^127: paths are limited to 2^28 cells)
+__device__ __forceinline__ void fx_advance(Fx96& p, const Fx96& d, long long k) {
+    const __int128 pp = (__int128(p.c) << 64) | (__int128(p.fh) << 32) | __int128(p.fl);
+    const __int128 dd = (__int128(d.c) << 64) | (__int128(d.fh) << 32) | __int128(d.fl);
+    const __int128 n = pp + dd * __int128(k);
+    p.c = int32_t(int64_t(n >> 64));
+    p.fh = uint32_t(uint64_t(n) >> 32);
+    p.fl = uint32_t(uint64_t(n));
 }
 
 // source coordinate a of source s, saturated to +-2^29 cells (rtmarch.h)

@@ -118,7 +118,8 @@ template <int NB, typename ACC> struct Stencil {
     }
 };
 
-template <int NB, typename ACC, int MINB>
+// STEP: the rt_march_step form -- start at substep P.k0 with (I, exp(-tau)) loaded from the ray state, store them back
+template <int NB, typename ACC, int MINB, bool STEP>
 __global__ void __launch_bounds__(kThreads, MINB) march_sliding_kernel(const MarchParams P) {
     RayId id;
     if (!ray_id(P, id)) return;
@@ -136,6 +137,7 @@ __global__ void __launch_bounds__(kThreads, MINB) march_sliding_kernel(const Mar
             A[a].p = fx_from_double(source_coord(P, id.src, a), neg ? kFxComplement : kFxPlain);
             A[a].d = fx_from_double(__dmul_rn(P.ds, nh[a]), neg ? kFxNegate : kFxPlain);
             A[a].sg = neg ? -1 : 1;
+            if (STEP) fx_advance(A[a].p, A[a].d, P.k0);      // x_k0 = x_0 + k0 ds n
         }
     }
     Stencil<NB, ACC> S;
@@ -146,6 +148,12 @@ __global__ void __launch_bounds__(kThreads, MINB) march_sliding_kernel(const Mar
     float I[NB], T[NB], att[NB];     // I scaled by 4 pi/N_Omega; T = exp(-tau); att = exp(-kappa ds) of the kappa cell
 #pragma unroll
     for (int b = 0; b < NB; ++b) { I[b] = 0.0f; T[b] = 1.0f; }
+    const size_t state_at = (size_t(id.src) * P.n_rays + id.index) * P.nb + size_t(id.group) * NB;
+    if (STEP) {                        // the ray's (I, exp(-tau)) carried from the previous call
+        const BinVec<NB> si = ld_bins<NB>(P.state_I + state_at), sT = ld_bins<NB>(P.state_T + state_at);
+#pragma unroll
+        for (int b = 0; b < NB; ++b) { I[b] = si.v[b]; T[b] = sT.v[b]; }
+    }
     // kappa: nearest neighbour at clamp(floor(x_k)) (D4) = trailing index, leading on descending axes
     auto load_att = [&]() {
         const int ko = S.off[0] + (A[0].dl & (A[0].sg >> 1)) + (A[1].dl & (A[1].sg >> 1)) + (A[2].dl & (A[2].sg >> 1));
@@ -211,6 +219,13 @@ __global__ void __launch_bounds__(kThreads, MINB) march_sliding_kernel(const Mar
         }
         S.flush_all(og);       // time-step boundary: the increments of step m are complete (rays continue, D7)
         og += P.snap_stride;
+    }
+    if (STEP) {
+#pragma unroll
+        for (int b = 0; b < NB; ++b) {
+            P.state_I[state_at + b] = I[b];
+            P.state_T[state_at + b] = T[b];
+        }
     }
 }
 

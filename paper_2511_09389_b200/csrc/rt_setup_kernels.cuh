@@ -97,5 +97,19 @@ __global__ void drain_kernel(double* master, float* scratch, long long n) {
     }
 }
 
+// rt_march_step: out = (accumulate ? out : 0) + float(increment), increment summed in fp64
+__global__ void step_finalize_kernel(const double* master, float* out, long long n, int accumulate) {
+    for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < n; e += (long long)gridDim.x * blockDim.x)
+        out[e] = float((accumulate ? double(out[e]) : 0.0) + master[e]);
+}
+
+// fresh ray state: I = 0, exp(-tau) = 1 (D11)
+__global__ void state_reset_kernel(float* state_I, float* state_T, long long n) {
+    for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < n; e += (long long)gridDim.x * blockDim.x) {
+        state_I[e] = 0.0f;
+        state_T[e] = 1.0f;
+    }
+}
+
 }  // namespace rt
 

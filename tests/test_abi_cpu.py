@@ -100,6 +100,11 @@ def test_argument_errors_are_caught_before_cuda(rt):
     assert L.rt_march_ex(p, p, 8, 8, 8, p, 1, 16, 1, 0.5, 1.0, 2.0, 1, p, p, 1 << 20, None, 7) == rt.RT_EINVAL
     assert L.rt_march_ex(p, p, 8, 8, 8, p, 1, 16, 1, 0.5, 1.0, 2.0, 1, p, p, 1 << 20, None, 128) == rt.RT_EINVAL
     assert L.rt_bench_red_ceiling(9, p, 8, 8, 8, 1, 100, 1, None, None) == rt.RT_EINVAL
+    assert L.rt_march_step(p, p, 8, 8, 8, p, 1, 16, 1, 0.5, 1.0, 2.0, 0, None, p, 0, p, 1 << 20, None) == rt.RT_EINVAL
+    assert L.rt_march_step(p, p, 8, 8, 8, p, 1, 16, 1, 0.5, 1.0, 2.0, 1 << 40, p, p, 0, p, 1 << 20, None) == rt.RT_EINVAL
+    assert L.rt_march_step(p, p, 8, 8, 8, p, 1, 16, 1, 0.5, 1.0, 2.0, 0, p, p, 0, p, 64, None) == rt.RT_EWORKSPACE
+    assert L.rt_state_reset(None, 1, 1, 1, None) == rt.RT_EINVAL
+    assert rt.rt_state_bytes(2, 3, 4) == 2 * 2 * 3 * 4 * 4 and rt.rt_state_bytes(0, 3, 4) == 0
     assert L.rt_directions(0, p, None) == rt.RT_EINVAL
     assert L.rt_ray_order(16, None, None) == rt.RT_EINVAL
 
