@@ -41,6 +41,9 @@ def parse():
     ap.add_argument("--config", default="C2", choices=["C0", "C1", "C2", "C3", "C4"])
     ap.add_argument("--impl", default="native", choices=["native", "reference"])
     ap.add_argument("--variant", type=int, default=0, help="RT_VARIANT_* (0 = the product path)")
+    ap.add_argument("--mode", default="march", choices=["march", "step"],
+                    help="march: one rt_march call per bench step (the headline); step: the same workload as n_steps "
+                         "rt_march_step calls with persistent ray state (DESIGN.md D17)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target host time of the oracle sample")
@@ -228,9 +231,21 @@ def run_native(args):
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB L2
     units_per_gpu = src.shape[0] * w.n_rays * w.n_steps * w.substeps_per_step * nb
 
+    if args.mode == "step":
+        state = rt.rt_state_reset(src.shape[0], w.n_rays, nb)
+        ws_step = torch.empty(max(16, rt.rt_step_workspace_bytes(nx, ny, nz, src.shape[0], w.n_rays, nb)),
+                              dtype=torch.uint8, device="cuda")
+
     def step():
-        rt.rt_march_ex(j, kappa, src, w.n_rays, w.step_size, w.c, w.dt, w.n_steps, out=out, workspace=ws,
-                       variant=args.variant)
+        if args.mode == "step":        # n_steps calls, the field of the last snapshot accumulated in out[-1]
+            rt.rt_state_reset(src.shape[0], w.n_rays, nb, state=state)
+            out[-1].zero_()
+            for m in range(w.n_steps):
+                rt.rt_march_step(j, kappa, src, w.n_rays, w.step_size, w.c, w.dt, m * w.substeps_per_step, state,
+                                 out=out[-1], accumulate=True, workspace=ws_step)
+        else:
+            rt.rt_march_ex(j, kappa, src, w.n_rays, w.step_size, w.c, w.dt, w.n_steps, out=out, workspace=ws,
+                           variant=args.variant)
         if world > 1:
             sharding.allreduce_field(out)
 
@@ -271,13 +286,13 @@ def run_native(args):
 
     line = None
     if rank == 0:
-        field_sum = float(out.double().sum().item())
+        field_sum = float((out[-1] if args.mode == "step" else out).double().sum().item())
         launches = rt.rt_launch_count(int(src.shape[0]), w.n_rays, nb, w.n_steps)
         cfg = describe(w, world)
         cfg["workload"] = cfg["workload"].replace(f"{w.n_src} sources/GPU", f"{n_src_per_gpu} sources/GPU")
         cfg.update({"timing": "CUDA events per step on the launch stream; 256 MiB L2 flush (memset) between "
                               "timed steps, outside the event pairs; inputs resident in HBM",
-                    "kernel_variant": args.variant, "field_checksum": field_sum})
+                    "kernel_variant": args.variant, "mode": args.mode, "field_checksum": field_sum})
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": 1e3 * total_s / args.steps, "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": cfg,
