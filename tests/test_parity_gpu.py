@@ -218,6 +218,33 @@ def test_out_is_overwritten_and_call_is_repeatable(rt, oracle_mod):
     parity.assert_parity(out.cpu().numpy(), oracle_march(oracle_mod, w), "repeat")
 
 
+@pytest.mark.parametrize("nb,n_src", [(1, 3), (1, 40), (4, 40), (8, 2), (3, 33)])
+def test_nothing_is_written_outside_out_workspace_and_state(rt, nb, n_src):
+    """Guard bands around every buffer the library writes (compute-sanitizer is closed on this pool): out, the
+    workspace and the ray state sit inside larger allocations whose margins must come back untouched."""
+    shape, n_rays, ds, dt, n_steps, g = (9, 7, 6), 21, 0.5, 4.0, 3, 4096
+    j, k = _random_medium(shape, nb, seed=nb + n_src)
+    src = np.random.default_rng(n_src).uniform(-3.0, 12.0, (n_src, 3)).astype(np.float32)
+    dj, dk, dsrc = _dev(j), _dev(k), _dev(src)
+    n_out = n_steps * j.size
+    obuf = torch.full((n_out + 2 * g,), 12345.0, device="cuda")
+    wbytes = max(rt.rt_workspace_bytes(*shape, n_src, n_rays, nb, n_steps), rt.rt_step_workspace_bytes(*shape, n_src, n_rays, nb))
+    wbuf = torch.full((wbytes + 2 * g,), 0xAB, dtype=torch.uint8, device="cuda")
+    sfl = rt.rt_state_bytes(n_src, n_rays, nb) // 4
+    sbuf = torch.full((sfl + 2 * g,), 777.0, device="cuda")
+    out, ws, state = obuf[g:g + n_out], wbuf[g:g + wbytes], sbuf[g:g + sfl]
+    for variant in (0, 1, 4, 5, 16, 32):
+        rt.rt_march_ex(dj, dk, dsrc, n_rays, ds, 1.0, dt, n_steps, out=out, workspace=ws, variant=variant)
+    rt.rt_state_reset(n_src, n_rays, nb, state=state)
+    for m in range(2):
+        rt.rt_march_step(dj, dk, dsrc, n_rays, ds, 1.0, dt, m * 8, state, out=out[:j.size], accumulate=bool(m), workspace=ws)
+    torch.cuda.synchronize()
+    assert (obuf[:g] == 12345.0).all() and (obuf[g + n_out:] == 12345.0).all()
+    assert (wbuf[:g] == 0xAB).all() and (wbuf[g + wbytes:] == 0xAB).all()
+    assert (sbuf[:g] == 777.0).all() and (sbuf[g + sfl:] == 777.0).all()
+    assert torch.isfinite(out).all() and torch.isfinite(state).all()
+
+
 def test_runs_on_a_side_stream(rt, oracle_mod):
     w = config("C0")
     st = torch.cuda.Stream()
