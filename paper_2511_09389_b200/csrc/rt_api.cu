@@ -93,8 +93,8 @@ int launch_march(const rt::MarchParams& P, bool sliding, cudaStream_t st) {
     if (blocks > 2147483647LL) return RT_EINVAL;
     const unsigned g = unsigned(blocks);
     if (sliding) {
-        // registers: 1 bin per thread fits 6 blocks/SM (80 registers) without spilling; 4 bins need ~155
-        constexpr int kMinBlocks = (NB == 1) ? 6 : 1;
+        // registers: 1 bin per thread runs 8 blocks/SM (64 registers, 16 bytes spilled); 4 bins need ~150
+        constexpr int kMinBlocks = (NB == 1) ? 8 : 1;
         if (P.state_I) rt::march_sliding_kernel<NB, ACC, kMinBlocks, true><<<g, rt::kThreads, 0, st>>>(P);
         else rt::march_sliding_kernel<NB, ACC, kMinBlocks, false><<<g, rt::kThreads, 0, st>>>(P);
     } else {

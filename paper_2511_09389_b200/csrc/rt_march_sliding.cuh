@@ -40,81 +40,91 @@ __device__ __forceinline__ float ex2_approx(float x) {
 
 struct TravelAxis {
     Fx96 p, d;          // position and per-substep increment in travel coordinates (d >= 0)
-    int t, dl;          // element offset of the trailing index; leading minus trailing offset (0 = merged)
-    int sg;             // +1 ascending, -1 descending
+    int dl;             // leading minus trailing element offset of this axis (0 = merged)
     uint32_t fmask;     // 0 while merged (dl == 0), else all ones
 };
 
-// element offset of u-cell c of axis AX (array index c or -c, clamped to the domain: PAPER.md:29)
-template <int AX> __device__ __forceinline__ int eoff(const MarchParams& P, int c, int sg) {
+// element offset of u-cell c of axis AX (array index c, or -c on a descending axis, clamped: PAPER.md:29)
+template <int AX> __device__ __forceinline__ int eoff(const MarchParams& P, int c, int negbits) {
     const int lim = (AX == 0 ? P.nx : (AX == 1 ? P.ny : P.nz)) - 1;
     const int stride = AX == 0 ? P.ny * P.nz * P.nb : (AX == 1 ? P.nz * P.nb : P.nb);
-    return min(max(c * sg, 0), lim) * stride;
+    const int idx = (negbits & (1 << AX)) ? -c : c;
+    return min(max(idx, 0), lim) * stride;
 }
 
+// The stencil: 8 register slots [x][y][z], 0 = trailing / 1 = leading per axis.  Slot s sits at element offset
+// base + (s&4 ? dl_x : 0) + (s&2 ? dl_y : 0) + (s&1 ? dl_z : 0); base includes the thread's bin offset.
 template <int NB, typename ACC> struct Stencil {
     BinVec<NB> acc[8];   // pending deposits for the 8 stencil voxels
     BinVec<NB> jc[8];    // j at the 8 stencil voxels
-    int off[8];          // their element offsets
+    int base;            // element offset of slot 0
 
-    __device__ __forceinline__ void flush_slot(ACC* og, int s) {
-        if (any_nonzero<NB>(acc[s])) red_bins(og + off[s], acc[s]);
+    __device__ __forceinline__ int off(int s, const TravelAxis (&A)[3]) const {
+        return base + ((s & 4) ? A[0].dl : 0) + ((s & 2) ? A[1].dl : 0) + ((s & 1) ? A[2].dl : 0);
+    }
+    __device__ __forceinline__ void flush_slot(ACC* og, int s, const TravelAxis (&A)[3]) {
+        if (any_nonzero<NB>(acc[s])) red_bins(og + off(s, A), acc[s]);
     }
     __device__ __forceinline__ void zero_slot(int s) {
 #pragma unroll
         for (int b = 0; b < NB; ++b) acc[s].v[b] = 0.0f;
     }
-    __device__ __forceinline__ void flush_all(ACC* og) {
+    __device__ __forceinline__ void flush_all(ACC* og, const TravelAxis (&A)[3]) {
 #pragma unroll
         for (int s = 0; s < 8; ++s) {
-            flush_slot(og, s);
+            flush_slot(og, s, A);
             zero_slot(s);
         }
     }
-    template <int AX> __device__ __forceinline__ void place(const MarchParams& P, TravelAxis& A) {
-        A.t = eoff<AX>(P, A.p.c, A.sg);
-        A.dl = eoff<AX>(P, A.p.c + 1, A.sg) - A.t;
-        A.fmask = A.dl ? 0xFFFFFFFFu : 0u;
+    template <int AX> __device__ __forceinline__ int place(const MarchParams& P, TravelAxis& X, int negbits) {
+        const int t = eoff<AX>(P, X.p.c, negbits);
+        X.dl = eoff<AX>(P, X.p.c + 1, negbits) - t;
+        X.fmask = X.dl ? 0xFFFFFFFFu : 0u;
+        return t;
     }
     // (re)build the stencil at the axes' current cells; pending deposits must have been flushed
-    __device__ __forceinline__ void restart(const MarchParams& P, TravelAxis (&A)[3], const float* jg) {
-        place<0>(P, A[0]);
-        place<1>(P, A[1]);
-        place<2>(P, A[2]);
+    __device__ __forceinline__ void restart(const MarchParams& P, TravelAxis (&A)[3], int negbits, int bin_off) {
+        base = bin_off + place<0>(P, A[0], negbits) + place<1>(P, A[1], negbits) + place<2>(P, A[2], negbits);
 #pragma unroll
-        for (int s = 0; s < 8; ++s) {
-            off[s] = A[0].t + A[1].t + A[2].t + ((s & 4) ? A[0].dl : 0) + ((s & 2) ? A[1].dl : 0) +
-                     ((s & 1) ? A[2].dl : 0);
-            jc[s] = ld_bins<NB>(jg + off[s]);
-        }
+        for (int s = 0; s < 8; ++s) jc[s] = ld_bins<NB>(P.j + off(s, A));
     }
     // Axis AX advanced by one cell.  The old leading plane is the new trailing plane (also under clamping: both
     // are clamp(c+1)), so the trailing index moves iff the axis was not merged; the new leading index is looked up.
     template <int AX>
-    __device__ __forceinline__ void axis_step(const MarchParams& P, TravelAxis& A, ACC* og, const float* jg) {
-        const int tn = A.t + A.dl;
-        const int dln = eoff<AX>(P, A.p.c + 1, A.sg) - tn;
-        const bool move = (A.dl != 0), load = (dln != 0);
-        if (move | load) {
+    __device__ __forceinline__ void axis_step(const MarchParams& P, TravelAxis (&A)[3], int negbits, ACC* og) {
+        TravelAxis& X = A[AX];
+        // new leading minus new trailing offset: +-stride while both indices are inside the domain, i.e. u-cell
+        // c in [0, lim-1] (ascending: indices c, c+1) or [-lim, -1] (descending: indices -c, -c-1); else 0
+        const int lim = (AX == 0 ? P.nx : (AX == 1 ? P.ny : P.nz)) - 1;
+        const int stride = AX == 0 ? P.ny * P.nz * P.nb : (AX == 1 ? P.nz * P.nb : P.nb);
+        const bool neg = (negbits & (1 << AX)) != 0;
+        const bool inside = uint32_t(X.p.c + (neg ? lim : 0)) < uint32_t(lim);
+        const int dln = inside ? (neg ? -stride : stride) : 0;
+        const bool move = (X.dl != 0), load = inside;
+        if (move) {
 #pragma unroll
             for (int u = 0; u < 2; ++u)
 #pragma unroll
                 for (int v = 0; v < 2; ++v) {
                     const int s0 = slot<AX>(0, u, v), s1 = slot<AX>(1, u, v);
-                    if (move) {
-                        flush_slot(og, s0);
-                        acc[s0] = acc[s1];
-                        jc[s0] = jc[s1];
-                        off[s0] = off[s1];
-                        zero_slot(s1);
-                    }
-                    off[s1] = off[s0] + dln;
-                    if (load) jc[s1] = ld_bins<NB>(jg + off[s1]);
+                    flush_slot(og, s0, A);
+                    acc[s0] = acc[s1];
+                    jc[s0] = jc[s1];
+                    zero_slot(s1);
                 }
         }
-        A.t = tn;
-        A.dl = dln;
-        A.fmask = dln ? 0xFFFFFFFFu : 0u;
+        base += X.dl;                 // the trailing index becomes the old leading one (dl = 0 when nothing moved)
+        X.dl = dln;
+        X.fmask = inside ? 0xFFFFFFFFu : 0u;
+        if (load) {
+#pragma unroll
+            for (int u = 0; u < 2; ++u)
+#pragma unroll
+                for (int v = 0; v < 2; ++v) {
+                    const int s1 = slot<AX>(1, u, v);
+                    jc[s1] = ld_bins<NB>(P.j + off(s1, A));
+                }
+        }
     }
 };
 
@@ -123,11 +133,10 @@ template <int NB, typename ACC, int MINB, bool STEP>
 __global__ void __launch_bounds__(kThreads, MINB) march_sliding_kernel(const MarchParams P) {
     RayId id;
     if (!ray_id(P, id)) return;
-    const float* jg = P.j + id.group * NB;
-    const float* kg = P.kappa + id.group * NB;
-    ACC* og = static_cast<ACC*>(P.acc) + id.group * NB;
+    ACC* og = static_cast<ACC*>(P.acc);      // the bin offset id.group * NB rides in the stencil's base offset
 
     TravelAxis A[3];
+    int negbits = 0;                         // bit a: the ray descends axis a
     {
         double nh[3];
         fib_direction(id.index, uint32_t(P.n_rays), nh);
@@ -136,14 +145,14 @@ __global__ void __launch_bounds__(kThreads, MINB) march_sliding_kernel(const Mar
             const bool neg = nh[a] < 0.0;
             A[a].p = fx_from_double(source_coord(P, id.src, a), neg ? kFxComplement : kFxPlain);
             A[a].d = fx_from_double(__dmul_rn(P.ds, nh[a]), neg ? kFxNegate : kFxPlain);
-            A[a].sg = neg ? -1 : 1;
+            negbits |= neg ? (1 << a) : 0;
             if (STEP) fx_advance(A[a].p, A[a].d, P.k0);      // x_k0 = x_0 + k0 ds n
         }
     }
     Stencil<NB, ACC> S;
 #pragma unroll
     for (int s = 0; s < 8; ++s) S.zero_slot(s);
-    S.restart(P, A, jg);
+    S.restart(P, A, negbits, id.group * NB);
 
     float I[NB], T[NB], att[NB];     // I scaled by 4 pi/N_Omega; T = exp(-tau); att = exp(-kappa ds) of the kappa cell
 #pragma unroll
@@ -156,8 +165,8 @@ __global__ void __launch_bounds__(kThreads, MINB) march_sliding_kernel(const Mar
     }
     // kappa: nearest neighbour at clamp(floor(x_k)) (D4) = trailing index, leading on descending axes
     auto load_att = [&]() {
-        const int ko = S.off[0] + (A[0].dl & (A[0].sg >> 1)) + (A[1].dl & (A[1].sg >> 1)) + (A[2].dl & (A[2].sg >> 1));
-        const BinVec<NB> kap = ld_bins<NB>(kg + ko);
+        const int ko = S.base + ((negbits & 1) ? A[0].dl : 0) + ((negbits & 2) ? A[1].dl : 0) + ((negbits & 4) ? A[2].dl : 0);
+        const BinVec<NB> kap = ld_bins<NB>(P.kappa + ko);
 #pragma unroll
         for (int b = 0; b < NB; ++b) att[b] = ex2_approx(kap.v[b] * P.att_scale);
     };
@@ -207,17 +216,17 @@ __global__ void __launch_bounds__(kThreads, MINB) march_sliding_kernel(const Mar
             for (int a = 0; a < 3; ++a) fx_add(A[a].p, A[a].d);
             if ((c0 ^ A[0].p.c) | (c1 ^ A[1].p.c) | (c2 ^ A[2].p.c)) {
                 if (long_steps && (((A[0].p.c - c0) | (A[1].p.c - c1) | (A[2].p.c - c2)) > 1)) {
-                    S.flush_all(og);               // a step longer than a cell: restart the stencil
-                    S.restart(P, A, jg);
+                    S.flush_all(og, A);            // a step longer than a cell: restart the stencil
+                    S.restart(P, A, negbits, id.group * NB);
                 } else {
-                    if (c0 != A[0].p.c) S.template axis_step<0>(P, A[0], og, jg);
-                    if (c1 != A[1].p.c) S.template axis_step<1>(P, A[1], og, jg);
-                    if (c2 != A[2].p.c) S.template axis_step<2>(P, A[2], og, jg);
+                    if (c0 != A[0].p.c) S.template axis_step<0>(P, A, negbits, og);
+                    if (c1 != A[1].p.c) S.template axis_step<1>(P, A, negbits, og);
+                    if (c2 != A[2].p.c) S.template axis_step<2>(P, A, negbits, og);
                 }
                 load_att();
             }
         }
-        S.flush_all(og);       // time-step boundary: the increments of step m are complete (rays continue, D7)
+        S.flush_all(og, A);    // time-step boundary: the increments of step m are complete (rays continue, D7)
         og += P.snap_stride;
     }
     if (STEP) {
