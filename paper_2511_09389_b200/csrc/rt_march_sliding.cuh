@@ -149,6 +149,7 @@ __global__ void __launch_bounds__(kThreads, MINB) march_sliding_kernel(const Mar
             if (STEP) fx_advance(A[a].p, A[a].d, P.k0);      // x_k0 = x_0 + k0 ds n
         }
     }
+    asm volatile("" : "+r"(negbits));        // opaque: keeps ptxas from re-deriving the signs with fp64 compares
     Stencil<NB, ACC> S;
 #pragma unroll
     for (int s = 0; s < 8; ++s) S.zero_slot(s);
