@@ -455,6 +455,6 @@ const char* rt_strerror(int code) {
     }
 }
 
-const char* rt_version(void) { return "rtmarch 0.3 (sm_100a; sliding-stencil RED march, 32 sources x 1 direction per warp, fp64 accumulation grid)"; }
+const char* rt_version(void) { return "rtmarch 0.4 (sm_100a; sliding-stencil RED march, 32 sources x 1 direction per warp, fp64 accumulation grid)"; }
 
 }  // extern "C"
