@@ -287,7 +287,7 @@ def run_native(args):
     line = None
     if rank == 0:
         field_sum = float((out[-1] if args.mode == "step" else out).double().sum().item())
-        launches = rt.rt_launch_count(int(src.shape[0]), w.n_rays, nb, w.n_steps)
+        launches = rt.rt_launch_count(nx, ny, nz, int(src.shape[0]), w.n_rays, nb, w.n_steps)
         cfg = describe(w, world)
         cfg["workload"] = cfg["workload"].replace(f"{w.n_src} sources/GPU", f"{n_src_per_gpu} sources/GPU")
         cfg.update({"timing": "CUDA events per step on the launch stream; 256 MiB L2 flush (memset) between "

@@ -118,7 +118,7 @@ size_t rt_workspace_bytes(int nx, int ny, int nz, int n_src, int n_rays, int n_b
 int rt_substeps_per_step(float step_size, float c, float dt);
 
 /* Number of kernels of this library that one rt_march call with these arguments enqueues (memsets excluded). */
-int rt_launch_count(int n_src, int n_rays, int n_bins, int n_steps);
+int rt_launch_count(int nx, int ny, int nz, int n_src, int n_rays, int n_bins, int n_steps);
 
 /* TEST HOOK.  Writes the library's direction lattice (D1) for i = 0..n_rays-1 into
  * nhat[n_rays][3] (float64, device), computed exactly as the march kernel does. */

@@ -53,7 +53,7 @@ def _load() -> ctypes.CDLL:
     L.rt_workspace_bytes.argtypes = [i] * 7
     L.rt_workspace_bytes.restype = sz
     L.rt_substeps_per_step.argtypes = [f, f, f]
-    L.rt_launch_count.argtypes = [i, i, i, i]
+    L.rt_launch_count.argtypes = [i] * 7
     L.rt_directions.argtypes = [i, vp, vp]
     L.rt_ray_order.argtypes = [i, vp, vp]
     L.rt_ray_slots.argtypes = [i]
@@ -97,8 +97,8 @@ def rt_workspace_bytes(nx, ny, nz, n_src, n_rays, n_bins, n_steps) -> int:
     return int(_lib.rt_workspace_bytes(nx, ny, nz, n_src, n_rays, n_bins, n_steps))
 
 
-def rt_launch_count(n_src: int, n_rays: int, n_bins: int, n_steps: int) -> int:
-    return int(_lib.rt_launch_count(n_src, n_rays, n_bins, n_steps))
+def rt_launch_count(nx, ny, nz, n_src: int, n_rays: int, n_bins: int, n_steps: int) -> int:
+    return int(_lib.rt_launch_count(nx, ny, nz, n_src, n_rays, n_bins, n_steps))
 
 
 def rt_ray_slots(n_rays: int) -> int:

@@ -114,6 +114,27 @@ int build_ray_order(int n_rays, uint32_t* order, cudaStream_t st) {
 
 constexpr int kMaxSortedSources = 65536;   // above this the O(n^2) source sort is skipped (identity order)
 
+// The batched fp32 path (4-bin kernels): a batch is a range of sources x a range of direction slots holding at most
+// 2^17 rays; the batches' fp32 sums are folded into the fp64 grid one by one.  It is used when the fp32 scratch
+// grid is small enough for the drains to be cheap; larger grids take the 1-bin kernel with fp64 reductions.
+constexpr long long kBatchRays = 1LL << 17;
+constexpr size_t kBatchedScratchLimit = size_t(256) << 20;
+struct Batching {
+    int src_per_batch, slots_per_batch;
+};
+Batching plan_batches(int n_src, int n_slots, bool map_src) {
+    Batching b;
+    if (map_src) b.src_per_batch = int(32 * std::max(1LL, kBatchRays / (32LL * n_slots)));
+    else b.src_per_batch = int(std::max(1LL, kBatchRays / (long long)n_slots));
+    b.src_per_batch = std::min(b.src_per_batch, map_src ? (n_src + 31) / 32 * 32 : n_src);
+    long long sl = std::max(128LL, kBatchRays / b.src_per_batch) / 128 * 128;      // whole blocks of slots
+    b.slots_per_batch = int(std::min<long long>(sl, n_slots));
+    return b;
+}
+bool use_batched_fp32(long long cells, int n_steps, int n_bins) {
+    return n_bins % 4 == 0 && size_t(cells) * size_t(n_steps) * sizeof(float) <= kBatchedScratchLimit;
+}
+
 // what a variant code means (rtmarch.h RT_VARIANT_*)
 struct Plan {
     bool sliding, coherent, map_src, acc64, one_bin;
@@ -136,7 +157,9 @@ struct StepArgs {
     int accumulate;
 };
 
-size_t step_scratch_bytes(long long cells, int n_bins) { return (n_bins % 4 == 0) ? size_t(cells) * sizeof(float) : 0; }
+size_t step_scratch_bytes(long long cells, int n_bins) {
+    return use_batched_fp32(cells, 1, n_bins) ? size_t(cells) * sizeof(float) : 0;
+}
 
 int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const float* sources, int n_src, int n_rays,
                int n_bins, float step_size, float c, float dt, int n_steps, float* out, void* workspace,
@@ -160,7 +183,7 @@ int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const
     rt::MarchParams P;
     P.j = j; P.kappa = kappa; P.sources = sources;
     P.nx = nx; P.ny = ny; P.nz = nz; P.nb = n_bins;
-    P.n_src = n_src; P.src_begin = 0; P.n_rays = n_rays;
+    P.n_src = n_src; P.src_begin = 0; P.slot_begin = 0; P.n_rays = n_rays;
     P.n_steps = n_steps; P.n_sub = int(ck.n_sub);
     P.ds = double(step_size); P.ds_f = step_size;
     P.emis = float(double(step_size) * 4.0 * 3.14159265358979323846 / double(n_rays));
@@ -193,32 +216,38 @@ int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const
     long long fin_blocks = (ck.cells + fin_threads - 1) / fin_threads;
     if (fin_blocks > 148 * 16) fin_blocks = 148 * 16;
 
-    // 4 bins per thread with 16-byte loads and 16-byte fp32 reductions when the layout allows it
-    const bool vec4 = (n_bins % 4 == 0) && !pl.one_bin && !((uintptr_t(j) | uintptr_t(kappa) | uintptr_t(out)) & 15u);
+    // 4 bins per thread (16-byte loads, 16-byte fp32 reductions) when the layout allows it -- and, with fp64
+    // accumulation, only on the batched path: there is no 16-byte fp64 reduction, and four scalar ones per voxel
+    // make the 4-bin kernel reduction bound, so larger grids march one bin per thread (bins in adjacent lanes
+    // share the sectors of their fp64 reductions)
+    const bool aligned4 = (n_bins % 4 == 0) && !((uintptr_t(j) | uintptr_t(kappa) | uintptr_t(out)) & 15u);
+    const bool batched = aligned4 && !pl.one_bin && pl.acc64 && pl.sliding && use_batched_fp32(ck.cells, n_steps, n_bins);
+    const bool vec4 = aligned4 && !pl.one_bin && (batched || !pl.acc64 || !pl.sliding);
     P.n_groups = vec4 ? n_bins / 4 : n_bins;
 
-    if (vec4 && pl.acc64 && pl.sliding) {
-        // Batched fp32: there is no 16-byte fp64 reduction, and four scalar fp64 reductions per voxel make the
-        // 4-bin kernel reduction bound.  So `out` is the fp32 scratch grid of ONE batch of sources (<= 2^18 rays:
-        // no fp32 sum grows past a batch, which bounds the stagnation error), reduced into with
-        // red.v4.f32 and folded into the fp64 grid after every batch.
-        // (rt_march_step may be accumulating into `out`: its scratch grid lives behind the fp64 grid instead)
+    if (batched) {
+        // `out` (rt_march_step: a grid behind the fp64 grid, it may be accumulating into out) is the fp32 scratch
+        // grid of ONE batch: no fp32 sum ever holds more than 2^17 rays, which bounds the error of fp32
+        // accumulation; after every batch drain_kernel folds it into the fp64 grid and zeroes it.
         float* scratch = step ? reinterpret_cast<float*>(ws + wl.total) : out;
         RT_CUDA(cudaMemsetAsync(master, 0, n_acc * sizeof(double), st));
         RT_CUDA(cudaMemsetAsync(scratch, 0, n_acc * sizeof(float), st));             // D14: overwrite
-        int per_batch = int(std::max(1LL, (1LL << 18) / (long long)n_rays));
-        if (pl.map_src) per_batch = (per_batch + 31) / 32 * 32;
+        const Batching bt = plan_batches(n_src, P.n_slots, pl.map_src);
+        const int all_slots = P.n_slots;
         P.acc = scratch;
-        for (int s0 = 0; s0 < n_src; s0 += per_batch) {
-            P.src_begin = s0;
-            P.n_src = std::min(per_batch, n_src - s0);
-            const int rcb = launch_march<4, float>(P, true, st);
-            if (rcb != RT_OK) return rcb;
-            long long db = ((long long)(n_acc / 4) + fin_threads - 1) / fin_threads;
-            if (db > 148 * 16) db = 148 * 16;
-            rt::drain_kernel<<<unsigned(db), fin_threads, 0, st>>>(master, scratch, (long long)n_acc);
-            RT_CUDA(cudaGetLastError());
-        }
+        long long db = ((long long)(n_acc / 4) + fin_threads - 1) / fin_threads;
+        if (db > 148 * 16) db = 148 * 16;
+        for (int s0 = 0; s0 < n_src; s0 += bt.src_per_batch)
+            for (int d0 = 0; d0 < all_slots; d0 += bt.slots_per_batch) {
+                P.src_begin = s0;
+                P.n_src = std::min(bt.src_per_batch, n_src - s0);
+                P.slot_begin = d0;
+                P.n_slots = std::min(bt.slots_per_batch, all_slots - d0);
+                const int rcb = launch_march<4, float>(P, true, st);
+                if (rcb != RT_OK) return rcb;
+                rt::drain_kernel<<<unsigned(db), fin_threads, 0, st>>>(master, scratch, (long long)n_acc);
+                RT_CUDA(cudaGetLastError());
+            }
         if (step)
             rt::step_finalize_kernel<<<unsigned(fin_blocks), fin_threads, 0, st>>>(master, out, ck.cells, step->accumulate);
         else
@@ -356,15 +385,17 @@ int rt_substeps_per_step(float step_size, float c, float dt) {
     return ns < 1 ? RT_EINVAL : int(ns);
 }
 
-int rt_launch_count(int n_src, int n_rays, int n_bins, int n_steps) {
-    if (n_src < 1 || n_rays < 1 || n_bins < 1 || n_steps < 1) return RT_EINVAL;
+int rt_launch_count(int nx, int ny, int nz, int n_src, int n_rays, int n_bins, int n_steps) {
+    if (nx < 1 || ny < 1 || nz < 1 || n_src < 1 || n_rays < 1 || n_bins < 1 || n_steps < 1) return RT_EINVAL;
     Plan pl;
     make_plan(RT_VARIANT_DEFAULT, n_src, &pl);
     const int setup = 1 + ((pl.map_src && n_src <= kMaxSortedSources) ? 1 : 0);     // ray order, (source order)
-    if (n_bins % 4 == 0) {                                                          // batched: (march, drain) per batch
-        int per_batch = int(std::max(1LL, (1LL << 18) / (long long)n_rays));
-        if (pl.map_src) per_batch = (per_batch + 31) / 32 * 32;
-        return setup + 2 * ((n_src + per_batch - 1) / per_batch) + 1;
+    if (use_batched_fp32((long long)nx * ny * nz * n_bins, n_steps, n_bins)) {      // (march, drain) per batch
+        const int slots = ray_slots(n_rays);
+        const Batching bt = plan_batches(n_src, slots, pl.map_src);
+        const int batches = ((n_src + bt.src_per_batch - 1) / bt.src_per_batch) *
+                            ((slots + bt.slots_per_batch - 1) / bt.slots_per_batch);
+        return setup + 2 * batches + 1;
     }
     return setup + 2;                                                               // march, snapshot finalisation
 }
@@ -387,7 +418,7 @@ int rt_trace_ray(const float* j, const float* kappa, int nx, int ny, int nz, int
     rt::MarchParams P{};
     P.j = j; P.kappa = kappa; P.sources = source_pos; P.acc = nullptr; P.ray_order = nullptr; P.src_order = nullptr; P.map_src = 0;
     P.nx = nx; P.ny = ny; P.nz = nz; P.nb = n_bins;
-    P.n_src = 1; P.src_begin = 0; P.n_rays = n_rays; P.n_slots = n_rays; P.n_groups = 1; P.n_steps = 1; P.n_sub = n_sub;
+    P.n_src = 1; P.src_begin = 0; P.slot_begin = 0; P.n_rays = n_rays; P.n_slots = n_rays; P.n_groups = 1; P.n_steps = 1; P.n_sub = n_sub;
     P.ds = double(step_size); P.ds_f = step_size; P.emis = step_size; P.att_scale = 0.0f; P.snap_stride = 0;
     P.state_I = nullptr; P.state_T = nullptr; P.k0 = 0;
     rt::trace_ray_kernel<<<1, 32, 0, static_cast<cudaStream_t>(stream)>>>(P, uint32_t(ray_index), n_sub, pos, trace_I,

@@ -20,6 +20,7 @@ struct MarchParams {
     int nx, ny, nz, nb;
     int n_src, n_rays, n_slots;  // n_src: sources of THIS launch, ranks src_begin .. src_begin + n_src - 1
     int src_begin;
+    int slot_begin;              // direction slots of THIS launch: slot_begin .. slot_begin + n_slots - 1
     int n_groups;                // bin groups per ray (nb / NB)
     int n_steps, n_sub;          // time steps, substeps per step (N_s)
     int map_src;                 // 0: the lanes of a warp are 32 directions of one source; 1: 32 sources, one direction
@@ -201,6 +202,7 @@ __device__ __forceinline__ bool ray_id(const MarchParams& P, RayId& id) {
     }
     if (slot >= uint32_t(P.n_slots) || s >= uint32_t(P.n_src)) return false;
     s += uint32_t(P.src_begin);
+    slot += uint32_t(P.slot_begin);
     id.src = int(P.src_order ? P.src_order[s] : s);
     id.index = P.ray_order ? P.ray_order[slot] : slot;
     return id.index != kPad && id.index < uint32_t(P.n_rays);

@@ -7,6 +7,9 @@ evaluated per snapshot (time step), all bins together.
 """
 from __future__ import annotations
 
+import json
+import os
+
 import numpy as np
 
 REL_L2_TOL = 1e-4
@@ -40,6 +43,11 @@ def compare(gpu: np.ndarray, ref: np.ndarray) -> list[dict]:
 
 def assert_parity(gpu, ref, what=""):
     rows = compare(gpu, ref)
+    report = os.environ.get("RT_PARITY_REPORT")       # optional: append every comparison to a JSON-lines file
+    if report:
+        with open(report, "a") as f:
+            for row in rows:
+                f.write(json.dumps(dict(row, what=str(what))) + "\n")
     for row in rows:
         assert row["nonfinite"] == 0, (what, row)
         assert row["mask_voxels"] > 0, (what, row)
