@@ -51,6 +51,10 @@ def lib() -> ctypes.CDLL:
             L.rt_march_oracle.argtypes = [fp, fp, ctypes.c_int, ctypes.c_int, ctypes.c_int, fp, ctypes.c_int,
                                           ctypes.c_int, ctypes.c_int, ctypes.c_float, ctypes.c_float,
                                           ctypes.c_float, ctypes.c_int, dp, ctypes.c_int]
+            L.rt_oracle_trace_ray_k.restype = ctypes.c_int
+            L.rt_oracle_trace_ray_k.argtypes = L.rt_oracle_trace_ray.argtypes + [ctypes.c_int]
+            L.rt_march_oracle_k.restype = ctypes.c_int
+            L.rt_march_oracle_k.argtypes = L.rt_march_oracle.argtypes + [ctypes.c_int]
             L.rt_oracle_step.restype = ctypes.c_int
             L.rt_oracle_step.argtypes = [fp, fp, ctypes.c_int, ctypes.c_int, ctypes.c_int, fp, ctypes.c_int,
                                          ctypes.c_int, ctypes.c_int, ctypes.c_float, ctypes.c_float, ctypes.c_float,
@@ -95,7 +99,7 @@ def direction(i: int, n: int) -> np.ndarray:
 
 
 def march(j, kappa, sources, n_rays, step_size, c, dt, n_steps, n_threads: int | None = None,
-          max_private_bytes: int = 24 << 30) -> np.ndarray:
+          max_private_bytes: int = 24 << 30, kappa_trilinear: bool = False) -> np.ndarray:
     """Oracle field: float64 ``[n_steps, nx, ny, nz, n_bins]`` (cumulative snapshots, scaled by 4π/N_Ω)."""
     j = _f32(j, 4)
     kappa = _f32(kappa, 4)
@@ -108,8 +112,8 @@ def march(j, kappa, sources, n_rays, step_size, c, dt, n_steps, n_threads: int |
     # each thread owns one private fp64 grid: bound the total
     n_threads = max(1, min(n_threads, max_private_bytes // max(1, j.size * 8)))
     out = np.empty((n_steps, nx, ny, nz, nb), dtype=np.float64)
-    rc = lib().rt_march_oracle(_fp(j), _fp(kappa), nx, ny, nz, _fp(sources), sources.shape[0], n_rays, nb,
-                               step_size, c, dt, n_steps, _dp(out), n_threads)
+    rc = lib().rt_march_oracle_k(_fp(j), _fp(kappa), nx, ny, nz, _fp(sources), sources.shape[0], n_rays, nb,
+                                 step_size, c, dt, n_steps, _dp(out), n_threads, int(kappa_trilinear))
     if rc:
         raise ValueError("rt_march_oracle: invalid arguments")
     return out
@@ -141,7 +145,8 @@ def step(j, kappa, sources, n_rays, step_size, c, dt, k_begin: int, state: np.nd
     return inc
 
 
-def trace_ray(j, kappa, source_pos, ray_index, n_rays, step_size, n_sub, deposit: bool = False):
+def trace_ray(j, kappa, source_pos, ray_index, n_rays, step_size, n_sub, deposit: bool = False,
+              kappa_trilinear: bool = False):
     """One ray from k=0: returns dict(I=[n_sub,B], tau=[n_sub,B], pos=[n_sub,3], acc=unnormalised grid|None)."""
     j = _f32(j, 4)
     kappa = _f32(kappa, 4)
@@ -151,8 +156,8 @@ def trace_ray(j, kappa, source_pos, ray_index, n_rays, step_size, n_sub, deposit
     tau = np.zeros((n_sub, nb))
     pos = np.zeros((n_sub, 3))
     acc = np.zeros((nx, ny, nz, nb)) if deposit else None
-    rc = lib().rt_oracle_trace_ray(_fp(j), _fp(kappa), nx, ny, nz, nb, _fp(src), ray_index, n_rays, step_size,
-                                   n_sub, _dp(I), _dp(tau), _dp(pos), _dp(acc))
+    rc = lib().rt_oracle_trace_ray_k(_fp(j), _fp(kappa), nx, ny, nz, nb, _fp(src), ray_index, n_rays, step_size,
+                                     n_sub, _dp(I), _dp(tau), _dp(pos), _dp(acc), int(kappa_trilinear))
     if rc:
         raise ValueError("rt_oracle_trace_ray: invalid arguments")
     return {"I": I, "tau": tau, "pos": pos, "acc": acc}

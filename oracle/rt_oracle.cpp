@@ -53,6 +53,7 @@ struct Medium {
     const float* j;
     const float* kappa;
     long nx, ny, nz, nb;
+    bool ktri = false;   // reading D18: kappa read by trilinear interpolation (the weights of j) instead of nearest neighbour
     size_t cell(long a, long b, long c) const { return ((size_t(a) * ny + b) * nz + c) * nb; }
 };
 
@@ -141,7 +142,11 @@ void march_ray(const Medium& M, const double x0[3], const double nhat[3], double
         }
         const size_t base = M.cell(lo[0], lo[1], lo[2]);
         for (long b = 0; b < M.nb; ++b) {
-            double kap = double(M.kappa[base + b]);
+            double kap = double(M.kappa[base + b]);                 // P:29 nearest neighbour at the cell of x_k (D4)
+            if (M.ktri) {                                            // D18 variant: the same trilinear weights as j
+                kap = 0.0;
+                for (int c = 0; c < 8; ++c) kap += w[c] * double(M.kappa[corner[c] + b]);
+            }
             double jv = 0.0;
             for (int c = 0; c < 8; ++c) jv += w[c] * double(M.j[corner[c] + b]);
             I[b] = I[b] * std::exp(-kap * ds) + jv * std::exp(-tau[b]) * ds;
@@ -174,12 +179,24 @@ int rt_oracle_direction(long i, long n, double* nhat) {
 
 // One ray, n_sub substeps from k = 0 (I_0 = tau_0 = 0, D11).  Records I_{k+1}, tau_{k+1} and x_k for every
 // substep and adds the UNNORMALISED deposits into acc (double [nx][ny][nz][B], caller-zeroed; may be null).
+int rt_oracle_trace_ray_k(const float* j, const float* kappa, int nx, int ny, int nz, int n_bins,
+                          const float* source_pos, long ray_index, long n_rays, float step_size, long n_sub,
+                          double* trace_I, double* trace_tau, double* trace_pos, double* acc, int kappa_trilinear);
+
 int rt_oracle_trace_ray(const float* j, const float* kappa, int nx, int ny, int nz, int n_bins,
                         const float* source_pos, long ray_index, long n_rays, float step_size, long n_sub,
                         double* trace_I, double* trace_tau, double* trace_pos, double* acc) {
+    return rt_oracle_trace_ray_k(j, kappa, nx, ny, nz, n_bins, source_pos, ray_index, n_rays, step_size, n_sub,
+                                 trace_I, trace_tau, trace_pos, acc, 0);
+}
+
+// The same with the kappa reading chosen: 0 = nearest neighbour (the paper), 1 = trilinear (D18).
+int rt_oracle_trace_ray_k(const float* j, const float* kappa, int nx, int ny, int nz, int n_bins,
+                          const float* source_pos, long ray_index, long n_rays, float step_size, long n_sub,
+                          double* trace_I, double* trace_tau, double* trace_pos, double* acc, int kappa_trilinear) {
     if (!j || !kappa || !source_pos || nx < 1 || ny < 1 || nz < 1 || n_bins < 1 || n_sub < 0 || bad(step_size))
         return -1;
-    Medium M{j, kappa, nx, ny, nz, n_bins};
+    Medium M{j, kappa, nx, ny, nz, n_bins, kappa_trilinear != 0};
     double nhat[3];
     if (rt_oracle_direction(ray_index, n_rays, nhat)) return -1;
     double x0[3] = {double(source_pos[0]), double(source_pos[1]), double(source_pos[2])};
@@ -192,15 +209,27 @@ int rt_oracle_trace_ray(const float* j, const float* kappa, int nx, int ny, int 
 // The multi-source march.  Host pointers.  out: double [n_steps][nx][ny][nz][n_bins],
 // overwritten; snapshot m is cumulative (D7) and scaled once by 4 pi / N_Omega (D8).
 // n_threads < 1 means 1.  Returns 0, or -1 on invalid arguments.
+int rt_march_oracle_k(const float* j, const float* kappa, int nx, int ny, int nz, const float* sources, int n_src,
+                      int n_rays, int n_bins, float step_size, float c, float dt, int n_steps, double* out,
+                      int n_threads, int kappa_trilinear);
+
 int rt_march_oracle(const float* j, const float* kappa, int nx, int ny, int nz, const float* sources, int n_src,
                     int n_rays, int n_bins, float step_size, float c, float dt, int n_steps, double* out,
                     int n_threads) {
+    return rt_march_oracle_k(j, kappa, nx, ny, nz, sources, n_src, n_rays, n_bins, step_size, c, dt, n_steps, out,
+                             n_threads, 0);
+}
+
+// The same with the kappa reading chosen: 0 = nearest neighbour (the paper), 1 = trilinear (D18).
+int rt_march_oracle_k(const float* j, const float* kappa, int nx, int ny, int nz, const float* sources, int n_src,
+                      int n_rays, int n_bins, float step_size, float c, float dt, int n_steps, double* out,
+                      int n_threads, int kappa_trilinear) {
     if (!j || !kappa || !sources || !out) return -1;
     if (nx < 1 || ny < 1 || nz < 1 || n_src < 1 || n_rays < 1 || n_bins < 1 || n_steps < 1) return -1;
     if (bad(step_size) || bad(c) || bad(dt)) return -1;
     const long Ns = substeps(double(step_size), double(c), double(dt));
     const double ds = double(step_size);
-    const Medium M{j, kappa, nx, ny, nz, n_bins};
+    const Medium M{j, kappa, nx, ny, nz, n_bins, kappa_trilinear != 0};
     const size_t grid = size_t(nx) * ny * nz * n_bins;
     const long total_rays = long(n_src) * n_rays;
     long T = std::max(1, n_threads);

@@ -636,3 +636,57 @@ def test_d17_a_step_sees_only_its_own_medium(oracle_mod):
     unit = oracle_mod.step(jz, kz, src, n_rays, ds, 1.0, dt, N, state1)
     assert np.abs(inc - I_N * unit).max() <= 1e-13 * inc.max()
     assert abs(unit.sum() - FOUR_PI * N) <= 1e-12 * unit.sum()
+
+
+# ------------------------------------------------------------------------------------------------------
+# D18  trilinear kappa variant (PAPER.md:29 samples kappa nearest-neighbour "(currently)")
+# ------------------------------------------------------------------------------------------------------
+def test_d18_uniform_kappa_cannot_tell_the_readings_apart(oracle_mod):
+    rho = W.lognormal_density(10, 9, 1.0)
+    j = np.ascontiguousarray((1e-2 * rho ** 2)[..., None], dtype=np.float32)
+    kap = np.full(j.shape, 0.15, dtype=np.float32)
+    src = np.array([[4.4, 5.1, 3.3]], dtype=np.float32)
+    a = oracle_mod.march(j, kap, src, 50, 0.5, 1.0, 6.0, 2)
+    b = oracle_mod.march(j, kap, src, 50, 0.5, 1.0, 6.0, 2, kappa_trilinear=True)
+    assert np.abs(a - b).max() <= 1e-13 * a.max()
+
+
+def test_d18_tau_is_the_riemann_sum_of_the_library_trilinear_read(oracle_mod):
+    """tau_k = ds * sum_{i<k} kappa(x_i) with kappa read by scipy's order-1 map_coordinates, mode 'nearest'
+    (= clamped indices), along rays that leave the box."""
+    from scipy.ndimage import map_coordinates
+    rng = np.random.default_rng(21)
+    shape = (7, 6, 5)
+    kap = rng.uniform(0.0, 0.6, shape + (2,)).astype(np.float32)
+    j = rng.uniform(0.1, 1.0, shape + (2,)).astype(np.float32)
+    src, ds, n_sub = (3.3, 2.6, 1.9), 0.37, 30
+    for ray in (0, 5, 11, 22):
+        tr = oracle_mod.trace_ray(j, kap, src, ray, 23, ds, n_sub, kappa_trilinear=True)
+        for b in range(2):
+            kx = map_coordinates(kap[..., b].astype(np.float64), tr["pos"].T, order=1, mode="nearest")
+            assert np.abs(tr["tau"][:, b] - f32(ds) * np.cumsum(kx)).max() <= 1e-12
+        nn = oracle_mod.trace_ray(j, kap, src, ray, 23, ds, n_sub)
+        assert np.abs(nn["tau"] - tr["tau"]).max() > 1e-3          # and it is a different reading from D4
+
+
+def test_d18_hand_trace_axis_ray(oracle_mod):
+    """N_Omega = 1 (nhat = (1,0,0)), source on a node: x-fractions alternate 0 and 1/2, so kappa is a cell value
+    or the mean of two neighbours; after the box, the boundary value (clamped)."""
+    J, K = _grid4()
+    J, K = J.astype(np.float64), K.astype(np.float64)
+    ds, y, z = 0.5, 1, 2
+    I = tau = 0.0
+    want = []
+    for k in range(10):
+        x = 1.0 + k * ds
+        i0, f = int(math.floor(x)), x - math.floor(x)
+        lo, hi = min(i0, 3), min(i0 + 1, 3)
+        kap = (1 - f) * K[lo, y, z] + f * K[hi, y, z]
+        jv = (1 - f) * J[lo, y, z] + f * J[hi, y, z]
+        I = I * math.exp(-kap * ds) + jv * math.exp(-tau) * ds
+        tau += kap * ds
+        want.append((I, tau))
+    j4, k4 = _grid4()
+    tr = oracle_mod.trace_ray(j4[..., None], k4[..., None], (1.0, 1.0, 2.0), 0, 1, ds, 10, kappa_trilinear=True)
+    assert np.allclose(tr["I"][:, 0], [w[0] for w in want], rtol=1e-14)
+    assert np.allclose(tr["tau"][:, 0], [w[1] for w in want], rtol=1e-14)
