@@ -41,9 +41,10 @@ def parse():
     ap.add_argument("--config", default="C2", choices=["C0", "C1", "C2", "C3", "C4"])
     ap.add_argument("--impl", default="native", choices=["native", "reference"])
     ap.add_argument("--variant", type=int, default=0, help="RT_VARIANT_* (0 = the product path)")
-    ap.add_argument("--mode", default="march", choices=["march", "step"],
+    ap.add_argument("--mode", default="march", choices=["march", "step", "trilinear_kappa"],
                     help="march: one rt_march call per bench step (the headline); step: the same workload as n_steps "
-                         "rt_march_step calls with persistent ray state (DESIGN.md D17)")
+                         "rt_march_step calls with persistent ray state (DESIGN.md D17); trilinear_kappa: "
+                         "rt_march_trilinear_kappa (DESIGN.md D18)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target host time of the oracle sample")
@@ -243,6 +244,8 @@ def run_native(args):
             for m in range(w.n_steps):
                 rt.rt_march_step(j, kappa, src, w.n_rays, w.step_size, w.c, w.dt, m * w.substeps_per_step, state,
                                  out=out[-1], accumulate=True, workspace=ws_step)
+        elif args.mode == "trilinear_kappa":
+            rt.rt_march_trilinear_kappa(j, kappa, src, w.n_rays, w.step_size, w.c, w.dt, w.n_steps, out=out, workspace=ws)
         else:
             rt.rt_march_ex(j, kappa, src, w.n_rays, w.step_size, w.c, w.dt, w.n_steps, out=out, workspace=ws,
                            variant=args.variant)

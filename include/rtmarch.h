@@ -69,6 +69,13 @@ int rt_march(const float* j, const float* kappa, int nx, int ny, int nz,
              void* workspace, size_t workspace_bytes, /* device scratch, >= rt_workspace_bytes(), 16-byte aligned */
              void* stream);
 
+/* rt_march with kappa read by TRILINEAR interpolation at x_k, with the weights of the j read, instead of nearest
+ * neighbour (reading D18: P:29 calls nearest neighbour the current choice).  Everything else as rt_march. */
+int rt_march_trilinear_kappa(const float* j, const float* kappa, int nx, int ny, int nz,
+                             const float* sources, int n_src, int n_rays, int n_bins,
+                             float step_size, float c, float dt, int n_steps, float* out,
+                             void* workspace, size_t workspace_bytes, void* stream);
+
 /* The paper's single-source kernel: rt_march with n_src = 1; source_pos = 3 floats (device). */
 int rt_march_single(const float* j, const float* kappa, int nx, int ny, int nz,
                     const float* source_pos, int n_rays, int n_bins,

@@ -24,7 +24,7 @@ RED_MODES = {"M1_scalar_random": 0, "M2_v4_random": 1, "M3_stencil": 2, "M4_one_
 EXPORTS = ("rt_march", "rt_march_single", "rt_march_ex", "rt_march_host", "rt_workspace_bytes",
            "rt_substeps_per_step", "rt_launch_count", "rt_directions", "rt_ray_order", "rt_ray_slots", "rt_trace_ray",
            "rt_bench_red_ceiling", "rt_strerror", "rt_version", "rt_state_bytes", "rt_state_reset",
-           "rt_step_workspace_bytes", "rt_march_step")
+           "rt_step_workspace_bytes", "rt_march_step", "rt_march_trilinear_kappa")
 
 
 class RtError(RuntimeError):
@@ -47,6 +47,7 @@ def _load() -> ctypes.CDLL:
     vp, i, f, sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_float, ctypes.c_size_t
     march_args = [vp, vp, i, i, i, vp, i, i, i, f, f, f, i, vp]
     L.rt_march.argtypes = march_args + [vp, sz, vp]
+    L.rt_march_trilinear_kappa.argtypes = march_args + [vp, sz, vp]
     L.rt_march_single.argtypes = [vp, vp, i, i, i, vp, i, i, f, f, f, i, vp, vp, sz, vp]
     L.rt_march_ex.argtypes = march_args + [vp, sz, vp, i]
     L.rt_march_host.argtypes = march_args
@@ -137,7 +138,7 @@ def alloc_workspace(nx, ny, nz, n_src, n_rays, n_bins, n_steps, device=None):
 
 
 def rt_march_ex(j, kappa, sources, n_rays, step_size, c, dt, n_steps, out=None, workspace=None, stream=None,
-                variant=RT_VARIANT_DEFAULT):
+                variant=RT_VARIANT_DEFAULT, _entry=None):
     """out[n_steps,nx,ny,nz,n_bins] = the march of include/rtmarch.h; asynchronous on the stream."""
     torch = _torch()
     _check_dev(j, "j", torch.float32, 4)
@@ -155,9 +156,9 @@ def rt_march_ex(j, kappa, sources, n_rays, step_size, c, dt, n_steps, out=None, 
             raise ValueError("out has the wrong size")
     if workspace is None:
         workspace = alloc_workspace(nx, ny, nz, n_src, n_rays, nb, n_steps, j.device)
-    rc = _lib.rt_march_ex(j.data_ptr(), kappa.data_ptr(), nx, ny, nz, sources.data_ptr(), n_src, n_rays, nb,
-                          step_size, c, dt, n_steps, out.data_ptr(), workspace.data_ptr(), workspace.numel(),
-                          _stream_ptr(stream), variant)
+    args = (j.data_ptr(), kappa.data_ptr(), nx, ny, nz, sources.data_ptr(), n_src, n_rays, nb, step_size, c, dt,
+            n_steps, out.data_ptr(), workspace.data_ptr(), workspace.numel(), _stream_ptr(stream))
+    rc = _entry(*args) if _entry is not None else _lib.rt_march_ex(*args, variant)
     if rc != RT_OK:
         raise RtError(rc, "rt_march")
     return out
@@ -166,6 +167,13 @@ def rt_march_ex(j, kappa, sources, n_rays, step_size, c, dt, n_steps, out=None, 
 def rt_march(j, kappa, sources, n_rays, step_size, c, dt, n_steps, out=None, workspace=None, stream=None):
     return rt_march_ex(j, kappa, sources, n_rays, step_size, c, dt, n_steps, out, workspace, stream,
                        RT_VARIANT_DEFAULT)
+
+
+def rt_march_trilinear_kappa(j, kappa, sources, n_rays, step_size, c, dt, n_steps, out=None, workspace=None,
+                             stream=None):
+    """rt_march with kappa read trilinearly (D18)."""
+    return rt_march_ex(j, kappa, sources, n_rays, step_size, c, dt, n_steps, out, workspace, stream,
+                       _entry=_lib.rt_march_trilinear_kappa)
 
 
 def rt_march_single(j, kappa, source_pos, n_rays, step_size, c, dt, n_steps, out=None, workspace=None,

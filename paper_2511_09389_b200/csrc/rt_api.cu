@@ -95,7 +95,8 @@ int launch_march(const rt::MarchParams& P, bool sliding, cudaStream_t st) {
     if (sliding) {
         // registers: 1 bin per thread runs 8 blocks/SM (64 registers, 16 bytes spilled); 4 bins need ~150
         constexpr int kMinBlocks = (NB == 1) ? 8 : 1;
-        if (P.state_I) rt::march_sliding_kernel<NB, ACC, kMinBlocks, true><<<g, rt::kThreads, 0, st>>>(P);
+        if (P.kappa_trilinear) rt::march_sliding_kernel<NB, ACC, 1, false, true><<<g, rt::kThreads, 0, st>>>(P);
+        else if (P.state_I) rt::march_sliding_kernel<NB, ACC, kMinBlocks, true><<<g, rt::kThreads, 0, st>>>(P);
         else rt::march_sliding_kernel<NB, ACC, kMinBlocks, false><<<g, rt::kThreads, 0, st>>>(P);
     } else {
         rt::march_direct_kernel<NB, ACC><<<g, rt::kThreads, 0, st>>>(P);
@@ -135,13 +136,17 @@ bool use_batched_fp32(long long cells, int n_steps, int n_bins) {
     return n_bins % 4 == 0 && size_t(cells) * size_t(n_steps) * sizeof(float) <= kBatchedScratchLimit;
 }
 
+constexpr int kVariantKappaTrilinear = 64;   // internal: rt_march_trilinear_kappa
+
 // what a variant code means (rtmarch.h RT_VARIANT_*)
 struct Plan {
-    bool sliding, coherent, map_src, acc64, one_bin;
+    bool sliding, coherent, map_src, acc64, one_bin, ktri;
 };
 bool make_plan(int variant, int n_src, Plan* pl) {
     const int kind = variant & 15;
-    if (variant < 0 || (variant & ~63) || kind > RT_VARIANT_SLIDING_BY_SOURCE) return false;
+    if (variant < 0 || (variant & ~127) || kind > RT_VARIANT_SLIDING_BY_SOURCE) return false;
+    pl->ktri = (variant & kVariantKappaTrilinear) != 0;
+    if (pl->ktri && (variant & ~kVariantKappaTrilinear)) return false;      // only with the default kernel path
     pl->acc64 = !(variant & RT_VARIANT_FLAG_ACC_F32);
     pl->one_bin = (variant & RT_VARIANT_FLAG_ONE_BIN) != 0;
     pl->sliding = !(kind == RT_VARIANT_DIRECT || kind == RT_VARIANT_DIRECT_COHERENT);
@@ -190,6 +195,8 @@ int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const
     P.att_scale = float(-double(step_size) * 1.4426950408889634074);
     P.snap_stride = ck.cells;
     P.map_src = pl.map_src ? 1 : 0;
+    P.kappa_trilinear = pl.ktri ? 1 : 0;
+    if (pl.ktri && step) return RT_EINVAL;
     P.state_I = step ? step->state : nullptr;
     P.state_T = step ? step->state + size_t(n_src) * size_t(n_rays) * size_t(n_bins) : nullptr;
     P.k0 = step ? step->k0 : 0;
@@ -291,6 +298,13 @@ int rt_march(const float* j, const float* kappa, int nx, int ny, int nz, const f
              size_t workspace_bytes, void* stream) {
     return march_impl(j, kappa, nx, ny, nz, sources, n_src, n_rays, n_bins, step_size, c, dt, n_steps, out, workspace,
                       workspace_bytes, stream, RT_VARIANT_DEFAULT);
+}
+
+int rt_march_trilinear_kappa(const float* j, const float* kappa, int nx, int ny, int nz, const float* sources, int n_src,
+                             int n_rays, int n_bins, float step_size, float c, float dt, int n_steps, float* out,
+                             void* workspace, size_t workspace_bytes, void* stream) {
+    return march_impl(j, kappa, nx, ny, nz, sources, n_src, n_rays, n_bins, step_size, c, dt, n_steps, out, workspace,
+                      workspace_bytes, stream, kVariantKappaTrilinear);
 }
 
 int rt_march_single(const float* j, const float* kappa, int nx, int ny, int nz, const float* source_pos, int n_rays,
@@ -420,7 +434,7 @@ int rt_trace_ray(const float* j, const float* kappa, int nx, int ny, int nz, int
     P.nx = nx; P.ny = ny; P.nz = nz; P.nb = n_bins;
     P.n_src = 1; P.src_begin = 0; P.slot_begin = 0; P.n_rays = n_rays; P.n_slots = n_rays; P.n_groups = 1; P.n_steps = 1; P.n_sub = n_sub;
     P.ds = double(step_size); P.ds_f = step_size; P.emis = step_size; P.att_scale = 0.0f; P.snap_stride = 0;
-    P.state_I = nullptr; P.state_T = nullptr; P.k0 = 0;
+    P.state_I = nullptr; P.state_T = nullptr; P.k0 = 0; P.kappa_trilinear = 0;
     rt::trace_ray_kernel<<<1, 32, 0, static_cast<cudaStream_t>(stream)>>>(P, uint32_t(ray_index), n_sub, pos, trace_I,
                                                                          trace_T);
     RT_CUDA(cudaGetLastError());

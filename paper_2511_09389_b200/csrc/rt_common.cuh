@@ -23,6 +23,7 @@ struct MarchParams {
     int slot_begin;              // direction slots of THIS launch: slot_begin .. slot_begin + n_slots - 1
     int n_groups;                // bin groups per ray (nb / NB)
     int n_steps, n_sub;          // time steps, substeps per step (N_s)
+    int kappa_trilinear;         // reading D18 instead of D4 (rt_march_trilinear_kappa)
     int map_src;                 // 0: the lanes of a warp are 32 directions of one source; 1: 32 sources, one direction
     double ds;                   // step_size as double
     float ds_f;                  // step_size

@@ -54,9 +54,11 @@ template <int AX> __device__ __forceinline__ int eoff(const MarchParams& P, int 
 
 // The stencil: 8 register slots [x][y][z], 0 = trailing / 1 = leading per axis.  Slot s sits at element offset
 // base + (s&4 ? dl_x : 0) + (s&2 ? dl_y : 0) + (s&1 ? dl_z : 0); base includes the thread's bin offset.
-template <int NB, typename ACC> struct Stencil {
+// KTRI (D18): kappa is read trilinearly too, so its 8 corner values are cached like j's.
+template <int NB, typename ACC, bool KTRI> struct Stencil {
     BinVec<NB> acc[8];   // pending deposits for the 8 stencil voxels
     BinVec<NB> jc[8];    // j at the 8 stencil voxels
+    BinVec<NB> kc[KTRI ? 8 : 1];   // kappa at the 8 stencil voxels (trilinear-kappa variant only)
     int base;            // element offset of slot 0
 
     __device__ __forceinline__ int off(int s, const TravelAxis (&A)[3]) const {
@@ -86,7 +88,10 @@ template <int NB, typename ACC> struct Stencil {
     __device__ __forceinline__ void restart(const MarchParams& P, TravelAxis (&A)[3], int negbits, int bin_off) {
         base = bin_off + place<0>(P, A[0], negbits) + place<1>(P, A[1], negbits) + place<2>(P, A[2], negbits);
 #pragma unroll
-        for (int s = 0; s < 8; ++s) jc[s] = ld_bins<NB>(P.j + off(s, A));
+        for (int s = 0; s < 8; ++s) {
+            jc[s] = ld_bins<NB>(P.j + off(s, A));
+            if constexpr (KTRI) kc[s] = ld_bins<NB>(P.kappa + off(s, A));
+        }
     }
     // Axis AX advanced by one cell.  The old leading plane is the new trailing plane (also under clamping: both
     // are clamp(c+1)), so the trailing index moves iff the axis was not merged; the new leading index is looked up.
@@ -110,6 +115,7 @@ template <int NB, typename ACC> struct Stencil {
                     flush_slot(og, s0, A);
                     acc[s0] = acc[s1];
                     jc[s0] = jc[s1];
+                    if constexpr (KTRI) kc[s0] = kc[s1];
                     zero_slot(s1);
                 }
         }
@@ -123,13 +129,14 @@ template <int NB, typename ACC> struct Stencil {
                 for (int v = 0; v < 2; ++v) {
                     const int s1 = slot<AX>(1, u, v);
                     jc[s1] = ld_bins<NB>(P.j + off(s1, A));
+                    if constexpr (KTRI) kc[s1] = ld_bins<NB>(P.kappa + off(s1, A));
                 }
         }
     }
 };
 
 // STEP: the rt_march_step form -- start at substep P.k0 with (I, exp(-tau)) loaded from the ray state, store them back
-template <int NB, typename ACC, int MINB, bool STEP>
+template <int NB, typename ACC, int MINB, bool STEP, bool KTRI = false>
 __global__ void __launch_bounds__(kThreads, MINB) march_sliding_kernel(const MarchParams P) {
     RayId id;
     if (!ray_id(P, id)) return;
@@ -150,7 +157,7 @@ __global__ void __launch_bounds__(kThreads, MINB) march_sliding_kernel(const Mar
         }
     }
     asm volatile("" : "+r"(negbits));        // opaque: keeps ptxas from re-deriving the signs with fp64 compares
-    Stencil<NB, ACC> S;
+    Stencil<NB, ACC, KTRI> S;
 #pragma unroll
     for (int s = 0; s < 8; ++s) S.zero_slot(s);
     S.restart(P, A, negbits, id.group * NB);
@@ -171,7 +178,7 @@ __global__ void __launch_bounds__(kThreads, MINB) march_sliding_kernel(const Mar
 #pragma unroll
         for (int b = 0; b < NB; ++b) att[b] = ex2_approx(kap.v[b] * P.att_scale);
     };
-    load_att();
+    if (!KTRI) load_att();
     const bool long_steps = !(P.ds_f < 1.0f);      // only then can one substep cross more than one cell plane
 
     for (int m = 0; m < P.n_steps; ++m) {
@@ -201,6 +208,15 @@ __global__ void __launch_bounds__(kThreads, MINB) march_sliding_kernel(const Mar
                 }
 #pragma unroll
             for (int b = 0; b < NB; ++b) jv[b] += ju[b];
+            if constexpr (KTRI) {          // kappa(x_k) with the weights of j(x_k); one exponential per substep
+#pragma unroll
+                for (int b = 0; b < NB; ++b) {
+                    float kv = 0.0f;
+#pragma unroll
+                    for (int s = 0; s < 8; ++s) kv = fmaf(w[s], S.kc[s].v[b], kv);
+                    att[b] = ex2_approx(kv * P.att_scale);
+                }
+            }
 #pragma unroll
             for (int b = 0; b < NB; ++b) {                       // eq. (2)
                 I[b] = fmaf(I[b], att[b], jv[b] * T[b] * P.emis);
@@ -224,7 +240,7 @@ __global__ void __launch_bounds__(kThreads, MINB) march_sliding_kernel(const Mar
                     if (c1 != A[1].p.c) S.template axis_step<1>(P, A, negbits, og);
                     if (c2 != A[2].p.c) S.template axis_step<2>(P, A, negbits, og);
                 }
-                load_att();
+                if (!KTRI) load_att();
             }
         }
         S.flush_all(og, A);    // time-step boundary: the increments of step m are complete (rays continue, D7)

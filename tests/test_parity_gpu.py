@@ -57,6 +57,10 @@ def config(name):
     return _cache[name]
 
 
+def _stratified(n_src, count):
+    return np.unique(np.linspace(0, n_src - 1, count).round().astype(int))
+
+
 VARIANTS = [0, 1, 2, 3, 4, 5, 16, 17, 21, 32, 36, 53]   # kinds 0..5; flags: 16 fp32 accumulation, 32 one bin per thread
 
 
@@ -207,6 +211,39 @@ def test_more_sources_than_the_sort_handles(rt, oracle_mod):
     parity.assert_parity(out.cpu().numpy(), ref, "66000 sources")
 
 
+# ------------------------------------------------------------------------------------------------
+# trilinear-kappa variant (D18)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("shape,nb,n_src,n_rays,ds,dt", [
+    ((5, 4, 3), 3, 2, 7, 0.5, 5.0),
+    ((6, 5, 7), 8, 1, 40, 0.5, 8.0),
+    ((9, 8, 7), 1, 40, 24, 0.25, 4.0),          # warp = 32 sources x 1 direction
+    ((8, 8, 8), 4, 3, 50, 1.7, 13.6),           # steps longer than a cell
+])
+def test_trilinear_kappa_small_cases(rt, oracle_mod, shape, nb, n_src, n_rays, ds, dt):
+    j, k = _random_medium(shape, nb, seed=sum(shape) + nb)
+    src = np.random.default_rng(n_src).uniform(-2.0, max(shape) + 1.0, (n_src, 3)).astype(np.float32)
+    src[0] = np.round(src[0])
+    for n_steps in (1, 3):
+        ref = oracle_mod.march(j, k, src, n_rays, ds, 1.0, dt, n_steps, kappa_trilinear=True)
+        nn = oracle_mod.march(j, k, src, n_rays, ds, 1.0, dt, n_steps)
+        out = rt.rt_march_trilinear_kappa(_dev(j), _dev(k), _dev(src), n_rays, ds, 1.0, dt, n_steps)
+        torch.cuda.synchronize()
+        parity.assert_parity(out.cpu().numpy(), ref, f"trilinear kappa {shape} nb={nb} steps={n_steps}")
+        assert np.abs(nn - ref).max() > 1e-3 * ref.max()        # the two readings really differ here
+
+
+@pytest.mark.parametrize("name", ["C1", "C3"])
+def test_trilinear_kappa_configs(rt, oracle_mod, name):
+    w = config(name)
+    src = w.sources if name == "C1" else np.ascontiguousarray(w.sources[_stratified(w.n_src, 40)])
+    ref = oracle_mod.march(w.j, w.kappa, src, w.n_rays, w.step_size, w.c, w.dt, w.n_steps, kappa_trilinear=True)
+    out = rt.rt_march_trilinear_kappa(_dev(w.j), _dev(w.kappa), _dev(src), w.n_rays, w.step_size, w.c, w.dt, w.n_steps)
+    torch.cuda.synchronize()
+    rows = parity.assert_parity(out.cpu().numpy(), ref, f"trilinear kappa {name}")
+    print(rows[-1])
+
+
 def test_out_is_overwritten_and_call_is_repeatable(rt, oracle_mod):
     w = config("C0")
     j, k, s = _dev(w.j), _dev(w.kappa), _dev(w.sources)
@@ -273,10 +310,6 @@ def test_error_codes_on_device(rt):
 # ------------------------------------------------------------------------------------------------
 # C2, C3, C4: oracle parity on stratified source subsets (all other arguments are the config's)
 # ------------------------------------------------------------------------------------------------
-def _stratified(n_src, count):
-    return np.unique(np.linspace(0, n_src - 1, count).round().astype(int))
-
-
 SUBSETS = {"C2": 48, "C3": 6, "C4": 3}
 
 
