@@ -55,6 +55,10 @@ def lib() -> ctypes.CDLL:
             L.rt_oracle_trace_ray_k.argtypes = L.rt_oracle_trace_ray.argtypes + [ctypes.c_int]
             L.rt_march_oracle_k.restype = ctypes.c_int
             L.rt_march_oracle_k.argtypes = L.rt_march_oracle.argtypes + [ctypes.c_int]
+            L.rt_adjoint_j_oracle.restype = ctypes.c_int
+            L.rt_adjoint_j_oracle.argtypes = [dp, fp, ctypes.c_int, ctypes.c_int, ctypes.c_int, fp, ctypes.c_int,
+                                              ctypes.c_int, ctypes.c_int, ctypes.c_float, ctypes.c_float,
+                                              ctypes.c_float, ctypes.c_int, dp, ctypes.c_int]
             L.rt_oracle_step.restype = ctypes.c_int
             L.rt_oracle_step.argtypes = [fp, fp, ctypes.c_int, ctypes.c_int, ctypes.c_int, fp, ctypes.c_int,
                                          ctypes.c_int, ctypes.c_int, ctypes.c_float, ctypes.c_float, ctypes.c_float,
@@ -117,6 +121,25 @@ def march(j, kappa, sources, n_rays, step_size, c, dt, n_steps, n_threads: int |
     if rc:
         raise ValueError("rt_march_oracle: invalid arguments")
     return out
+
+
+def adjoint_j(gbar, kappa, sources, n_rays, step_size, c, dt, n_steps, n_threads: int | None = None) -> np.ndarray:
+    """dL/dj for dL/d out[m] = gbar[m]: float64 [nx, ny, nz, n_bins] (the march is linear in j; D19)."""
+    kappa = _f32(kappa, 4)
+    sources = _f32(sources, 2)
+    nx, ny, nz, nb = kappa.shape
+    gbar = np.ascontiguousarray(gbar, dtype=np.float64)
+    if gbar.shape != (n_steps, nx, ny, nz, nb):
+        raise ValueError("gbar must be [n_steps, nx, ny, nz, n_bins]")
+    if n_threads is None:
+        n_threads = host_threads()
+    n_threads = max(1, min(n_threads, (24 << 30) // max(1, kappa.size * 8)))
+    grad = np.empty((nx, ny, nz, nb), dtype=np.float64)
+    rc = lib().rt_adjoint_j_oracle(_dp(gbar), _fp(kappa), nx, ny, nz, _fp(sources), sources.shape[0], n_rays, nb,
+                                   step_size, c, dt, n_steps, _dp(grad), n_threads)
+    if rc:
+        raise ValueError("rt_adjoint_j_oracle: invalid arguments")
+    return grad
 
 
 def new_state(n_src: int, n_rays: int, n_bins: int) -> np.ndarray:

@@ -320,6 +320,97 @@ int rt_oracle_step(const float* j, const float* kappa, int nx, int ny, int nz, c
     return 0;
 }
 
+// ADJOINT of the march with respect to j ("its Jacobians with respect to (j, kappa) are well defined";
+// DESIGN.md reading D19).  For fixed kappa the field is linear in j, out[m] = A_m j.  Given gbar[m] = dL/d out[m]
+// this returns grad_j = sum_m A_m^T gbar[m], i.e. dL/dj.  Derived from eq. (2) and the deposit rule:
+//   I_{k+1} = a_k I_k + T_k ds (w_k . j),  a_k = exp(-kappa_k ds),  T_k = exp(-tau_k);   out[m] += s w_k I_{k+1}
+//   for every substep k of time steps 0..m, s = 4 pi / N_Omega.  Hence L = sum_k G_k I_{k+1} with
+//   G_k = s w_k . (sum_{m >= step(k)} gbar[m]),   lambda_{k+1} := dL/dI_{k+1} = G_k + a_{k+1} lambda_{k+2} (lambda_{K+1} = 0),
+//   grad_j[corner_c] += lambda_{k+1} T_k ds w_k[c].
+// Written as it reads: a forward sweep that records (corners, weights, a_k, T_k) of every substep of a ray, then the
+// backward recurrence.  gbar: double [n_steps][nx][ny][nz][B]; grad_j: double [nx][ny][nz][B], overwritten.
+int rt_adjoint_j_oracle(const double* gbar, const float* kappa, int nx, int ny, int nz, const float* sources, int n_src,
+                        int n_rays, int n_bins, float step_size, float c, float dt, int n_steps, double* grad_j,
+                        int n_threads) {
+    if (!gbar || !kappa || !sources || !grad_j) return -1;
+    if (nx < 1 || ny < 1 || nz < 1 || n_src < 1 || n_rays < 1 || n_bins < 1 || n_steps < 1) return -1;
+    if (bad(step_size) || bad(c) || bad(dt)) return -1;
+    const long Ns = substeps(double(step_size), double(c), double(dt)), K = Ns * n_steps;
+    const double ds = double(step_size);
+    const long N[3] = {nx, ny, nz};
+    const Medium M{nullptr, kappa, nx, ny, nz, n_bins};
+    const size_t grid = size_t(nx) * ny * nz * n_bins;
+    const double scale = double(4.0L * kPiL / (long double)n_rays);
+    std::vector<double> gsuf(gbar, gbar + grid * size_t(n_steps));          // gsuf[m] = sum_{m' >= m} gbar[m']
+    for (long m = n_steps - 2; m >= 0; --m)
+        for (size_t v = 0; v < grid; ++v) gsuf[size_t(m) * grid + v] += gsuf[size_t(m + 1) * grid + v];
+    const long total_rays = long(n_src) * n_rays;
+    const long T = std::min<long>(std::max(1, n_threads), total_rays);
+    std::vector<std::vector<double>> acc(T);
+    for (auto& a : acc) a.assign(grid, 0.0);
+    auto work = [&](long t) {
+        std::vector<size_t> corner(size_t(K) * 8);
+        std::vector<double> w(size_t(K) * 8), att(size_t(K) * n_bins), tr(size_t(K) * n_bins);
+        for (long r = total_rays * t / T; r < total_rays * (t + 1) / T; ++r) {
+            const long s = r / n_rays, i = r % n_rays;
+            double nhat[3];
+            fib_direction(i, n_rays, nhat);
+            fx_t X0[3], D[3];
+            for (int a = 0; a < 3; ++a) {
+                X0[a] = fx(double(sources[3 * s + a]));
+                volatile double step = ds * nhat[a];
+                D[a] = fx(step);
+            }
+            std::vector<double> tau(n_bins, 0.0);
+            for (long k = 0; k < K; ++k) {                                  // forward sweep: geometry, a_k, T_k
+                long lo[3], hi[3];
+                double f[3];
+                for (int a = 0; a < 3; ++a) {
+                    const fx_t X = X0[a] + fx_t(k) * D[a];
+                    const long i0 = long((long long)(X >> 64));
+                    f[a] = double((unsigned long long)X) * 5.42101086242752217e-20;
+                    lo[a] = clampl(i0, 0, N[a] - 1);
+                    hi[a] = clampl(i0 + 1, 0, N[a] - 1);
+                }
+                for (int cc = 0; cc < 8; ++cc) {
+                    int dx = (cc >> 2) & 1, dy = (cc >> 1) & 1, dz = cc & 1;
+                    corner[k * 8 + cc] = M.cell(dx ? hi[0] : lo[0], dy ? hi[1] : lo[1], dz ? hi[2] : lo[2]);
+                    w[k * 8 + cc] = (dx ? f[0] : 1.0 - f[0]) * (dy ? f[1] : 1.0 - f[1]) * (dz ? f[2] : 1.0 - f[2]);
+                }
+                const size_t base = M.cell(lo[0], lo[1], lo[2]);
+                for (long b = 0; b < n_bins; ++b) {
+                    const double kap = double(kappa[base + b]);
+                    att[k * n_bins + b] = std::exp(-kap * ds);
+                    tr[k * n_bins + b] = std::exp(-tau[b]);
+                    tau[b] += kap * ds;
+                }
+            }
+            for (long b = 0; b < n_bins; ++b) {                             // backward recurrence
+                double lambda = 0.0, a_next = 0.0;
+                for (long k = K - 1; k >= 0; --k) {
+                    const double* gs = gsuf.data() + size_t(k / Ns) * grid;
+                    double G = 0.0;
+                    for (int cc = 0; cc < 8; ++cc) G += w[k * 8 + cc] * gs[corner[k * 8 + cc] + b];
+                    lambda = scale * G + a_next * lambda;
+                    a_next = att[k * n_bins + b];
+                    const double v = lambda * tr[k * n_bins + b] * ds;
+                    for (int cc = 0; cc < 8; ++cc) acc[t][corner[k * 8 + cc] + b] += w[k * 8 + cc] * v;
+                }
+            }
+        }
+    };
+    std::vector<std::thread> pool;
+    for (long t = 1; t < T; ++t) pool.emplace_back(work, t);
+    work(0);
+    for (auto& th : pool) th.join();
+    for (size_t v = 0; v < grid; ++v) {
+        double sum = 0.0;
+        for (long u = 0; u < T; ++u) sum += acc[u][v];
+        grad_j[v] = sum;
+    }
+    return 0;
+}
+
 const char* rt_oracle_version(void) { return "rt_oracle 1 (fp64, PAPER.md eq. 2)"; }
 
 }  // extern "C"

@@ -690,3 +690,67 @@ def test_d18_hand_trace_axis_ray(oracle_mod):
     tr = oracle_mod.trace_ray(j4[..., None], k4[..., None], (1.0, 1.0, 2.0), 0, 1, ds, 10, kappa_trilinear=True)
     assert np.allclose(tr["I"][:, 0], [w[0] for w in want], rtol=1e-14)
     assert np.allclose(tr["tau"][:, 0], [w[1] for w in want], rtol=1e-14)
+
+
+# ------------------------------------------------------------------------------------------------------
+# D19  adjoint of the march with respect to j.  The forward oracle is pinned above; the adjoint
+#      is pinned against it by the identity that DEFINES a transpose, <A j, g> = <j, A^T g>, for random j and g.
+# ------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("shape,nb,n_src,n_rays,ds,dt,n_steps", [
+    ((6, 5, 7), 1, 2, 13, 0.5, 4.0, 1),
+    ((5, 4, 3), 3, 3, 7, 0.37, 2.6, 3),         # several snapshots: gbar[m] acts on the CUMULATIVE field of step m
+    ((4, 4, 4), 2, 1, 1, 0.5, 5.0, 2),          # the axis ray, leaving the box (clamped deposits)
+])
+def test_d19_adjoint_is_the_transpose_of_the_march(oracle_mod, shape, nb, n_src, n_rays, ds, dt, n_steps):
+    rng = np.random.default_rng(sum(shape) + nb)
+    kap = rng.uniform(0.0, 0.6, shape + (nb,)).astype(np.float32)
+    src = rng.uniform(-1.0, max(shape), (n_src, 3)).astype(np.float32)
+    for trial in range(3):
+        j = rng.uniform(-1.0, 1.0, shape + (nb,)).astype(np.float32)           # signs allowed: the map is linear
+        g = rng.standard_normal((n_steps,) + shape + (nb,))
+        out = oracle_mod.march(j, kap, src, n_rays, ds, 1.0, dt, n_steps)
+        grad = oracle_mod.adjoint_j(g, kap, src, n_rays, ds, 1.0, dt, n_steps)
+        lhs, rhs = float((out * g).sum()), float((j.astype(np.float64) * grad).sum())
+        assert abs(lhs - rhs) <= 1e-11 * max(np.abs(out * g).sum(), 1e-300), (lhs, rhs)
+
+
+def test_d19_column_of_the_operator(oracle_mod):
+    """grad_j for gbar = a unit impulse at voxel v is row v of A: it equals the response at v to unit emissivity
+    placed voxel by voxel (brute force over all 27 cells of a 3^3 grid)."""
+    shape, n_rays, ds, dt = (3, 3, 3), 6, 0.5, 2.0
+    rng = np.random.default_rng(3)
+    kap = rng.uniform(0.1, 0.5, shape + (1,)).astype(np.float32)
+    src = np.array([[1.2, 0.9, 1.4]], dtype=np.float32)
+    v = (2, 1, 0, 0)
+    g = np.zeros((1,) + shape + (1,))
+    g[(0,) + v] = 1.0
+    grad = oracle_mod.adjoint_j(g, kap, src, n_rays, ds, 1.0, dt, 1)
+    for cell in np.ndindex(*shape):
+        j = np.zeros(shape + (1,), dtype=np.float32)
+        j[cell + (0,)] = 1.0
+        resp = oracle_mod.march(j, kap, src, n_rays, ds, 1.0, dt, 1)[(0,) + v]
+        assert abs(resp - grad[cell + (0,)]) <= 1e-13 * max(abs(resp), 1e-30)
+
+
+def test_d19_scalar_amplitude_inversion_matches_the_closed_form(oracle_mod):
+    """The paper's demo (P:62): recover A in j = A e0 from I_ref by minimising the MSE.  The loss is a parabola in A;
+    gradient descent with dL/dA = <e0, A^T (2/n)(A_op(A e0) - I_ref)> reaches the closed-form minimiser
+    <F, I_ref>/<F, F>, F = A_op e0."""
+    n = 8
+    rho = W.lognormal_density(n, 4, 0.8)
+    e0 = np.ascontiguousarray((rho ** 2)[..., None], dtype=np.float32)
+    kap = np.ascontiguousarray((0.1 * rho)[..., None], dtype=np.float32)
+    src = np.array([[3.5, 3.5, 3.5]], dtype=np.float32)
+    args = (src, 24, 0.5, 1.0, 3.0, 1)
+    F = oracle_mod.march(e0, kap, *args)
+    A_true = 2.5
+    I_ref = A_true * F + 0.01 * F.max() * np.random.default_rng(0).standard_normal(F.shape)
+    A_star = float((F * I_ref).sum() / (F * F).sum())
+    A = 0.3
+    lip = 2.0 * float((F * F).sum()) / F.size
+    for _ in range(40):
+        resid = A * F - I_ref
+        dLdA = float((e0.astype(np.float64) * oracle_mod.adjoint_j(2.0 * resid / F.size, kap, *args)).sum())
+        assert abs(dLdA - 2.0 * float((resid * F).sum()) / F.size) <= 1e-11 * 2.0 * float(np.abs(resid * F).sum()) / F.size
+        A -= dLdA / lip
+    assert abs(A - A_star) <= 1e-9 * abs(A_star)
