@@ -41,10 +41,11 @@ def parse():
     ap.add_argument("--config", default="C2", choices=["C0", "C1", "C2", "C3", "C4"])
     ap.add_argument("--impl", default="native", choices=["native", "reference"])
     ap.add_argument("--variant", type=int, default=0, help="RT_VARIANT_* (0 = the product path)")
-    ap.add_argument("--mode", default="march", choices=["march", "step", "trilinear_kappa"],
+    ap.add_argument("--mode", default="march", choices=["march", "step", "trilinear_kappa", "adjoint_j"],
                     help="march: one rt_march call per bench step (the headline); step: the same workload as n_steps "
                          "rt_march_step calls with persistent ray state (DESIGN.md D17); trilinear_kappa: "
-                         "rt_march_trilinear_kappa (DESIGN.md D18)")
+                         "rt_march_trilinear_kappa (DESIGN.md D18); adjoint_j: rt_march_adjoint_j, dL/dj for a "
+                         "random dL/d out (DESIGN.md D19; `out` then holds nothing useful)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target host time of the oracle sample")
@@ -237,7 +238,17 @@ def run_native(args):
         ws_step = torch.empty(max(16, rt.rt_step_workspace_bytes(nx, ny, nz, src.shape[0], w.n_rays, nb)),
                               dtype=torch.uint8, device="cuda")
 
+    if args.mode == "adjoint_j":
+        gbar = torch.rand((w.n_steps, nx, ny, nz, nb), dtype=torch.float32, device="cuda")
+        grad_j = torch.empty((nx, ny, nz, nb), dtype=torch.float32, device="cuda")
+        ws_adj = torch.empty(max(16, rt.rt_adjoint_workspace_bytes(nx, ny, nz, src.shape[0], w.n_rays, nb, w.n_steps)),
+                             dtype=torch.uint8, device="cuda")
+
     def step():
+        if args.mode == "adjoint_j":
+            rt.rt_march_adjoint_j(gbar, kappa, src, w.n_rays, w.step_size, w.c, w.dt, w.n_steps, grad_j=grad_j,
+                                  workspace=ws_adj)
+            return
         if args.mode == "step":        # n_steps calls, the field of the last snapshot accumulated in out[-1]
             rt.rt_state_reset(src.shape[0], w.n_rays, nb, state=state)
             out[-1].zero_()

@@ -107,6 +107,19 @@ int rt_march_step(const float* j, const float* kappa, int nx, int ny, int nz,
                   float step_size, float c, float dt, long long k_begin, float* state,
                   float* out, int accumulate, void* workspace, size_t workspace_bytes, void* stream);
 
+/* ADJOINT WITH RESPECT TO j (P:62-64 differentiability; reading D19).  For fixed kappa the field of
+ * rt_march is linear in j: out[m] = A_m j.  Given gbar[n_steps][nx][ny][nz][n_bins] = dL/d out[m] (device, fp32)
+ * this writes grad_j[nx][ny][nz][n_bins] = sum_m A_m^T gbar[m] = dL/dj (device, fp32, OVERWRITTEN; summed in fp64):
+ * the backward recurrence of eq. (2), marched along every ray from its last substep to its first with the same
+ * clamped trilinear stencils, gather and deposit exchanged.  <rt_march(j), gbar> = <j, grad_j> up to rounding.
+ * kappa is read nearest neighbour (as rt_march).  Same argument rules, limits and error codes as rt_march;
+ * workspace: rt_adjoint_workspace_bytes() bytes. */
+size_t rt_adjoint_workspace_bytes(int nx, int ny, int nz, int n_src, int n_rays, int n_bins, int n_steps);
+int rt_march_adjoint_j(const float* gbar, const float* kappa, int nx, int ny, int nz,
+                       const float* sources, int n_src, int n_rays, int n_bins,
+                       float step_size, float c, float dt, int n_steps, float* grad_j,
+                       void* workspace, size_t workspace_bytes, void* stream);
+
 /* End-to-end form with HOST pointers (j, kappa, sources, out are host memory, pinned or pageable).
  * Allocates device buffers, copies the inputs in, marches, copies out[] back, frees, and returns after the
  * copy has completed (SYNCHRONOUS).  Same semantics, limits and error codes as rt_march. */

@@ -10,6 +10,7 @@
 
 #include "rt_ceiling_kernels.cuh"
 #include "rt_march_direct.cuh"
+#include "rt_adjoint.cuh"
 #include "rt_march_sliding.cuh"
 #include "rt_setup_kernels.cuh"
 
@@ -319,6 +320,73 @@ int rt_march_ex(const float* j, const float* kappa, int nx, int ny, int nz, cons
                 size_t workspace_bytes, void* stream, int variant) {
     return march_impl(j, kappa, nx, ny, nz, sources, n_src, n_rays, n_bins, step_size, c, dt, n_steps, out, workspace,
                       workspace_bytes, stream, variant);
+}
+
+size_t rt_adjoint_workspace_bytes(int nx, int ny, int nz, int n_src, int n_rays, int n_bins, int n_steps) {
+    const size_t base = rt_workspace_bytes(nx, ny, nz, n_src, n_rays, n_bins, 1);
+    if (!base || n_steps < 1) return 0;
+    const size_t cells = size_t(nx) * ny * nz * n_bins;
+    return align_up(base, 256) + (n_steps > 1 ? cells * size_t(n_steps) * sizeof(float) : 0);
+}
+
+int rt_march_adjoint_j(const float* gbar, const float* kappa, int nx, int ny, int nz, const float* sources, int n_src,
+                       int n_rays, int n_bins, float step_size, float c, float dt, int n_steps, float* grad_j,
+                       void* workspace, size_t workspace_bytes, void* stream) {
+    Checked ck;
+    const int rc = check_args(gbar, kappa, nx, ny, nz, sources, n_src, n_rays, n_bins, step_size, c, dt, n_steps,
+                              grad_j, &ck);
+    if (rc != RT_OK) return rc;
+    const Workspace wl = workspace_layout(ck.cells, n_src, n_rays, 1);
+    const size_t need = rt_adjoint_workspace_bytes(nx, ny, nz, n_src, n_rays, n_bins, n_steps);
+    if (!workspace || workspace_bytes < need || (uintptr_t(workspace) & 15u)) return RT_EWORKSPACE;
+    char* ws = static_cast<char*>(workspace);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    Plan pl;
+    make_plan(RT_VARIANT_DEFAULT, n_src, &pl);
+
+    rt::MarchParams P{};
+    P.j = nullptr; P.kappa = kappa; P.sources = sources;
+    P.nx = nx; P.ny = ny; P.nz = nz; P.nb = n_bins;
+    P.n_src = n_src; P.src_begin = 0; P.slot_begin = 0; P.n_rays = n_rays;
+    P.n_groups = n_bins;
+    P.n_steps = n_steps; P.n_sub = int(ck.n_sub);
+    P.ds = double(step_size); P.ds_f = step_size;
+    P.emis = float(double(step_size) * 4.0 * 3.14159265358979323846 / double(n_rays));
+    P.att_scale = float(-double(step_size) * 1.4426950408889634074);
+    P.snap_stride = ck.cells;
+    P.map_src = pl.map_src ? 1 : 0;
+    P.kappa_trilinear = 0; P.state_I = nullptr; P.state_T = nullptr; P.k0 = 0;
+    P.ray_order = reinterpret_cast<const uint32_t*>(ws);
+    P.n_slots = ray_slots(n_rays);
+    const int rc2 = build_ray_order(n_rays, reinterpret_cast<uint32_t*>(ws), st);
+    if (rc2 != RT_OK) return rc2;
+    P.src_order = nullptr;
+    if (pl.map_src && n_src <= kMaxSortedSources) {
+        uint32_t* so = reinterpret_cast<uint32_t*>(ws + wl.src_order_at);
+        rt::src_order_kernel<<<(n_src + 3) / 4, 128, 0, st>>>(so, sources, n_src, nx, ny, nz);
+        RT_CUDA(cudaGetLastError());
+        P.src_order = so;
+    }
+    double* master = reinterpret_cast<double*>(ws + wl.acc_at);
+    P.acc = master;
+    RT_CUDA(cudaMemsetAsync(master, 0, size_t(ck.cells) * sizeof(double), st));
+    const int threads = 256;
+    long long blocks = (ck.cells + threads - 1) / threads;
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    const float* gsuf = gbar;
+    if (n_steps > 1) {                       // the snapshots are cumulative: step m feeds gbar[m], gbar[m+1], ...
+        float* gs = reinterpret_cast<float*>(ws + align_up(wl.total, 256));
+        rt::suffix_sum_kernel<<<unsigned(blocks), threads, 0, st>>>(gbar, gs, ck.cells, n_steps);
+        RT_CUDA(cudaGetLastError());
+        gsuf = gs;
+    }
+    const long long mb = rt::march_blocks(n_src, P.n_slots, P.n_groups, P.map_src);
+    if (mb > 2147483647LL) return RT_EINVAL;
+    rt::adjoint_j_kernel<6><<<unsigned(mb), rt::kThreads, 0, st>>>(P, gsuf);
+    RT_CUDA(cudaGetLastError());
+    rt::snapshot_finalize_kernel<double><<<unsigned(blocks), threads, 0, st>>>(master, grad_j, ck.cells, 1);
+    RT_CUDA(cudaGetLastError());
+    return RT_OK;
 }
 
 size_t rt_state_bytes(int n_src, int n_rays, int n_bins) {

@@ -85,18 +85,25 @@ template <int NB, typename ACC, bool KTRI> struct Stencil {
         return t;
     }
     // (re)build the stencil at the axes' current cells; pending deposits must have been flushed
-    __device__ __forceinline__ void restart(const MarchParams& P, TravelAxis (&A)[3], int negbits, int bin_off) {
+    __device__ __forceinline__ void restart(const MarchParams& P, TravelAxis (&A)[3], int negbits, int bin_off,
+                                            const float* jsrc) {
         base = bin_off + place<0>(P, A[0], negbits) + place<1>(P, A[1], negbits) + place<2>(P, A[2], negbits);
 #pragma unroll
+        reload(P, A, jsrc);
+    }
+    // (re)read the cached values of the 8 stencil voxels from `jsrc`
+    __device__ __forceinline__ void reload(const MarchParams& P, const TravelAxis (&A)[3], const float* jsrc) {
+#pragma unroll
         for (int s = 0; s < 8; ++s) {
-            jc[s] = ld_bins<NB>(P.j + off(s, A));
+            jc[s] = ld_bins<NB>(jsrc + off(s, A));
             if constexpr (KTRI) kc[s] = ld_bins<NB>(P.kappa + off(s, A));
         }
     }
     // Axis AX advanced by one cell.  The old leading plane is the new trailing plane (also under clamping: both
     // are clamp(c+1)), so the trailing index moves iff the axis was not merged; the new leading index is looked up.
     template <int AX>
-    __device__ __forceinline__ void axis_step(const MarchParams& P, TravelAxis (&A)[3], int negbits, ACC* og) {
+    __device__ __forceinline__ void axis_step(const MarchParams& P, TravelAxis (&A)[3], int negbits, ACC* og,
+                                              const float* jsrc) {
         TravelAxis& X = A[AX];
         // new leading minus new trailing offset: +-stride while both indices are inside the domain, i.e. u-cell
         // c in [0, lim-1] (ascending: indices c, c+1) or [-lim, -1] (descending: indices -c, -c-1); else 0
@@ -128,7 +135,7 @@ template <int NB, typename ACC, bool KTRI> struct Stencil {
 #pragma unroll
                 for (int v = 0; v < 2; ++v) {
                     const int s1 = slot<AX>(1, u, v);
-                    jc[s1] = ld_bins<NB>(P.j + off(s1, A));
+                    jc[s1] = ld_bins<NB>(jsrc + off(s1, A));
                     if constexpr (KTRI) kc[s1] = ld_bins<NB>(P.kappa + off(s1, A));
                 }
         }
@@ -160,7 +167,7 @@ __global__ void __launch_bounds__(kThreads, MINB) march_sliding_kernel(const Mar
     Stencil<NB, ACC, KTRI> S;
 #pragma unroll
     for (int s = 0; s < 8; ++s) S.zero_slot(s);
-    S.restart(P, A, negbits, id.group * NB);
+    S.restart(P, A, negbits, id.group * NB, P.j);
 
     float I[NB], T[NB], att[NB];     // I scaled by 4 pi/N_Omega; T = exp(-tau); att = exp(-kappa ds) of the kappa cell
 #pragma unroll
@@ -234,11 +241,11 @@ __global__ void __launch_bounds__(kThreads, MINB) march_sliding_kernel(const Mar
             if ((c0 ^ A[0].p.c) | (c1 ^ A[1].p.c) | (c2 ^ A[2].p.c)) {
                 if (long_steps && (((A[0].p.c - c0) | (A[1].p.c - c1) | (A[2].p.c - c2)) > 1)) {
                     S.flush_all(og, A);            // a step longer than a cell: restart the stencil
-                    S.restart(P, A, negbits, id.group * NB);
+                    S.restart(P, A, negbits, id.group * NB, P.j);
                 } else {
-                    if (c0 != A[0].p.c) S.template axis_step<0>(P, A, negbits, og);
-                    if (c1 != A[1].p.c) S.template axis_step<1>(P, A, negbits, og);
-                    if (c2 != A[2].p.c) S.template axis_step<2>(P, A, negbits, og);
+                    if (c0 != A[0].p.c) S.template axis_step<0>(P, A, negbits, og, P.j);
+                    if (c1 != A[1].p.c) S.template axis_step<1>(P, A, negbits, og, P.j);
+                    if (c2 != A[2].p.c) S.template axis_step<2>(P, A, negbits, og, P.j);
                 }
                 if (!KTRI) load_att();
             }

@@ -1,0 +1,99 @@
+"""rt_march_adjoint_j (dL/dj, reading D19) against the fp64 oracle's adjoint, element by
+element, and against the forward CUDA march through the transpose identity <A j, g> = <j, A^T g>."""
+import numpy as np
+import pytest
+
+import parity
+from paper_2511_09389_b200 import workloads
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def rt():
+    if not torch.cuda.is_available():
+        pytest.fail("-m gpu tests need a CUDA device")
+    import paper_2511_09389_b200 as rt
+    return rt
+
+
+def _dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+@pytest.mark.parametrize("shape,nb,n_src,n_rays,ds,dt,n_steps", [
+    ((4, 4, 4), 1, 1, 1, 0.5, 4.0, 1),            # the axis ray through and out of a 4-cube
+    ((5, 4, 3), 3, 2, 7, 0.5, 5.0, 1),            # rays landing exactly on cell planes (rational z_i)
+    ((6, 5, 7), 8, 1, 40, 0.5, 8.0, 3),           # source outside the box, three snapshots
+    ((9, 8, 7), 1, 40, 24, 0.25, 4.0, 2),         # warp = 32 sources x 1 direction, ragged group
+    ((7, 6, 9), 4, 33, 11, 0.5, 4.0, 2),          # 4 bins, cell-centred and duplicate sources
+    ((8, 8, 8), 2, 3, 50, 1.7, 13.6, 1),          # steps longer than a cell
+])
+def test_adjoint_matches_the_oracle(rt, oracle_mod, shape, nb, n_src, n_rays, ds, dt, n_steps):
+    rng = np.random.default_rng(sum(shape) + nb + n_src)
+    kap = rng.uniform(0.0, 0.6, shape + (nb,)).astype(np.float32)
+    src = rng.uniform(-2.0, max(shape) + 1.0, (n_src, 3))
+    if n_src > 3:
+        src = np.round(src)
+        src[1] = src[0]
+    src = src.astype(np.float32)
+    if n_src == 1 and n_rays == 1:
+        src = np.array([[1.0, 2.0, 1.0]], dtype=np.float32)
+    gbar = rng.uniform(0.0, 1.0, (n_steps,) + shape + (nb,)).astype(np.float32)      # >= 0: no cancellation in grad
+    ref = oracle_mod.adjoint_j(gbar, kap, src, n_rays, ds, 1.0, dt, n_steps)
+    got = rt.rt_march_adjoint_j(_dev(gbar), _dev(kap), _dev(src), n_rays, ds, 1.0, dt, n_steps)
+    torch.cuda.synchronize()
+    parity.assert_parity(got.cpu().numpy()[None], ref[None], f"adjoint {shape} nb={nb} n_src={n_src} steps={n_steps}")
+
+
+@pytest.mark.parametrize("name,n_sub_src", [("C1", None), ("C2", 96), ("C3", 40)])
+def test_adjoint_is_the_transpose_of_the_cuda_march(rt, name, n_sub_src):
+    w = workloads.make_config(name)
+    src = w.sources if n_sub_src is None else np.ascontiguousarray(
+        w.sources[np.unique(np.linspace(0, w.n_src - 1, n_sub_src).round().astype(int))])
+    rng = np.random.default_rng(7)
+    j = _dev(w.j)
+    kap, dsrc = _dev(w.kappa), _dev(src)
+    out = rt.rt_march(j, kap, dsrc, w.n_rays, w.step_size, w.c, w.dt, w.n_steps)
+    for trial in range(2):
+        g = torch.from_numpy(rng.uniform(0.0, 1.0, tuple(out.shape)).astype(np.float32)).cuda()
+        grad = rt.rt_march_adjoint_j(g, kap, dsrc, w.n_rays, w.step_size, w.c, w.dt, w.n_steps)
+        torch.cuda.synchronize()
+        lhs = float((out.double() * g.double()).sum())
+        rhs = float((j.double() * grad.double()).sum())
+        assert abs(lhs - rhs) <= 2e-5 * abs(lhs), (name, lhs, rhs)
+
+
+def test_scalar_amplitude_inversion_on_the_gpu(rt):
+    """recover A in j = A e0 from a reference field by gradient descent on the MSE, the gradient from
+    the adjoint; the minimiser is the closed form <F, I_ref>/<F, F>."""
+    w = workloads.make_config("C1")
+    e0, kap, src = _dev(w.j), _dev(w.kappa), _dev(w.sources)
+    args = (w.n_rays, w.step_size, w.c, w.dt, w.n_steps)
+    F = rt.rt_march(e0, kap, src, *args).double()
+    noise = torch.from_numpy(np.random.default_rng(1).standard_normal(tuple(F.shape))).cuda()
+    I_ref = 1.8 * F + 0.02 * F.max() * noise
+    A_star = float((F * I_ref).sum() / (F * F).sum())
+    n = F.numel()
+    lip = 2.0 * float((F * F).sum()) / n
+    A = 0.2
+    for _ in range(25):
+        resid = (A * F - I_ref)
+        grad_j = rt.rt_march_adjoint_j((2.0 * resid / n).float(), kap, src, *args)
+        A -= float((e0.double() * grad_j.double()).sum()) / lip
+    torch.cuda.synchronize()
+    assert abs(A - A_star) <= 2e-4 * abs(A_star), (A, A_star)
+
+
+def test_adjoint_argument_errors(rt):
+    n = 6
+    k = torch.zeros((n, n, n, 1), device="cuda")
+    g = torch.zeros((1, n, n, n, 1), device="cuda")
+    s = torch.zeros((1, 3), device="cuda")
+    with pytest.raises(rt.RtError) as e:
+        rt.rt_march_adjoint_j(g, k, s, 16, 0.5, 1.0, 2.0, 1, workspace=torch.empty(16, dtype=torch.uint8, device="cuda"))
+    assert e.value.code == rt.RT_EWORKSPACE
+    with pytest.raises(ValueError):
+        rt.rt_march_adjoint_j(g, k, s, 16, 0.5, 1.0, 2.0, 2)
