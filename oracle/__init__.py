@@ -59,6 +59,10 @@ def lib() -> ctypes.CDLL:
             L.rt_adjoint_j_oracle.argtypes = [dp, fp, ctypes.c_int, ctypes.c_int, ctypes.c_int, fp, ctypes.c_int,
                                               ctypes.c_int, ctypes.c_int, ctypes.c_float, ctypes.c_float,
                                               ctypes.c_float, ctypes.c_int, dp, ctypes.c_int]
+            L.rt_adjoint_kappa_oracle.restype = ctypes.c_int
+            L.rt_adjoint_kappa_oracle.argtypes = [dp, fp, fp, ctypes.c_int, ctypes.c_int, ctypes.c_int, fp, ctypes.c_int,
+                                                  ctypes.c_int, ctypes.c_int, ctypes.c_float, ctypes.c_float,
+                                                  ctypes.c_float, ctypes.c_int, dp, ctypes.c_int]
             L.rt_oracle_step.restype = ctypes.c_int
             L.rt_oracle_step.argtypes = [fp, fp, ctypes.c_int, ctypes.c_int, ctypes.c_int, fp, ctypes.c_int,
                                          ctypes.c_int, ctypes.c_int, ctypes.c_float, ctypes.c_float, ctypes.c_float,
@@ -139,6 +143,26 @@ def adjoint_j(gbar, kappa, sources, n_rays, step_size, c, dt, n_steps, n_threads
                                    step_size, c, dt, n_steps, _dp(grad), n_threads)
     if rc:
         raise ValueError("rt_adjoint_j_oracle: invalid arguments")
+    return grad
+
+
+def adjoint_kappa(gbar, j, kappa, sources, n_rays, step_size, c, dt, n_steps, n_threads: int | None = None) -> np.ndarray:
+    """dL/dkappa for dL/d out[m] = gbar[m]: float64 [nx, ny, nz, n_bins] (D19)."""
+    j = _f32(j, 4)
+    kappa = _f32(kappa, 4)
+    sources = _f32(sources, 2)
+    nx, ny, nz, nb = kappa.shape
+    gbar = np.ascontiguousarray(gbar, dtype=np.float64)
+    if gbar.shape != (n_steps, nx, ny, nz, nb) or j.shape != kappa.shape:
+        raise ValueError("gbar must be [n_steps, nx, ny, nz, n_bins] and j must have kappa's shape")
+    if n_threads is None:
+        n_threads = host_threads()
+    n_threads = max(1, min(n_threads, (24 << 30) // max(1, kappa.size * 8)))
+    grad = np.empty((nx, ny, nz, nb), dtype=np.float64)
+    rc = lib().rt_adjoint_kappa_oracle(_dp(gbar), _fp(j), _fp(kappa), nx, ny, nz, _fp(sources), sources.shape[0], n_rays,
+                                       nb, step_size, c, dt, n_steps, _dp(grad), n_threads)
+    if rc:
+        raise ValueError("rt_adjoint_kappa_oracle: invalid arguments")
     return grad
 
 

@@ -411,6 +411,99 @@ int rt_adjoint_j_oracle(const double* gbar, const float* kappa, int nx, int ny, 
     return 0;
 }
 
+// ADJOINT with respect to kappa (the other half of P:64's Jacobian; reading D19).  kappa enters eq. (2)
+// through a_k = exp(-kappa_k ds) and T_k = exp(-ds sum_{i<k} kappa_i), kappa_i = kappa[cell of x_i] (nearest
+// neighbour, P:29 / D4; the cells do not depend on kappa).  Unrolling eq. (2), I_{k+1} = T_{k+1} sum_{m<=k} ds J_m / a_m
+// with J_m = w_m . j, so for L = sum_k G_k I_{k+1}, G_k = s w_k . gsuf[step(k)]:
+//     dL/dkappa_i = ds [ ds J_i T_i lambda_{i+1} - R_i ],   R_i = sum_{k >= i} G_k I_{k+1},
+// lambda as in rt_adjoint_j_oracle.  Forward sweep recording every substep, then the backward sums, as it reads.
+// grad_kappa: double [nx][ny][nz][B], overwritten.
+int rt_adjoint_kappa_oracle(const double* gbar, const float* j, const float* kappa, int nx, int ny, int nz,
+                            const float* sources, int n_src, int n_rays, int n_bins, float step_size, float c, float dt,
+                            int n_steps, double* grad_kappa, int n_threads) {
+    if (!gbar || !j || !kappa || !sources || !grad_kappa) return -1;
+    if (nx < 1 || ny < 1 || nz < 1 || n_src < 1 || n_rays < 1 || n_bins < 1 || n_steps < 1) return -1;
+    if (bad(step_size) || bad(c) || bad(dt)) return -1;
+    const long Ns = substeps(double(step_size), double(c), double(dt)), K = Ns * n_steps;
+    const double ds = double(step_size);
+    const long N[3] = {nx, ny, nz};
+    const Medium M{j, kappa, nx, ny, nz, n_bins};
+    const size_t grid = size_t(nx) * ny * nz * n_bins;
+    const double scale = double(4.0L * kPiL / (long double)n_rays);
+    std::vector<double> gsuf(gbar, gbar + grid * size_t(n_steps));
+    for (long m = n_steps - 2; m >= 0; --m)
+        for (size_t v = 0; v < grid; ++v) gsuf[size_t(m) * grid + v] += gsuf[size_t(m + 1) * grid + v];
+    const long total_rays = long(n_src) * n_rays;
+    const long T = std::min<long>(std::max(1, n_threads), total_rays);
+    std::vector<std::vector<double>> acc(T);
+    for (auto& a : acc) a.assign(grid, 0.0);
+    auto work = [&](long t) {
+        std::vector<size_t> corner(size_t(K) * 8), cell(K);
+        std::vector<double> w(size_t(K) * 8), att(K), tr(K), Inext(K), Jv(K);
+        for (long r = total_rays * t / T; r < total_rays * (t + 1) / T; ++r) {
+            const long s = r / n_rays, i = r % n_rays;
+            double nhat[3];
+            fib_direction(i, n_rays, nhat);
+            fx_t X0[3], D[3];
+            for (int a = 0; a < 3; ++a) {
+                X0[a] = fx(double(sources[3 * s + a]));
+                volatile double step = ds * nhat[a];
+                D[a] = fx(step);
+            }
+            for (long b = 0; b < n_bins; ++b) {
+                double I = 0.0, tau = 0.0;
+                for (long k = 0; k < K; ++k) {                              // forward sweep, eq. (2)
+                    long lo[3], hi[3];
+                    double f[3];
+                    for (int a = 0; a < 3; ++a) {
+                        const fx_t X = X0[a] + fx_t(k) * D[a];
+                        const long i0 = long((long long)(X >> 64));
+                        f[a] = double((unsigned long long)X) * 5.42101086242752217e-20;
+                        lo[a] = clampl(i0, 0, N[a] - 1);
+                        hi[a] = clampl(i0 + 1, 0, N[a] - 1);
+                    }
+                    double jv = 0.0;
+                    for (int cc = 0; cc < 8; ++cc) {
+                        int dx = (cc >> 2) & 1, dy = (cc >> 1) & 1, dz = cc & 1;
+                        corner[k * 8 + cc] = M.cell(dx ? hi[0] : lo[0], dy ? hi[1] : lo[1], dz ? hi[2] : lo[2]);
+                        w[k * 8 + cc] = (dx ? f[0] : 1.0 - f[0]) * (dy ? f[1] : 1.0 - f[1]) * (dz ? f[2] : 1.0 - f[2]);
+                        jv += w[k * 8 + cc] * double(j[corner[k * 8 + cc] + b]);
+                    }
+                    cell[k] = M.cell(lo[0], lo[1], lo[2]);
+                    const double kap = double(kappa[cell[k] + b]);
+                    att[k] = std::exp(-kap * ds);
+                    tr[k] = std::exp(-tau);
+                    Jv[k] = jv;
+                    I = I * att[k] + jv * tr[k] * ds;
+                    tau += kap * ds;
+                    Inext[k] = I;
+                }
+                double lambda = 0.0, a_next = 0.0, R = 0.0;
+                for (long k = K - 1; k >= 0; --k) {                         // backward sums
+                    const double* gs = gsuf.data() + size_t(k / Ns) * grid;
+                    double G = 0.0;
+                    for (int cc = 0; cc < 8; ++cc) G += w[k * 8 + cc] * gs[corner[k * 8 + cc] + b];
+                    G *= scale;
+                    lambda = G + a_next * lambda;
+                    a_next = att[k];
+                    R += G * Inext[k];
+                    acc[t][cell[k] + b] += ds * (ds * Jv[k] * tr[k] * lambda - R);
+                }
+            }
+        }
+    };
+    std::vector<std::thread> pool;
+    for (long t = 1; t < T; ++t) pool.emplace_back(work, t);
+    work(0);
+    for (auto& th : pool) th.join();
+    for (size_t v = 0; v < grid; ++v) {
+        double sum = 0.0;
+        for (long u = 0; u < T; ++u) sum += acc[u][v];
+        grad_kappa[v] = sum;
+    }
+    return 0;
+}
+
 const char* rt_oracle_version(void) { return "rt_oracle 1 (fp64, PAPER.md eq. 2)"; }
 
 }  // extern "C"
