@@ -41,7 +41,7 @@ def parse():
     ap.add_argument("--config", default="C2", choices=["C0", "C1", "C2", "C3", "C4"])
     ap.add_argument("--impl", default="native", choices=["native", "reference"])
     ap.add_argument("--variant", type=int, default=0, help="RT_VARIANT_* (0 = the product path)")
-    ap.add_argument("--mode", default="march", choices=["march", "step", "trilinear_kappa", "adjoint_j"],
+    ap.add_argument("--mode", default="march", choices=["march", "step", "trilinear_kappa", "adjoint_j", "adjoint_kappa"],
                     help="march: one rt_march call per bench step (the headline); step: the same workload as n_steps "
                          "rt_march_step calls with persistent ray state (DESIGN.md D17); trilinear_kappa: "
                          "rt_march_trilinear_kappa (DESIGN.md D18); adjoint_j: rt_march_adjoint_j, dL/dj for a "
@@ -244,7 +244,18 @@ def run_native(args):
         ws_adj = torch.empty(max(16, rt.rt_adjoint_workspace_bytes(nx, ny, nz, src.shape[0], w.n_rays, nb, w.n_steps)),
                              dtype=torch.uint8, device="cuda")
 
+    if args.mode == "adjoint_kappa":
+        gbar = torch.rand((w.n_steps, nx, ny, nz, nb), dtype=torch.float32, device="cuda")
+        grad_j = torch.empty((nx, ny, nz, nb), dtype=torch.float32, device="cuda")
+        ws_adj = torch.empty(max(16, rt.rt_adjoint_kappa_workspace_bytes(nx, ny, nz, src.shape[0], w.n_rays, nb, w.step_size,
+                                                                         w.c, w.dt, w.n_steps)),
+                             dtype=torch.uint8, device="cuda")
+
     def step():
+        if args.mode == "adjoint_kappa":
+            rt.rt_march_adjoint_kappa(gbar, j, kappa, src, w.n_rays, w.step_size, w.c, w.dt, w.n_steps, grad_kappa=grad_j,
+                                      workspace=ws_adj)
+            return
         if args.mode == "adjoint_j":
             rt.rt_march_adjoint_j(gbar, kappa, src, w.n_rays, w.step_size, w.c, w.dt, w.n_steps, grad_j=grad_j,
                                   workspace=ws_adj)

@@ -120,6 +120,20 @@ int rt_march_adjoint_j(const float* gbar, const float* kappa, int nx, int ny, in
                        float step_size, float c, float dt, int n_steps, float* grad_j,
                        void* workspace, size_t workspace_bytes, void* stream);
 
+/* ADJOINT WITH RESPECT TO kappa (the other half of P:64's Jacobian; reading D19).  Writes
+ * grad_kappa[nx][ny][nz][n_bins] = dL/dkappa (device, fp32, OVERWRITTEN; summed in fp64) for gbar[m] = dL/d out[m] of
+ * rt_march(j, kappa, ...): kappa enters eq. (2) through exp(-kappa ds) and exp(-tau), read nearest neighbour at the
+ * cell of x_k, so dL/dkappa_i = ds [P_i lambda_{i+1} - sum_{k>=i} G_k I_{k+1}] summed into that cell.  The forward
+ * intensities are recorded (8 bytes per ray-substep-bin, sources in batches so the record stays below 2 GiB) and the
+ * rays are then marched backwards.  Same argument rules, limits and error codes as rt_march; workspace:
+ * rt_adjoint_kappa_workspace_bytes() bytes (0 on invalid arguments). */
+size_t rt_adjoint_kappa_workspace_bytes(int nx, int ny, int nz, int n_src, int n_rays, int n_bins,
+                                        float step_size, float c, float dt, int n_steps);
+int rt_march_adjoint_kappa(const float* gbar, const float* j, const float* kappa, int nx, int ny, int nz,
+                           const float* sources, int n_src, int n_rays, int n_bins,
+                           float step_size, float c, float dt, int n_steps, float* grad_kappa,
+                           void* workspace, size_t workspace_bytes, void* stream);
+
 /* End-to-end form with HOST pointers (j, kappa, sources, out are host memory, pinned or pageable).
  * Allocates device buffers, copies the inputs in, marches, copies out[] back, frees, and returns after the
  * copy has completed (SYNCHRONOUS).  Same semantics, limits and error codes as rt_march. */

@@ -25,7 +25,7 @@ EXPORTS = ("rt_march", "rt_march_single", "rt_march_ex", "rt_march_host", "rt_wo
            "rt_substeps_per_step", "rt_launch_count", "rt_directions", "rt_ray_order", "rt_ray_slots", "rt_trace_ray",
            "rt_bench_red_ceiling", "rt_strerror", "rt_version", "rt_state_bytes", "rt_state_reset",
            "rt_step_workspace_bytes", "rt_march_step", "rt_march_trilinear_kappa", "rt_adjoint_workspace_bytes",
-           "rt_march_adjoint_j")
+           "rt_march_adjoint_j", "rt_adjoint_kappa_workspace_bytes", "rt_march_adjoint_kappa")
 
 
 class RtError(RuntimeError):
@@ -52,6 +52,9 @@ def _load() -> ctypes.CDLL:
     L.rt_adjoint_workspace_bytes.argtypes = [i] * 7
     L.rt_adjoint_workspace_bytes.restype = sz
     L.rt_march_adjoint_j.argtypes = march_args + [vp, sz, vp]
+    L.rt_adjoint_kappa_workspace_bytes.argtypes = [i] * 6 + [f, f, f, i]
+    L.rt_adjoint_kappa_workspace_bytes.restype = sz
+    L.rt_march_adjoint_kappa.argtypes = [vp] + march_args + [vp, sz, vp]
     L.rt_march_single.argtypes = [vp, vp, i, i, i, vp, i, i, f, f, f, i, vp, vp, sz, vp]
     L.rt_march_ex.argtypes = march_args + [vp, sz, vp, i]
     L.rt_march_host.argtypes = march_args
@@ -208,8 +211,42 @@ def rt_march_adjoint_j(gbar, kappa, sources, n_rays, step_size, c, dt, n_steps, 
                                  step_size, c, dt, n_steps, grad_j.data_ptr(), workspace.data_ptr(), workspace.numel(),
                                  _stream_ptr(stream))
     if rc != RT_OK:
-        raise RtError(rc, "rt_march_adjoint_j")
+        raise RtError(rc, "rt_march_adjoint_j", "rt_adjoint_kappa_workspace_bytes", "rt_march_adjoint_kappa")
     return grad_j
+
+
+def rt_adjoint_kappa_workspace_bytes(nx, ny, nz, n_src, n_rays, n_bins, step_size, c, dt, n_steps) -> int:
+    return int(_lib.rt_adjoint_kappa_workspace_bytes(nx, ny, nz, n_src, n_rays, n_bins, step_size, c, dt, n_steps))
+
+
+def rt_march_adjoint_kappa(gbar, j, kappa, sources, n_rays, step_size, c, dt, n_steps, grad_kappa=None, workspace=None,
+                           stream=None):
+    """grad_kappa [nx,ny,nz,n_bins] = dL/dkappa for gbar [n_steps,nx,ny,nz,n_bins] = dL/d out (D19)."""
+    torch = _torch()
+    _check_dev(gbar, "gbar", torch.float32, 5)
+    _check_dev(j, "j", torch.float32, 4)
+    _check_dev(kappa, "kappa", torch.float32, 4)
+    _check_dev(sources, "sources", torch.float32, 2)
+    nx, ny, nz, nb = kappa.shape
+    if tuple(gbar.shape) != (n_steps, nx, ny, nz, nb) or j.shape != kappa.shape or sources.shape[1] != 3:
+        raise ValueError("gbar must be [n_steps, nx, ny, nz, n_bins], j like kappa, sources [n_src, 3]")
+    n_src = sources.shape[0]
+    if grad_kappa is None:
+        grad_kappa = torch.empty((nx, ny, nz, nb), dtype=torch.float32, device=kappa.device)
+    else:
+        _check_dev(grad_kappa, "grad_kappa", torch.float32)
+        if grad_kappa.numel() != kappa.numel():
+            raise ValueError("grad_kappa has the wrong size")
+    if workspace is None:
+        workspace = torch.empty(max(16, rt_adjoint_kappa_workspace_bytes(nx, ny, nz, n_src, n_rays, nb, step_size, c, dt,
+                                                                         n_steps)),
+                                dtype=torch.uint8, device=kappa.device)
+    rc = _lib.rt_march_adjoint_kappa(gbar.data_ptr(), j.data_ptr(), kappa.data_ptr(), nx, ny, nz, sources.data_ptr(),
+                                     n_src, n_rays, nb, step_size, c, dt, n_steps, grad_kappa.data_ptr(),
+                                     workspace.data_ptr(), workspace.numel(), _stream_ptr(stream))
+    if rc != RT_OK:
+        raise RtError(rc, "rt_march_adjoint_kappa")
+    return grad_kappa
 
 
 def rt_march_single(j, kappa, source_pos, n_rays, step_size, c, dt, n_steps, out=None, workspace=None,

@@ -13,14 +13,22 @@
 // the forward ray's, bit for bit, hence the same cells and the same weight bits.  tau_k is recovered by
 // subtracting kappa_k ds in fp64 (an fp32 running difference would lose 1e-3 of T over a few hundred substeps).
 #pragma once
+#include "rt_march_direct.cuh"
 #include "rt_march_sliding.cuh"
 
 namespace rt {
 
-template <int MINB>
-__global__ void __launch_bounds__(kThreads, MINB) adjoint_j_kernel(const MarchParams P, const float* gsuf) {
+// WRT_KAPPA = false: dL/dj as described above.  WRT_KAPPA = true: dL/dkappa (D19).  Unrolling eq. (2),
+// I_{k+1} = T_{k+1} sum_{m<=k} ds J_m / a_m, so with G_k = w_k . gsuf and P_i = ds J_i T_i (the emission term of
+// substep i) dL/dkappa_i = ds [P_i lambda_{i+1} - R_i], R_i = sum_{k>=i} G_k I_{k+1}: the same backward march,
+// fed with (I_{k+1}, P_k) of every substep as recorded by forward_store_kernel, summing into the kappa cell of x_i
+// (nearest neighbour: one voxel per substep, reduced when the cell changes).
+template <int MINB, bool WRT_KAPPA>
+__global__ void __launch_bounds__(kThreads, MINB) adjoint_kernel(const MarchParams P, const float* gsuf,
+                                                                 const float2* fwd, long long fwd_stride) {
     RayId id;
     if (!ray_id(P, id)) return;
+    const long long tid = (long long)blockIdx.x * kThreads + threadIdx.x;
     const int bin = id.group;                       // one bin per thread (n_groups = n_bins)
     double* og = static_cast<double*>(P.acc);
 
@@ -40,12 +48,17 @@ __global__ void __launch_bounds__(kThreads, MINB) adjoint_j_kernel(const MarchPa
     const int sx = P.ny * P.nz * P.nb, sy = P.nz * P.nb, sz = P.nb;
     double tau = 0.0;
     const long long K = (long long)P.n_steps * P.n_sub;
-    for (long long k = 0; k < K; ++k) {
-        const int o = min(max(X[0].c, 0), P.nx - 1) * sx + min(max(X[1].c, 0), P.ny - 1) * sy +
-                      min(max(X[2].c, 0), P.nz - 1) * sz;
-        tau = fma(double(__ldg(P.kappa + o + bin)), P.ds, tau);
+    if (WRT_KAPPA) {                                 // tau is not needed: jump to x_K
 #pragma unroll
-        for (int a = 0; a < 3; ++a) fx_add(X[a], D[a]);
+        for (int a = 0; a < 3; ++a) fx_advance(X[a], D[a], K);
+    } else {
+        for (long long k = 0; k < K; ++k) {
+            const int o = min(max(X[0].c, 0), P.nx - 1) * sx + min(max(X[1].c, 0), P.ny - 1) * sy +
+                          min(max(X[2].c, 0), P.nz - 1) * sz;
+            tau = fma(double(__ldg(P.kappa + o + bin)), P.ds, tau);
+#pragma unroll
+            for (int a = 0; a < 3; ++a) fx_add(X[a], D[a]);
+        }
     }
     // phase 2: backwards from x_{K-1}
     TravelAxis A[3];
@@ -74,12 +87,20 @@ __global__ void __launch_bounds__(kThreads, MINB) adjoint_j_kernel(const MarchPa
     S.restart(P, A, negbits, bin, gs);
 
     float lambda = 0.0f, a_next = 0.0f, kap = 0.0f, att = 1.0f;
+    double Rsum = 0.0, kacc = 0.0;                   // WRT_KAPPA: R_i and the pending sum for the current kappa cell (fp64:
+                                                     // P_i lambda_{i+1} - R_i cancels)
+    int ko = 0;
     auto load_kappa = [&]() {
-        const int ko = S.base + ((negbits & 1) ? A[0].dl : 0) + ((negbits & 2) ? A[1].dl : 0) + ((negbits & 4) ? A[2].dl : 0);
+        ko = S.base + ((negbits & 1) ? A[0].dl : 0) + ((negbits & 2) ? A[1].dl : 0) + ((negbits & 4) ? A[2].dl : 0);
         kap = __ldg(P.kappa + ko);
         att = ex2_approx(kap * P.att_scale);
     };
+    auto flush_kappa = [&]() {
+        if (kacc != 0.0) asm volatile("red.global.add.f64 [%0], %1;" ::"l"(og + ko), "d"(kacc) : "memory");
+        kacc = 0.0;
+    };
     load_kappa();
+    long long kk = K - 1;                            // global substep index of the backward sweep
 
     for (int m = P.n_steps - 1; m >= 0; --m) {
         if (m != P.n_steps - 1) {                    // an earlier time step sees the suffix sum of one more snapshot
@@ -102,13 +123,22 @@ __global__ void __launch_bounds__(kThreads, MINB) adjoint_j_kernel(const MarchPa
                 gv = fmaf(w[s], S.jc[s].v[0], gv);
                 gu = fmaf(w[s + 1], S.jc[s + 1].v[0], gu);
             }
-            tau = fma(-double(kap), P.ds, tau);                                   // tau_k = tau_{k+1} - kappa_k ds
-            const float T = ex2_approx(float(tau * -1.4426950408889634));         // exp(-tau_k)
-            lambda = fmaf(a_next, lambda, (gv + gu) * P.emis);                    // lambda_{k+1} ds
-            a_next = att;
-            const float v = lambda * T;
+            if (WRT_KAPPA) {
+                const float2 rec = __ldg(fwd + kk * fwd_stride + tid);            // (I_{k+1}, P_k), both x 4 pi/N_Omega
+                lambda = fmaf(a_next, lambda, gv + gu);
+                a_next = att;
+                Rsum = fma(double(gv + gu), double(rec.x), Rsum);
+                kacc = fma(fma(double(rec.y), double(lambda), -Rsum), P.ds, kacc);
+                --kk;
+            } else {
+                tau = fma(-double(kap), P.ds, tau);                               // tau_k = tau_{k+1} - kappa_k ds
+                const float T = ex2_approx(float(tau * -1.4426950408889634));     // exp(-tau_k)
+                lambda = fmaf(a_next, lambda, (gv + gu) * P.emis);                // lambda_{k+1} ds
+                a_next = att;
+                const float v = lambda * T;
 #pragma unroll
-            for (int s = 0; s < 8; ++s) S.acc[s].v[0] = fmaf(w[s], v, S.acc[s].v[0]);
+                for (int s = 0; s < 8; ++s) S.acc[s].v[0] = fmaf(w[s], v, S.acc[s].v[0]);
+            }
 
             const int c0 = A[0].p.c, c1 = A[1].p.c, c2 = A[2].p.c;
 #pragma unroll
@@ -122,11 +152,53 @@ __global__ void __launch_bounds__(kThreads, MINB) adjoint_j_kernel(const MarchPa
                     if (c1 != A[1].p.c) S.template axis_step<1>(P, A, negbits, og, gs);
                     if (c2 != A[2].p.c) S.template axis_step<2>(P, A, negbits, og, gs);
                 }
-                load_kappa();
+                if (WRT_KAPPA) {                     // the kappa cell may have changed: reduce the old one's sum
+                    const int ko_old = ko;
+                    load_kappa();
+                    if (ko != ko_old) {
+                        if (kacc != 0.0)
+                            asm volatile("red.global.add.f64 [%0], %1;" ::"l"(og + ko_old), "d"(kacc) : "memory");
+                        kacc = 0.0;
+                    }
+                } else {
+                    load_kappa();
+                }
             }
         }
     }
-    S.flush_all(og, A);
+    if (WRT_KAPPA) flush_kappa();
+    else S.flush_all(og, A);
+}
+
+// The forward march of eq. (2) with nothing deposited: records (I_{k+1}, P_k = ds J_k T_k), both scaled
+// by 4 pi / N_Omega, of every substep of every ray of the launch, laid out [substep][thread] so a warp writes one
+// 256-byte run per substep.  Same thread -> ray mapping as adjoint_kernel (same MarchParams).
+__global__ void __launch_bounds__(kThreads) forward_store_kernel(const MarchParams P, float2* fwd, long long fwd_stride) {
+    RayId id;
+    if (!ray_id(P, id)) return;
+    const long long tid = (long long)blockIdx.x * kThreads + threadIdx.x;
+    const int bin = id.group;
+    RaySetup R = ray_setup(P, id);
+    const int sx = P.ny * P.nz * P.nb, sy = P.nz * P.nb, sz = P.nb;
+    float I = 0.0f, T = 1.0f;
+    const long long K = (long long)P.n_steps * P.n_sub;
+    for (long long k = 0; k < K; ++k) {
+        const AxisLoHi ax = axis_lohi(R.p[0], P.nx - 1), ay = axis_lohi(R.p[1], P.ny - 1), az = axis_lohi(R.p[2], P.nz - 1);
+        const int ox[2] = {ax.lo * sx, ax.hi * sx}, oy[2] = {ay.lo * sy, ay.hi * sy}, oz[2] = {az.lo * sz, az.hi * sz};
+        const float wx[2] = {ax.g, ax.f}, wy[2] = {ay.g, ay.f}, wz[2] = {az.g, az.f};
+        const float kap = __ldg(P.kappa + ox[0] + oy[0] + oz[0] + bin);
+        float jv = 0.0f;
+#pragma unroll
+        for (int c = 0; c < 8; ++c)
+            jv = fmaf(wx[c >> 2] * wy[(c >> 1) & 1] * wz[c & 1], __ldg(P.j + ox[c >> 2] + oy[(c >> 1) & 1] + oz[c & 1] + bin), jv);
+        const float a = ex2_approx(kap * P.att_scale);
+        const float Pk = jv * T * P.emis;
+        I = fmaf(I, a, Pk);
+        T *= a;
+        fwd[k * fwd_stride + tid] = make_float2(I, Pk);
+#pragma unroll
+        for (int q = 0; q < 3; ++q) fx_add(R.p[q], R.d[q]);
+    }
 }
 
 // gsuf[m] = gbar[m] + gbar[m+1] + ... (the snapshots of the forward march are cumulative, D7)

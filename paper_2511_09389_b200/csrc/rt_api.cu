@@ -382,9 +382,114 @@ int rt_march_adjoint_j(const float* gbar, const float* kappa, int nx, int ny, in
     }
     const long long mb = rt::march_blocks(n_src, P.n_slots, P.n_groups, P.map_src);
     if (mb > 2147483647LL) return RT_EINVAL;
-    rt::adjoint_j_kernel<6><<<unsigned(mb), rt::kThreads, 0, st>>>(P, gsuf);
+    rt::adjoint_kernel<6, false><<<unsigned(mb), rt::kThreads, 0, st>>>(P, gsuf, nullptr, 0);
     RT_CUDA(cudaGetLastError());
     rt::snapshot_finalize_kernel<double><<<unsigned(blocks), threads, 0, st>>>(master, grad_j, ck.cells, 1);
+    RT_CUDA(cudaGetLastError());
+    return RT_OK;
+}
+
+// rt_march_adjoint_kappa records (I_{k+1}, P_k) of every substep of every ray of a launch: 8 bytes per
+// ray-substep-bin.  Sources are marched in batches so that this record stays below kForwardRecordLimit.
+constexpr size_t kForwardRecordLimit = size_t(2) << 30;
+struct KappaBatch {
+    int src_per_batch;
+    size_t record_bytes;
+};
+KappaBatch plan_kappa_batches(int n_src, int n_slots, int n_groups, bool map_src, long long K) {
+    const int unit = map_src ? 32 : 1;                               // sources come in whole warps' worth
+    const int n_units = (n_src + unit - 1) / unit;
+    auto bytes_for = [&](int n) {
+        return size_t(rt::march_blocks(n, n_slots, n_groups, map_src ? 1 : 0)) * rt::kThreads * size_t(K) * sizeof(float2);
+    };
+    int units = int(std::max<size_t>(1, kForwardRecordLimit / std::max<size_t>(1, bytes_for(unit))));
+    units = std::min(units, n_units);
+    KappaBatch kb;
+    kb.src_per_batch = std::min(units * unit, map_src ? n_units * unit : n_src);
+    kb.record_bytes = bytes_for(std::min(kb.src_per_batch, n_src));
+    return kb;
+}
+
+size_t rt_adjoint_kappa_workspace_bytes(int nx, int ny, int nz, int n_src, int n_rays, int n_bins, float step_size,
+                                        float c, float dt, int n_steps) {
+    const size_t base = rt_adjoint_workspace_bytes(nx, ny, nz, n_src, n_rays, n_bins, n_steps);
+    if (!base || !positive_finite(step_size) || !positive_finite(c) || !positive_finite(dt)) return 0;
+    const long long ns = substeps(step_size, c, dt);
+    if (ns < 1 || ns * n_steps > 2147483647LL) return 0;
+    Plan pl;
+    make_plan(RT_VARIANT_DEFAULT, n_src, &pl);
+    return align_up(base, 256) + plan_kappa_batches(n_src, ray_slots(n_rays), n_bins, pl.map_src, ns * n_steps).record_bytes;
+}
+
+int rt_march_adjoint_kappa(const float* gbar, const float* j, const float* kappa, int nx, int ny, int nz,
+                           const float* sources, int n_src, int n_rays, int n_bins, float step_size, float c, float dt,
+                           int n_steps, float* grad_kappa, void* workspace, size_t workspace_bytes, void* stream) {
+    if (!gbar) return RT_EINVAL;
+    Checked ck;
+    const int rc = check_args(j, kappa, nx, ny, nz, sources, n_src, n_rays, n_bins, step_size, c, dt, n_steps,
+                              grad_kappa, &ck);
+    if (rc != RT_OK) return rc;
+    if (uintptr_t(gbar) & 3u) return RT_EALIGN;
+    const Workspace wl = workspace_layout(ck.cells, n_src, n_rays, 1);
+    const size_t base = rt_adjoint_workspace_bytes(nx, ny, nz, n_src, n_rays, n_bins, n_steps);
+    const size_t need = rt_adjoint_kappa_workspace_bytes(nx, ny, nz, n_src, n_rays, n_bins, step_size, c, dt, n_steps);
+    if (!workspace || workspace_bytes < need || (uintptr_t(workspace) & 15u)) return RT_EWORKSPACE;
+    char* ws = static_cast<char*>(workspace);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    Plan pl;
+    make_plan(RT_VARIANT_DEFAULT, n_src, &pl);
+
+    rt::MarchParams P{};
+    P.j = j; P.kappa = kappa; P.sources = sources;
+    P.nx = nx; P.ny = ny; P.nz = nz; P.nb = n_bins;
+    P.n_src = n_src; P.src_begin = 0; P.slot_begin = 0; P.n_rays = n_rays;
+    P.n_groups = n_bins;
+    P.n_steps = n_steps; P.n_sub = int(ck.n_sub);
+    P.ds = double(step_size); P.ds_f = step_size;
+    P.emis = float(double(step_size) * 4.0 * 3.14159265358979323846 / double(n_rays));
+    P.att_scale = float(-double(step_size) * 1.4426950408889634074);
+    P.snap_stride = ck.cells;
+    P.map_src = pl.map_src ? 1 : 0;
+    P.kappa_trilinear = 0; P.state_I = nullptr; P.state_T = nullptr; P.k0 = 0;
+    P.ray_order = reinterpret_cast<const uint32_t*>(ws);
+    P.n_slots = ray_slots(n_rays);
+    const int rc2 = build_ray_order(n_rays, reinterpret_cast<uint32_t*>(ws), st);
+    if (rc2 != RT_OK) return rc2;
+    P.src_order = nullptr;
+    if (pl.map_src && n_src <= kMaxSortedSources) {
+        uint32_t* so = reinterpret_cast<uint32_t*>(ws + wl.src_order_at);
+        rt::src_order_kernel<<<(n_src + 3) / 4, 128, 0, st>>>(so, sources, n_src, nx, ny, nz);
+        RT_CUDA(cudaGetLastError());
+        P.src_order = so;
+    }
+    double* master = reinterpret_cast<double*>(ws + wl.acc_at);
+    P.acc = master;
+    RT_CUDA(cudaMemsetAsync(master, 0, size_t(ck.cells) * sizeof(double), st));
+    const int threads = 256;
+    long long blocks = (ck.cells + threads - 1) / threads;
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    const float* gsuf = gbar;
+    if (n_steps > 1) {
+        float* gs = reinterpret_cast<float*>(ws + align_up(wl.total, 256));
+        rt::suffix_sum_kernel<<<unsigned(blocks), threads, 0, st>>>(gbar, gs, ck.cells, n_steps);
+        RT_CUDA(cudaGetLastError());
+        gsuf = gs;
+    }
+    const long long K = ck.n_sub * n_steps;
+    const KappaBatch kb = plan_kappa_batches(n_src, P.n_slots, P.n_groups, pl.map_src, K);
+    float2* fwd = reinterpret_cast<float2*>(ws + align_up(base, 256));
+    for (int s0 = 0; s0 < n_src; s0 += kb.src_per_batch) {
+        P.src_begin = s0;
+        P.n_src = std::min(kb.src_per_batch, n_src - s0);
+        const long long mb = rt::march_blocks(P.n_src, P.n_slots, P.n_groups, P.map_src);
+        if (mb > 2147483647LL) return RT_EINVAL;
+        const long long stride = mb * rt::kThreads;
+        rt::forward_store_kernel<<<unsigned(mb), rt::kThreads, 0, st>>>(P, fwd, stride);
+        RT_CUDA(cudaGetLastError());
+        rt::adjoint_kernel<4, true><<<unsigned(mb), rt::kThreads, 0, st>>>(P, gsuf, fwd, stride);
+        RT_CUDA(cudaGetLastError());
+    }
+    rt::snapshot_finalize_kernel<double><<<unsigned(blocks), threads, 0, st>>>(master, grad_kappa, ck.cells, 1);
     RT_CUDA(cudaGetLastError());
     return RT_OK;
 }

@@ -97,3 +97,66 @@ def test_adjoint_argument_errors(rt):
     assert e.value.code == rt.RT_EWORKSPACE
     with pytest.raises(ValueError):
         rt.rt_march_adjoint_j(g, k, s, 16, 0.5, 1.0, 2.0, 2)
+
+
+# ------------------------------------------------------------------------------------------------
+# dL/dkappa
+# ------------------------------------------------------------------------------------------------
+def _signed_compare(got, ref, what):
+    """Gradients with respect to kappa have both signs and cancel: compare against the largest entry."""
+    scale = np.abs(ref).max()
+    rel_l2 = np.linalg.norm(got - ref) / np.linalg.norm(ref)
+    worst = np.abs(got - ref).max() / scale
+    assert np.isfinite(got).all(), what
+    assert rel_l2 <= parity.REL_L2_TOL, (what, rel_l2, worst)
+    assert worst <= parity.REL_L2_TOL, (what, rel_l2, worst)           # per entry: 1e-4 of the largest entry
+    return rel_l2, worst
+
+
+@pytest.mark.parametrize("shape,nb,n_src,n_rays,ds,dt,n_steps", [
+    ((4, 4, 4), 1, 1, 1, 0.5, 4.0, 1),
+    ((5, 4, 3), 3, 2, 7, 0.5, 5.0, 1),
+    ((6, 5, 7), 8, 1, 40, 0.5, 8.0, 3),
+    ((9, 8, 7), 1, 40, 24, 0.25, 4.0, 2),
+    ((7, 6, 9), 4, 33, 11, 0.5, 4.0, 2),
+    ((8, 8, 8), 2, 3, 50, 1.7, 13.6, 1),
+])
+def test_kappa_adjoint_matches_the_oracle(rt, oracle_mod, shape, nb, n_src, n_rays, ds, dt, n_steps):
+    rng = np.random.default_rng(sum(shape) + nb + n_src)
+    kap = rng.uniform(0.0, 0.6, shape + (nb,)).astype(np.float32)
+    j = rng.uniform(0.1, 1.0, shape + (nb,)).astype(np.float32)
+    src = rng.uniform(-2.0, max(shape) + 1.0, (n_src, 3))
+    if n_src > 3:
+        src = np.round(src)
+        src[1] = src[0]
+    src = src.astype(np.float32)
+    if n_src == 1 and n_rays == 1:
+        src = np.array([[1.0, 2.0, 1.0]], dtype=np.float32)
+    gbar = rng.standard_normal((n_steps,) + shape + (nb,)).astype(np.float32)
+    ref = oracle_mod.adjoint_kappa(gbar, j, kap, src, n_rays, ds, 1.0, dt, n_steps)
+    got = rt.rt_march_adjoint_kappa(_dev(gbar), _dev(j), _dev(kap), _dev(src), n_rays, ds, 1.0, dt, n_steps)
+    torch.cuda.synchronize()
+    print(_signed_compare(got.cpu().numpy().astype(np.float64), ref, f"kappa adjoint {shape} nb={nb} n_src={n_src}"))
+
+
+def test_kappa_adjoint_on_c1_against_the_oracle_and_a_directional_difference(rt, oracle_mod):
+    w = workloads.make_config("C1")
+    rng = np.random.default_rng(5)
+    j, kap, src = _dev(w.j), _dev(w.kappa), _dev(w.sources)
+    args = (w.n_rays, w.step_size, w.c, w.dt, w.n_steps)
+    out = rt.rt_march(j, kap, src, *args)
+    g = torch.from_numpy(rng.uniform(0.0, 1.0, tuple(out.shape)).astype(np.float32)).cuda()
+    grad = rt.rt_march_adjoint_kappa(g, j, kap, src, *args)
+    torch.cuda.synchronize()
+    ref = oracle_mod.adjoint_kappa(g.cpu().numpy(), w.j, w.kappa, w.sources, *args)
+    print(_signed_compare(grad.cpu().numpy().astype(np.float64), ref, "kappa adjoint C1"))
+    # d/d eps L(kappa (1 + eps d)) at 0, by central differences of the CUDA march
+    d = torch.from_numpy(rng.uniform(0.5, 1.5, w.kappa.shape).astype(np.float32)).cuda() * kap
+    eps = 1e-2
+
+    def loss(k):
+        return float((rt.rt_march(j, k.contiguous(), src, *args).double() * g.double()).sum())
+
+    fd = (loss(kap + eps * d) - loss(kap - eps * d)) / (2 * eps)
+    an = float((grad.double() * d.double()).sum())
+    assert abs(fd - an) <= 2e-3 * abs(an), (fd, an)
