@@ -211,7 +211,7 @@ def rt_march_adjoint_j(gbar, kappa, sources, n_rays, step_size, c, dt, n_steps, 
                                  step_size, c, dt, n_steps, grad_j.data_ptr(), workspace.data_ptr(), workspace.numel(),
                                  _stream_ptr(stream))
     if rc != RT_OK:
-        raise RtError(rc, "rt_march_adjoint_j", "rt_adjoint_kappa_workspace_bytes", "rt_march_adjoint_kappa")
+        raise RtError(rc, "rt_march_adjoint_j")
     return grad_j
 
 

@@ -1,4 +1,5 @@
-// rt_adjoint.cuh — adjoint of the march with respect to j (reading D19), sm_100a.
+// rt_adjoint.cuh — adjoints of the march with respect to j and to kappa (reading D19),
+// sm_100a.  The j part first; the kappa part is described at adjoint_kernel.
 //
 // For fixed kappa the field is linear in j.  With gbar[m] = dL/d out[m] and gsuf[m] = sum_{m' >= m} gbar[m'] (the
 // snapshots are cumulative, D7), eq. (2) and the deposit rule give, per ray,

@@ -88,7 +88,6 @@ template <int NB, typename ACC, bool KTRI> struct Stencil {
     __device__ __forceinline__ void restart(const MarchParams& P, TravelAxis (&A)[3], int negbits, int bin_off,
                                             const float* jsrc) {
         base = bin_off + place<0>(P, A[0], negbits) + place<1>(P, A[1], negbits) + place<2>(P, A[2], negbits);
-#pragma unroll
         reload(P, A, jsrc);
     }
     // (re)read the cached values of the 8 stencil voxels from `jsrc`
