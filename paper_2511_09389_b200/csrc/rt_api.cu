@@ -94,8 +94,8 @@ int launch_march(const rt::MarchParams& P, bool sliding, cudaStream_t st) {
     if (blocks > 2147483647LL) return RT_EINVAL;
     const unsigned g = unsigned(blocks);
     if (sliding) {
-        // registers: 1 bin per thread runs 8 blocks/SM (64 registers, 16 bytes spilled); 4 bins need ~150
-        constexpr int kMinBlocks = (NB == 1) ? 8 : 1;
+        // registers: 1 bin per thread runs 8 blocks/SM (64 registers); 4 bins 4 blocks/SM (128 registers, 8 bytes spilled)
+        constexpr int kMinBlocks = (NB == 1) ? 8 : 4;
         if (P.kappa_trilinear) rt::march_sliding_kernel<NB, ACC, 1, false, true><<<g, rt::kThreads, 0, st>>>(P);
         else if (P.state_I) rt::march_sliding_kernel<NB, ACC, kMinBlocks, true><<<g, rt::kThreads, 0, st>>>(P);
         else rt::march_sliding_kernel<NB, ACC, kMinBlocks, false><<<g, rt::kThreads, 0, st>>>(P);

@@ -244,6 +244,29 @@ def test_trilinear_kappa_configs(rt, oracle_mod, name):
     print(rows[-1])
 
 
+def test_one_source_a_hundred_thousand_rays(rt, oracle_mod):
+    """N_Omega far above a warp and not a power of two (ragged last ray band, padded slots), one source."""
+    shape, n_rays = (6, 7, 5), 100003
+    j, k = _random_medium(shape, 1, seed=9)
+    src = np.array([[2.4, 3.1, 1.7]], dtype=np.float32)
+    ref = oracle_mod.march(j, k, src, n_rays, 0.5, 1.0, 3.0, 1)
+    out = rt.rt_march(_dev(j), _dev(k), _dev(src), n_rays, 0.5, 1.0, 3.0, 1)
+    torch.cuda.synchronize()
+    parity.assert_parity(out.cpu().numpy(), ref, "100003 rays")
+
+
+@pytest.mark.parametrize("nb", [1, 4])
+def test_many_time_steps_of_one_substep(rt, oracle_mod, nb):
+    """n_steps = 40 snapshots with N_s = 1: every substep is a time-step boundary (flush, next slice)."""
+    shape = (6, 6, 6)
+    j, k = _random_medium(shape, nb, seed=nb)
+    src = np.array([[2.5, 2.5, 2.5], [0.0, 5.0, 3.0]], dtype=np.float32)
+    ref = oracle_mod.march(j, k, src, 30, 0.5, 1.0, 0.5, 40)
+    out = rt.rt_march(_dev(j), _dev(k), _dev(src), 30, 0.5, 1.0, 0.5, 40)
+    torch.cuda.synchronize()
+    parity.assert_parity(out.cpu().numpy(), ref, f"40 steps nb={nb}")
+
+
 def test_out_is_overwritten_and_call_is_repeatable(rt, oracle_mod):
     w = config("C0")
     j, k, s = _dev(w.j), _dev(w.kappa), _dev(w.sources)
