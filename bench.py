@@ -186,7 +186,7 @@ def measure_ceilings(rt, torch, shape, n_bins):
         g = grid64 if mode in (6, 7) else grid
         if mode == 1 and grid.numel() % 4:
             continue
-        n_red = (1 << 24) if mode == 3 else (1 << 28)
+        n_red = (1 << 24) if mode in (3, 8) else (1 << 28)
         best = None
         for rep in range(6):
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)

@@ -183,7 +183,9 @@ int rt_ray_slots(int n_rays);
  *   mode 5  M3 issued along a random walk of half a cell per step (ray-like locality)     (M6)
  *   mode 6  scalar red.global.add.f64, uniformly random addresses                         (M1 in fp64)
  *   mode 7  the stencil pattern of mode 2 with n_bins scalar red.global.add.f64 per corner (M3 in fp64)
- * `grid` holds nx*ny*nz*n_bins floats (modes 0-5) or doubles (modes 6, 7).
+ *   mode 8  scalar reds spread over the 8 corner voxels of the grid                          (M4, 8 addresses)
+ *   mode 9  scalar reds to uniformly random voxels of the boundary shell                     (M4, shell)
+ * `grid` holds nx*ny*nz*n_bins floats (modes 0-5, 8, 9) or doubles (modes 6, 7).
  * The grid is only accumulated into (caller zero-fills if the content matters). */
 int rt_bench_red_ceiling(int mode, void* grid, int nx, int ny, int nz, int n_bins,
                          long long n_red, unsigned int seed, long long* n_issued, void* stream);

@@ -19,7 +19,8 @@ RT_VARIANT_DEFAULT, RT_VARIANT_DIRECT, RT_VARIANT_DIRECT_COHERENT, RT_VARIANT_SL
 RT_VARIANT_SLIDING_BY_DIRECTION, RT_VARIANT_SLIDING_BY_SOURCE, RT_VARIANT_FLAG_ACC_F32 = 4, 5, 16
 RT_VARIANT_FLAG_ONE_BIN = 32
 RED_MODES = {"M1_scalar_random": 0, "M2_v4_random": 1, "M3_stencil": 2, "M4_one_address": 3,
-             "M5_coalesced": 4, "M6_stencil_walk": 5, "M1_f64_scalar_random": 6, "M3_f64_stencil": 7}
+             "M5_coalesced": 4, "M6_stencil_walk": 5, "M1_f64_scalar_random": 6, "M3_f64_stencil": 7,
+             "M4_eight_corners": 8, "M4_boundary_shell": 9}
 
 EXPORTS = ("rt_march", "rt_march_single", "rt_march_ex", "rt_march_host", "rt_workspace_bytes",
            "rt_substeps_per_step", "rt_launch_count", "rt_directions", "rt_ray_order", "rt_ray_slots", "rt_trace_ray",

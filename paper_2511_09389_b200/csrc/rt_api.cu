@@ -626,12 +626,12 @@ int rt_ray_order(int n_rays, unsigned int* order, void* stream) {
 
 int rt_bench_red_ceiling(int mode, void* grid, int nx, int ny, int nz, int n_bins, long long n_red, unsigned int seed,
                          long long* n_issued, void* stream) {
-    if (!grid || mode < 0 || mode > 7 || nx < 2 || ny < 2 || nz < 2 || n_bins < 1 || n_red < 1) return RT_EINVAL;
+    if (!grid || mode < 0 || mode > 9 || nx < 2 || ny < 2 || nz < 2 || n_bins < 1 || n_red < 1) return RT_EINVAL;
     const long long elems = (long long)nx * ny * nz * n_bins;
     if (elems > 2147483647LL || elems < 32) return RT_EINVAL;
     const bool vec = (n_bins % 4 == 0) && !(uintptr_t(grid) & 15u);
     if (mode == 1 && (elems % 4 || (uintptr_t(grid) & 15u))) return RT_EALIGN;
-    if (mode >= 6 && (uintptr_t(grid) & 7u)) return RT_EALIGN;
+    if ((mode == 6 || mode == 7) && (uintptr_t(grid) & 7u)) return RT_EALIGN;
     const int threads = 256, blocks = 148 * 8;
     // reductions (red instructions x lanes) one thread issues per iteration
     long long per_iter = 8LL;
@@ -653,6 +653,8 @@ int rt_bench_red_ceiling(int mode, void* grid, int nx, int ny, int nz, int n_bin
         case 4: rt::red_ceiling_kernel<4, 1><<<blocks, threads, 0, st>>>(P); break;
         case 6: rt::red_ceiling_kernel<6, 1><<<blocks, threads, 0, st>>>(P); break;
         case 7: rt::red_ceiling_kernel<7, 1><<<blocks, threads, 0, st>>>(P); break;
+        case 8: rt::red_ceiling_kernel<8, 1><<<blocks, threads, 0, st>>>(P); break;
+        case 9: rt::red_ceiling_kernel<9, 1><<<blocks, threads, 0, st>>>(P); break;
         default:
             if (vec) rt::red_ceiling_kernel<5, 4><<<blocks, threads, 0, st>>>(P);
             else rt::red_ceiling_kernel<5, 1><<<blocks, threads, 0, st>>>(P);

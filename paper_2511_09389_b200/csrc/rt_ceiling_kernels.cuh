@@ -81,6 +81,26 @@ __global__ void __launch_bounds__(256) red_ceiling_kernel(const CeilingParams P)
         for (int it = 0; it < P.iters; ++it)
 #pragma unroll
             for (int u = 0; u < 8; ++u) red1(P.grid + 32 * size_t(below(xorshift32(ws), n_elem / 32)) + (tid & 31), v);
+    } else if (MODE == 8) {     // M4b: every reduction to one of the 8 corner voxels of the grid (clamped far field)
+        const size_t sy = size_t(P.nz) * P.nb, sx = sy * P.ny;
+        for (int it = 0; it < P.iters; ++it)
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const uint32_t r = xorshift32(s);
+                red1(P.grid + ((r & 1) ? (P.nx - 1) * sx : 0) + ((r & 2) ? (P.ny - 1) * sy : 0) +
+                         ((r & 4) ? size_t(P.nz - 1) * P.nb : 0), v);
+            }
+    } else if (MODE == 9) {     // M4c: uniformly random voxels of the boundary shell (where clamped rays deposit)
+        const size_t sy = size_t(P.nz) * P.nb, sx = sy * P.ny;
+        for (int it = 0; it < P.iters; ++it)
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                int x = below(xorshift32(s), P.nx), y = below(xorshift32(s), P.ny), z = below(xorshift32(s), P.nz);
+                const uint32_t f = below(xorshift32(s), 6);
+                if (f == 0) x = 0; else if (f == 1) x = P.nx - 1; else if (f == 2) y = 0;
+                else if (f == 3) y = P.ny - 1; else if (f == 4) z = 0; else z = P.nz - 1;
+                red1(P.grid + x * sx + y * sy + size_t(z) * P.nb, v);
+            }
     } else if (MODE == 6) {     // M1 in fp64: scalar, uniformly random
         double* g = reinterpret_cast<double*>(P.grid);
         for (int it = 0; it < P.iters; ++it)

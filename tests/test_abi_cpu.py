@@ -100,7 +100,7 @@ def test_argument_errors_are_caught_before_cuda(rt):
     assert L.rt_march_host(None, p, 8, 8, 8, p, 1, 16, 1, 0.5, 1.0, 2.0, 1, p) == rt.RT_EINVAL
     assert L.rt_march_ex(p, p, 8, 8, 8, p, 1, 16, 1, 0.5, 1.0, 2.0, 1, p, p, 1 << 20, None, 7) == rt.RT_EINVAL
     assert L.rt_march_ex(p, p, 8, 8, 8, p, 1, 16, 1, 0.5, 1.0, 2.0, 1, p, p, 1 << 20, None, 128) == rt.RT_EINVAL
-    assert L.rt_bench_red_ceiling(9, p, 8, 8, 8, 1, 100, 1, None, None) == rt.RT_EINVAL
+    assert L.rt_bench_red_ceiling(10, p, 8, 8, 8, 1, 100, 1, None, None) == rt.RT_EINVAL
     assert L.rt_march_step(p, p, 8, 8, 8, p, 1, 16, 1, 0.5, 1.0, 2.0, 0, None, p, 0, p, 1 << 20, None) == rt.RT_EINVAL
     assert L.rt_march_step(p, p, 8, 8, 8, p, 1, 16, 1, 0.5, 1.0, 2.0, 1 << 40, p, p, 0, p, 1 << 20, None) == rt.RT_EINVAL
     assert L.rt_march_step(p, p, 8, 8, 8, p, 1, 16, 1, 0.5, 1.0, 2.0, 0, p, p, 0, p, 64, None) == rt.RT_EWORKSPACE
