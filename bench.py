@@ -343,7 +343,7 @@ def run_native(args):
                 torch.cuda.synchronize()
             call_s.append(time.perf_counter() - tc)
         barrier()
-        # median call (a stray cudaMalloc/cudaFree hiccup of the driver once took 10x on a shared box)
+        # median call (robust against a stray hiccup of a shared box)
         e2e_s = torch.tensor([sorted(call_s)[len(call_s) // 2] * n_e2e], dtype=torch.float64, device="cuda")
         if world > 1:
             dist.all_reduce(e2e_s, op=dist.ReduceOp.MAX)
@@ -351,7 +351,7 @@ def run_native(args):
             line["e2e"] = {"value": units_per_gpu * world * n_e2e / float(e2e_s.item()), "unit": UNIT,
                            "h2d_bytes_per_step": int(hj.numel() * 4 + hk.numel() * 4 + hs.numel() * 4),
                            "d2h_bytes_per_step": int(hout.numel() * 4), "steps": n_e2e,
-                           "api": "rt_march_host (cudaMalloc + H2D + march + D2H + free inside the call), "
+                           "api": "rt_march_host (device buffers from the library's memory pool + H2D + march + D2H inside the call), "
                                   "wall clock around each synchronous call (median call x steps), pinned host buffers", "call_ms": [1e3 * t for t in call_s]}
 
     # ---- roofline of the dominant kernel (the march kernel) against the measured L2-reduction ceiling

@@ -136,10 +136,14 @@ int rt_march_adjoint_kappa(const float* gbar, const float* j, const float* kappa
 
 /* End-to-end form with HOST pointers (j, kappa, sources, out are host memory, pinned or pageable).
  * Allocates device buffers, copies the inputs in, marches, copies out[] back, frees, and returns after the
- * copy has completed (SYNCHRONOUS).  Same semantics, limits and error codes as rt_march. */
+ * copy has completed (SYNCHRONOUS).  Same semantics, limits and error codes as rt_march.  The device buffers come
+ * from a private stream-ordered memory pool per device that keeps its memory between calls (the library's only
+ * retained state); rt_host_release() gives it back. */
 int rt_march_host(const float* j, const float* kappa, int nx, int ny, int nz,
                   const float* sources, int n_src, int n_rays, int n_bins,
                   float step_size, float c, float dt, int n_steps, float* out);
+
+int rt_host_release(void);
 
 /* Bytes of device scratch one rt_march call needs: the ray-order and source-order tables and the fp64
  * accumulation grid (n_steps * nx*ny*nz*n_bins doubles: deposits are summed in fp64 and rounded to fp32 once,

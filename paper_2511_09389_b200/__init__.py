@@ -8,7 +8,7 @@ from .binding import (RT_EALIGN, RT_ECUDA, RT_EINVAL, RT_EWORKSPACE, RT_OK, RT_V
                       RT_VARIANT_DIRECT, RT_VARIANT_DIRECT_COHERENT, RT_VARIANT_FLAG_ACC_F32, RT_VARIANT_FLAG_ONE_BIN,
                       RT_VARIANT_SLIDING_BY_DIRECTION,
                       RT_VARIANT_SLIDING_BY_SOURCE, RT_VARIANT_SLIDING_LATTICE, RtError,
-                      alloc_workspace, library_path, rt_bench_red_ceiling, rt_directions, rt_launch_count,
+                      alloc_workspace, library_path, rt_bench_red_ceiling, rt_directions, rt_host_release, rt_launch_count,
                       rt_adjoint_kappa_workspace_bytes, rt_adjoint_workspace_bytes, rt_march, rt_march_adjoint_j,
                       rt_march_adjoint_kappa, rt_march_ex, rt_march_host, rt_march_single, rt_march_step, rt_march_trilinear_kappa,
                       rt_state_bytes,

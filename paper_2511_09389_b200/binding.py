@@ -26,7 +26,7 @@ EXPORTS = ("rt_march", "rt_march_single", "rt_march_ex", "rt_march_host", "rt_wo
            "rt_substeps_per_step", "rt_launch_count", "rt_directions", "rt_ray_order", "rt_ray_slots", "rt_trace_ray",
            "rt_bench_red_ceiling", "rt_strerror", "rt_version", "rt_state_bytes", "rt_state_reset",
            "rt_step_workspace_bytes", "rt_march_step", "rt_march_trilinear_kappa", "rt_adjoint_workspace_bytes",
-           "rt_march_adjoint_j", "rt_adjoint_kappa_workspace_bytes", "rt_march_adjoint_kappa")
+           "rt_march_adjoint_j", "rt_adjoint_kappa_workspace_bytes", "rt_march_adjoint_kappa", "rt_host_release")
 
 
 class RtError(RuntimeError):
@@ -398,6 +398,11 @@ def rt_march_host(j, kappa, sources, n_rays, step_size, c, dt, n_steps, out=None
     if rc != RT_OK:
         raise RtError(rc, "rt_march_host")
     return out
+
+
+def rt_host_release() -> None:
+    """Give back the device memory rt_march_host keeps between calls."""
+    _lib.rt_host_release()
 
 
 def raw():

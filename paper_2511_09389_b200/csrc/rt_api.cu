@@ -7,6 +7,7 @@
 #include <cstdint>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 
 #include "rt_ceiling_kernels.cuh"
 #include "rt_march_direct.cuh"
@@ -522,6 +523,42 @@ int rt_march_step(const float* j, const float* kappa, int nx, int ny, int nz, co
                       workspace_bytes, stream, RT_VARIANT_DEFAULT, &sa);
 }
 
+// rt_march_host's device buffers come from a private stream-ordered memory pool per device that keeps what it has
+// been given (release threshold = max), so repeated calls do not pay cudaMalloc/cudaFree; rt_host_release() trims it.
+static std::mutex g_pool_mutex;
+static cudaMemPool_t g_pools[64] = {};
+
+static cudaError_t host_pool(cudaMemPool_t* pool) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_pool_mutex);
+    if (!g_pools[dev]) {
+        cudaMemPoolProps props = {};
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        e = cudaMemPoolCreate(&g_pools[dev], &props);
+        if (e != cudaSuccess) { g_pools[dev] = nullptr; return e; }
+        unsigned long long keep = ~0ull;
+        cudaMemPoolSetAttribute(g_pools[dev], cudaMemPoolAttrReleaseThreshold, &keep);
+    }
+    *pool = g_pools[dev];
+    return cudaSuccess;
+}
+
+int rt_host_release(void) {
+    std::lock_guard<std::mutex> lock(g_pool_mutex);
+    for (auto& p : g_pools)
+        if (p) {
+            cudaMemPoolDestroy(p);
+            p = nullptr;
+        }
+    return RT_OK;
+}
+
 int rt_march_host(const float* j, const float* kappa, int nx, int ny, int nz, const float* sources, int n_src,
                   int n_rays, int n_bins, float step_size, float c, float dt, int n_steps, float* out) {
     Checked ck;
@@ -530,31 +567,33 @@ int rt_march_host(const float* j, const float* kappa, int nx, int ny, int nz, co
     const size_t grid_b = size_t(ck.cells) * sizeof(float), out_b = grid_b * size_t(n_steps);
     const size_t src_b = size_t(n_src) * 3 * sizeof(float);
     const size_t ws_b = rt_workspace_bytes(nx, ny, nz, n_src, n_rays, n_bins, n_steps);
-    float *dj = nullptr, *dk = nullptr, *ds = nullptr, *dout = nullptr;
-    void* dws = nullptr;
+    // one allocation: [j][kappa][out][workspace][sources], every part 256-byte aligned
+    const size_t at_k = align_up(grid_b, 256), at_out = at_k + align_up(grid_b, 256), at_ws = at_out + align_up(out_b, 256),
+                 at_src = at_ws + align_up(ws_b, 256), total = at_src + align_up(src_b, 256);
+    char* base = nullptr;
+    cudaMemPool_t pool = nullptr;
     cudaStream_t st = nullptr;
     int result = RT_OK;
     auto ok = [&](cudaError_t err, const char* where) {
         if (err != cudaSuccess && result == RT_OK) result = cuda_fail(err, where);
         return err == cudaSuccess;
     };
-    if (ok(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking), "cudaStreamCreate") &&
-        ok(cudaMalloc(&dj, grid_b), "cudaMalloc j") && ok(cudaMalloc(&dk, grid_b), "cudaMalloc kappa") &&
-        ok(cudaMalloc(&ds, src_b), "cudaMalloc sources") && ok(cudaMalloc(&dout, out_b), "cudaMalloc out") &&
-        ok(cudaMalloc(&dws, ws_b), "cudaMalloc workspace") &&
-        ok(cudaMemcpyAsync(dj, j, grid_b, cudaMemcpyHostToDevice, st), "H2D j") &&
-        ok(cudaMemcpyAsync(dk, kappa, grid_b, cudaMemcpyHostToDevice, st), "H2D kappa") &&
-        ok(cudaMemcpyAsync(ds, sources, src_b, cudaMemcpyHostToDevice, st), "H2D sources")) {
-        result = march_impl(dj, dk, nx, ny, nz, ds, n_src, n_rays, n_bins, step_size, c, dt, n_steps, dout, dws, ws_b,
-                            st, RT_VARIANT_DEFAULT);
-        if (result == RT_OK) {
-            ok(cudaMemcpyAsync(out, dout, out_b, cudaMemcpyDeviceToHost, st), "D2H out");
-            ok(cudaStreamSynchronize(st), "cudaStreamSynchronize");
-        }
+    if (ok(host_pool(&pool), "cudaMemPoolCreate") &&
+        ok(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking), "cudaStreamCreate") &&
+        ok(cudaMallocFromPoolAsync(reinterpret_cast<void**>(&base), total, pool, st), "cudaMallocFromPoolAsync") &&
+        ok(cudaMemcpyAsync(base, j, grid_b, cudaMemcpyHostToDevice, st), "H2D j") &&
+        ok(cudaMemcpyAsync(base + at_k, kappa, grid_b, cudaMemcpyHostToDevice, st), "H2D kappa") &&
+        ok(cudaMemcpyAsync(base + at_src, sources, src_b, cudaMemcpyHostToDevice, st), "H2D sources")) {
+        result = march_impl(reinterpret_cast<float*>(base), reinterpret_cast<float*>(base + at_k), nx, ny, nz,
+                            reinterpret_cast<float*>(base + at_src), n_src, n_rays, n_bins, step_size, c, dt, n_steps,
+                            reinterpret_cast<float*>(base + at_out), base + at_ws, ws_b, st, RT_VARIANT_DEFAULT);
+        if (result == RT_OK) ok(cudaMemcpyAsync(out, base + at_out, out_b, cudaMemcpyDeviceToHost, st), "D2H out");
     }
-    if (st) cudaStreamSynchronize(st);
-    cudaFree(dj); cudaFree(dk); cudaFree(ds); cudaFree(dout); cudaFree(dws);
-    if (st) cudaStreamDestroy(st);
+    if (base) cudaFreeAsync(base, st);
+    if (st) {
+        ok(cudaStreamSynchronize(st), "cudaStreamSynchronize");
+        cudaStreamDestroy(st);
+    }
     return result;
 }
 
