@@ -14,7 +14,6 @@
 // the forward ray's, bit for bit, hence the same cells and the same weight bits.  tau_k is recovered by
 // subtracting kappa_k ds in fp64 (an fp32 running difference would lose 1e-3 of T over a few hundred substeps).
 #pragma once
-#include "rt_march_direct.cuh"
 #include "rt_march_sliding.cuh"
 
 namespace rt {
@@ -22,7 +21,7 @@ namespace rt {
 // WRT_KAPPA = false: dL/dj as described above.  WRT_KAPPA = true: dL/dkappa (D19).  Unrolling eq. (2),
 // I_{k+1} = T_{k+1} sum_{m<=k} ds J_m / a_m, so with G_k = w_k . gsuf and P_i = ds J_i T_i (the emission term of
 // substep i) dL/dkappa_i = ds [P_i lambda_{i+1} - R_i], R_i = sum_{k>=i} G_k I_{k+1}: the same backward march,
-// fed with (I_{k+1}, P_k) of every substep as recorded by forward_store_kernel, summing into the kappa cell of x_i
+// fed with (I_{k+1}, P_k) of every substep as recorded by march_sliding_kernel<..., RECORD = true>, summing into the kappa cell of x_i
 // (nearest neighbour: one voxel per substep, reduced when the cell changes).
 template <int MINB, bool WRT_KAPPA>
 __global__ void __launch_bounds__(kThreads, MINB) adjoint_kernel(const MarchParams P, const float* gsuf,
@@ -169,37 +168,6 @@ __global__ void __launch_bounds__(kThreads, MINB) adjoint_kernel(const MarchPara
     }
     if (WRT_KAPPA) flush_kappa();
     else S.flush_all(og, A);
-}
-
-// The forward march of eq. (2) with nothing deposited: records (I_{k+1}, P_k = ds J_k T_k), both scaled
-// by 4 pi / N_Omega, of every substep of every ray of the launch, laid out [substep][thread] so a warp writes one
-// 256-byte run per substep.  Same thread -> ray mapping as adjoint_kernel (same MarchParams).
-__global__ void __launch_bounds__(kThreads) forward_store_kernel(const MarchParams P, float2* fwd, long long fwd_stride) {
-    RayId id;
-    if (!ray_id(P, id)) return;
-    const long long tid = (long long)blockIdx.x * kThreads + threadIdx.x;
-    const int bin = id.group;
-    RaySetup R = ray_setup(P, id);
-    const int sx = P.ny * P.nz * P.nb, sy = P.nz * P.nb, sz = P.nb;
-    float I = 0.0f, T = 1.0f;
-    const long long K = (long long)P.n_steps * P.n_sub;
-    for (long long k = 0; k < K; ++k) {
-        const AxisLoHi ax = axis_lohi(R.p[0], P.nx - 1), ay = axis_lohi(R.p[1], P.ny - 1), az = axis_lohi(R.p[2], P.nz - 1);
-        const int ox[2] = {ax.lo * sx, ax.hi * sx}, oy[2] = {ay.lo * sy, ay.hi * sy}, oz[2] = {az.lo * sz, az.hi * sz};
-        const float wx[2] = {ax.g, ax.f}, wy[2] = {ay.g, ay.f}, wz[2] = {az.g, az.f};
-        const float kap = __ldg(P.kappa + ox[0] + oy[0] + oz[0] + bin);
-        float jv = 0.0f;
-#pragma unroll
-        for (int c = 0; c < 8; ++c)
-            jv = fmaf(wx[c >> 2] * wy[(c >> 1) & 1] * wz[c & 1], __ldg(P.j + ox[c >> 2] + oy[(c >> 1) & 1] + oz[c & 1] + bin), jv);
-        const float a = ex2_approx(kap * P.att_scale);
-        const float Pk = jv * T * P.emis;
-        I = fmaf(I, a, Pk);
-        T *= a;
-        fwd[k * fwd_stride + tid] = make_float2(I, Pk);
-#pragma unroll
-        for (int q = 0; q < 3; ++q) fx_add(R.p[q], R.d[q]);
-    }
 }
 
 // gsuf[m] = gbar[m] + gbar[m+1] + ... (the snapshots of the forward march are cumulative, D7)

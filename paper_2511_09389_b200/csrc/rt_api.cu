@@ -485,7 +485,7 @@ int rt_march_adjoint_kappa(const float* gbar, const float* j, const float* kappa
         const long long mb = rt::march_blocks(P.n_src, P.n_slots, P.n_groups, P.map_src);
         if (mb > 2147483647LL) return RT_EINVAL;
         const long long stride = mb * rt::kThreads;
-        rt::forward_store_kernel<<<unsigned(mb), rt::kThreads, 0, st>>>(P, fwd, stride);
+        rt::march_sliding_kernel<1, double, 8, false, false, true><<<unsigned(mb), rt::kThreads, 0, st>>>(P, fwd, stride);
         RT_CUDA(cudaGetLastError());
         rt::adjoint_kernel<4, true><<<unsigned(mb), rt::kThreads, 0, st>>>(P, gsuf, fwd, stride);
         RT_CUDA(cudaGetLastError());

@@ -142,8 +142,11 @@ template <int NB, typename ACC, bool KTRI> struct Stencil {
 };
 
 // STEP: the rt_march_step form -- start at substep P.k0 with (I, exp(-tau)) loaded from the ray state, store them back
-template <int NB, typename ACC, int MINB, bool STEP, bool KTRI = false>
-__global__ void __launch_bounds__(kThreads, MINB) march_sliding_kernel(const MarchParams P) {
+// RECORD (rt_march_adjoint_kappa): nothing is deposited; (I_{k+1}, P_k = ds J_k T_k), both scaled by 4 pi/N_Omega, of
+// every substep go to record[k * record_stride + thread], a warp writing one 256-byte run per substep.
+template <int NB, typename ACC, int MINB, bool STEP, bool KTRI = false, bool RECORD = false>
+__global__ void __launch_bounds__(kThreads, MINB) march_sliding_kernel(const MarchParams P, float2* record = nullptr,
+                                                                       long long record_stride = 0) {
     RayId id;
     if (!ray_id(P, id)) return;
     ACC* og = static_cast<ACC*>(P.acc);      // the bin offset id.group * NB rides in the stencil's base offset
@@ -225,13 +228,19 @@ __global__ void __launch_bounds__(kThreads, MINB) march_sliding_kernel(const Mar
             }
 #pragma unroll
             for (int b = 0; b < NB; ++b) {                       // eq. (2)
-                I[b] = fmaf(I[b], att[b], jv[b] * T[b] * P.emis);
+                const float emitted = jv[b] * T[b] * P.emis;
+                I[b] = fmaf(I[b], att[b], emitted);
                 T[b] *= att[b];
+                if (RECORD && b == 0)
+                    record[((long long)m * P.n_sub + k) * record_stride + (long long)blockIdx.x * kThreads + threadIdx.x] =
+                        make_float2(I[0], emitted);
             }
+            if (!RECORD) {
 #pragma unroll
-            for (int s = 0; s < 8; ++s)
+                for (int s = 0; s < 8; ++s)
 #pragma unroll
-                for (int b = 0; b < NB; ++b) S.acc[s].v[b] = fmaf(w[s], I[b], S.acc[s].v[b]);
+                    for (int b = 0; b < NB; ++b) S.acc[s].v[b] = fmaf(w[s], I[b], S.acc[s].v[b]);
+            }
 
             // x_{k+1} = x_k + n ds; a changed cell word is a crossing (increments are >= 0 in travel coordinates)
             const int c0 = A[0].p.c, c1 = A[1].p.c, c2 = A[2].p.c;
