@@ -80,3 +80,19 @@ def test_source_slices_partition_the_sources():
             assert (seen == 1).all() and max(sizes) - min(sizes) <= 1
     with pytest.raises(ValueError):
         source_slice(4, 2, 2)
+
+
+def test_bench_weak_scaling_workload_extends_the_source_list():
+    """bench.py --gpus N: rank r marches the r-th block of N * n_src sources placed by the config's own rule."""
+    sys.path.insert(0, ROOT)
+    import bench
+    from paper_2511_09389_b200.sharding import source_slice
+    one = bench.make_workload("C1", 1)
+    two = bench.make_workload("C1", 2)
+    assert two.n_src == 2 * one.n_src and two.sources.dtype == np.float32
+    assert np.array_equal(two.j, one.j) and np.array_equal(two.kappa, one.kappa)
+    blocks = [two.sources[source_slice(two.n_src, r, 2)] for r in range(2)]
+    assert all(len(b) == one.n_src for b in blocks)
+    assert len(np.unique(np.concatenate(blocks), axis=0)) == two.n_src          # disjoint, all distinct
+    desc = bench.describe(one, 2)
+    assert "2 GPU" in desc["parallelism"] and desc["updates_per_gpu"] == one.updates
