@@ -329,9 +329,10 @@ def run_native(args):
         hj, hk = torch.from_numpy(w.j).pin_memory(), torch.from_numpy(w.kappa).pin_memory()
         hs = torch.from_numpy(np.ascontiguousarray(w.sources[sl])).pin_memory()
         hout = torch.empty((w.n_steps, nx, ny, nz, nb), dtype=torch.float32).pin_memory()
-        n_e2e = max(1, min(args.steps, 5))
-        rt.rt_march_host(hj.numpy(), hk.numpy(), hs.numpy(), w.n_rays, w.step_size, w.c, w.dt, w.n_steps,
-                         out=hout.numpy())
+        n_e2e = max(1, min(args.steps, 11))
+        for _ in range(3):             # untimed: pool allocation, page-locking, clocks back up after the idle gap
+            rt.rt_march_host(hj.numpy(), hk.numpy(), hs.numpy(), w.n_rays, w.step_size, w.c, w.dt, w.n_steps,
+                             out=hout.numpy())
         barrier()
         call_s = []
         for _ in range(n_e2e):
