@@ -255,6 +255,24 @@ def test_one_source_a_hundred_thousand_rays(rt, oracle_mod):
     parity.assert_parity(out.cpu().numpy(), ref, "100003 rays")
 
 
+@pytest.mark.parametrize("nb,n_src", [(1, 3), (1, 40), (4, 3), (8, 40)])
+@pytest.mark.parametrize("log2_scale", [-100, 90])
+def test_emissivities_of_any_magnitude(rt, oracle_mod, nb, n_src, log2_scale):
+    """The field is linear in j (eq. (2)) and the weights are formed before they meet j, so j in
+    physical units (1e-30 or 1e+27 instead of O(1)) loses nothing: oracle parity at that scale, and the field
+    is the O(1) field times the (power of two, hence exact) scale up to the order of the reductions."""
+    shape, n_rays = (6, 5, 7), 50
+    j, k = _random_medium(shape, nb, seed=11)
+    src = np.random.default_rng(12).uniform(-1.0, 7.0, (n_src, 3)).astype(np.float32)
+    scale = np.float32(2.0) ** log2_scale
+    js = (j * scale).astype(np.float32)
+    ref = oracle_mod.march(js, k, src, n_rays, 0.5, 1.0, 5.0, 2)
+    got = rt.rt_march(_dev(js), _dev(k), _dev(src), n_rays, 0.5, 1.0, 5.0, 2).cpu().numpy()
+    parity.assert_parity(got, ref, f"j x 2^{log2_scale} nb={nb}")
+    unit = rt.rt_march(_dev(j), _dev(k), _dev(src), n_rays, 0.5, 1.0, 5.0, 2).cpu().numpy()
+    assert np.abs(got / scale - unit).max() <= 1e-6 * np.abs(unit).max()
+
+
 @pytest.mark.parametrize("nb", [1, 4])
 def test_many_time_steps_of_one_substep(rt, oracle_mod, nb):
     """n_steps = 40 snapshots with N_s = 1: every substep is a time-step boundary (flush, next slice)."""
