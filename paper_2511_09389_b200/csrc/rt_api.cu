@@ -79,21 +79,41 @@ size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 // workspace layout: [ray order: slots u32][source order: n_src u32][fp64 accumulation grid]
 struct Workspace {
-    size_t src_order_at, acc_at, total;
+    size_t src_order_at, acc_at, scratch2_at, total;
 };
-Workspace workspace_layout(long long cells, int n_src, int n_rays, int n_steps) {
+bool use_batched_fp32(long long cells, int n_steps, int n_bins);
+Workspace workspace_layout(long long cells, int n_src, int n_rays, int n_steps, int n_bins) {
     Workspace w;
     w.src_order_at = align_up(size_t(ray_slots(n_rays)) * sizeof(uint32_t), 16);
     w.acc_at = align_up(w.src_order_at + size_t(n_src) * sizeof(uint32_t), 256);
-    w.total = w.acc_at + size_t(cells) * size_t(n_steps) * sizeof(double);
+    w.scratch2_at = align_up(w.acc_at + size_t(cells) * size_t(n_steps) * sizeof(double), 256);
+    // the batched fp32 path marches two batches at a time: `out` and this second fp32 grid are their scratch grids
+    w.total = w.scratch2_at + (use_batched_fp32(cells, n_steps, n_bins) ? size_t(cells) * size_t(n_steps) * sizeof(float) : 0);
     return w;
 }
 
+// overlap_previous: programmatic stream serialization -- this grid may start while the tail of the previous kernel
+// of the stream (a march_sliding_kernel<4, ...> it does not depend on) is still running
 template <int NB, typename ACC>
-int launch_march(const rt::MarchParams& P, bool sliding, cudaStream_t st) {
+int launch_march(const rt::MarchParams& P, bool sliding, cudaStream_t st, bool overlap_previous = false) {
     const long long blocks = rt::march_blocks(P.n_src, P.n_slots, P.n_groups, P.map_src);
     if (blocks > 2147483647LL) return RT_EINVAL;
     const unsigned g = unsigned(blocks);
+    if (overlap_previous) {
+        if (!sliding || NB != 4 || P.kappa_trilinear || P.state_I) return RT_EINVAL;
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(g);
+        cfg.blockDim = dim3(rt::kThreads);
+        cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        RT_CUDA(cudaLaunchKernelEx(&cfg, rt::march_sliding_kernel<NB, ACC, 4, false, false, false>, P,
+                                   static_cast<float2*>(nullptr), 0LL));
+        return RT_OK;
+    }
     if (sliding) {
         // registers: 1 bin per thread runs 8 blocks/SM (64 registers); 4 bins 4 blocks/SM (128 registers, 8 bytes spilled)
         constexpr int kMinBlocks = (NB == 1) ? 8 : 4;
@@ -176,7 +196,7 @@ int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const
     if (rc != RT_OK) return rc;
     Plan pl;
     if (!make_plan(variant, n_src, &pl)) return RT_EINVAL;
-    const Workspace wl = workspace_layout(ck.cells, n_src, n_rays, n_steps);
+    const Workspace wl = workspace_layout(ck.cells, n_src, n_rays, n_steps, n_bins);
     const size_t need = wl.total + (step ? step_scratch_bytes(ck.cells, n_bins) : 0);
     if (!workspace || workspace_bytes < need || (uintptr_t(workspace) & 15u)) return RT_EWORKSPACE;
     char* ws = static_cast<char*>(workspace);
@@ -246,17 +266,32 @@ int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const
         P.acc = scratch;
         long long db = ((long long)(n_acc / 4) + fin_threads - 1) / fin_threads;
         if (db > 148 * 16) db = 148 * 16;
-        for (int s0 = 0; s0 < n_src; s0 += bt.src_per_batch)
-            for (int d0 = 0; d0 < all_slots; d0 += bt.slots_per_batch) {
-                P.src_begin = s0;
-                P.n_src = std::min(bt.src_per_batch, n_src - s0);
-                P.slot_begin = d0;
-                P.n_slots = std::min(bt.slots_per_batch, all_slots - d0);
-                const int rcb = launch_march<4, float>(P, true, st);
-                if (rcb != RT_OK) return rcb;
-                rt::drain_kernel<<<unsigned(db), fin_threads, 0, st>>>(master, scratch, (long long)n_acc);
-                RT_CUDA(cudaGetLastError());
+        // two batches at a time, each into its own scratch grid; the second overlaps the tail of the first
+        float* scratch2 = (step || pl.ktri) ? nullptr : reinterpret_cast<float*>(ws + wl.scratch2_at);
+        if (scratch2) RT_CUDA(cudaMemsetAsync(scratch2, 0, n_acc * sizeof(float), st));
+        const int sb = (n_src + bt.src_per_batch - 1) / bt.src_per_batch, db_n = (all_slots + bt.slots_per_batch - 1) / bt.slots_per_batch;
+        auto select = [&](int b) {
+            const int s0 = (b / db_n) * bt.src_per_batch, d0 = (b % db_n) * bt.slots_per_batch;
+            P.src_begin = s0;
+            P.n_src = std::min(bt.src_per_batch, n_src - s0);
+            P.slot_begin = d0;
+            P.n_slots = std::min(bt.slots_per_batch, all_slots - d0);
+        };
+        for (int b = 0; b < sb * db_n; b += scratch2 ? 2 : 1) {
+            select(b);
+            P.acc = scratch;
+            const int rcb = launch_march<4, float>(P, true, st);
+            if (rcb != RT_OK) return rcb;
+            const bool pair = scratch2 && b + 1 < sb * db_n;
+            if (pair) {
+                select(b + 1);
+                P.acc = scratch2;
+                const int rcc = launch_march<4, float>(P, true, st, true);
+                if (rcc != RT_OK) return rcc;
             }
+            rt::drain_kernel<<<unsigned(db), fin_threads, 0, st>>>(master, scratch, pair ? scratch2 : nullptr, (long long)n_acc);
+            RT_CUDA(cudaGetLastError());
+        }
         if (step)
             rt::step_finalize_kernel<<<unsigned(fin_blocks), fin_threads, 0, st>>>(master, out, ck.cells, step->accumulate);
         else
@@ -337,7 +372,7 @@ int rt_march_adjoint_j(const float* gbar, const float* kappa, int nx, int ny, in
     const int rc = check_args(gbar, kappa, nx, ny, nz, sources, n_src, n_rays, n_bins, step_size, c, dt, n_steps,
                               grad_j, &ck);
     if (rc != RT_OK) return rc;
-    const Workspace wl = workspace_layout(ck.cells, n_src, n_rays, 1);
+    const Workspace wl = workspace_layout(ck.cells, n_src, n_rays, 1, n_bins);
     const size_t need = rt_adjoint_workspace_bytes(nx, ny, nz, n_src, n_rays, n_bins, n_steps);
     if (!workspace || workspace_bytes < need || (uintptr_t(workspace) & 15u)) return RT_EWORKSPACE;
     char* ws = static_cast<char*>(workspace);
@@ -431,7 +466,7 @@ int rt_march_adjoint_kappa(const float* gbar, const float* j, const float* kappa
                               grad_kappa, &ck);
     if (rc != RT_OK) return rc;
     if (uintptr_t(gbar) & 3u) return RT_EALIGN;
-    const Workspace wl = workspace_layout(ck.cells, n_src, n_rays, 1);
+    const Workspace wl = workspace_layout(ck.cells, n_src, n_rays, 1, n_bins);
     const size_t base = rt_adjoint_workspace_bytes(nx, ny, nz, n_src, n_rays, n_bins, n_steps);
     const size_t need = rt_adjoint_kappa_workspace_bytes(nx, ny, nz, n_src, n_rays, n_bins, step_size, c, dt, n_steps);
     if (!workspace || workspace_bytes < need || (uintptr_t(workspace) & 15u)) return RT_EWORKSPACE;
@@ -602,7 +637,7 @@ size_t rt_workspace_bytes(int nx, int ny, int nz, int n_src, int n_rays, int n_b
         return 0;
     const long long cells = (long long)nx * ny;
     if (cells > 2147483647LL || cells * nz > 2147483647LL || cells * nz * n_bins > 2147483647LL) return 0;
-    return workspace_layout(cells * nz * n_bins, n_src, n_rays, n_steps).total;
+    return workspace_layout(cells * nz * n_bins, n_src, n_rays, n_steps, n_bins).total;
 }
 
 int rt_substeps_per_step(float step_size, float c, float dt) {
@@ -621,7 +656,7 @@ int rt_launch_count(int nx, int ny, int nz, int n_src, int n_rays, int n_bins, i
         const Batching bt = plan_batches(n_src, slots, pl.map_src);
         const int batches = ((n_src + bt.src_per_batch - 1) / bt.src_per_batch) *
                             ((slots + bt.slots_per_batch - 1) / bt.slots_per_batch);
-        return setup + 2 * batches + 1;
+        return setup + batches + (batches + 1) / 2 + 1;         // batches march in pairs, one drain per pair
     }
     return setup + 2;                                                               // march, snapshot finalisation
 }

@@ -147,6 +147,9 @@ template <int NB, typename ACC, bool KTRI> struct Stencil {
 template <int NB, typename ACC, int MINB, bool STEP, bool KTRI = false, bool RECORD = false>
 __global__ void __launch_bounds__(kThreads, MINB) march_sliding_kernel(const MarchParams P, float2* record = nullptr,
                                                                        long long record_stride = 0) {
+    // the batched path launches the next batch (other scratch grid, no dependence on this one) with programmatic
+    // stream serialization: it may start as soon as every block of this grid has started, filling this grid's tail
+    if constexpr (NB == 4) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     RayId id;
     if (!ray_id(P, id)) return;
     ACC* og = static_cast<ACC*>(P.acc);      // the bin offset id.group * NB rides in the stencil's base offset

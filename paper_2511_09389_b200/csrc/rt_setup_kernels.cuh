@@ -80,19 +80,25 @@ __global__ void snapshot_finalize_kernel(const ACC* acc, float* out, long long s
     }
 }
 
-// master += scratch; scratch = 0 (the batched fp32 path of rt_api.cu: fp32 reductions of one batch of sources are
-// folded into the fp64 grid before the next batch, so no fp32 sum grows past one batch)
-__global__ void drain_kernel(double* master, float* scratch, long long n) {
+// master += scratch (+ scratch2); scratch = scratch2 = 0 (the batched fp32 path of rt_api.cu: fp32 reductions of one
+// batch of sources are folded into the fp64 grid before that scratch grid is used again, so no fp32 sum grows past
+// one batch)
+__global__ void drain_kernel(double* master, float* scratch, float* scratch2, long long n) {
     const long long n4 = n / 4;
     for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < n4;
          e += (long long)gridDim.x * blockDim.x) {
         const float4 v = reinterpret_cast<float4*>(scratch)[e];
-        if (v.x != 0.0f || v.y != 0.0f || v.z != 0.0f || v.w != 0.0f) {
+        const float4 u = scratch2 ? reinterpret_cast<float4*>(scratch2)[e] : make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+        const bool nv = v.x != 0.0f || v.y != 0.0f || v.z != 0.0f || v.w != 0.0f;
+        const bool nu = u.x != 0.0f || u.y != 0.0f || u.z != 0.0f || u.w != 0.0f;
+        if (nv || nu) {
             double2* m = reinterpret_cast<double2*>(master) + 2 * e;
             double2 a = m[0], b = m[1];
-            a.x += double(v.x); a.y += double(v.y); b.x += double(v.z); b.y += double(v.w);
+            a.x += double(v.x) + double(u.x); a.y += double(v.y) + double(u.y);
+            b.x += double(v.z) + double(u.z); b.y += double(v.w) + double(u.w);
             m[0] = a; m[1] = b;
-            reinterpret_cast<float4*>(scratch)[e] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+            if (nv) reinterpret_cast<float4*>(scratch)[e] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+            if (nu) reinterpret_cast<float4*>(scratch2)[e] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
         }
     }
 }

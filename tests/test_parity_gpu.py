@@ -273,6 +273,21 @@ def test_emissivities_of_any_magnitude(rt, oracle_mod, nb, n_src, log2_scale):
     assert np.abs(got / scale - unit).max() <= 1e-6 * np.abs(unit).max()
 
 
+@pytest.mark.parametrize("nb,n_src", [(1, 2), (1, 33), (4, 2)])
+def test_vacuum_and_opaque_cells(rt, oracle_mod, nb, n_src):
+    """kappa = 0 (vacuum), kappa ds ~ 1, ~ 20 and ~ 5000 (exp(-kappa ds) underflows to 0 in fp32 and in fp64) mixed
+    cell by cell: attenuation factors from 1 down to exactly 0 along one ray."""
+    shape, n_rays = (8, 7, 6), 60
+    rng = np.random.default_rng(21)
+    j = rng.uniform(0.1, 1.0, shape + (nb,)).astype(np.float32)
+    k = rng.choice(np.array([0.0, 2.0, 40.0, 1.0e4], dtype=np.float32), size=shape + (nb,), p=[0.4, 0.4, 0.15, 0.05])
+    src = rng.uniform(0.0, 6.0, (n_src, 3)).astype(np.float32)
+    ref = oracle_mod.march(j, k, src, n_rays, 0.5, 1.0, 6.0, 2)
+    got = rt.rt_march(_dev(j), _dev(k), _dev(src), n_rays, 0.5, 1.0, 6.0, 2).cpu().numpy()
+    assert np.isfinite(got).all()
+    parity.assert_parity(got, ref, f"vacuum/opaque nb={nb} n_src={n_src}")
+
+
 @pytest.mark.parametrize("nb", [1, 4])
 def test_many_time_steps_of_one_substep(rt, oracle_mod, nb):
     """n_steps = 40 snapshots with N_s = 1: every substep is a time-step boundary (flush, next slice)."""
