@@ -366,9 +366,9 @@ def run_native(args):
         hbm_bytes = int((2 + 3 * w.n_steps) * nx * ny * nz * nb * 4)      # j, kappa read; fp64 grid zeroed+read; out written
         roof = {
             "bound": "l2_red", "achieved": achieved, "peak": peak, "unit": "Gred/s", "frac": achieved / peak,
-            "traffic": None, "kernel": "march_sliding_kernel",
+            "traffic": None, "kernel": "march_table_kernel / march_sliding_kernel",
             "how": "achieved = ALGORITHMIC reductions (8 corners x bin-groups x ray-substeps) / mean CUDA-event "
-                   "time of the whole rt_march call (the march kernel is 99% of it at C2, profiles/r01b); peak = "
+                   "time of the whole rt_march call (the march kernel is 99% of it at C2, profiles/r01f); peak = "
                    "M3 stencil-pattern red.global.add ceiling measured in this process on a grid of the same "
                    "size (DESIGN.md §8), of measured; frac > 1: the sliding stencil sums a voxel's deposits in "
                    "registers, so fewer reductions are issued than the method states (see `issued`)",
@@ -389,6 +389,7 @@ def run_native(args):
                            "peak_Ginst_per_s": 148 * 4 * sm_hz / 1e9,
                            "frac": cnt["warp_instructions"] / step_s / (148 * 4 * sm_hz),
                            "peak_how": "148 SMs x 4 schedulers x 1 warp-instruction/clk x SM clock sampled in the run"}
+            roof["kernel"] = cnt["kernel"]
             roof["counters_from"] = cnt["source"]
         line["roofline"] = roof
         if not args.no_cpu_baseline and world == 1:
@@ -410,7 +411,7 @@ def _ncu_counters(config, variant):
             for row in csv.DictReader(f):
                 if row["case"] == f"{config}:v{variant}" and row["library"] == _lib_version():
                     return {"warp_instructions": float(row["warp_instructions"]), "red_sectors": float(row["red_sectors"]),
-                            "dram_bytes": float(row["dram_bytes"]), "source": row["source"]}
+                            "dram_bytes": float(row["dram_bytes"]), "source": row["source"], "kernel": row["kernel"]}
     except (OSError, KeyError, ValueError):
         pass
     return None

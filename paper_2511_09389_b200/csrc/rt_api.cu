@@ -13,6 +13,7 @@
 #include "rt_march_direct.cuh"
 #include "rt_adjoint.cuh"
 #include "rt_march_sliding.cuh"
+#include "rt_march_table.cuh"
 #include "rt_setup_kernels.cuh"
 
 namespace {
@@ -77,16 +78,24 @@ int check_args(const void* j, const void* kappa, int nx, int ny, int nz, const v
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
-// workspace layout: [ray order: slots u32][source order: n_src u32][fp64 accumulation grid]
+// workspace layout: [ray order: slots u32][source order: n_src u32][flag][fp64 accumulation grid x copies][fp32 scratch]
 struct Workspace {
-    size_t src_order_at, acc_at, scratch2_at, total;
+    size_t src_order_at, flag_at, acc_at, scratch2_at, total;
+    int acc_copies;
 };
 bool use_batched_fp32(long long cells, int n_steps, int n_bins);
+// The table march (rt_march_table.cuh) is in play for the default one-bin march with >= 32 sources (warp = 32
+// sources x 1 direction); it spreads its reductions over up to 4 copies of the fp64 grid, 48 MiB in all
+constexpr size_t kAccCopiesBytes = size_t(48) << 20;
+bool table_march_sizes(int n_src, int n_bins) { return n_bins == 1 && n_src >= 32; }
 Workspace workspace_layout(long long cells, int n_src, int n_rays, int n_steps, int n_bins) {
     Workspace w;
+    const size_t grid = size_t(cells) * size_t(n_steps) * sizeof(double);
+    w.acc_copies = table_march_sizes(n_src, n_bins) ? int(std::min<size_t>(4, std::max<size_t>(1, kAccCopiesBytes / grid))) : 1;
     w.src_order_at = align_up(size_t(ray_slots(n_rays)) * sizeof(uint32_t), 16);
-    w.acc_at = align_up(w.src_order_at + size_t(n_src) * sizeof(uint32_t), 256);
-    w.scratch2_at = align_up(w.acc_at + size_t(cells) * size_t(n_steps) * sizeof(double), 256);
+    w.flag_at = align_up(w.src_order_at + size_t(n_src) * sizeof(uint32_t), 16);      // same-fraction flag (table march)
+    w.acc_at = align_up(w.flag_at + 16, 256);
+    w.scratch2_at = align_up(w.acc_at + grid * size_t(w.acc_copies), 256);
     // the batched fp32 path marches two batches at a time: `out` and this second fp32 grid are their scratch grids
     w.total = w.scratch2_at + (use_batched_fp32(cells, n_steps, n_bins) ? size_t(cells) * size_t(n_steps) * sizeof(float) : 0);
     return w;
@@ -207,7 +216,8 @@ int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const
     }
 
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    rt::MarchParams P;
+    rt::MarchParams P{};
+    P.acc_copies = 1;
     P.j = j; P.kappa = kappa; P.sources = sources;
     P.nx = nx; P.ny = ny; P.nz = nz; P.nb = n_bins;
     P.n_src = n_src; P.src_begin = 0; P.slot_begin = 0; P.n_rays = n_rays;
@@ -305,6 +315,26 @@ int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const
         const int rcs = vec4 ? launch_march<4, double>(P, true, st) : launch_march<1, double>(P, true, st);
         if (rcs != RT_OK) return rcs;
         rt::step_finalize_kernel<<<unsigned(fin_blocks), fin_threads, 0, st>>>(master, out, ck.cells, step->accumulate);
+        RT_CUDA(cudaGetLastError());
+        return RT_OK;
+    }
+
+    if (variant == RT_VARIANT_DEFAULT && pl.map_src && table_march_sizes(n_src, n_bins)) {
+        // Sources that share their cell fractions (decided on the device) are marched by march_table_kernel, others
+        // by the gated march_sliding_kernel: each of the two returns at once when the flag says it is the other's call
+        int* flag = reinterpret_cast<int*>(ws + wl.flag_at);
+        P.acc = master;
+        P.same_frac = flag;
+        P.acc_copies = wl.acc_copies;
+        P.acc_copy_stride = (long long)n_acc;
+        RT_CUDA(cudaMemsetAsync(master, 0, n_acc * sizeof(double) * size_t(wl.acc_copies), st));                // D14: overwrite
+        const long long tb = rt::march_blocks(P.n_src, P.n_slots, 1, 1);
+        if (tb > 2147483647LL) return RT_EINVAL;
+        rt::same_fraction_kernel<<<1, 256, 0, st>>>(flag, sources, n_src, step_size);
+        rt::march_table_kernel<8><<<unsigned(tb), rt::kThreads, 0, st>>>(P);
+        rt::march_sliding_kernel<1, double, 8, false, false, false, true><<<unsigned(tb), rt::kThreads, 0, st>>>(P);
+        rt::snapshot_finalize_kernel<double><<<unsigned(fin_blocks), fin_threads, 0, st>>>(master, out, ck.cells, n_steps,
+                                                                                          wl.acc_copies, (long long)n_acc);
         RT_CUDA(cudaGetLastError());
         return RT_OK;
     }
@@ -658,7 +688,8 @@ int rt_launch_count(int nx, int ny, int nz, int n_src, int n_rays, int n_bins, i
                             ((slots + bt.slots_per_batch - 1) / bt.slots_per_batch);
         return setup + batches + (batches + 1) / 2 + 1;         // batches march in pairs, one drain per pair
     }
-    return setup + 2;                                                               // march, snapshot finalisation
+    // march, snapshot finalisation; the one-bin march with >= 32 sources: fraction test, table march, gated march
+    return setup + 2 + (table_march_sizes(n_src, n_bins) ? 2 : 0);
 }
 
 int rt_directions(int n_rays, double* nhat, void* stream) {
@@ -749,6 +780,6 @@ const char* rt_strerror(int code) {
     }
 }
 
-const char* rt_version(void) { return "rtmarch 0.4 (sm_100a; sliding-stencil RED march, 32 sources x 1 direction per warp, fp64 accumulation grid)"; }
+const char* rt_version(void) { return "rtmarch 0.5 (sm_100a; sliding-stencil RED march, 32 sources x 1 direction per warp, per-warp weight table for sources sharing their cell fractions, fp64 accumulation grid)"; }
 
 }  // extern "C"

@@ -200,6 +200,34 @@ def test_many_sources_fill_warps_raggedly(rt, oracle_mod, n_src, integer, varian
     parity.assert_parity(out.cpu().numpy(), ref, f"n_src={n_src} variant={variant}")
 
 
+@pytest.mark.parametrize("case", ["quarter_fractions", "one_source_off", "integer_outside", "long_steps", "two_warps"])
+def test_sources_sharing_their_cell_fractions(rt, oracle_mod, case):
+    """rt_march with >= 32 sources and one bin launches march_table_kernel (all sources share their fractional cell
+    offsets: one weight table per warp) and the gated march_sliding_kernel (they do not, or step_size >= 1); a flag
+    computed on the device decides which of the two does the work.  Both against the oracle and against the plain
+    kernel; substeps per step not a multiple of the 32-row table, a ragged last source group (dark padding lanes)."""
+    shape, n_rays, ds, dt, n_steps = (9, 7, 8), 37, 0.25, 9.25, 3            # 37 substeps per step
+    rng = np.random.default_rng(77)
+    n_src = 45
+    src = rng.integers(-1, 10, (n_src, 3)).astype(np.float64)
+    if case == "quarter_fractions":
+        src += (0.25, 0.5, 0.75)
+    elif case == "one_source_off":
+        src += (0.25, 0.5, 0.75)
+        src[31, 1] += 0.125
+    elif case == "long_steps":
+        ds, dt = 1.5, 12.0
+    elif case == "two_warps":
+        src = rng.integers(0, 7, (64, 3)).astype(np.float64)
+    src = src.astype(np.float32)
+    j, k = _random_medium(shape, 1, seed=78)
+    ref = oracle_mod.march(j, k, src, n_rays, ds, 1.0, dt, n_steps)
+    got = rt.rt_march(_dev(j), _dev(k), _dev(src), n_rays, ds, 1.0, dt, n_steps).cpu().numpy()
+    parity.assert_parity(got, ref, f"shared fractions: {case}")
+    plain = rt.rt_march_ex(_dev(j), _dev(k), _dev(src), n_rays, ds, 1.0, dt, n_steps, variant=5).cpu().numpy()
+    assert np.abs(got - plain).max() <= 1e-6 * np.abs(plain).max()      # same arithmetic per ray, other summation order
+
+
 def test_more_sources_than_the_sort_handles(rt, oracle_mod):
     """Above 65,536 sources the spatial source sort is skipped (identity order); same field."""
     shape, n_src = (4, 4, 4), 66000
