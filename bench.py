@@ -366,7 +366,7 @@ def run_native(args):
         hbm_bytes = int((2 + 3 * w.n_steps) * nx * ny * nz * nb * 4)      # j, kappa read; fp64 grid zeroed+read; out written
         roof = {
             "bound": "l2_red", "achieved": achieved, "peak": peak, "unit": "Gred/s", "frac": achieved / peak,
-            "traffic": None, "kernel": "march_table_kernel / march_sliding_kernel",
+            "traffic": None, "kernel": "march_sliding_kernel",
             "how": "achieved = ALGORITHMIC reductions (8 corners x bin-groups x ray-substeps) / mean CUDA-event "
                    "time of the whole rt_march call (the march kernel is 99% of it at C2, profiles/r01f); peak = "
                    "M3 stencil-pattern red.global.add ceiling measured in this process on a grid of the same "

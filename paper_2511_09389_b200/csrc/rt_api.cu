@@ -13,7 +13,6 @@
 #include "rt_march_direct.cuh"
 #include "rt_adjoint.cuh"
 #include "rt_march_sliding.cuh"
-#include "rt_march_table.cuh"
 #include "rt_setup_kernels.cuh"
 
 namespace {
@@ -78,23 +77,21 @@ int check_args(const void* j, const void* kappa, int nx, int ny, int nz, const v
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
-// workspace layout: [ray order: slots u32][source order: n_src u32][flag][fp64 accumulation grid x copies][fp32 scratch]
+// workspace layout: [ray order: slots u32][source order: n_src u32][fp64 accumulation grid x copies][fp32 scratch]
 struct Workspace {
-    size_t src_order_at, flag_at, acc_at, scratch2_at, total;
+    size_t src_order_at, acc_at, scratch2_at, total;
     int acc_copies;
 };
 bool use_batched_fp32(long long cells, int n_steps, int n_bins);
-// The table march (rt_march_table.cuh) is in play for the default one-bin march with >= 32 sources (warp = 32
-// sources x 1 direction); it spreads its reductions over up to 4 copies of the fp64 grid, 48 MiB in all
+// One-bin-per-thread marches with fp64 reductions spread them over up to 4 copies of the grid, 48 MiB in all (C2: 3
+// copies of 16 MiB; C4's 4 GiB grid: 1)
 constexpr size_t kAccCopiesBytes = size_t(48) << 20;
-bool table_march_sizes(int n_src, int n_bins) { return n_bins == 1 && n_src >= 32; }
 Workspace workspace_layout(long long cells, int n_src, int n_rays, int n_steps, int n_bins) {
     Workspace w;
     const size_t grid = size_t(cells) * size_t(n_steps) * sizeof(double);
-    w.acc_copies = table_march_sizes(n_src, n_bins) ? int(std::min<size_t>(4, std::max<size_t>(1, kAccCopiesBytes / grid))) : 1;
+    w.acc_copies = use_batched_fp32(cells, n_steps, n_bins) ? 1 : int(std::min<size_t>(4, std::max<size_t>(1, kAccCopiesBytes / grid)));
     w.src_order_at = align_up(size_t(ray_slots(n_rays)) * sizeof(uint32_t), 16);
-    w.flag_at = align_up(w.src_order_at + size_t(n_src) * sizeof(uint32_t), 16);      // same-fraction flag (table march)
-    w.acc_at = align_up(w.flag_at + 16, 256);
+    w.acc_at = align_up(w.src_order_at + size_t(n_src) * sizeof(uint32_t), 256);
     w.scratch2_at = align_up(w.acc_at + grid * size_t(w.acc_copies), 256);
     // the batched fp32 path marches two batches at a time: `out` and this second fp32 grid are their scratch grids
     w.total = w.scratch2_at + (use_batched_fp32(cells, n_steps, n_bins) ? size_t(cells) * size_t(n_steps) * sizeof(float) : 0);
@@ -128,6 +125,7 @@ int launch_march(const rt::MarchParams& P, bool sliding, cudaStream_t st, bool o
         constexpr int kMinBlocks = (NB == 1) ? 8 : 4;
         if (P.kappa_trilinear) rt::march_sliding_kernel<NB, ACC, 1, false, true><<<g, rt::kThreads, 0, st>>>(P);
         else if (P.state_I) rt::march_sliding_kernel<NB, ACC, kMinBlocks, true><<<g, rt::kThreads, 0, st>>>(P);
+        else if (P.acc_copies > 1) rt::march_sliding_kernel<NB, ACC, kMinBlocks, false, false, false, true><<<g, rt::kThreads, 0, st>>>(P);
         else rt::march_sliding_kernel<NB, ACC, kMinBlocks, false><<<g, rt::kThreads, 0, st>>>(P);
     } else {
         rt::march_direct_kernel<NB, ACC><<<g, rt::kThreads, 0, st>>>(P);
@@ -319,35 +317,20 @@ int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const
         return RT_OK;
     }
 
-    if (variant == RT_VARIANT_DEFAULT && pl.map_src && table_march_sizes(n_src, n_bins)) {
-        // Sources that share their cell fractions (decided on the device) are marched by march_table_kernel, others
-        // by the gated march_sliding_kernel: each of the two returns at once when the flag says it is the other's call
-        int* flag = reinterpret_cast<int*>(ws + wl.flag_at);
-        P.acc = master;
-        P.same_frac = flag;
-        P.acc_copies = wl.acc_copies;
-        P.acc_copy_stride = (long long)n_acc;
-        RT_CUDA(cudaMemsetAsync(master, 0, n_acc * sizeof(double) * size_t(wl.acc_copies), st));                // D14: overwrite
-        const long long tb = rt::march_blocks(P.n_src, P.n_slots, 1, 1);
-        if (tb > 2147483647LL) return RT_EINVAL;
-        rt::same_fraction_kernel<<<1, 256, 0, st>>>(flag, sources, n_src, step_size);
-        rt::march_table_kernel<8><<<unsigned(tb), rt::kThreads, 0, st>>>(P);
-        rt::march_sliding_kernel<1, double, 8, false, false, false, true><<<unsigned(tb), rt::kThreads, 0, st>>>(P);
-        rt::snapshot_finalize_kernel<double><<<unsigned(fin_blocks), fin_threads, 0, st>>>(master, out, ck.cells, n_steps,
-                                                                                          wl.acc_copies, (long long)n_acc);
-        RT_CUDA(cudaGetLastError());
-        return RT_OK;
-    }
-
     // the accumulation grid: fp64 in the workspace (default), or `out` itself (RT_VARIANT_FLAG_ACC_F32)
     P.acc = pl.acc64 ? static_cast<void*>(master) : static_cast<void*>(out);
-    RT_CUDA(cudaMemsetAsync(P.acc, 0, n_acc * (pl.acc64 ? sizeof(double) : sizeof(float)), st));   // D14: overwrite
+    if (pl.acc64 && pl.sliding && !vec4 && !pl.ktri) {       // the one-bin kernel spreads its reductions over copies
+        P.acc_copies = wl.acc_copies;
+        P.acc_copy_stride = (long long)n_acc;
+    }
+    RT_CUDA(cudaMemsetAsync(P.acc, 0, n_acc * (pl.acc64 ? sizeof(double) * size_t(P.acc_copies) : sizeof(float)), st));   // D14: overwrite
     int rc3;
     if (vec4) rc3 = pl.acc64 ? launch_march<4, double>(P, pl.sliding, st) : launch_march<4, float>(P, pl.sliding, st);
     else rc3 = pl.acc64 ? launch_march<1, double>(P, pl.sliding, st) : launch_march<1, float>(P, pl.sliding, st);
     if (rc3 != RT_OK) return rc3;
     if (pl.acc64) {
-        rt::snapshot_finalize_kernel<double><<<unsigned(fin_blocks), fin_threads, 0, st>>>(master, out, ck.cells, n_steps);
+        rt::snapshot_finalize_kernel<double><<<unsigned(fin_blocks), fin_threads, 0, st>>>(master, out, ck.cells, n_steps,
+                                                                                          P.acc_copies, P.acc_copy_stride);
         RT_CUDA(cudaGetLastError());
     } else if (n_steps > 1) {
         rt::snapshot_finalize_kernel<float><<<unsigned(fin_blocks), fin_threads, 0, st>>>(out, out, ck.cells, n_steps);
@@ -688,8 +671,7 @@ int rt_launch_count(int nx, int ny, int nz, int n_src, int n_rays, int n_bins, i
                             ((slots + bt.slots_per_batch - 1) / bt.slots_per_batch);
         return setup + batches + (batches + 1) / 2 + 1;         // batches march in pairs, one drain per pair
     }
-    // march, snapshot finalisation; the one-bin march with >= 32 sources: fraction test, table march, gated march
-    return setup + 2 + (table_march_sizes(n_src, n_bins) ? 2 : 0);
+    return setup + 2;                                                               // march, snapshot finalisation
 }
 
 int rt_directions(int n_rays, double* nhat, void* stream) {
@@ -780,6 +762,6 @@ const char* rt_strerror(int code) {
     }
 }
 
-const char* rt_version(void) { return "rtmarch 0.5 (sm_100a; sliding-stencil RED march, 32 sources x 1 direction per warp, per-warp weight table for sources sharing their cell fractions, fp64 accumulation grid)"; }
+const char* rt_version(void) { return "rtmarch 0.5 (sm_100a; sliding-stencil RED march, 32 sources x 1 direction per warp, fp64 accumulation grid in up to 4 copies)"; }
 
 }  // extern "C"

@@ -144,21 +144,17 @@ template <int NB, typename ACC, bool KTRI> struct Stencil {
 // STEP: the rt_march_step form -- start at substep P.k0 with (I, exp(-tau)) loaded from the ray state, store them back
 // RECORD (rt_march_adjoint_kappa): nothing is deposited; (I_{k+1}, P_k = ds J_k T_k), both scaled by 4 pi/N_Omega, of
 // every substep go to record[k * record_stride + thread], a warp writing one 256-byte run per substep.
-// GATED: the launch that follows march_table_kernel (rt_march_table.cuh) -- returns at once if that kernel has marched
-// the call, and spreads its reductions over the copies of the accumulation grid like it.  (A separate instantiation:
-// the plain kernel's code stays as it is.)
-template <int NB, typename ACC, int MINB, bool STEP, bool KTRI = false, bool RECORD = false, bool GATED = false>
+// COPIES: block b reduces into copy b % P.acc_copies of the accumulation grid.  ncu shows this march loading the L2
+// slices unevenly (atomic input 19-67 % busy across slices: the voxels next to the sources and on the faces are
+// hot); a few copies of a small grid spread a hot voxel over as many addresses, snapshot_finalize_kernel adds them
+// up (C2: 18.1 -> 17.2 ms with 3 copies).  A separate instantiation: the plain kernel's code stays as it is.
+template <int NB, typename ACC, int MINB, bool STEP, bool KTRI = false, bool RECORD = false, bool COPIES = false>
 __global__ void __launch_bounds__(kThreads, MINB) march_sliding_kernel(const MarchParams P, float2* record = nullptr,
                                                                        long long record_stride = 0) {
-    if constexpr (GATED)
-        if (*P.same_frac) return;
-    // the batched path launches the next batch (other scratch grid, no dependence on this one) with programmatic
-    // stream serialization: it may start as soon as every block of this grid has started, filling this grid's tail
-    if constexpr (NB == 4) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     RayId id;
     if (!ray_id(P, id)) return;
     ACC* og = static_cast<ACC*>(P.acc);      // the bin offset id.group * NB rides in the stencil's base offset
-    if constexpr (GATED) og += (blockIdx.x % unsigned(P.acc_copies)) * P.acc_copy_stride;
+    if constexpr (COPIES) og += (blockIdx.x % unsigned(P.acc_copies)) * P.acc_copy_stride;
 
     TravelAxis A[3];
     int negbits = 0;                         // bit a: the ray descends axis a

@@ -68,7 +68,8 @@ __global__ void directions_kernel(double* nhat, int n_rays) {
 
 // out[m] <- acc[0] + ... + acc[m]: per-step increments become the cumulative snapshots (D7).
 // ACC = float with acc == out: in place; ACC = double: the fp64 accumulation grid is summed in fp64 and rounded once.
-// `copies` grids, `copy_stride` elements apart, are added first (the table march spreads its reductions over them).
+// `copies` grids, `copy_stride` elements apart, are added first (march_sliding_kernel<..., COPIES> spreads its
+// reductions over them).
 template <typename ACC>
 __global__ void snapshot_finalize_kernel(const ACC* acc, float* out, long long stride, int n_steps, int copies = 1,
                                          long long copy_stride = 0) {

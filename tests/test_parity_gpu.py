@@ -202,10 +202,11 @@ def test_many_sources_fill_warps_raggedly(rt, oracle_mod, n_src, integer, varian
 
 @pytest.mark.parametrize("case", ["quarter_fractions", "one_source_off", "integer_outside", "long_steps", "two_warps"])
 def test_sources_sharing_their_cell_fractions(rt, oracle_mod, case):
-    """rt_march with >= 32 sources and one bin launches march_table_kernel (all sources share their fractional cell
-    offsets: one weight table per warp) and the gated march_sliding_kernel (they do not, or step_size >= 1); a flag
-    computed on the device decides which of the two does the work.  Both against the oracle and against the plain
-    kernel; substeps per step not a multiple of the 32-row table, a ragged last source group (dark padding lanes)."""
+    """>= 32 sources, one bin: warp = 32 sorted sources x 1 direction.  Sources that share their fractional cell
+    offsets (the lanes then cross cell planes in the same substep) with non-zero fractions, one source breaking the
+    pattern, sources outside the box, substeps longer than a cell, a ragged last source group and exactly two full
+    groups; reductions spread over the copies of the accumulation grid.  Against the oracle and against the
+    textbook-order kernel variant."""
     shape, n_rays, ds, dt, n_steps = (9, 7, 8), 37, 0.25, 9.25, 3            # 37 substeps per step
     rng = np.random.default_rng(77)
     n_src = 45
