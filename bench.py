@@ -169,7 +169,7 @@ class ClockSampler:
         sm = sorted(float(r[0]) for r in rows)
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         reasons = [n for i, n in enumerate(names) if any(r[3 + i].lower().startswith("active") for r in rows)]
-        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(rows[0][1]), "reasons": reasons,
+        return {"sm_mhz": sm[len(sm) // 2], "sm_min_mhz": sm[0], "sm_max_mhz": float(rows[0][1]), "reasons": reasons,
                 "power_w_max": max(float(r[2]) for r in rows), "samples": len(rows)}
 
 
@@ -334,6 +334,11 @@ def run_native(args):
             rt.rt_march_host(hj.numpy(), hk.numpy(), hs.numpy(), w.n_rays, w.step_size, w.c, w.dt, w.n_steps,
                              out=hout.numpy())
         barrier()
+        e2e_sampler = ClockSampler(local)
+        if rank == 0:
+            e2e_sampler.start()
+            time.sleep(0.1)
+        te0 = time.perf_counter()
         call_s = []
         for _ in range(n_e2e):
             tc = time.perf_counter()
@@ -343,7 +348,11 @@ def run_native(args):
                 dist.all_reduce(hout.cuda(), op=dist.ReduceOp.SUM)
                 torch.cuda.synchronize()
             call_s.append(time.perf_counter() - tc)
+        te1 = time.perf_counter()
         barrier()
+        if rank == 0:
+            time.sleep(0.1)
+            e2e_sampler.stop()
         # median call (robust against a stray hiccup of a shared box)
         e2e_s = torch.tensor([sorted(call_s)[len(call_s) // 2] * n_e2e], dtype=torch.float64, device="cuda")
         if world > 1:
@@ -353,7 +362,8 @@ def run_native(args):
                            "h2d_bytes_per_step": int(hj.numel() * 4 + hk.numel() * 4 + hs.numel() * 4),
                            "d2h_bytes_per_step": int(hout.numel() * 4), "steps": n_e2e,
                            "api": "rt_march_host (device buffers from the library's memory pool + H2D + march + D2H inside the call), "
-                                  "wall clock around each synchronous call (median call x steps), pinned host buffers", "call_ms": [1e3 * t for t in call_s]}
+                                  "wall clock around each synchronous call (median call x steps), pinned host buffers", "call_ms": [1e3 * t for t in call_s],
+                           "min_call_ms": 1e3 * min(call_s), "clocks": e2e_sampler.summary(te0, te1)}
 
     # ---- roofline of the dominant kernel (the march kernel) against the measured L2-reduction ceiling
     if rank == 0:

@@ -13,6 +13,7 @@
 #include "rt_march_direct.cuh"
 #include "rt_adjoint.cuh"
 #include "rt_march_sliding.cuh"
+#include "rt_march_table.cuh"
 #include "rt_setup_kernels.cuh"
 
 namespace {
@@ -77,9 +78,9 @@ int check_args(const void* j, const void* kappa, int nx, int ny, int nz, const v
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
-// workspace layout: [ray order: slots u32][source order: n_src u32][fp64 accumulation grid x copies][fp32 scratch]
+// workspace layout: [ray order: slots u32][source order: n_src u32][flag][fp64 accumulation grid x copies][fp32 scratch]
 struct Workspace {
-    size_t src_order_at, acc_at, scratch2_at, total;
+    size_t src_order_at, flag_at, acc_at, scratch2_at, total;
     int acc_copies;
 };
 bool use_batched_fp32(long long cells, int n_steps, int n_bins);
@@ -91,7 +92,8 @@ Workspace workspace_layout(long long cells, int n_src, int n_rays, int n_steps, 
     const size_t grid = size_t(cells) * size_t(n_steps) * sizeof(double);
     w.acc_copies = use_batched_fp32(cells, n_steps, n_bins) ? 1 : int(std::min<size_t>(4, std::max<size_t>(1, kAccCopiesBytes / grid)));
     w.src_order_at = align_up(size_t(ray_slots(n_rays)) * sizeof(uint32_t), 16);
-    w.acc_at = align_up(w.src_order_at + size_t(n_src) * sizeof(uint32_t), 256);
+    w.flag_at = align_up(w.src_order_at + size_t(n_src) * sizeof(uint32_t), 16);      // same-fraction flag (table march)
+    w.acc_at = align_up(w.flag_at + 16, 256);
     w.scratch2_at = align_up(w.acc_at + grid * size_t(w.acc_copies), 256);
     // the batched fp32 path marches two batches at a time: `out` and this second fp32 grid are their scratch grids
     w.total = w.scratch2_at + (use_batched_fp32(cells, n_steps, n_bins) ? size_t(cells) * size_t(n_steps) * sizeof(float) : 0);
@@ -125,7 +127,8 @@ int launch_march(const rt::MarchParams& P, bool sliding, cudaStream_t st, bool o
         constexpr int kMinBlocks = (NB == 1) ? 8 : 4;
         if (P.kappa_trilinear) rt::march_sliding_kernel<NB, ACC, 1, false, true><<<g, rt::kThreads, 0, st>>>(P);
         else if (P.state_I) rt::march_sliding_kernel<NB, ACC, kMinBlocks, true><<<g, rt::kThreads, 0, st>>>(P);
-        else if (P.acc_copies > 1) rt::march_sliding_kernel<NB, ACC, kMinBlocks, false, false, false, true><<<g, rt::kThreads, 0, st>>>(P);
+        else if (P.acc_copies > 1 || P.same_frac)
+            rt::march_sliding_kernel<NB, ACC, kMinBlocks, false, false, false, true><<<g, rt::kThreads, 0, st>>>(P);
         else rt::march_sliding_kernel<NB, ACC, kMinBlocks, false><<<g, rt::kThreads, 0, st>>>(P);
     } else {
         rt::march_direct_kernel<NB, ACC><<<g, rt::kThreads, 0, st>>>(P);
@@ -182,6 +185,12 @@ bool make_plan(int variant, int n_src, Plan* pl) {
     pl->coherent = !(kind == RT_VARIANT_DIRECT || kind == RT_VARIANT_SLIDING_LATTICE);
     pl->map_src = (kind == RT_VARIANT_SLIDING_BY_SOURCE) || (kind == RT_VARIANT_DEFAULT && n_src >= 32);
     return true;
+}
+
+// rt_march_table.cuh: in play for the default one-bin march with 32 sources per warp (whether the sources qualify is
+// decided on the device)
+bool use_table_march(int variant, const Plan& pl, int n_bins) {
+    return variant == RT_VARIANT_DEFAULT && pl.map_src && n_bins == 1;
 }
 
 // rt_march_step: one time step from substep k0 with the ray state carried in `state`
@@ -324,6 +333,17 @@ int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const
         P.acc_copy_stride = (long long)n_acc;
     }
     RT_CUDA(cudaMemsetAsync(P.acc, 0, n_acc * (pl.acc64 ? sizeof(double) * size_t(P.acc_copies) : sizeof(float)), st));   // D14: overwrite
+    if (use_table_march(variant, pl, n_bins)) {
+        // Sources that share their cell fractions (decided on the device) are marched by march_table_kernel, others by
+        // march_sliding_kernel<..., COPIES> below: each returns at once when the flag says it is the other's call
+        int* flag = reinterpret_cast<int*>(ws + wl.flag_at);
+        rt::same_fraction_kernel<<<1, 256, 0, st>>>(flag, sources, n_src, step_size);
+        P.same_frac = flag;
+        const long long tb = rt::march_blocks(P.n_src, P.n_slots, 1, 1);
+        if (tb > 2147483647LL) return RT_EINVAL;
+        rt::march_table_kernel<10><<<unsigned(tb), rt::kThreads, 0, st>>>(P);
+        RT_CUDA(cudaGetLastError());
+    }
     int rc3;
     if (vec4) rc3 = pl.acc64 ? launch_march<4, double>(P, pl.sliding, st) : launch_march<4, float>(P, pl.sliding, st);
     else rc3 = pl.acc64 ? launch_march<1, double>(P, pl.sliding, st) : launch_march<1, float>(P, pl.sliding, st);
@@ -671,7 +691,9 @@ int rt_launch_count(int nx, int ny, int nz, int n_src, int n_rays, int n_bins, i
                             ((slots + bt.slots_per_batch - 1) / bt.slots_per_batch);
         return setup + batches + (batches + 1) / 2 + 1;         // batches march in pairs, one drain per pair
     }
-    return setup + 2;                                                               // march, snapshot finalisation
+    // march, snapshot finalisation; the one-bin march with >= 32 sources also launches the fraction test and
+    // march_table_kernel (one of the two march kernels returns at once)
+    return setup + 2 + (use_table_march(RT_VARIANT_DEFAULT, pl, n_bins) ? 2 : 0);
 }
 
 int rt_directions(int n_rays, double* nhat, void* stream) {
@@ -762,6 +784,6 @@ const char* rt_strerror(int code) {
     }
 }
 
-const char* rt_version(void) { return "rtmarch 0.5 (sm_100a; sliding-stencil RED march, 32 sources x 1 direction per warp, fp64 accumulation grid in up to 4 copies)"; }
+const char* rt_version(void) { return "rtmarch 0.6 (sm_100a; sliding-stencil RED march, 32 sources x 1 direction per warp, weight table per warp for sources sharing their cell fractions, fp64 accumulation grid in up to 4 copies)"; }
 
 }  // extern "C"

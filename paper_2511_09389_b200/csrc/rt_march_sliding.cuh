@@ -151,6 +151,8 @@ template <int NB, typename ACC, bool KTRI> struct Stencil {
 template <int NB, typename ACC, int MINB, bool STEP, bool KTRI = false, bool RECORD = false, bool COPIES = false>
 __global__ void __launch_bounds__(kThreads, MINB) march_sliding_kernel(const MarchParams P, float2* record = nullptr,
                                                                        long long record_stride = 0) {
+    if constexpr (COPIES)
+        if (P.same_frac && *P.same_frac) return;     // march_table_kernel has marched this call (rt_march_table.cuh)
     RayId id;
     if (!ray_id(P, id)) return;
     ACC* og = static_cast<ACC*>(P.acc);      // the bin offset id.group * NB rides in the stencil's base offset
