@@ -26,8 +26,9 @@
 
 namespace rt {
 
-// flag = 1 iff ds < 1 and every source has the fractional cell offsets of source 0 (exact: the fixed-point fraction of a float
-// coordinate is the float's own fraction, and the saturation of source_coord maps to whole cells)
+// flag = 1 iff ds < 1 and every source has the fractional cell offsets of source 0 -- compared as the 64 fraction
+// bits of the fixed-point coordinates the kernels march with (exact; float arithmetic on x - floor(x) would round
+// e.g. -1e-10 and -3e-10 to the same 1.0f)
 __global__ void same_fraction_kernel(int* flag, const float* sources, int n_src, float ds) {
     __shared__ int differs;
     if (threadIdx.x == 0) differs = (ds < 1.0f) ? 0 : 1;      // a substep of a cell or more may cross two planes
@@ -35,9 +36,10 @@ __global__ void same_fraction_kernel(int* flag, const float* sources, int n_src,
     int bad = 0;
     for (int s = threadIdx.x; s < n_src; s += blockDim.x)
         for (int a = 0; a < 3; ++a) {
-            const float x = fminf(fmaxf(sources[3 * size_t(s) + a], -536870912.0f), 536870912.0f);
-            const float x0 = fminf(fmaxf(sources[a], -536870912.0f), 536870912.0f);
-            bad |= !((x - floorf(x)) == (x0 - floorf(x0)));      // also true for a NaN coordinate
+            const float x = sources[3 * size_t(s) + a], x0 = sources[a];
+            const Fx96 p = fx_from_double(double(fminf(fmaxf(x, -536870912.0f), 536870912.0f)));
+            const Fx96 p0 = fx_from_double(double(fminf(fmaxf(x0, -536870912.0f), 536870912.0f)));
+            bad |= (p.fh != p0.fh) | (p.fl != p0.fl) | !(x == x);      // a NaN coordinate: leave it to the plain kernel
         }
     if (bad) atomicOr(&differs, 1);
     __syncthreads();

@@ -200,7 +200,8 @@ def test_many_sources_fill_warps_raggedly(rt, oracle_mod, n_src, integer, varian
     parity.assert_parity(out.cpu().numpy(), ref, f"n_src={n_src} variant={variant}")
 
 
-@pytest.mark.parametrize("case", ["quarter_fractions", "one_source_off", "integer_outside", "long_steps", "two_warps"])
+@pytest.mark.parametrize("case", ["quarter_fractions", "one_source_off", "integer_outside", "long_steps", "two_warps",
+                                  "tiny_negative_offsets"])
 def test_sources_sharing_their_cell_fractions(rt, oracle_mod, case):
     """>= 32 sources, one bin: warp = 32 sorted sources x 1 direction.  Sources that share their fractional cell
     offsets (the lanes then cross cell planes in the same substep) with non-zero fractions, one source breaking the
@@ -218,6 +219,8 @@ def test_sources_sharing_their_cell_fractions(rt, oracle_mod, case):
         src[31, 1] += 0.125
     elif case == "long_steps":
         ds, dt = 1.5, 12.0
+    elif case == "tiny_negative_offsets":        # fractions 1 - 1e-10, 1 - 3e-10, ...: equal in float arithmetic, not equal
+        src = src - rng.choice([1e-10, 3e-10, 7e-10], size=src.shape)
     elif case == "two_warps":
         src = rng.integers(0, 7, (64, 3)).astype(np.float64)
     src = src.astype(np.float32)
