@@ -149,7 +149,7 @@ int rt_host_release(void);
  * accumulation grid (n_steps * nx*ny*nz*n_bins doubles: deposits are summed in fp64 and rounded to fp32 once,
  * DESIGN.md §7; where several copies of it fit 48 MiB the march spreads its reductions over up to 4 copies), plus
  * one fp32 grid of n_steps * nx*ny*nz*n_bins floats where the batched multi-bin path runs
- * (n_bins % 4 == 0 and that grid <= 256 MiB).  0 on invalid arguments. */
+ * (n_bins % 4 == 0 and that grid <= 128 MiB).  0 on invalid arguments. */
 size_t rt_workspace_bytes(int nx, int ny, int nz, int n_src, int n_rays, int n_bins, int n_steps);
 
 /* N_s as the library computes it (D6): ceil(c dt / step_size), a ratio within 1e-6 (relative) of an

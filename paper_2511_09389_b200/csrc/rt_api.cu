@@ -151,7 +151,7 @@ constexpr int kMaxSortedSources = 65536;   // above this the O(n^2) source sort 
 // 2^17 rays; the batches' fp32 sums are folded into the fp64 grid one by one.  It is used when the fp32 scratch
 // grid is small enough for the drains to be cheap; larger grids take the 1-bin kernel with fp64 reductions.
 constexpr long long kBatchRays = 1LL << 17;
-constexpr size_t kBatchedScratchLimit = size_t(256) << 20;
+constexpr size_t kBatchedScratchLimit = size_t(128) << 20;
 struct Batching {
     int src_per_batch, slots_per_batch;
 };

@@ -153,6 +153,9 @@ __global__ void __launch_bounds__(kThreads, MINB) march_sliding_kernel(const Mar
                                                                        long long record_stride = 0) {
     if constexpr (COPIES)
         if (P.same_frac && *P.same_frac) return;     // march_table_kernel has marched this call (rt_march_table.cuh)
+    // the batched path launches the next batch (other scratch grid, no dependence on this one) with programmatic
+    // stream serialization: it may start as soon as every block of this grid has started, filling this grid's tail
+    if constexpr (NB == 4) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     RayId id;
     if (!ray_id(P, id)) return;
     ACC* og = static_cast<ACC*>(P.acc);      // the bin offset id.group * NB rides in the stencil's base offset
