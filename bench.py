@@ -6,7 +6,11 @@
 A "step" is one pass of the whole hot path: one rt_march call (zero-fill, ray-order, march, snapshot
 prefix) over the full workload.  Default workload = BASELINE.json configs[2] ("C2": 128^3, 4,096 rays,
 2,097 sources at the density peaks, 444 substeps), the configuration the metric is quoted on.
-One JSON line is printed by rank 0; see DESIGN.md §8 for every field.
+One JSON line is printed by rank 0; see DESIGN.md §8 for every field.  Besides the headline (C2) the default
+single-GPU run also times, a few steps each, the other large configs (`per_config`: C3, C4, and C2 with its sources
+jittered off the cell nodes -- the general-position cost of the headline) and the other entry points on C2
+(`modes`: step, trilinear_kappa, adjoint_j, adjoint_kappa), each with its own roofline and a checksum
+(--no-extras skips them).
 
 N > 1 (under torchrun): weak scaling — rank r marches sources [r*n_src, (r+1)*n_src) of the N*n_src
 highest-density cells, then one NCCL sum all-reduce of the field (sharding.py).
@@ -48,6 +52,8 @@ def parse():
                          "random dL/d out (DESIGN.md D19; `out` then holds nothing useful)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip the per_config and modes objects")
+    ap.add_argument("--extra-steps", type=int, default=5, help="timed steps of each per_config / modes entry")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target host time of the oracle sample")
     return ap.parse_args()
 
@@ -55,7 +61,7 @@ def parse():
 def make_workload(name, world_size=1):
     """Config `name`; for world_size > 1 the source list is extended to world_size * n_src sources by the
     config's own placement rule (weak scaling: per-GPU work fixed)."""
-    from paper_2511_09389_b200 import workloads
+    import workloads
     w = workloads.make_config(name)
     if world_size > 1:
         n = w.n_src * world_size
@@ -176,13 +182,17 @@ class ClockSampler:
 # ----------------------------------------------------------------------------------------------------
 # the CUDA path
 # ----------------------------------------------------------------------------------------------------
-def measure_ceilings(rt, torch, shape, n_bins):
+def measure_ceilings(rt, torch, shape, n_bins, only=None):
     """Reduction-throughput ceilings on a grid of the workload's size, in this process, back to back with
     the march: best of 5 launches of >= 2^28 reductions each, CUDA events.  Greds/s."""
     grid = torch.zeros(shape + (n_bins,), dtype=torch.float32, device="cuda")
-    grid64 = torch.zeros(shape + (n_bins,), dtype=torch.float64, device="cuda")
+    grid64 = None
     res = {}
     for name, mode in rt.binding.RED_MODES.items():
+        if only is not None and name not in only:
+            continue
+        if mode in (6, 7) and grid64 is None:
+            grid64 = torch.zeros(shape + (n_bins,), dtype=torch.float64, device="cuda")
         g = grid64 if mode in (6, 7) else grid
         if mode == 1 and grid.numel() % 4:
             continue
@@ -203,11 +213,114 @@ def measure_ceilings(rt, torch, shape, n_bins):
     return res
 
 
+class Case:
+    """One workload resident on the device with the buffers of one entry point (`mode`); step() is one pass of the
+    whole hot path through the C ABI."""
+
+    def __init__(self, rt, torch, w, sources, mode="march", variant=0):
+        self.rt, self.torch, self.w, self.mode, self.variant = rt, torch, w, mode, variant
+        nx, ny, nz = w.shape
+        nb = w.n_bins
+        self.j, self.kappa = torch.from_numpy(w.j).cuda(), torch.from_numpy(w.kappa).cuda()
+        self.src = torch.from_numpy(np.ascontiguousarray(sources)).cuda()
+        n_src = int(self.src.shape[0])
+        self.units = n_src * w.n_rays * w.n_steps * w.substeps_per_step * nb
+        u8 = torch.uint8
+        if mode in ("adjoint_j", "adjoint_kappa"):
+            self.gbar = torch.rand((w.n_steps, nx, ny, nz, nb), dtype=torch.float32, device="cuda")
+            self.result = torch.empty((nx, ny, nz, nb), dtype=torch.float32, device="cuda")
+            nbytes = (rt.rt_adjoint_workspace_bytes(nx, ny, nz, n_src, w.n_rays, nb, w.n_steps) if mode == "adjoint_j" else
+                      rt.rt_adjoint_kappa_workspace_bytes(nx, ny, nz, n_src, w.n_rays, nb, w.step_size, w.c, w.dt, w.n_steps))
+        elif mode == "step":
+            self.state = rt.rt_state_reset(n_src, w.n_rays, nb)
+            self.result = torch.empty((nx, ny, nz, nb), dtype=torch.float32, device="cuda")
+            nbytes = rt.rt_step_workspace_bytes(nx, ny, nz, n_src, w.n_rays, nb)
+        else:
+            self.result = torch.empty((w.n_steps, nx, ny, nz, nb), dtype=torch.float32, device="cuda")
+            nbytes = rt.rt_workspace_bytes(nx, ny, nz, n_src, w.n_rays, nb, w.n_steps)
+        self.ws = torch.empty(max(16, nbytes), dtype=u8, device="cuda")
+
+    def step(self):
+        rt, w = self.rt, self.w
+        a = (w.n_rays, w.step_size, w.c, w.dt)
+        if self.mode == "adjoint_kappa":
+            rt.rt_march_adjoint_kappa(self.gbar, self.j, self.kappa, self.src, *a, w.n_steps, grad_kappa=self.result,
+                                      workspace=self.ws)
+        elif self.mode == "adjoint_j":
+            rt.rt_march_adjoint_j(self.gbar, self.kappa, self.src, *a, w.n_steps, grad_j=self.result, workspace=self.ws)
+        elif self.mode == "step":        # n_steps calls with persistent ray state, the field accumulated in `result`
+            rt.rt_state_reset(int(self.src.shape[0]), w.n_rays, w.n_bins, state=self.state)
+            for m in range(w.n_steps):
+                rt.rt_march_step(self.j, self.kappa, self.src, *a, m * w.substeps_per_step, self.state, out=self.result,
+                                 accumulate=bool(m), workspace=self.ws)
+        elif self.mode == "trilinear_kappa":
+            rt.rt_march_trilinear_kappa(self.j, self.kappa, self.src, *a, w.n_steps, out=self.result, workspace=self.ws)
+        else:
+            rt.rt_march_ex(self.j, self.kappa, self.src, *a, w.n_steps, out=self.result, workspace=self.ws,
+                           variant=self.variant)
+
+    def checksum(self):
+        return float(self.result.double().sum().item())
+
+
+def time_steps(torch, flush, fn, steps, warmup, barrier=None):
+    """`warmup` untimed then `steps` timed calls of fn(); a 256 MiB memset between calls (outside the event pairs)
+    flushes the L2.  Returns the per-step milliseconds (CUDA events on the launch stream)."""
+    for _ in range(max(warmup, 0)):
+        flush.zero_()
+        fn()
+    (barrier or torch.cuda.synchronize)()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    for e0, e1 in ev:
+        flush.zero_()
+        e0.record()
+        fn()
+        e1.record()
+    (barrier or torch.cuda.synchronize)()
+    return [e0.elapsed_time(e1) for e0, e1 in ev]
+
+
+L2_BYTES = 126e6
+
+
+def roofline_of(rt, torch, w, n_src, step_s, ceil=None, mode="march"):
+    """The roofline object of one measured case.  Grids that stay L2 resident are bounded by the L2
+    reduction rate (peak = M3, the stencil-pattern ceiling measured here on a grid of the same size and bin count);
+    grids larger than the L2 by HBM traffic (peak = the measured copy bandwidth)."""
+    nx, ny, nz = w.shape
+    nb = w.n_bins
+    cells = nx * ny * nz * nb
+    substeps = n_src * w.n_rays * w.n_steps * w.substeps_per_step
+    groups = nb // 4 if nb % 4 == 0 else nb
+    alg_reds = 8 * groups * substeps
+    hbm_bytes = int((2 + 3 * w.n_steps) * cells * 4)        # j, kappa read; fp64 grid zeroed+read (as 2 fp32 units); out written
+    resident = cells * 4 <= L2_BYTES / 1.5         # one fp32 grid against the L2 (C3: 64 MiB, the v4 reduction rate bounds it; C4: 256 MiB, HBM)
+    if ceil is None:
+        ceil = measure_ceilings(rt, torch, (nx, ny, nz), nb, only=("M3_stencil", "M6_stencil_walk"))
+    red = {"achieved": alg_reds / step_s / 1e9, "peak": ceil["M3_stencil"], "unit": "Gred/s",
+           "frac": alg_reds / step_s / 1e9 / ceil["M3_stencil"], "M6_stencil_walk": ceil.get("M6_stencil_walk")}
+    hbm = {"algorithmic_bytes": hbm_bytes, "achieved": hbm_bytes / step_s / 1e9, "peak": _measured_hbm(), "unit": "GB/s",
+           "frac": hbm_bytes / step_s / 1e9 / _measured_hbm(), "peak_is": "MEASURED_PEAKS.json hbm_gbs (of measured)"
+           if _have_measured_hbm() else "fallback of B200_PROFILING.md (of fallback)"}
+    if resident:
+        roof = {"bound": "l2_red", **red, "traffic": None, "hbm": hbm}
+    else:
+        roof = {"bound": "hbm", **{k: hbm[k] for k in ("achieved", "peak", "unit", "frac")}, "traffic": None,
+                "algorithmic_bytes": hbm_bytes, "peak_is": hbm["peak_is"], "l2_red": red}
+    roof["how"] = ("achieved = ALGORITHMIC units / mean CUDA-event time of the whole call; l2_red: 8 corners x bin groups x "
+                   "ray-substeps against M3 measured in this process (frac > 1: the sliding stencil sums a voxel's deposits "
+                   "in registers and issues fewer reductions than the method states); hbm: (2 + 3 n_steps) grids of fp32 "
+                   "size against the measured copy bandwidth")
+    if mode != "march":
+        roof["note"] = f"mode {mode}: the same algorithmic count as the forward march of this workload"
+    return roof
+
+
 def run_native(args):
     import torch
     import torch.distributed as dist
 
-    import paper_2511_09389_b200 as rt          # raises if librtmarch.so is missing: no fallback
+    import paper_2511_09389_b200 as rt          # raises on first use if librtmarch.so is missing: no fallback
     from paper_2511_09389_b200 import sharding
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -217,6 +330,8 @@ def run_native(args):
         raise RuntimeError("bench.py needs a CUDA device (use --impl reference for the CPU oracle)")
     torch.cuda.set_device(local)
     if world > 1:
+        os.environ.setdefault("NCCL_DEBUG", "INFO")             # the communicator lines (ranks, NVLS) stay in the log
+        os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     if world != args.gpus and rank == 0:
         print(f"warning: --gpus {args.gpus} but WORLD_SIZE={world}", file=sys.stderr)
@@ -226,53 +341,15 @@ def run_native(args):
     sl = sharding.source_slice(w.n_src, rank, world)
     nx, ny, nz = w.shape
     nb = w.n_bins
-    j, kappa = torch.from_numpy(w.j).cuda(), torch.from_numpy(w.kappa).cuda()
-    src = torch.from_numpy(np.ascontiguousarray(w.sources[sl])).cuda()
-    out = torch.empty((w.n_steps, nx, ny, nz, nb), dtype=torch.float32, device="cuda")
-    ws = rt.alloc_workspace(nx, ny, nz, src.shape[0], w.n_rays, nb, w.n_steps)
+    case = Case(rt, torch, w, w.sources[sl], args.mode, args.variant)
+    n_src = int(case.src.shape[0])
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB L2
-    units_per_gpu = src.shape[0] * w.n_rays * w.n_steps * w.substeps_per_step * nb
-
-    if args.mode == "step":
-        state = rt.rt_state_reset(src.shape[0], w.n_rays, nb)
-        ws_step = torch.empty(max(16, rt.rt_step_workspace_bytes(nx, ny, nz, src.shape[0], w.n_rays, nb)),
-                              dtype=torch.uint8, device="cuda")
-
-    if args.mode == "adjoint_j":
-        gbar = torch.rand((w.n_steps, nx, ny, nz, nb), dtype=torch.float32, device="cuda")
-        grad_j = torch.empty((nx, ny, nz, nb), dtype=torch.float32, device="cuda")
-        ws_adj = torch.empty(max(16, rt.rt_adjoint_workspace_bytes(nx, ny, nz, src.shape[0], w.n_rays, nb, w.n_steps)),
-                             dtype=torch.uint8, device="cuda")
-
-    if args.mode == "adjoint_kappa":
-        gbar = torch.rand((w.n_steps, nx, ny, nz, nb), dtype=torch.float32, device="cuda")
-        grad_j = torch.empty((nx, ny, nz, nb), dtype=torch.float32, device="cuda")
-        ws_adj = torch.empty(max(16, rt.rt_adjoint_kappa_workspace_bytes(nx, ny, nz, src.shape[0], w.n_rays, nb, w.step_size,
-                                                                         w.c, w.dt, w.n_steps)),
-                             dtype=torch.uint8, device="cuda")
+    units_per_gpu = case.units
 
     def step():
-        if args.mode == "adjoint_kappa":
-            rt.rt_march_adjoint_kappa(gbar, j, kappa, src, w.n_rays, w.step_size, w.c, w.dt, w.n_steps, grad_kappa=grad_j,
-                                      workspace=ws_adj)
-            return
-        if args.mode == "adjoint_j":
-            rt.rt_march_adjoint_j(gbar, kappa, src, w.n_rays, w.step_size, w.c, w.dt, w.n_steps, grad_j=grad_j,
-                                  workspace=ws_adj)
-            return
-        if args.mode == "step":        # n_steps calls, the field of the last snapshot accumulated in out[-1]
-            rt.rt_state_reset(src.shape[0], w.n_rays, nb, state=state)
-            out[-1].zero_()
-            for m in range(w.n_steps):
-                rt.rt_march_step(j, kappa, src, w.n_rays, w.step_size, w.c, w.dt, m * w.substeps_per_step, state,
-                                 out=out[-1], accumulate=True, workspace=ws_step)
-        elif args.mode == "trilinear_kappa":
-            rt.rt_march_trilinear_kappa(j, kappa, src, w.n_rays, w.step_size, w.c, w.dt, w.n_steps, out=out, workspace=ws)
-        else:
-            rt.rt_march_ex(j, kappa, src, w.n_rays, w.step_size, w.c, w.dt, w.n_steps, out=out, workspace=ws,
-                           variant=args.variant)
+        case.step()
         if world > 1:
-            sharding.allreduce_field(out)
+            sharding.allreduce_field(case.result)
 
     def barrier():
         torch.cuda.synchronize()
@@ -288,17 +365,9 @@ def run_native(args):
     if rank == 0:
         sampler.start()
         time.sleep(0.3)
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    barrier()
     t0 = time.perf_counter()
-    for e0, e1 in ev:
-        flush.zero_()                 # L2 flush between timed iterations (outside the event pair)
-        e0.record()
-        step()
-        e1.record()
-    barrier()
+    step_ms = time_steps(torch, flush, step, args.steps, 0, barrier)
     t1 = time.perf_counter()
-    step_ms = [e0.elapsed_time(e1) for e0, e1 in ev]
     total_ms = torch.tensor([sum(step_ms)], dtype=torch.float64, device="cuda")
     if world > 1:
         dist.all_reduce(total_ms, op=dist.ReduceOp.MAX)
@@ -311,13 +380,12 @@ def run_native(args):
 
     line = None
     if rank == 0:
-        field_sum = float((out[-1] if args.mode == "step" else out).double().sum().item())
-        launches = rt.rt_launch_count(nx, ny, nz, int(src.shape[0]), w.n_rays, nb, w.n_steps)
+        launches = rt.rt_launch_count(nx, ny, nz, n_src, w.n_rays, nb, w.n_steps)
         cfg = describe(w, world)
         cfg["workload"] = cfg["workload"].replace(f"{w.n_src} sources/GPU", f"{n_src_per_gpu} sources/GPU")
         cfg.update({"timing": "CUDA events per step on the launch stream; 256 MiB L2 flush (memset) between "
                               "timed steps, outside the event pairs; inputs resident in HBM",
-                    "kernel_variant": args.variant, "mode": args.mode, "field_checksum": field_sum})
+                    "kernel_variant": args.variant, "mode": args.mode, "field_checksum": case.checksum()})
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": 1e3 * total_s / args.steps, "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": cfg,
@@ -329,10 +397,20 @@ def run_native(args):
         hj, hk = torch.from_numpy(w.j).pin_memory(), torch.from_numpy(w.kappa).pin_memory()
         hs = torch.from_numpy(np.ascontiguousarray(w.sources[sl])).pin_memory()
         hout = torch.empty((w.n_steps, nx, ny, nz, nb), dtype=torch.float32).pin_memory()
+        dfield = torch.empty_like(hout, device="cuda") if world > 1 else None
         n_e2e = max(1, min(args.steps, 11))
-        for _ in range(3):             # untimed: pool allocation, page-locking, clocks back up after the idle gap
+
+        def e2e_call():
             rt.rt_march_host(hj.numpy(), hk.numpy(), hs.numpy(), w.n_rays, w.step_size, w.c, w.dt, w.n_steps,
                              out=hout.numpy())
+            if world > 1:          # the field leaves the call on the host: sum it over the ranks and bring the sum back
+                dfield.copy_(hout, non_blocking=True)
+                dist.all_reduce(dfield, op=dist.ReduceOp.SUM)
+                hout.copy_(dfield, non_blocking=True)
+                torch.cuda.synchronize()
+
+        for _ in range(3):             # untimed: pool allocation, page-locking, clocks back up after the idle gap
+            e2e_call()
         barrier()
         e2e_sampler = ClockSampler(local)
         if rank == 0:
@@ -342,11 +420,7 @@ def run_native(args):
         call_s = []
         for _ in range(n_e2e):
             tc = time.perf_counter()
-            rt.rt_march_host(hj.numpy(), hk.numpy(), hs.numpy(), w.n_rays, w.step_size, w.c, w.dt, w.n_steps,
-                             out=hout.numpy())
-            if world > 1:          # the field leaves the call on the host: reduce it there
-                dist.all_reduce(hout.cuda(), op=dist.ReduceOp.SUM)
-                torch.cuda.synchronize()
+            e2e_call()
             call_s.append(time.perf_counter() - tc)
         te1 = time.perf_counter()
         barrier()
@@ -358,50 +432,55 @@ def run_native(args):
         if world > 1:
             dist.all_reduce(e2e_s, op=dist.ReduceOp.MAX)
         if rank == 0:
+            extra = int(hout.numel() * 4) if world > 1 else 0
             line["e2e"] = {"value": units_per_gpu * world * n_e2e / float(e2e_s.item()), "unit": UNIT,
-                           "h2d_bytes_per_step": int(hj.numel() * 4 + hk.numel() * 4 + hs.numel() * 4),
-                           "d2h_bytes_per_step": int(hout.numel() * 4), "steps": n_e2e,
+                           "h2d_bytes_per_step": int(hj.numel() * 4 + hk.numel() * 4 + hs.numel() * 4) + extra,
+                           "d2h_bytes_per_step": int(hout.numel() * 4) + extra, "steps": n_e2e,
                            "api": "rt_march_host (device buffers from the library's memory pool + H2D + march + D2H inside the call), "
-                                  "wall clock around each synchronous call (median call x steps), pinned host buffers", "call_ms": [1e3 * t for t in call_s],
+                                  "wall clock around each synchronous call (median call x steps), pinned host buffers"
+                                  + ("; N > 1: the host field goes back to the device, one NCCL sum all-reduce, and back" if world > 1 else ""),
+                           "call_ms": [1e3 * t for t in call_s],
                            "min_call_ms": 1e3 * min(call_s), "clocks": e2e_sampler.summary(te0, te1)}
+        del hj, hk, hs, hout
 
     # ---- roofline of the dominant kernel (the march kernel) against the measured L2-reduction ceiling
     if rank == 0:
         ceil = measure_ceilings(rt, torch, (nx, ny, nz), nb)
         step_s = total_s / args.steps
-        reds_per_substep = 8 * (nb // 4 if nb % 4 == 0 else nb)           # algorithmic: 8 corners x bin groups
-        alg_reds = reds_per_substep * src.shape[0] * w.n_rays * w.n_steps * w.substeps_per_step
-        achieved = alg_reds / step_s / 1e9
-        peak = ceil["M3_stencil"]
-        hbm_bytes = int((2 + 3 * w.n_steps) * nx * ny * nz * nb * 4)      # j, kappa read; fp64 grid zeroed+read; out written
-        roof = {
-            "bound": "l2_red", "achieved": achieved, "peak": peak, "unit": "Gred/s", "frac": achieved / peak,
-            "traffic": None, "kernel": "march_sliding_kernel",
-            "how": "achieved = ALGORITHMIC reductions (8 corners x bin-groups x ray-substeps) / mean CUDA-event "
-                   "time of the whole rt_march call (the march kernel is 99% of it at C2, profiles/r01f); peak = "
-                   "M3 stencil-pattern red.global.add ceiling measured in this process on a grid of the same "
-                   "size (DESIGN.md §8), of measured; frac > 1: the sliding stencil sums a voxel's deposits in "
-                   "registers, so fewer reductions are issued than the method states (see `issued`)",
-            "best_step_frac": alg_reds / (min(step_ms) * 1e-3) / 1e9 / peak if world == 1 else None,
-            "ceilings_Gred_per_s": ceil,
-            "hbm": {"algorithmic_bytes": hbm_bytes, "achieved_GBps": hbm_bytes / step_s / 1e9,
-                    "peak_GBps": _measured_hbm(), "note": "grids are L2 resident at C0-C2: HBM is not the bound"}}
-        cnt = _ncu_counters(args.config, args.variant)
+        roof = roofline_of(rt, torch, w, n_src, step_s, ceil, args.mode)
+        roof["kernel"] = "march kernel of the call"
+        roof["ceilings_Gred_per_s"] = ceil
+        if world == 1:
+            red = roof if roof["bound"] == "l2_red" else roof["l2_red"]
+            red["best_step_frac"] = red["frac"] * step_s / (min(step_ms) * 1e-3)
+        cnt = _ncu_counters(args.config, args.variant) if args.mode == "march" else None
         if cnt and world == 1:
             sm_hz = (clocks.get("sm_mhz") or 1965.0) * 1e6
+            substeps = n_src * w.n_rays * w.n_steps * w.substeps_per_step
             roof["traffic"] = cnt["dram_bytes"]
             roof["issued"] = {"red_sectors_per_launch": cnt["red_sectors"],
-                              "red_sectors_per_ray_substep": cnt["red_sectors"] / (alg_reds / reds_per_substep),
+                              "red_sectors_per_ray_substep": cnt["red_sectors"] / substeps,
                               "achieved_Gsectors_per_s": cnt["red_sectors"] / step_s / 1e9,
                               "frac_of_M3": cnt["red_sectors"] / step_s / 1e9 / ceil["M3_f64_stencil"]}
             roof["alu"] = {"warp_instructions_per_launch": cnt["warp_instructions"],
+                           "warp_instructions_per_warp_substep": cnt["warp_instructions"] / (substeps / 32),
                            "achieved_Ginst_per_s": cnt["warp_instructions"] / step_s / 1e9,
                            "peak_Ginst_per_s": 148 * 4 * sm_hz / 1e9,
                            "frac": cnt["warp_instructions"] / step_s / (148 * 4 * sm_hz),
                            "peak_how": "148 SMs x 4 schedulers x 1 warp-instruction/clk x SM clock sampled in the run"}
             roof["kernel"] = cnt["kernel"]
             roof["counters_from"] = cnt["source"]
+            roof["how"] += ("; `traffic`, `issued` and `alu` are REPLAYED from the committed ncu capture named in "
+                            "`counters_from` (same library version string), divided by the step time measured here")
         line["roofline"] = roof
+
+    # ---- the other large configs and the other entry points, a few steps each (single GPU, default run only)
+    if rank == 0 and world == 1 and not args.no_extras and args.config == "C2" and args.mode == "march" and args.variant == 0:
+        del case
+        torch.cuda.empty_cache()
+        line["per_config"], line["modes"] = run_extras(rt, torch, w, flush, args.extra_steps)
+
+    if rank == 0:
         if not args.no_cpu_baseline and world == 1:
             ups, cores, what, _, _ = oracle_sample(make_workload(args.config), args.cpu_seconds)
             line["cpu_baseline"] = {"value": ups, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": what}
@@ -410,6 +489,39 @@ def run_native(args):
         dist.barrier()
         dist.destroy_process_group()
     return 0
+
+
+def run_extras(rt, torch, w_c2, flush, steps):
+    """per_config: C3, C4 and C2 with its sources jittered by +-0.5 cell (sources in general position: no shared cell
+    fractions, divergent stencil slides); modes: the other entry points on C2.  Each: `steps` timed calls after 3
+    warm-ups, CUDA events, L2 flushed between calls; its own roofline; a checksum of the result."""
+    import workloads
+
+    def measure(w, sources, mode="march", label=None):
+        case = Case(rt, torch, w, sources, mode)
+        ms = time_steps(torch, flush, case.step, steps, 3)
+        mean_s = sum(ms) / len(ms) * 1e-3
+        n_src = int(case.src.shape[0])
+        row = {"workload": label or describe(w, 1)["workload"], "mode": mode, "steps": steps, "warmup": 3,
+               "ms_per_step": 1e3 * mean_s, "step_ms_each": ms, "updates_per_s": case.units / mean_s,
+               "ray_substeps_per_s": case.units / w.n_bins / mean_s, "checksum": case.checksum(),
+               "gpu_launches_per_step": rt.rt_launch_count(*w.shape, n_src, w.n_rays, w.n_bins, w.n_steps) if mode == "march" else None,
+               "roofline": roofline_of(rt, torch, w, n_src, mean_s, None, mode)}
+        del case
+        torch.cuda.empty_cache()
+        return row
+
+    modes = {m: measure(w_c2, w_c2.sources, m) for m in ("step", "trilinear_kappa", "adjoint_j", "adjoint_kappa")}
+    per_config = {}
+    jit = (w_c2.sources.astype(np.float64) + np.random.default_rng(939912).uniform(-0.5, 0.5, w_c2.sources.shape))
+    jit = np.clip(jit, 0.0, w_c2.shape[0] - 1.0).astype(np.float32)
+    per_config["C2_jittered"] = measure(w_c2, jit, label=describe(w_c2, 1)["workload"] +
+                                        "; sources moved off the cell nodes by uniform(-0.5, 0.5) per axis (seed 939912)")
+    for name in ("C3", "C4"):
+        w = workloads.make_config(name)
+        per_config[name] = measure(w, w.sources)
+        del w
+    return per_config, modes
 
 
 def _ncu_counters(config, variant):
@@ -437,6 +549,10 @@ def _measured_hbm():
         return json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
     except (OSError, KeyError, ValueError):
         return 6650.0      # fallback of B200_PROFILING.md
+
+
+def _have_measured_hbm():
+    return os.path.exists(os.path.join(ROOT, "MEASURED_PEAKS.json"))
 
 
 if __name__ == "__main__":

@@ -23,7 +23,8 @@
  * CUDA device, owned by the caller (e.g. a torch tensor's data_ptr()); the library never frees or keeps
  * it.  rt_march* are ASYNCHRONOUS: all work is enqueued on `stream` (a cudaStream_t passed as void*; NULL =
  * the legacy default stream) and the caller synchronises.  j, kappa, sources, out and workspace must not
- * overlap.  No global state; re-entrant per stream (each concurrent call needs its own workspace and out).
+ * overlap.  Re-entrant per stream (each concurrent call needs its own workspace and out); the only state the
+ * library keeps between calls is rt_march_host's memory pool (below) and a thread-local CUDA error string.
  *
  * ERRORS.  Functions returning int give RT_OK (0) or a negative RT_E* code; rt_strerror() names it.
  * Argument errors are detected on the host BEFORE any CUDA call, so they can be exercised without a GPU.
@@ -133,6 +134,16 @@ int rt_march_adjoint_kappa(const float* gbar, const float* j, const float* kappa
                            const float* sources, int n_src, int n_rays, int n_bins,
                            float step_size, float c, float dt, int n_steps, float* grad_kappa,
                            void* workspace, size_t workspace_bytes, void* stream);
+
+/* TEST HOOK.  rt_march_adjoint_kappa with the bound on the forward record of one source batch given explicitly
+ * (record_limit bytes; 0 = the library's 2 GiB), so that tests can drive the source-batch loop on small cases.  A batch
+ * never holds fewer than 32 sources (n_src >= 32) or 1 source (n_src < 32).  Same result for every limit. */
+size_t rt_adjoint_kappa_workspace_bytes_ex(int nx, int ny, int nz, int n_src, int n_rays, int n_bins,
+                                           float step_size, float c, float dt, int n_steps, size_t record_limit);
+int rt_march_adjoint_kappa_ex(const float* gbar, const float* j, const float* kappa, int nx, int ny, int nz,
+                              const float* sources, int n_src, int n_rays, int n_bins,
+                              float step_size, float c, float dt, int n_steps, float* grad_kappa,
+                              void* workspace, size_t workspace_bytes, void* stream, size_t record_limit);
 
 /* End-to-end form with HOST pointers (j, kappa, sources, out are host memory, pinned or pageable).
  * Allocates device buffers, copies the inputs in, marches, copies out[] back, frees, and returns after the

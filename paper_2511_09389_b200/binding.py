@@ -26,7 +26,8 @@ EXPORTS = ("rt_march", "rt_march_single", "rt_march_ex", "rt_march_host", "rt_wo
            "rt_substeps_per_step", "rt_launch_count", "rt_directions", "rt_ray_order", "rt_ray_slots", "rt_trace_ray",
            "rt_bench_red_ceiling", "rt_strerror", "rt_version", "rt_state_bytes", "rt_state_reset",
            "rt_step_workspace_bytes", "rt_march_step", "rt_march_trilinear_kappa", "rt_adjoint_workspace_bytes",
-           "rt_march_adjoint_j", "rt_adjoint_kappa_workspace_bytes", "rt_march_adjoint_kappa", "rt_host_release")
+           "rt_march_adjoint_j", "rt_adjoint_kappa_workspace_bytes", "rt_march_adjoint_kappa",
+           "rt_adjoint_kappa_workspace_bytes_ex", "rt_march_adjoint_kappa_ex", "rt_host_release")
 
 
 class RtError(RuntimeError):
@@ -39,11 +40,11 @@ def _load() -> ctypes.CDLL:
     path = _build.LIB_PATH
     if not os.path.exists(path):
         path = _build.build_library()          # raises if nvcc is missing: no fallback
-    elif _build.is_stale():                    # sources newer than the library: rebuild if a compiler is here
-        try:
+    elif _build.is_stale():                    # sources newer than the library: rebuild, or fail -- never run stale
+        try:                                   # code silently (RT_ALLOW_STALE_LIB=1 overrides, for a box without nvcc)
             path = _build.build_library()
         except RuntimeError:
-            if os.environ.get("RT_REQUIRE_FRESH_LIB"):
+            if not os.environ.get("RT_ALLOW_STALE_LIB"):
                 raise
     L = ctypes.CDLL(path)
     vp, i, f, sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_float, ctypes.c_size_t
@@ -56,6 +57,9 @@ def _load() -> ctypes.CDLL:
     L.rt_adjoint_kappa_workspace_bytes.argtypes = [i] * 6 + [f, f, f, i]
     L.rt_adjoint_kappa_workspace_bytes.restype = sz
     L.rt_march_adjoint_kappa.argtypes = [vp] + march_args + [vp, sz, vp]
+    L.rt_adjoint_kappa_workspace_bytes_ex.argtypes = [i] * 6 + [f, f, f, i, sz]
+    L.rt_adjoint_kappa_workspace_bytes_ex.restype = sz
+    L.rt_march_adjoint_kappa_ex.argtypes = [vp] + march_args + [vp, sz, vp, sz]
     L.rt_march_single.argtypes = [vp, vp, i, i, i, vp, i, i, f, f, f, i, vp, vp, sz, vp]
     L.rt_march_ex.argtypes = march_args + [vp, sz, vp, i]
     L.rt_march_host.argtypes = march_args
@@ -122,10 +126,43 @@ def _torch():
     return torch
 
 
-def _stream_ptr(stream):
+def _stream_ptr(stream, device=None):
+    """cudaStream_t of ``stream`` (a torch stream or a raw handle), else torch's current stream ON ``device``."""
     if stream is None:
-        return _torch().cuda.current_stream().cuda_stream
+        return _torch().cuda.current_stream(device).cuda_stream
     return getattr(stream, "cuda_stream", stream)
+
+
+class _Call:
+    """Context of one device call: makes the tensors' device current (the library launches on the current CUDA
+    device) and resolves the stream there.  ``scratch()`` allocates a buffer the call owns: if the launch stream is
+    not torch's current stream the buffer is recorded on it, so the caching allocator cannot hand the block to
+    another allocation while the enqueued kernels still use it."""
+
+    def __init__(self, stream, *tensors):
+        torch = _torch()
+        self.device = tensors[0].device
+        for t in tensors:
+            if t is not None and t.device != self.device:
+                raise ValueError(f"all tensors must be on one CUDA device: {t.device} vs {self.device}")
+        self._guard = torch.cuda.device(self.device)
+        self._stream = stream
+
+    def __enter__(self):
+        self._guard.__enter__()
+        self.stream_ptr = _stream_ptr(self._stream, self.device)
+        return self
+
+    def __exit__(self, *exc):
+        return self._guard.__exit__(*exc)
+
+    def scratch(self, shape, dtype):
+        torch = _torch()
+        t = torch.empty(shape, dtype=dtype, device=self.device)
+        cur = torch.cuda.current_stream(self.device)
+        if self.stream_ptr != cur.cuda_stream:
+            t.record_stream(torch.cuda.ExternalStream(self.stream_ptr, device=self.device))
+        return t
 
 
 def _check_dev(t, name, dtype, ndim=None):
@@ -145,6 +182,32 @@ def alloc_workspace(nx, ny, nz, n_src, n_rays, n_bins, n_steps, device=None):
     return torch.empty(n, dtype=torch.uint8, device=device or "cuda")
 
 
+def _out_or_new(call, out, shape, name):
+    """The caller's ``out`` (validated: float32, contiguous, on the call's device, right size) or a fresh one."""
+    torch = _torch()
+    n = 1
+    for d in shape:
+        n *= d
+    if out is None:
+        return call.scratch(shape, torch.float32)
+    _check_dev(out, name, torch.float32)
+    if out.device != call.device:
+        raise ValueError(f"{name} is on {out.device}, the inputs on {call.device}")
+    if out.numel() != n:
+        raise ValueError(f"{name} has the wrong size")
+    return out
+
+
+def _workspace_or_new(call, workspace, nbytes):
+    torch = _torch()
+    if workspace is None:
+        return call.scratch((max(16, nbytes),), torch.uint8)
+    _check_dev(workspace, "workspace", torch.uint8)
+    if workspace.device != call.device:
+        raise ValueError(f"workspace is on {workspace.device}, the inputs on {call.device}")
+    return workspace
+
+
 def rt_march_ex(j, kappa, sources, n_rays, step_size, c, dt, n_steps, out=None, workspace=None, stream=None,
                 variant=RT_VARIANT_DEFAULT, _entry=None):
     """out[n_steps,nx,ny,nz,n_bins] = the march of include/rtmarch.h; asynchronous on the stream."""
@@ -156,17 +219,12 @@ def rt_march_ex(j, kappa, sources, n_rays, step_size, c, dt, n_steps, out=None, 
         raise ValueError("kappa must have j's shape and sources must be [n_src, 3]")
     nx, ny, nz, nb = j.shape
     n_src = sources.shape[0]
-    if out is None:
-        out = torch.empty((n_steps, nx, ny, nz, nb), dtype=torch.float32, device=j.device)
-    else:
-        _check_dev(out, "out", torch.float32)
-        if out.numel() != n_steps * j.numel():
-            raise ValueError("out has the wrong size")
-    if workspace is None:
-        workspace = alloc_workspace(nx, ny, nz, n_src, n_rays, nb, n_steps, j.device)
-    args = (j.data_ptr(), kappa.data_ptr(), nx, ny, nz, sources.data_ptr(), n_src, n_rays, nb, step_size, c, dt,
-            n_steps, out.data_ptr(), workspace.data_ptr(), workspace.numel(), _stream_ptr(stream))
-    rc = _entry(*args) if _entry is not None else _lib.rt_march_ex(*args, variant)
+    with _Call(stream, j, kappa, sources) as call:
+        out = _out_or_new(call, out, (n_steps, nx, ny, nz, nb), "out")
+        workspace = _workspace_or_new(call, workspace, rt_workspace_bytes(nx, ny, nz, n_src, n_rays, nb, n_steps))
+        args = (j.data_ptr(), kappa.data_ptr(), nx, ny, nz, sources.data_ptr(), n_src, n_rays, nb, step_size, c, dt,
+                n_steps, out.data_ptr(), workspace.data_ptr(), workspace.numel(), call.stream_ptr)
+        rc = _entry(*args) if _entry is not None else _lib.rt_march_ex(*args, variant)
     if rc != RT_OK:
         raise RtError(rc, "rt_march")
     return out
@@ -199,18 +257,12 @@ def rt_march_adjoint_j(gbar, kappa, sources, n_rays, step_size, c, dt, n_steps, 
     if tuple(gbar.shape) != (n_steps, nx, ny, nz, nb) or sources.shape[1] != 3:
         raise ValueError("gbar must be [n_steps, nx, ny, nz, n_bins] and sources [n_src, 3]")
     n_src = sources.shape[0]
-    if grad_j is None:
-        grad_j = torch.empty((nx, ny, nz, nb), dtype=torch.float32, device=kappa.device)
-    else:
-        _check_dev(grad_j, "grad_j", torch.float32)
-        if grad_j.numel() != kappa.numel():
-            raise ValueError("grad_j has the wrong size")
-    if workspace is None:
-        workspace = torch.empty(max(16, rt_adjoint_workspace_bytes(nx, ny, nz, n_src, n_rays, nb, n_steps)),
-                                dtype=torch.uint8, device=kappa.device)
-    rc = _lib.rt_march_adjoint_j(gbar.data_ptr(), kappa.data_ptr(), nx, ny, nz, sources.data_ptr(), n_src, n_rays, nb,
-                                 step_size, c, dt, n_steps, grad_j.data_ptr(), workspace.data_ptr(), workspace.numel(),
-                                 _stream_ptr(stream))
+    with _Call(stream, gbar, kappa, sources) as call:
+        grad_j = _out_or_new(call, grad_j, (nx, ny, nz, nb), "grad_j")
+        workspace = _workspace_or_new(call, workspace, rt_adjoint_workspace_bytes(nx, ny, nz, n_src, n_rays, nb, n_steps))
+        rc = _lib.rt_march_adjoint_j(gbar.data_ptr(), kappa.data_ptr(), nx, ny, nz, sources.data_ptr(), n_src, n_rays,
+                                     nb, step_size, c, dt, n_steps, grad_j.data_ptr(), workspace.data_ptr(),
+                                     workspace.numel(), call.stream_ptr)
     if rc != RT_OK:
         raise RtError(rc, "rt_march_adjoint_j")
     return grad_j
@@ -220,9 +272,16 @@ def rt_adjoint_kappa_workspace_bytes(nx, ny, nz, n_src, n_rays, n_bins, step_siz
     return int(_lib.rt_adjoint_kappa_workspace_bytes(nx, ny, nz, n_src, n_rays, n_bins, step_size, c, dt, n_steps))
 
 
-def rt_march_adjoint_kappa(gbar, j, kappa, sources, n_rays, step_size, c, dt, n_steps, grad_kappa=None, workspace=None,
-                           stream=None):
-    """grad_kappa [nx,ny,nz,n_bins] = dL/dkappa for gbar [n_steps,nx,ny,nz,n_bins] = dL/d out (DESIGN.md D19)."""
+def rt_adjoint_kappa_workspace_bytes_ex(nx, ny, nz, n_src, n_rays, n_bins, step_size, c, dt, n_steps,
+                                        record_limit: int) -> int:
+    return int(_lib.rt_adjoint_kappa_workspace_bytes_ex(nx, ny, nz, n_src, n_rays, n_bins, step_size, c, dt, n_steps,
+                                                        record_limit))
+
+
+def rt_march_adjoint_kappa_ex(gbar, j, kappa, sources, n_rays, step_size, c, dt, n_steps, grad_kappa=None,
+                              workspace=None, stream=None, record_limit: int = 0):
+    """rt_march_adjoint_kappa with the forward-record bound of one source batch given in bytes (0 = the library's
+    2 GiB): the test hook that drives the source-batch loop on small cases."""
     torch = _torch()
     _check_dev(gbar, "gbar", torch.float32, 5)
     _check_dev(j, "j", torch.float32, 4)
@@ -232,22 +291,24 @@ def rt_march_adjoint_kappa(gbar, j, kappa, sources, n_rays, step_size, c, dt, n_
     if tuple(gbar.shape) != (n_steps, nx, ny, nz, nb) or j.shape != kappa.shape or sources.shape[1] != 3:
         raise ValueError("gbar must be [n_steps, nx, ny, nz, n_bins], j like kappa, sources [n_src, 3]")
     n_src = sources.shape[0]
-    if grad_kappa is None:
-        grad_kappa = torch.empty((nx, ny, nz, nb), dtype=torch.float32, device=kappa.device)
-    else:
-        _check_dev(grad_kappa, "grad_kappa", torch.float32)
-        if grad_kappa.numel() != kappa.numel():
-            raise ValueError("grad_kappa has the wrong size")
-    if workspace is None:
-        workspace = torch.empty(max(16, rt_adjoint_kappa_workspace_bytes(nx, ny, nz, n_src, n_rays, nb, step_size, c, dt,
-                                                                         n_steps)),
-                                dtype=torch.uint8, device=kappa.device)
-    rc = _lib.rt_march_adjoint_kappa(gbar.data_ptr(), j.data_ptr(), kappa.data_ptr(), nx, ny, nz, sources.data_ptr(),
-                                     n_src, n_rays, nb, step_size, c, dt, n_steps, grad_kappa.data_ptr(),
-                                     workspace.data_ptr(), workspace.numel(), _stream_ptr(stream))
+    with _Call(stream, gbar, j, kappa, sources) as call:
+        grad_kappa = _out_or_new(call, grad_kappa, (nx, ny, nz, nb), "grad_kappa")
+        workspace = _workspace_or_new(call, workspace, rt_adjoint_kappa_workspace_bytes_ex(
+            nx, ny, nz, n_src, n_rays, nb, step_size, c, dt, n_steps, record_limit))
+        rc = _lib.rt_march_adjoint_kappa_ex(gbar.data_ptr(), j.data_ptr(), kappa.data_ptr(), nx, ny, nz,
+                                            sources.data_ptr(), n_src, n_rays, nb, step_size, c, dt, n_steps,
+                                            grad_kappa.data_ptr(), workspace.data_ptr(), workspace.numel(),
+                                            call.stream_ptr, record_limit)
     if rc != RT_OK:
         raise RtError(rc, "rt_march_adjoint_kappa")
     return grad_kappa
+
+
+def rt_march_adjoint_kappa(gbar, j, kappa, sources, n_rays, step_size, c, dt, n_steps, grad_kappa=None, workspace=None,
+                           stream=None):
+    """grad_kappa [nx,ny,nz,n_bins] = dL/dkappa for gbar [n_steps,nx,ny,nz,n_bins] = dL/d out (DESIGN.md D19)."""
+    return rt_march_adjoint_kappa_ex(gbar, j, kappa, sources, n_rays, step_size, c, dt, n_steps, grad_kappa, workspace,
+                                     stream, 0)
 
 
 def rt_march_single(j, kappa, source_pos, n_rays, step_size, c, dt, n_steps, out=None, workspace=None,
@@ -259,13 +320,12 @@ def rt_march_single(j, kappa, source_pos, n_rays, step_size, c, dt, n_steps, out
     if source_pos.numel() != 3 or kappa.shape != j.shape:
         raise ValueError("source_pos must hold 3 floats and kappa must have j's shape")
     nx, ny, nz, nb = j.shape
-    if out is None:
-        out = torch.empty((n_steps, nx, ny, nz, nb), dtype=torch.float32, device=j.device)
-    if workspace is None:
-        workspace = alloc_workspace(nx, ny, nz, 1, n_rays, nb, n_steps, j.device)
-    rc = _lib.rt_march_single(j.data_ptr(), kappa.data_ptr(), nx, ny, nz, source_pos.data_ptr(), n_rays, nb,
-                              step_size, c, dt, n_steps, out.data_ptr(), workspace.data_ptr(),
-                              workspace.numel(), _stream_ptr(stream))
+    with _Call(stream, j, kappa, source_pos) as call:
+        out = _out_or_new(call, out, (n_steps, nx, ny, nz, nb), "out")
+        workspace = _workspace_or_new(call, workspace, rt_workspace_bytes(nx, ny, nz, 1, n_rays, nb, n_steps))
+        rc = _lib.rt_march_single(j.data_ptr(), kappa.data_ptr(), nx, ny, nz, source_pos.data_ptr(), n_rays, nb,
+                                  step_size, c, dt, n_steps, out.data_ptr(), workspace.data_ptr(),
+                                  workspace.numel(), call.stream_ptr)
     if rc != RT_OK:
         raise RtError(rc, "rt_march_single")
     return out
@@ -279,15 +339,18 @@ def rt_step_workspace_bytes(nx, ny, nz, n_src, n_rays, n_bins) -> int:
     return int(_lib.rt_step_workspace_bytes(nx, ny, nz, n_src, n_rays, n_bins))
 
 
-def rt_state_reset(n_src: int, n_rays: int, n_bins: int, state=None, stream=None):
-    """Fresh ray state (I = 0, exp(-tau) = 1): float32 [2, n_src, n_rays, n_bins] on the current device."""
+def rt_state_reset(n_src: int, n_rays: int, n_bins: int, state=None, stream=None, device=None):
+    """Fresh ray state (I = 0, exp(-tau) = 1): float32 [2, n_src, n_rays, n_bins] on ``device`` (default: ``state``'s
+    device, else the current CUDA device)."""
     torch = _torch()
     if state is None:
-        state = torch.empty((2, n_src, n_rays, n_bins), dtype=torch.float32, device="cuda")
+        dev = torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
+        state = torch.empty((2, n_src, n_rays, n_bins), dtype=torch.float32, device=dev)
     _check_dev(state, "state", torch.float32)
     if state.numel() * 4 != rt_state_bytes(n_src, n_rays, n_bins):
         raise ValueError("state has the wrong size")
-    rc = _lib.rt_state_reset(state.data_ptr(), n_src, n_rays, n_bins, _stream_ptr(stream))
+    with _Call(stream, state) as call:
+        rc = _lib.rt_state_reset(state.data_ptr(), n_src, n_rays, n_bins, call.stream_ptr)
     if rc != RT_OK:
         raise RtError(rc, "rt_state_reset")
     return state
@@ -308,38 +371,39 @@ def rt_march_step(j, kappa, sources, n_rays, step_size, c, dt, k_begin: int, sta
     n_src = sources.shape[0]
     if state.numel() * 4 != rt_state_bytes(n_src, n_rays, nb):
         raise ValueError("state has the wrong size")
-    if out is None:
-        if accumulate:
-            raise ValueError("accumulate needs the running field in `out`")
-        out = torch.empty((nx, ny, nz, nb), dtype=torch.float32, device=j.device)
-    else:
-        _check_dev(out, "out", torch.float32)
-        if out.numel() != j.numel():
-            raise ValueError("out has the wrong size")
-    if workspace is None:
-        workspace = torch.empty(max(16, rt_step_workspace_bytes(nx, ny, nz, n_src, n_rays, nb)), dtype=torch.uint8,
-                                device=j.device)
-    rc = _lib.rt_march_step(j.data_ptr(), kappa.data_ptr(), nx, ny, nz, sources.data_ptr(), n_src, n_rays, nb,
-                            step_size, c, dt, int(k_begin), state.data_ptr(), out.data_ptr(), int(bool(accumulate)),
-                            workspace.data_ptr(), workspace.numel(), _stream_ptr(stream))
+    if out is None and accumulate:
+        raise ValueError("accumulate needs the running field in `out`")
+    with _Call(stream, j, kappa, sources, state) as call:
+        out = _out_or_new(call, out, (nx, ny, nz, nb), "out")
+        workspace = _workspace_or_new(call, workspace, rt_step_workspace_bytes(nx, ny, nz, n_src, n_rays, nb))
+        rc = _lib.rt_march_step(j.data_ptr(), kappa.data_ptr(), nx, ny, nz, sources.data_ptr(), n_src, n_rays, nb,
+                                step_size, c, dt, int(k_begin), state.data_ptr(), out.data_ptr(),
+                                int(bool(accumulate)), workspace.data_ptr(), workspace.numel(), call.stream_ptr)
     if rc != RT_OK:
         raise RtError(rc, "rt_march_step")
     return out
 
 
-def rt_directions(n_rays: int, stream=None):
+def _current_device(device):
     torch = _torch()
-    nhat = torch.empty((n_rays, 3), dtype=torch.float64, device="cuda")
-    rc = _lib.rt_directions(n_rays, nhat.data_ptr(), _stream_ptr(stream))
+    return torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
+
+
+def rt_directions(n_rays: int, stream=None, device=None):
+    torch = _torch()
+    nhat = torch.empty((n_rays, 3), dtype=torch.float64, device=_current_device(device))
+    with _Call(stream, nhat) as call:
+        rc = _lib.rt_directions(n_rays, nhat.data_ptr(), call.stream_ptr)
     if rc != RT_OK:
         raise RtError(rc, "rt_directions")
     return nhat
 
 
-def rt_ray_order(n_rays: int, stream=None):
+def rt_ray_order(n_rays: int, stream=None, device=None):
     torch = _torch()
-    order = torch.empty(rt_ray_slots(n_rays), dtype=torch.int32, device="cuda")
-    rc = _lib.rt_ray_order(n_rays, order.data_ptr(), _stream_ptr(stream))
+    order = torch.empty(rt_ray_slots(n_rays), dtype=torch.int32, device=_current_device(device))
+    with _Call(stream, order) as call:
+        rc = _lib.rt_ray_order(n_rays, order.data_ptr(), call.stream_ptr)
     if rc != RT_OK:
         raise RtError(rc, "rt_ray_order")
     return order
@@ -352,11 +416,13 @@ def rt_trace_ray(j, kappa, source_pos, ray_index: int, n_rays: int, step_size: f
     _check_dev(kappa, "kappa", torch.float32, 4)
     _check_dev(source_pos, "source_pos", torch.float32)
     nx, ny, nz, nb = j.shape
-    pos = torch.empty((n_sub, 3), dtype=torch.float64, device=j.device)
-    tr_i = torch.empty((n_sub, nb), dtype=torch.float32, device=j.device)
-    tr_t = torch.empty((n_sub, nb), dtype=torch.float32, device=j.device)
-    rc = _lib.rt_trace_ray(j.data_ptr(), kappa.data_ptr(), nx, ny, nz, nb, source_pos.data_ptr(), ray_index, n_rays,
-                           step_size, n_sub, pos.data_ptr(), tr_i.data_ptr(), tr_t.data_ptr(), _stream_ptr(stream))
+    with _Call(stream, j, kappa, source_pos) as call:
+        pos = call.scratch((n_sub, 3), torch.float64)
+        tr_i = call.scratch((n_sub, nb), torch.float32)
+        tr_t = call.scratch((n_sub, nb), torch.float32)
+        rc = _lib.rt_trace_ray(j.data_ptr(), kappa.data_ptr(), nx, ny, nz, nb, source_pos.data_ptr(), ray_index,
+                               n_rays, step_size, n_sub, pos.data_ptr(), tr_i.data_ptr(), tr_t.data_ptr(),
+                               call.stream_ptr)
     if rc != RT_OK:
         raise RtError(rc, "rt_trace_ray")
     return {"pos": pos, "I": tr_i, "T": tr_t}
@@ -369,8 +435,9 @@ def rt_bench_red_ceiling(mode: int, grid, n_red: int, seed: int = 1, stream=None
     _check_dev(grid, "grid", torch.float64 if mode in (6, 7) else torch.float32, 4)
     nx, ny, nz, nb = grid.shape
     issued = ctypes.c_longlong(0)
-    rc = _lib.rt_bench_red_ceiling(mode, grid.data_ptr(), nx, ny, nz, nb, n_red, seed, ctypes.byref(issued),
-                                   _stream_ptr(stream))
+    with _Call(stream, grid) as call:
+        rc = _lib.rt_bench_red_ceiling(mode, grid.data_ptr(), nx, ny, nz, nb, n_red, seed, ctypes.byref(issued),
+                                       call.stream_ptr)
     if rc != RT_OK:
         raise RtError(rc, "rt_bench_red_ceiling")
     return int(issued.value)

@@ -1,5 +1,6 @@
 // rt_api.cu — the C ABI of librtmarch.so (include/rtmarch.h): argument checks on the host, then kernel
-// launches on the caller's stream.  No torch types, no global state besides a thread-local error string.
+// launches on the caller's stream.  No torch types; the only state kept between calls is a thread-local error
+// string and rt_march_host's per-device memory pool.
 #include "../../include/rtmarch.h"
 
 #include <algorithm>
@@ -8,6 +9,7 @@
 #include <cstdio>
 #include <cstring>
 #include <mutex>
+#include <shared_mutex>
 
 #include "rt_ceiling_kernels.cuh"
 #include "rt_march_direct.cuh"
@@ -193,6 +195,52 @@ bool use_table_march(int variant, const Plan& pl, int n_bins) {
     return variant == RT_VARIANT_DEFAULT && pl.map_src && n_bins == 1;
 }
 
+// the plan of RT_VARIANT_DEFAULT (make_plan cannot fail for it)
+Plan default_plan(int n_src) {
+    Plan pl{};
+    const bool ok = make_plan(RT_VARIANT_DEFAULT, n_src, &pl);
+    (void)ok;
+    return pl;
+}
+
+// The launch parameters every march / adjoint entry shares: medium, geometry, substep constants (emission quadrature
+// weight ds * 4 pi / N_Omega of D8, attenuation scale -ds log2 e), one launch covering all sources and direction slots.
+rt::MarchParams base_params(const float* j, const float* kappa, int nx, int ny, int nz, const float* sources, int n_src,
+                            int n_rays, int n_bins, float step_size, int n_steps, const Checked& ck, const Plan& pl) {
+    rt::MarchParams P{};
+    P.acc_copies = 1;
+    P.j = j; P.kappa = kappa; P.sources = sources;
+    P.nx = nx; P.ny = ny; P.nz = nz; P.nb = n_bins;
+    P.n_src = n_src; P.src_begin = 0; P.slot_begin = 0; P.n_rays = n_rays;
+    P.n_groups = n_bins;
+    P.n_steps = n_steps; P.n_sub = int(ck.n_sub);
+    P.ds = double(step_size); P.ds_f = step_size;
+    P.emis = float(double(step_size) * 4.0 * 3.14159265358979323846 / double(n_rays));
+    P.att_scale = float(-double(step_size) * 1.4426950408889634074);
+    P.snap_stride = ck.cells;
+    P.map_src = pl.map_src ? 1 : 0;
+    P.kappa_trilinear = pl.ktri ? 1 : 0;
+    P.n_slots = n_rays;
+    return P;
+}
+
+// the coherent ray order and the spatial source order of a plan, built on the stream into the head of the workspace
+int build_orders(rt::MarchParams& P, const Plan& pl, const Workspace& wl, char* ws, cudaStream_t st) {
+    if (pl.coherent) {
+        P.ray_order = reinterpret_cast<const uint32_t*>(ws);
+        P.n_slots = ray_slots(P.n_rays);
+        const int rc = build_ray_order(P.n_rays, reinterpret_cast<uint32_t*>(ws), st);
+        if (rc != RT_OK) return rc;
+    }
+    if (pl.map_src && P.n_src <= kMaxSortedSources) {
+        uint32_t* so = reinterpret_cast<uint32_t*>(ws + wl.src_order_at);
+        rt::src_order_kernel<<<(P.n_src + 3) / 4, 128, 0, st>>>(so, P.sources, P.n_src, P.nx, P.ny, P.nz);
+        RT_CUDA(cudaGetLastError());
+        P.src_order = so;
+    }
+    return RT_OK;
+}
+
 // rt_march_step: one time step from substep k0 with the ray state carried in `state`
 struct StepArgs {
     float* state;
@@ -223,39 +271,13 @@ int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const
     }
 
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    rt::MarchParams P{};
-    P.acc_copies = 1;
-    P.j = j; P.kappa = kappa; P.sources = sources;
-    P.nx = nx; P.ny = ny; P.nz = nz; P.nb = n_bins;
-    P.n_src = n_src; P.src_begin = 0; P.slot_begin = 0; P.n_rays = n_rays;
-    P.n_steps = n_steps; P.n_sub = int(ck.n_sub);
-    P.ds = double(step_size); P.ds_f = step_size;
-    P.emis = float(double(step_size) * 4.0 * 3.14159265358979323846 / double(n_rays));
-    P.att_scale = float(-double(step_size) * 1.4426950408889634074);
-    P.snap_stride = ck.cells;
-    P.map_src = pl.map_src ? 1 : 0;
-    P.kappa_trilinear = pl.ktri ? 1 : 0;
     if (pl.ktri && step) return RT_EINVAL;
+    rt::MarchParams P = base_params(j, kappa, nx, ny, nz, sources, n_src, n_rays, n_bins, step_size, n_steps, ck, pl);
     P.state_I = step ? step->state : nullptr;
     P.state_T = step ? step->state + size_t(n_src) * size_t(n_rays) * size_t(n_bins) : nullptr;
     P.k0 = step ? step->k0 : 0;
-    if (pl.coherent) {
-        P.ray_order = reinterpret_cast<const uint32_t*>(ws);
-        P.n_slots = ray_slots(n_rays);
-        const int rc2 = build_ray_order(n_rays, reinterpret_cast<uint32_t*>(ws), st);
-        if (rc2 != RT_OK) return rc2;
-    } else {
-        P.ray_order = nullptr;
-        P.n_slots = n_rays;
-    }
-    if (pl.map_src && n_src <= kMaxSortedSources) {
-        uint32_t* so = reinterpret_cast<uint32_t*>(ws + wl.src_order_at);
-        rt::src_order_kernel<<<(n_src + 3) / 4, 128, 0, st>>>(so, sources, n_src, nx, ny, nz);
-        RT_CUDA(cudaGetLastError());
-        P.src_order = so;
-    } else {
-        P.src_order = nullptr;
-    }
+    const int rco = build_orders(P, pl, wl, ws, st);
+    if (rco != RT_OK) return rco;
     const size_t n_acc = size_t(ck.cells) * size_t(n_steps);
     double* master = reinterpret_cast<double*>(ws + wl.acc_at);
     const int fin_threads = 256;
@@ -410,32 +432,10 @@ int rt_march_adjoint_j(const float* gbar, const float* kappa, int nx, int ny, in
     if (!workspace || workspace_bytes < need || (uintptr_t(workspace) & 15u)) return RT_EWORKSPACE;
     char* ws = static_cast<char*>(workspace);
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    Plan pl;
-    make_plan(RT_VARIANT_DEFAULT, n_src, &pl);
-
-    rt::MarchParams P{};
-    P.j = nullptr; P.kappa = kappa; P.sources = sources;
-    P.nx = nx; P.ny = ny; P.nz = nz; P.nb = n_bins;
-    P.n_src = n_src; P.src_begin = 0; P.slot_begin = 0; P.n_rays = n_rays;
-    P.n_groups = n_bins;
-    P.n_steps = n_steps; P.n_sub = int(ck.n_sub);
-    P.ds = double(step_size); P.ds_f = step_size;
-    P.emis = float(double(step_size) * 4.0 * 3.14159265358979323846 / double(n_rays));
-    P.att_scale = float(-double(step_size) * 1.4426950408889634074);
-    P.snap_stride = ck.cells;
-    P.map_src = pl.map_src ? 1 : 0;
-    P.kappa_trilinear = 0; P.state_I = nullptr; P.state_T = nullptr; P.k0 = 0;
-    P.ray_order = reinterpret_cast<const uint32_t*>(ws);
-    P.n_slots = ray_slots(n_rays);
-    const int rc2 = build_ray_order(n_rays, reinterpret_cast<uint32_t*>(ws), st);
+    const Plan pl = default_plan(n_src);
+    rt::MarchParams P = base_params(nullptr, kappa, nx, ny, nz, sources, n_src, n_rays, n_bins, step_size, n_steps, ck, pl);
+    const int rc2 = build_orders(P, pl, wl, ws, st);
     if (rc2 != RT_OK) return rc2;
-    P.src_order = nullptr;
-    if (pl.map_src && n_src <= kMaxSortedSources) {
-        uint32_t* so = reinterpret_cast<uint32_t*>(ws + wl.src_order_at);
-        rt::src_order_kernel<<<(n_src + 3) / 4, 128, 0, st>>>(so, sources, n_src, nx, ny, nz);
-        RT_CUDA(cudaGetLastError());
-        P.src_order = so;
-    }
     double* master = reinterpret_cast<double*>(ws + wl.acc_at);
     P.acc = master;
     RT_CUDA(cudaMemsetAsync(master, 0, size_t(ck.cells) * sizeof(double), st));
@@ -465,13 +465,16 @@ struct KappaBatch {
     int src_per_batch;
     size_t record_bytes;
 };
-KappaBatch plan_kappa_batches(int n_src, int n_slots, int n_groups, bool map_src, long long K) {
+// record_limit: bytes the record of one batch may take (0 = kForwardRecordLimit; the _ex entries let tests force
+// several batches on small cases); a batch is never smaller than one warp's worth of sources
+KappaBatch plan_kappa_batches(int n_src, int n_slots, int n_groups, bool map_src, long long K, size_t record_limit) {
+    if (!record_limit) record_limit = kForwardRecordLimit;
     const int unit = map_src ? 32 : 1;                               // sources come in whole warps' worth
     const int n_units = (n_src + unit - 1) / unit;
     auto bytes_for = [&](int n) {
         return size_t(rt::march_blocks(n, n_slots, n_groups, map_src ? 1 : 0)) * rt::kThreads * size_t(K) * sizeof(float2);
     };
-    int units = int(std::max<size_t>(1, kForwardRecordLimit / std::max<size_t>(1, bytes_for(unit))));
+    int units = int(std::max<size_t>(1, record_limit / std::max<size_t>(1, bytes_for(unit))));
     units = std::min(units, n_units);
     KappaBatch kb;
     kb.src_per_batch = std::min(units * unit, map_src ? n_units * unit : n_src);
@@ -479,20 +482,33 @@ KappaBatch plan_kappa_batches(int n_src, int n_slots, int n_groups, bool map_src
     return kb;
 }
 
-size_t rt_adjoint_kappa_workspace_bytes(int nx, int ny, int nz, int n_src, int n_rays, int n_bins, float step_size,
-                                        float c, float dt, int n_steps) {
+size_t rt_adjoint_kappa_workspace_bytes_ex(int nx, int ny, int nz, int n_src, int n_rays, int n_bins, float step_size,
+                                           float c, float dt, int n_steps, size_t record_limit) {
     const size_t base = rt_adjoint_workspace_bytes(nx, ny, nz, n_src, n_rays, n_bins, n_steps);
     if (!base || !positive_finite(step_size) || !positive_finite(c) || !positive_finite(dt)) return 0;
     const long long ns = substeps(step_size, c, dt);
     if (ns < 1 || ns * n_steps > 2147483647LL) return 0;
-    Plan pl;
-    make_plan(RT_VARIANT_DEFAULT, n_src, &pl);
-    return align_up(base, 256) + plan_kappa_batches(n_src, ray_slots(n_rays), n_bins, pl.map_src, ns * n_steps).record_bytes;
+    const Plan pl = default_plan(n_src);
+    return align_up(base, 256) +
+           plan_kappa_batches(n_src, ray_slots(n_rays), n_bins, pl.map_src, ns * n_steps, record_limit).record_bytes;
+}
+
+size_t rt_adjoint_kappa_workspace_bytes(int nx, int ny, int nz, int n_src, int n_rays, int n_bins, float step_size,
+                                        float c, float dt, int n_steps) {
+    return rt_adjoint_kappa_workspace_bytes_ex(nx, ny, nz, n_src, n_rays, n_bins, step_size, c, dt, n_steps, 0);
 }
 
 int rt_march_adjoint_kappa(const float* gbar, const float* j, const float* kappa, int nx, int ny, int nz,
                            const float* sources, int n_src, int n_rays, int n_bins, float step_size, float c, float dt,
                            int n_steps, float* grad_kappa, void* workspace, size_t workspace_bytes, void* stream) {
+    return rt_march_adjoint_kappa_ex(gbar, j, kappa, nx, ny, nz, sources, n_src, n_rays, n_bins, step_size, c, dt, n_steps,
+                                     grad_kappa, workspace, workspace_bytes, stream, 0);
+}
+
+int rt_march_adjoint_kappa_ex(const float* gbar, const float* j, const float* kappa, int nx, int ny, int nz,
+                              const float* sources, int n_src, int n_rays, int n_bins, float step_size, float c, float dt,
+                              int n_steps, float* grad_kappa, void* workspace, size_t workspace_bytes, void* stream,
+                              size_t record_limit) {
     if (!gbar) return RT_EINVAL;
     Checked ck;
     const int rc = check_args(j, kappa, nx, ny, nz, sources, n_src, n_rays, n_bins, step_size, c, dt, n_steps,
@@ -501,36 +517,15 @@ int rt_march_adjoint_kappa(const float* gbar, const float* j, const float* kappa
     if (uintptr_t(gbar) & 3u) return RT_EALIGN;
     const Workspace wl = workspace_layout(ck.cells, n_src, n_rays, 1, n_bins);
     const size_t base = rt_adjoint_workspace_bytes(nx, ny, nz, n_src, n_rays, n_bins, n_steps);
-    const size_t need = rt_adjoint_kappa_workspace_bytes(nx, ny, nz, n_src, n_rays, n_bins, step_size, c, dt, n_steps);
+    const size_t need = rt_adjoint_kappa_workspace_bytes_ex(nx, ny, nz, n_src, n_rays, n_bins, step_size, c, dt, n_steps,
+                                                            record_limit);
     if (!workspace || workspace_bytes < need || (uintptr_t(workspace) & 15u)) return RT_EWORKSPACE;
     char* ws = static_cast<char*>(workspace);
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    Plan pl;
-    make_plan(RT_VARIANT_DEFAULT, n_src, &pl);
-
-    rt::MarchParams P{};
-    P.j = j; P.kappa = kappa; P.sources = sources;
-    P.nx = nx; P.ny = ny; P.nz = nz; P.nb = n_bins;
-    P.n_src = n_src; P.src_begin = 0; P.slot_begin = 0; P.n_rays = n_rays;
-    P.n_groups = n_bins;
-    P.n_steps = n_steps; P.n_sub = int(ck.n_sub);
-    P.ds = double(step_size); P.ds_f = step_size;
-    P.emis = float(double(step_size) * 4.0 * 3.14159265358979323846 / double(n_rays));
-    P.att_scale = float(-double(step_size) * 1.4426950408889634074);
-    P.snap_stride = ck.cells;
-    P.map_src = pl.map_src ? 1 : 0;
-    P.kappa_trilinear = 0; P.state_I = nullptr; P.state_T = nullptr; P.k0 = 0;
-    P.ray_order = reinterpret_cast<const uint32_t*>(ws);
-    P.n_slots = ray_slots(n_rays);
-    const int rc2 = build_ray_order(n_rays, reinterpret_cast<uint32_t*>(ws), st);
+    const Plan pl = default_plan(n_src);
+    rt::MarchParams P = base_params(j, kappa, nx, ny, nz, sources, n_src, n_rays, n_bins, step_size, n_steps, ck, pl);
+    const int rc2 = build_orders(P, pl, wl, ws, st);
     if (rc2 != RT_OK) return rc2;
-    P.src_order = nullptr;
-    if (pl.map_src && n_src <= kMaxSortedSources) {
-        uint32_t* so = reinterpret_cast<uint32_t*>(ws + wl.src_order_at);
-        rt::src_order_kernel<<<(n_src + 3) / 4, 128, 0, st>>>(so, sources, n_src, nx, ny, nz);
-        RT_CUDA(cudaGetLastError());
-        P.src_order = so;
-    }
     double* master = reinterpret_cast<double*>(ws + wl.acc_at);
     P.acc = master;
     RT_CUDA(cudaMemsetAsync(master, 0, size_t(ck.cells) * sizeof(double), st));
@@ -545,7 +540,7 @@ int rt_march_adjoint_kappa(const float* gbar, const float* j, const float* kappa
         gsuf = gs;
     }
     const long long K = ck.n_sub * n_steps;
-    const KappaBatch kb = plan_kappa_batches(n_src, P.n_slots, P.n_groups, pl.map_src, K);
+    const KappaBatch kb = plan_kappa_batches(n_src, P.n_slots, P.n_groups, pl.map_src, K, record_limit);
     float2* fwd = reinterpret_cast<float2*>(ws + align_up(base, 256));
     for (int s0 = 0; s0 < n_src; s0 += kb.src_per_batch) {
         P.src_begin = s0;
@@ -593,7 +588,10 @@ int rt_march_step(const float* j, const float* kappa, int nx, int ny, int nz, co
 
 // rt_march_host's device buffers come from a private stream-ordered memory pool per device that keeps what it has
 // been given (release threshold = max), so repeated calls do not pay cudaMalloc/cudaFree; rt_host_release() trims it.
+// rt_march_host holds g_pool_use shared for the whole call, rt_host_release takes it exclusively: a pool is never
+// destroyed under a call that is using it.
 static std::mutex g_pool_mutex;
+static std::shared_mutex g_pool_use;
 static cudaMemPool_t g_pools[64] = {};
 
 static cudaError_t host_pool(cudaMemPool_t* pool) {
@@ -618,6 +616,7 @@ static cudaError_t host_pool(cudaMemPool_t* pool) {
 }
 
 int rt_host_release(void) {
+    std::unique_lock<std::shared_mutex> idle(g_pool_use);       // waits for running rt_march_host calls
     std::lock_guard<std::mutex> lock(g_pool_mutex);
     for (auto& p : g_pools)
         if (p) {
@@ -642,6 +641,7 @@ int rt_march_host(const float* j, const float* kappa, int nx, int ny, int nz, co
     cudaMemPool_t pool = nullptr;
     cudaStream_t st = nullptr;
     int result = RT_OK;
+    std::shared_lock<std::shared_mutex> in_use(g_pool_use);
     auto ok = [&](cudaError_t err, const char* where) {
         if (err != cudaSuccess && result == RT_OK) result = cuda_fail(err, where);
         return err == cudaSuccess;
@@ -681,8 +681,7 @@ int rt_substeps_per_step(float step_size, float c, float dt) {
 
 int rt_launch_count(int nx, int ny, int nz, int n_src, int n_rays, int n_bins, int n_steps) {
     if (nx < 1 || ny < 1 || nz < 1 || n_src < 1 || n_rays < 1 || n_bins < 1 || n_steps < 1) return RT_EINVAL;
-    Plan pl;
-    make_plan(RT_VARIANT_DEFAULT, n_src, &pl);
+    const Plan pl = default_plan(n_src);
     const int setup = 1 + ((pl.map_src && n_src <= kMaxSortedSources) ? 1 : 0);     // ray order, (source order)
     if (use_batched_fp32((long long)nx * ny * nz * n_bins, n_steps, n_bins)) {      // (march, drain) per batch
         const int slots = ray_slots(n_rays);

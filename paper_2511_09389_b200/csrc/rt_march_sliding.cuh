@@ -155,6 +155,7 @@ __global__ void __launch_bounds__(kThreads, MINB) march_sliding_kernel(const Mar
         if (P.same_frac && *P.same_frac) return;     // march_table_kernel has marched this call (rt_march_table.cuh)
     // the batched path launches the next batch (other scratch grid, no dependence on this one) with programmatic
     // stream serialization: it may start as soon as every block of this grid has started, filling this grid's tail
+    // (and waits for this grid's completion at its own end: griddepcontrol.wait below)
     if constexpr (NB == 4) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     RayId id;
     if (!ray_id(P, id)) return;
@@ -278,6 +279,11 @@ __global__ void __launch_bounds__(kThreads, MINB) march_sliding_kernel(const Mar
             P.state_T[state_at + b] = T[b];
         }
     }
+    // A grid launched with programmatic stream serialization (the second batch of a pair) must not COMPLETE before
+    // its prerequisite grid has: the drain_kernel that follows is ordered behind this grid only.  The wait comes
+    // last, so the overlap is kept (this grid's tail is later than the first grid's anyway); it returns at once in a
+    // normally launched grid.
+    if constexpr (NB == 4) asm volatile("griddepcontrol.wait;" ::: "memory");
 }
 
 }  // namespace rt

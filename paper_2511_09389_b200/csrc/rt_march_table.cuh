@@ -46,10 +46,20 @@ __global__ void same_fraction_kernel(int* flag, const float* sources, int n_src,
     if (threadIdx.x == 0) *flag = differs ? 0 : 1;
 }
 
-struct TableRow {            // substep g of a direction: 16 bytes, one shared-memory load per substep
-    uint32_t h[3];           // top 32 fraction bits of x_g per axis (travel coordinates, rt_march_sliding.cuh)
+struct TableRow {            // substep g of a direction: 32 bytes, two 16-byte shared-memory loads per substep
+    float tx, lx, ty, ly;    // trailing / leading weight of x_g per axis, unscaled: float(~h), float(h) of the top 32
+    float tz, lz;            // fraction bits h (travel coordinates, rt_march_sliding.cuh); the z pair carries 2^-96
     int cross;               // bit a: the cell word of axis a goes up between x_g and x_{g+1}
+    int pad;
 };
+
+// (t, l) of an axis with the clamping mask of the lane applied: m = ~0 leaves the pair, m = 0 -- both
+// indices of the axis clamp to one voxel -- makes it exactly (one, 0), `one` being float(~0u) = 2^32 (times 2^-96 on z).
+// The same values as masking the fraction word before the conversions, bit for bit.
+__device__ __forceinline__ void mask_pair(float& t, float& l, uint32_t m, uint32_t one_bits) {
+    t = __uint_as_float((__float_as_uint(t) & m) | (one_bits & ~m));
+    l = __uint_as_float(__float_as_uint(l) & m);
+}
 
 template <int MINB>
 __global__ void __launch_bounds__(kThreads, MINB) march_table_kernel(const MarchParams P) {
@@ -91,7 +101,7 @@ __global__ void __launch_bounds__(kThreads, MINB) march_table_kernel(const March
 #pragma unroll
     for (int s = 0; s < 8; ++s) S.zero_slot(s);
     S.restart(P, A, negbits, 0, P.j);
-    float I = 0.0f, T = live ? 1.0f : 0.0f, att;
+    float I = 0.0f, T = live ? P.emis : 0.0f, att;   // T = exp(-tau) ds 4 pi/N_Omega: the emission weight rides on it
     auto load_att = [&]() {
         const int ko = S.base + ((negbits & 1) ? A[0].dl : 0) + ((negbits & 2) ? A[1].dl : 0) + ((negbits & 4) ? A[2].dl : 0);
         att = ex2_approx(__ldg(P.kappa + ko) * P.att_scale);
@@ -99,34 +109,51 @@ __global__ void __launch_bounds__(kThreads, MINB) march_table_kernel(const March
     load_att();
     __syncwarp();
 
+    // shared-window address of this warp's table, kept in a register (opaque to the compiler, which would
+    // otherwise rebuild it from the thread index every substep), and the byte offset of the current row
+    uint32_t tbase = uint32_t(__cvta_generic_to_shared(&table[warp][0]));
+    asm volatile("" : "+r"(tbase));
+    uint32_t roff = 0;
+
     int g = 0;                               // substep index since x_0
     for (int m = 0; m < P.n_steps; ++m) {
         for (int k = 0; k < P.n_sub; ++k, ++g) {
-            if ((g & 31) == 0) {             // lane l writes the row of substep g + l
+            if (roff == 0) {                 // lane l writes the row of substep g + l
                 __syncwarp();
                 TableRow row;
                 row.cross = 0;
+                row.pad = 0;
+                uint32_t h[3];
 #pragma unroll
                 for (int a = 0; a < 3; ++a) {
                     Fx96 p = ref[warp][a];
                     const Fx96 d = ref[warp][3 + a];
                     fx_advance(p, d, (long long)g + lane);
-                    row.h[a] = p.fh;
+                    h[a] = p.fh;
                     const int c = p.c;
                     fx_add(p, d);
                     row.cross |= (p.c != c) ? (1 << a) : 0;
                 }
+                row.tx = __uint2float_rn(~h[0]); row.lx = __uint2float_rn(h[0]);
+                row.ty = __uint2float_rn(~h[1]); row.ly = __uint2float_rn(h[1]);
+                row.tz = __uint2float_rn(~h[2]) * 1.2621774483536189e-29f;      // 2^-96
+                row.lz = __uint2float_rn(h[2]) * 1.2621774483536189e-29f;
                 table[warp][lane] = row;
                 __syncwarp();
             }
-            const uint4 row = *reinterpret_cast<const uint4*>(&table[warp][g & 31]);
-            // from here on the substep is march_sliding_kernel's: masked fractions, unscaled weights, 2^-96 on z
-            const uint32_t hx = row.x & A[0].fmask, hy = row.y & A[1].fmask, hz = row.z & A[2].fmask;
-            const float lx = __uint2float_rn(hx), tx = __uint2float_rn(~hx);
-            const float ly = __uint2float_rn(hy), ty = __uint2float_rn(~hy);
-            const float wz[2] = {__uint2float_rn(~hz) * 1.2621774483536189e-29f,      // 2^-96
-                                 __uint2float_rn(hz) * 1.2621774483536189e-29f};
-            const int cross = int(row.w);
+            float4 rxy, rz;
+            asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];"
+                         : "=f"(rxy.x), "=f"(rxy.y), "=f"(rxy.z), "=f"(rxy.w) : "r"(tbase + roff));
+            asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4+16];"
+                         : "=f"(rz.x), "=f"(rz.y), "=f"(rz.z), "=f"(rz.w) : "r"(tbase + roff));
+            roff = (roff + 32u) & 1023u;
+            // from here on the substep is march_sliding_kernel's: the lane's clamping masks, unscaled weights, 2^-96 on z
+            float tx = rxy.x, lx = rxy.y, ty = rxy.z, ly = rxy.w, tz = rz.x, lz = rz.y;
+            mask_pair(tx, lx, A[0].fmask, 0x4F800000u);          // 2^32
+            mask_pair(ty, ly, A[1].fmask, 0x4F800000u);
+            mask_pair(tz, lz, A[2].fmask, 0x1F800000u);          // 2^-64 = 2^32 2^-96
+            const int cross = __float_as_int(rz.z);
+            const float wz[2] = {tz, lz};
             const float wxy[4] = {tx * ty, tx * ly, lx * ty, lx * ly};
             float w[8];
 #pragma unroll
@@ -137,7 +164,7 @@ __global__ void __launch_bounds__(kThreads, MINB) march_table_kernel(const March
                 jv = fmaf(w[s], S.jc[s].v[0], jv);
                 ju = fmaf(w[s + 1], S.jc[s + 1].v[0], ju);
             }
-            I = fmaf(I, att, (jv + ju) * T * P.emis);                  // eq. (2)
+            I = fmaf(I, att, (jv + ju) * T);                           // eq. (2)
             T *= att;
 #pragma unroll
             for (int s = 0; s < 8; ++s) S.acc[s].v[0] = fmaf(w[s], I, S.acc[s].v[0]);

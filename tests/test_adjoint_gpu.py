@@ -4,7 +4,7 @@ import numpy as np
 import pytest
 
 import parity
-from paper_2511_09389_b200 import workloads
+import workloads
 
 pytestmark = pytest.mark.gpu
 
@@ -160,3 +160,107 @@ def test_kappa_adjoint_on_c1_against_the_oracle_and_a_directional_difference(rt,
     fd = (loss(kap + eps * d) - loss(kap - eps * d)) / (2 * eps)
     an = float((grad.double() * d.double()).sum())
     assert abs(fd - an) <= 2e-3 * abs(an), (fd, an)
+
+
+# ------------------------------------------------------------------------------------------------
+# paths that only exist at size: oracle parity (not GPU-vs-GPU) on stratified subsets of C2 / C3 / C4, and the source-batch
+# loop of rt_march_adjoint_kappa (taken when the forward record of all sources exceeds the record limit)
+# ------------------------------------------------------------------------------------------------
+def _stratified(n_src, count):
+    return np.unique(np.linspace(0, n_src - 1, count).round().astype(int))
+
+
+@pytest.mark.parametrize("name,count", [("C2", 40), ("C3", 36), ("C4", 2)])
+def test_adjoint_j_on_config_subsets_matches_the_oracle(rt, oracle_mod, name, count):
+    """rt_march_adjoint_j with the config's own grid, rays, substeps, steps and bins on a stratified subset of its
+    sources (the adjoint is a plain sum over sources, like the field): >= 32 cell-centred sources for C2 / C3 (warp =
+    32 sources x 1 direction), 2 of C4's random sources on the 256^3 x 4 grid with 8 snapshots (suffix sums)."""
+    w = workloads.make_config(name)
+    src = np.ascontiguousarray(w.sources[_stratified(w.n_src, count)])
+    rng = np.random.default_rng(11)
+    gbar = rng.uniform(0.0, 1.0, (w.n_steps,) + w.j.shape).astype(np.float32)
+    got = rt.rt_march_adjoint_j(_dev(gbar), _dev(w.kappa), _dev(src), w.n_rays, w.step_size, w.c, w.dt, w.n_steps)
+    torch.cuda.synchronize()
+    got = got.cpu().numpy()
+    ref = oracle_mod.adjoint_j(gbar, w.kappa, src, w.n_rays, w.step_size, w.c, w.dt, w.n_steps)
+    rows = parity.assert_parity(got[None], ref[None], f"adjoint_j {name} subset of {len(src)} sources")
+    print(name, rows[-1])
+
+
+@pytest.mark.parametrize("n_src,n_rays,nb,limit_sources", [
+    (70, 24, 1, 32),        # warp = 32 sources x 1 direction: batches of 32, 32 and a ragged 6
+    (100, 11, 2, 64),       # two bins: batches of 64 and 36
+    (5, 40, 1, 2),          # fewer than 32 sources (warp = 32 directions of one source): batches of 2, 2, 1
+])
+def test_kappa_adjoint_source_batches_match_the_oracle(rt, oracle_mod, n_src, n_rays, nb, limit_sources):
+    """The source-batch loop of rt_march_adjoint_kappa (src_begin offsets, the record stride of each batch, reuse of
+    the record buffer), forced on a small case by a record limit of `limit_sources` sources' worth of record
+    (rt_march_adjoint_kappa_ex): against the oracle entry by entry, and against the one-batch call."""
+    shape, ds, dt, n_steps = (9, 8, 7), 0.25, 4.0, 2
+    rng = np.random.default_rng(n_src + nb)
+    kap = rng.uniform(0.0, 0.6, shape + (nb,)).astype(np.float32)
+    j = rng.uniform(0.1, 1.0, shape + (nb,)).astype(np.float32)
+    src = rng.uniform(-2.0, 10.0, (n_src, 3))
+    src[: n_src // 2] = np.round(src[: n_src // 2])
+    src = src.astype(np.float32)
+    gbar = rng.standard_normal((n_steps,) + shape + (nb,)).astype(np.float32)
+    K = rt.rt_substeps_per_step(ds, 1.0, dt) * n_steps
+    slots = rt.rt_ray_slots(n_rays)
+    if n_src >= 32:     # record bytes of one batch = blocks(4 direction slots x 32 (source, bin) pairs) x 128 threads x K x 8
+        blocks = ((slots + 3) // 4) * ((limit_sources * nb + 31) // 32)
+    else:
+        blocks = ((slots * nb + 127) // 128) * limit_sources
+    limit = blocks * 128 * K * 8
+    args = (_dev(gbar), _dev(j), _dev(kap), _dev(src), n_rays, ds, 1.0, dt, n_steps)
+    one = rt.rt_march_adjoint_kappa(*args)
+    ws_one = rt.rt_adjoint_kappa_workspace_bytes(*shape, n_src, n_rays, nb, ds, 1.0, dt, n_steps)
+    ws_many = rt.rt_adjoint_kappa_workspace_bytes_ex(*shape, n_src, n_rays, nb, ds, 1.0, dt, n_steps, limit)
+    assert ws_many < ws_one                                   # the record buffer holds one batch only
+    many = rt.rt_march_adjoint_kappa_ex(*args, record_limit=limit)
+    torch.cuda.synchronize()
+    ref = oracle_mod.adjoint_kappa(gbar, j, kap, src, n_rays, ds, 1.0, dt, n_steps)
+    print(_signed_compare(many.cpu().numpy().astype(np.float64), ref, f"kappa adjoint, batches of {limit_sources} of {n_src}"))
+    print(_signed_compare(one.cpu().numpy().astype(np.float64), ref, f"kappa adjoint, one batch of {n_src}"))
+    scale = float(one.abs().max())
+    assert float((one - many).abs().max()) <= 2e-6 * scale    # same per-ray arithmetic, other order of the fp64 sums
+
+
+def test_kappa_adjoint_c2_subset_in_batches_matches_the_oracle(rt, oracle_mod):
+    """C2's grid, rays and substeps with 72 of its sources: the record of all of them (72 x 4,096 x 444 x 8 B = 1 GB)
+    is cut into batches of 32 sources by the record limit, as the full config is cut by the 2 GiB default."""
+    w = workloads.make_config("C2")
+    src = np.ascontiguousarray(w.sources[_stratified(w.n_src, 72)])
+    rng = np.random.default_rng(13)
+    gbar = rng.uniform(0.0, 1.0, (w.n_steps,) + w.j.shape).astype(np.float32)
+    K = w.n_steps * w.substeps_per_step
+    limit = (rt.rt_ray_slots(w.n_rays) // 4) * 128 * K * 8               # one group of 32 sources
+    got = rt.rt_march_adjoint_kappa_ex(_dev(gbar), _dev(w.j), _dev(w.kappa), _dev(src), w.n_rays, w.step_size, w.c, w.dt,
+                                       w.n_steps, record_limit=limit)
+    torch.cuda.synchronize()
+    ref = oracle_mod.adjoint_kappa(gbar, w.j, w.kappa, src, w.n_rays, w.step_size, w.c, w.dt, w.n_steps)
+    print(_signed_compare(got.cpu().numpy().astype(np.float64), ref, "kappa adjoint C2, 72 sources in 3 batches"))
+
+
+def test_relative_mse_amplitude_inversion_on_the_gpu(rt):
+    """PAPER.md:62 names two losses.  The relative MSE weights every voxel by 1 / (I_ref^2 + eps^2) (D20): still
+    a parabola in A, minimiser <w F, I_ref> / <w F, F>; the gradient comes from the same adjoint with gbar = 2 w r / n."""
+    w = workloads.make_config("C1")
+    e0, kap, src = _dev(w.j), _dev(w.kappa), _dev(w.sources)
+    args = (w.n_rays, w.step_size, w.c, w.dt, w.n_steps)
+    F = rt.rt_march(e0, kap, src, *args).double()
+    noise = torch.from_numpy(np.random.default_rng(2).standard_normal(tuple(F.shape))).cuda()
+    I_ref = 1.8 * F * (1.0 + 0.05 * noise)
+    eps = 1e-3 * float(I_ref.max())
+    wgt = 1.0 / (I_ref * I_ref + eps * eps)
+    A_star = float((wgt * F * I_ref).sum() / (wgt * F * F).sum())
+    n = F.numel()
+    lip = 2.0 * float((wgt * F * F).sum()) / n
+    A = 0.2
+    for _ in range(25):
+        resid = A * F - I_ref
+        grad_j = rt.rt_march_adjoint_j((2.0 * wgt * resid / n).float(), kap, src, *args)
+        A -= float((e0.double() * grad_j.double()).sum()) / lip
+    torch.cuda.synchronize()
+    assert abs(A - A_star) <= 2e-4 * abs(A_star), (A, A_star)
+    plain = float((F * I_ref).sum() / (F * F).sum())
+    assert abs(plain - A_star) > 1e-4 * abs(A_star)        # the weighting matters: another minimiser than the plain MSE's

@@ -11,7 +11,7 @@ import math
 import numpy as np
 import pytest
 
-from paper_2511_09389_b200 import workloads as W
+import workloads as W
 
 FOUR_PI = 4.0 * math.pi
 
@@ -754,6 +754,32 @@ def test_d19_scalar_amplitude_inversion_matches_the_closed_form(oracle_mod):
         assert abs(dLdA - 2.0 * float((resid * F).sum()) / F.size) <= 1e-11 * 2.0 * float(np.abs(resid * F).sum()) / F.size
         A -= dLdA / lip
     assert abs(A - A_star) <= 1e-9 * abs(A_star)
+
+
+def test_d20_relative_mse_inversion_matches_its_closed_form(oracle_mod):
+    """The paper's other loss ("either a plain MSE or a relative MSE"; reading D20): L(A) = mean(w (A F - I_ref)^2),
+    w = 1 / (I_ref^2 + eps^2).  Still a parabola in A: gradient descent with dL/dA = <e0, A^T (2/n) w (A F - I_ref)>
+    reaches <w F, I_ref> / <w F, F> ("the corresponding closed-form minimizer (under the chosen weighting)"), which
+    differs from the plain-MSE minimiser."""
+    n = 8
+    rho = W.lognormal_density(n, 4, 0.8)
+    e0 = np.ascontiguousarray((rho ** 2)[..., None], dtype=np.float32)
+    kap = np.ascontiguousarray((0.1 * rho)[..., None], dtype=np.float32)
+    src = np.array([[3.5, 3.5, 3.5]], dtype=np.float32)
+    args = (src, 24, 0.5, 1.0, 3.0, 1)
+    F = oracle_mod.march(e0, kap, *args)
+    I_ref = 2.5 * F * (1.0 + 0.1 * np.random.default_rng(0).standard_normal(F.shape))
+    eps = 1e-3 * I_ref.max()
+    wgt = 1.0 / (I_ref ** 2 + eps ** 2)
+    A_star = float((wgt * F * I_ref).sum() / (wgt * F * F).sum())
+    lip = 2.0 * float((wgt * F * F).sum()) / F.size
+    A = 0.3
+    for _ in range(40):
+        resid = A * F - I_ref
+        dLdA = float((e0.astype(np.float64) * oracle_mod.adjoint_j(2.0 * wgt * resid / F.size, kap, *args)).sum())
+        A -= dLdA / lip
+    assert abs(A - A_star) <= 1e-9 * abs(A_star)
+    assert abs(float((F * I_ref).sum() / (F * F).sum()) - A_star) > 1e-3 * abs(A_star)
 
 
 # ------------------------------------------------------------------------------------------------------

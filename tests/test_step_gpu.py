@@ -4,7 +4,7 @@ import numpy as np
 import pytest
 
 import parity
-from paper_2511_09389_b200 import workloads
+import workloads
 
 pytestmark = pytest.mark.gpu
 
@@ -71,6 +71,34 @@ def test_steps_with_a_changing_medium_match_the_oracle(rt, oracle_mod, n, nb, n_
         scale = 4.0 * np.pi / n_rays
         assert np.abs(g[0] - scale * ostate[:, :, 0, :]).max() <= 2e-5 * scale * ostate[:, :, 0, :].max()
         assert np.abs(g[1] - np.exp(-ostate[:, :, 1, :])).max() <= 2e-5
+
+
+def test_steps_on_a_c4_shaped_grid_with_a_changing_medium_match_the_oracle(rt, oracle_mod):
+    """The branch C4 takes in rt_march_step: a 256^3 x 4-bin grid is too large for the batched fp32 path, so the step
+    marches one bin per thread with fp64 reductions into the workspace grid.  C4's own grid, rays, step size and
+    substeps per step, 2 of its sources, 3 time steps, the medium advected and rescaled between steps."""
+    w = workloads.make_config("C4")
+    src = np.ascontiguousarray(w.sources[[5, 41]])
+    n, nb, ns = w.shape[0], w.n_bins, w.substeps_per_step
+    ostate = oracle_mod.new_state(len(src), w.n_rays, nb)
+    gstate = rt.rt_state_reset(len(src), w.n_rays, nb)
+    dsrc = _dev(src)
+    running = torch.zeros(w.j.shape, dtype=torch.float32, device="cuda")
+    ref_running = np.zeros(w.j.shape)
+    for m in range(3):
+        j = np.ascontiguousarray(np.roll(w.j, shift=(3 * m, -2 * m, m), axis=(0, 1, 2)) * np.float32(1.0 + 0.5 * m))
+        k = np.ascontiguousarray(np.roll(w.kappa, shift=(3 * m, -2 * m, m), axis=(0, 1, 2)) * np.float32(1.0 + 0.25 * m))
+        ref = oracle_mod.step(j, k, src, w.n_rays, w.step_size, w.c, w.dt, m * ns, ostate)
+        rt.rt_march_step(_dev(j), _dev(k), dsrc, w.n_rays, w.step_size, w.c, w.dt, m * ns, gstate, out=running,
+                         accumulate=True)
+        torch.cuda.synchronize()
+        ref_running += ref
+        rows = parity.assert_parity(running.cpu().numpy()[None], ref_running[None], f"C4-shaped step {m} accumulated")
+        print(rows[-1])
+    g = gstate.cpu().numpy().astype(np.float64)
+    scale = 4.0 * np.pi / w.n_rays
+    assert np.abs(g[0] - scale * ostate[:, :, 0, :]).max() <= 2e-5 * scale * ostate[:, :, 0, :].max()
+    assert np.abs(g[1] - np.exp(-ostate[:, :, 1, :])).max() <= 2e-5
 
 
 def test_steps_in_a_static_medium_reproduce_rt_march(rt, oracle_mod):

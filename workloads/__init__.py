@@ -1,6 +1,6 @@
 """Seeded synthetic inputs for the ray-march hot path (configs C0..C4 of BASELINE.json).
 
-This module is the ONE piece shared by the CUDA path's tests/bench and the oracle's tests: it only
+This top-level module is the ONE piece shared by the CUDA path's tests/bench and the oracle's tests: it only
 builds input arrays (j, kappa, sources) and the scalar call arguments.  It holds none of the
 method's arithmetic (no marching, no interpolation, no direction lattice) and imports neither the
 CUDA binding nor ``oracle/``.
