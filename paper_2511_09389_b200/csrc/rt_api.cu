@@ -14,6 +14,7 @@
 #include "rt_ceiling_kernels.cuh"
 #include "rt_march_direct.cuh"
 #include "rt_adjoint.cuh"
+#include "rt_brick.cuh"
 #include "rt_march_sliding.cuh"
 #include "rt_march_table.cuh"
 #include "rt_setup_kernels.cuh"
@@ -81,16 +82,28 @@ int check_args(const void* j, const void* kappa, int nx, int ny, int nz, const v
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 // workspace layout: [ray order: slots u32][source order: n_src u32][flag][fp64 accumulation grid x copies][fp32 scratch]
+// [fp32 brick scratch of the table march]
 struct Workspace {
-    size_t src_order_at, flag_at, acc_at, scratch2_at, total;
+    size_t src_order_at, flag_at, acc_at, scratch2_at, brick_at, brick_bytes, total;
     int acc_copies;
 };
+// march_table_kernel (one bin, >= 32 sources) deposits into an fp32 brick scratch (rt_brick.cuh): one 16-byte brick per
+// 2 x 2 (y, z) window of each time step's grid, ~4.1 x the fp32 grid; the table march is used while that stays below
+// kBrickScratchLimit
+constexpr size_t kBrickScratchLimit = size_t(1) << 30;
+size_t brick_scratch_bytes(int nx, int ny, int nz, int n_src, int n_steps, int n_bins) {
+    if (n_bins != 1 || n_src < 32) return 0;
+    const rt::BrickGeom g = rt::brick_geom(nx, ny, nz);
+    const double bytes = double(g.step_stride) * double(n_steps) * sizeof(float);
+    return bytes <= double(kBrickScratchLimit) ? size_t(g.step_stride) * size_t(n_steps) * sizeof(float) : 0;
+}
 bool use_batched_fp32(long long cells, int n_steps, int n_bins);
 // One-bin-per-thread marches with fp64 reductions spread them over up to 4 copies of the grid, 48 MiB in all (C2: 3
 // copies of 16 MiB; C4's 4 GiB grid: 1)
 constexpr size_t kAccCopiesBytes = size_t(48) << 20;
-Workspace workspace_layout(long long cells, int n_src, int n_rays, int n_steps, int n_bins) {
+Workspace workspace_layout(int nx, int ny, int nz, int n_src, int n_rays, int n_steps, int n_bins) {
     Workspace w;
+    const long long cells = (long long)nx * ny * nz * n_bins;
     const size_t grid = size_t(cells) * size_t(n_steps) * sizeof(double);
     w.acc_copies = use_batched_fp32(cells, n_steps, n_bins) ? 1 : int(std::min<size_t>(4, std::max<size_t>(1, kAccCopiesBytes / grid)));
     w.src_order_at = align_up(size_t(ray_slots(n_rays)) * sizeof(uint32_t), 16);
@@ -98,7 +111,9 @@ Workspace workspace_layout(long long cells, int n_src, int n_rays, int n_steps, 
     w.acc_at = align_up(w.flag_at + 16, 256);
     w.scratch2_at = align_up(w.acc_at + grid * size_t(w.acc_copies), 256);
     // the batched fp32 path marches two batches at a time: `out` and this second fp32 grid are their scratch grids
-    w.total = w.scratch2_at + (use_batched_fp32(cells, n_steps, n_bins) ? size_t(cells) * size_t(n_steps) * sizeof(float) : 0);
+    w.brick_at = align_up(w.scratch2_at + (use_batched_fp32(cells, n_steps, n_bins) ? size_t(cells) * size_t(n_steps) * sizeof(float) : 0), 256);
+    w.brick_bytes = brick_scratch_bytes(nx, ny, nz, n_src, n_steps, n_bins);
+    w.total = w.brick_at + w.brick_bytes;
     return w;
 }
 
@@ -260,7 +275,7 @@ int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const
     if (rc != RT_OK) return rc;
     Plan pl;
     if (!make_plan(variant, n_src, &pl)) return RT_EINVAL;
-    const Workspace wl = workspace_layout(ck.cells, n_src, n_rays, n_steps, n_bins);
+    const Workspace wl = workspace_layout(nx, ny, nz, n_src, n_rays, n_steps, n_bins);
     const size_t need = wl.total + (step ? step_scratch_bytes(ck.cells, n_bins) : 0);
     if (!workspace || workspace_bytes < need || (uintptr_t(workspace) & 15u)) return RT_EWORKSPACE;
     char* ws = static_cast<char*>(workspace);
@@ -355,21 +370,34 @@ int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const
         P.acc_copy_stride = (long long)n_acc;
     }
     RT_CUDA(cudaMemsetAsync(P.acc, 0, n_acc * (pl.acc64 ? sizeof(double) * size_t(P.acc_copies) : sizeof(float)), st));   // D14: overwrite
-    if (use_table_march(variant, pl, n_bins)) {
+    const bool table = use_table_march(variant, pl, n_bins) && wl.brick_bytes;
+    if (table) {
         // Sources that share their cell fractions (decided on the device) are marched by march_table_kernel, others by
-        // march_sliding_kernel<..., COPIES> below: each returns at once when the flag says it is the other's call
+        // march_sliding_kernel<..., COPIES> below: each returns at once when the flag says it is the other's call.  The
+        // table march deposits into the fp32 brick scratch, which it drains into the fp64 grid as it goes (rt_brick.cuh).
         int* flag = reinterpret_cast<int*>(ws + wl.flag_at);
         rt::same_fraction_kernel<<<1, 256, 0, st>>>(flag, sources, n_src, step_size);
         P.same_frac = flag;
+        P.scratch = reinterpret_cast<float*>(ws + wl.brick_at);
+        RT_CUDA(cudaMemsetAsync(P.scratch, 0, wl.brick_bytes, st));
         const long long tb = rt::march_blocks(P.n_src, P.n_slots, 1, 1);
         if (tb > 2147483647LL) return RT_EINVAL;
-        rt::march_table_kernel<10><<<unsigned(tb), rt::kThreads, 0, st>>>(P);
+        P.n_bricks = (long long)(wl.brick_bytes / (4 * sizeof(float)));
+        const long long per = (P.n_bricks * rt::kDrainRounds + tb - 1) / tb;
+        P.drain_bricks_per_block = int(std::min<long long>(std::max<long long>(per, 1), rt::kDrainMaxBricks));
+        rt::march_table_kernel<RT_TABLE_MINB><<<unsigned(tb), rt::kThreads, 0, st>>>(P);
         RT_CUDA(cudaGetLastError());
     }
     int rc3;
     if (vec4) rc3 = pl.acc64 ? launch_march<4, double>(P, pl.sliding, st) : launch_march<4, float>(P, pl.sliding, st);
     else rc3 = pl.acc64 ? launch_march<1, double>(P, pl.sliding, st) : launch_march<1, float>(P, pl.sliding, st);
     if (rc3 != RT_OK) return rc3;
+    if (table) {                       // what the table march left in the brick scratch
+        long long db = (P.n_bricks + 255) / 256;
+        if (db > 148 * 16) db = 148 * 16;
+        rt::drain_all_kernel<<<unsigned(db), 256, 0, st>>>(P.scratch, master, rt::brick_geom(nx, ny, nz), nx, ny, nz, P.n_bricks);
+        RT_CUDA(cudaGetLastError());
+    }
     if (pl.acc64) {
         rt::snapshot_finalize_kernel<double><<<unsigned(fin_blocks), fin_threads, 0, st>>>(master, out, ck.cells, n_steps,
                                                                                           P.acc_copies, P.acc_copy_stride);
@@ -427,7 +455,7 @@ int rt_march_adjoint_j(const float* gbar, const float* kappa, int nx, int ny, in
     const int rc = check_args(gbar, kappa, nx, ny, nz, sources, n_src, n_rays, n_bins, step_size, c, dt, n_steps,
                               grad_j, &ck);
     if (rc != RT_OK) return rc;
-    const Workspace wl = workspace_layout(ck.cells, n_src, n_rays, 1, n_bins);
+    const Workspace wl = workspace_layout(nx, ny, nz, n_src, n_rays, 1, n_bins);
     const size_t need = rt_adjoint_workspace_bytes(nx, ny, nz, n_src, n_rays, n_bins, n_steps);
     if (!workspace || workspace_bytes < need || (uintptr_t(workspace) & 15u)) return RT_EWORKSPACE;
     char* ws = static_cast<char*>(workspace);
@@ -515,7 +543,7 @@ int rt_march_adjoint_kappa_ex(const float* gbar, const float* j, const float* ka
                               grad_kappa, &ck);
     if (rc != RT_OK) return rc;
     if (uintptr_t(gbar) & 3u) return RT_EALIGN;
-    const Workspace wl = workspace_layout(ck.cells, n_src, n_rays, 1, n_bins);
+    const Workspace wl = workspace_layout(nx, ny, nz, n_src, n_rays, 1, n_bins);
     const size_t base = rt_adjoint_workspace_bytes(nx, ny, nz, n_src, n_rays, n_bins, n_steps);
     const size_t need = rt_adjoint_kappa_workspace_bytes_ex(nx, ny, nz, n_src, n_rays, n_bins, step_size, c, dt, n_steps,
                                                             record_limit);
@@ -670,7 +698,7 @@ size_t rt_workspace_bytes(int nx, int ny, int nz, int n_src, int n_rays, int n_b
         return 0;
     const long long cells = (long long)nx * ny;
     if (cells > 2147483647LL || cells * nz > 2147483647LL || cells * nz * n_bins > 2147483647LL) return 0;
-    return workspace_layout(cells * nz * n_bins, n_src, n_rays, n_steps, n_bins).total;
+    return workspace_layout(nx, ny, nz, n_src, n_rays, n_steps, n_bins).total;
 }
 
 int rt_substeps_per_step(float step_size, float c, float dt) {
@@ -692,7 +720,8 @@ int rt_launch_count(int nx, int ny, int nz, int n_src, int n_rays, int n_bins, i
     }
     // march, snapshot finalisation; the one-bin march with >= 32 sources also launches the fraction test and
     // march_table_kernel (one of the two march kernels returns at once)
-    return setup + 2 + (use_table_march(RT_VARIANT_DEFAULT, pl, n_bins) ? 2 : 0);
+    // march_table_kernel and the final drain of its scratch (one of the two march kernels returns at once)
+    return setup + 2 + ((use_table_march(RT_VARIANT_DEFAULT, pl, n_bins) && brick_scratch_bytes(nx, ny, nz, n_src, n_steps, n_bins)) ? 3 : 0);
 }
 
 int rt_directions(int n_rays, double* nhat, void* stream) {

@@ -1,0 +1,94 @@
+// rt_brick.cuh — the fp32 BRICK SCRATCH of the one-bin table march (sm_100a): vector reductions, concurrent drain.
+//
+// WHY.  ncu on C2 (profiles/r02b): the march is bound by the L1/LSU data pipe, and three quarters of its wavefronts
+// are the deposits -- every lane of a red.global.add is its own 32-byte sector on its way to the L2, whatever it
+// carries.  A stencil slide flushes a PLANE of 2 x 2 pending sums (the deposit has the trilinear
+// footprint), so the payload of one reduction can be the whole plane: red.global.add.v4.f32 / .v2.f32 (there is no
+// vector form for f64).  That needs (a) the 4 voxels of a plane contiguous and 16-byte aligned wherever the stencil
+// sits, and (b) fp32 sums that stay accurate.
+//
+// (a) LAYOUT.  The scratch grid is indexed by WINDOW: S[x][Y0][Z0][4] holds, for the 2 x 2 (y, z) window that starts at
+// (y0, z0) = (Y0 - 1, Z0 - 1), its four voxels (y0, z0), (y0, z0+1), (y0+1, z0), (y0+1, z0+1) as one 16-byte BRICK;
+// Y0 in [0, ny], Z0 in [0, nz], so every window of the padded index range [-1, N] has its own aligned brick (a voxel
+// lies in four windows: its sum is spread over four bricks, 4.1 x the memory of the grid).  Then
+//     x-slide:  the trailing x-plane (2 x 2 in y, z)            -> 1 red.v4
+//     y-slide:  per x slot, the z pair of the trailing y row    -> 2 red.v2  (the window that starts at that row)
+//     z-slide:  per x slot, the y pair of the trailing z column -> 2 red.v4 {a, 0, b, 0}
+// 1.67 reductions per slide instead of 4, and a brick's address is the lane's window offset, kept incrementally.
+// Windows that start one z apart are neighbours in memory, so rays from z-adjacent sources (the lanes of a warp are
+// sorted sources) share 32-byte sectors.  Index -1 and N (a clamped axis: both stencil indices are the same voxel,
+// the other element of the pair carries an exact zero) are padding and only ever receive zeros.
+//
+// (b) ACCURACY.  A voxel's fp32 sum must not collect too many addends (stagnation at the hot voxels).
+// Every block, when its rays are done, DRAINS one slice of the scratch into the fp64 accumulation grid:
+// atom.exch.b32(element, 0) takes the element's sum and zeroes it in one indivisible step -- a reduction that arrives
+// before the exchange is in the value taken, one that arrives after stays for the next drain, none is lost -- and
+// the value is added to the fp64 grid with red.global.add.f64.  The slices rotate with the block index so that the
+// whole scratch is drained kDrainRounds times per launch; a last pass after the march takes what is left.
+// (Vector reductions are performed element by element, so every access to an element is a 4-byte atomic.)
+#pragma once
+#include "rt_common.cuh"
+
+namespace rt {
+
+constexpr int kDrainRounds = 32;          // the scratch is drained about this often per march launch
+constexpr int kDrainMaxBricks = 8192;     // bricks one block drains at most
+
+struct BrickGeom {
+    int wy, wz;                   // windows per column / row: ny + 1, nz + 1
+    int sx, sy;                   // floats per step of x, of Y0 (a step of Z0 is 4)
+    long long step_stride;        // floats per time step: nx * wy * wz * 4
+};
+
+__host__ __device__ inline BrickGeom brick_geom(int nx, int ny, int nz) {
+    BrickGeom g;
+    g.wy = ny + 1;
+    g.wz = nz + 1;
+    g.sy = g.wz * 4;
+    g.sx = g.wy * g.sy;
+    g.step_stride = (long long)nx * g.sx;
+    return g;
+}
+
+__device__ __forceinline__ void red_v4(float* p, float a, float b, float c, float d) {
+    if ((__float_as_uint(a) | __float_as_uint(b) | __float_as_uint(c) | __float_as_uint(d)) != 0u)
+        asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
+}
+__device__ __forceinline__ void red_v2(float* p, float a, float b) {
+    if ((__float_as_uint(a) | __float_as_uint(b)) != 0u)
+        asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(p), "f"(a), "f"(b) : "memory");
+}
+
+// Drain bricks [b_begin, b_end) of the scratch (all time steps: brick b = ((m * nx + x) * wy + Y0) * wz + Z0) into the
+// fp64 grid master[m][x][y][z]; thread `t` of `n_threads` takes every n_threads-th brick.
+// CONCURRENT: safe while other blocks reduce into the same elements (see above).
+__device__ __forceinline__ void drain_bricks(float* scratch, double* master, const BrickGeom& G, int nx, int ny, int nz,
+                                             long long b_begin, long long b_end, int t, int n_threads) {
+    for (long long b = b_begin + t; b < b_end; b += n_threads) {
+        float* e = scratch + 4 * b;
+        const float4 peek = __ldcg(reinterpret_cast<const float4*>(e));      // a hint only: all zero -> nothing to take
+        if (peek.x == 0.0f && peek.y == 0.0f && peek.z == 0.0f && peek.w == 0.0f) continue;
+        const long long r = b / G.wz;
+        const int Z0 = int(b - r * G.wz);
+        const long long mx = r / G.wy;                      // m * nx + x
+        const int Y0 = int(r - mx * G.wy);
+        double* row = master + mx * ((long long)ny * nz);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int y = Y0 - 1 + (i >> 1), z = Z0 - 1 + (i & 1);
+            if (uint32_t(y) >= uint32_t(ny) || uint32_t(z) >= uint32_t(nz)) continue;      // padding: only zeros arrive
+            uint32_t bits;
+            asm volatile("atom.global.exch.b32 %0, [%1], %2;" : "=r"(bits) : "l"(e + i), "r"(0u) : "memory");
+            const float v = __uint_as_float(bits);
+            if (v != 0.0f)
+                asm volatile("red.global.add.f64 [%0], %1;" ::"l"(row + (long long)y * nz + z), "d"(double(v)) : "memory");
+        }
+    }
+}
+
+// the pass after the march: everything that is left in the scratch goes to the fp64 grid
+__global__ void drain_all_kernel(float* scratch, double* master, BrickGeom G, int nx, int ny, int nz, long long n_bricks) {
+    drain_bricks(scratch, master, G, nx, ny, nz, 0, n_bricks, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
+}
+
+}  // namespace rt

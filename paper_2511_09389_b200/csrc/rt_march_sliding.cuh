@@ -71,12 +71,17 @@ template <int NB, typename ACC, bool KTRI> struct Stencil {
 #pragma unroll
         for (int b = 0; b < NB; ++b) acc[s].v[b] = 0.0f;
     }
-    __device__ __forceinline__ void flush_all(ACC* og, const TravelAxis (&A)[3]) {
+    // ACT (here and in axis_step): bit a set = axis a is ACTIVE.  An inactive axis is one every ray of the warp has
+    // left the box through for good (march_table_kernel's lower-dimensional phases): its leading slots hold exactly
+    // zero and are skipped, i.e. only the slots whose index bit (4 >> a) is clear are touched.  ACT = 7: all 8 slots.
+    template <int ACT = 7> __device__ __forceinline__ void flush_all(ACC* og, const TravelAxis (&A)[3]) {
+        constexpr int kBits = ((ACT & 1) ? 4 : 0) | ((ACT & 2) ? 2 : 0) | ((ACT & 4) ? 1 : 0);
 #pragma unroll
-        for (int s = 0; s < 8; ++s) {
-            flush_slot(og, s, A);
-            zero_slot(s);
-        }
+        for (int s = 0; s < 8; ++s)
+            if ((s & ~kBits) == 0) {
+                flush_slot(og, s, A);
+                zero_slot(s);
+            }
     }
     template <int AX> __device__ __forceinline__ int place(const MarchParams& P, TravelAxis& X, int negbits) {
         const int t = eoff<AX>(P, X.p.c, negbits);
@@ -100,9 +105,12 @@ template <int NB, typename ACC, bool KTRI> struct Stencil {
     }
     // Axis AX advanced by one cell.  The old leading plane is the new trailing plane (also under clamping: both
     // are clamp(c+1)), so the trailing index moves iff the axis was not merged; the new leading index is looked up.
-    template <int AX>
-    __device__ __forceinline__ void axis_step(const MarchParams& P, TravelAxis (&A)[3], int negbits, ACC* og,
-                                              const float* jsrc) {
+    // flush_plane() reduces the pending sums of the trailing plane of AX to memory (called before anything moves, with
+    // base / dl still those of the old stencil; the cell word of AX may already be the new one).
+    template <int AX, int ACT = 7, class FlushPlane>
+    __device__ __forceinline__ void axis_step_with(const MarchParams& P, TravelAxis (&A)[3], int negbits, const float* jsrc,
+                                                   FlushPlane&& flush_plane) {
+        constexpr int kBits = ((ACT & 1) ? 4 : 0) | ((ACT & 2) ? 2 : 0) | ((ACT & 4) ? 1 : 0);
         TravelAxis& X = A[AX];
         // new leading minus new trailing offset: +-stride while both indices are inside the domain, i.e. u-cell
         // c in [0, lim-1] (ascending: indices c, c+1) or [-lim, -1] (descending: indices -c, -c-1); else 0
@@ -113,12 +121,13 @@ template <int NB, typename ACC, bool KTRI> struct Stencil {
         const int dln = inside ? (neg ? -stride : stride) : 0;
         const bool move = (X.dl != 0), load = inside;
         if (move) {
+            flush_plane();
 #pragma unroll
             for (int u = 0; u < 2; ++u)
 #pragma unroll
                 for (int v = 0; v < 2; ++v) {
                     const int s0 = slot<AX>(0, u, v), s1 = slot<AX>(1, u, v);
-                    flush_slot(og, s0, A);
+                    if (s1 & ~kBits) continue;       // a slot on the leading side of an inactive axis
                     acc[s0] = acc[s1];
                     jc[s0] = jc[s1];
                     if constexpr (KTRI) kc[s0] = kc[s1];
@@ -134,10 +143,26 @@ template <int NB, typename ACC, bool KTRI> struct Stencil {
 #pragma unroll
                 for (int v = 0; v < 2; ++v) {
                     const int s1 = slot<AX>(1, u, v);
+                    if (s1 & ~kBits) continue;
                     jc[s1] = ld_bins<NB>(jsrc + off(s1, A));
                     if constexpr (KTRI) kc[s1] = ld_bins<NB>(P.kappa + off(s1, A));
                 }
         }
+    }
+    // the slide with the trailing plane reduced slot by slot into the accumulation grid `og`
+    template <int AX, int ACT = 7>
+    __device__ __forceinline__ void axis_step(const MarchParams& P, TravelAxis (&A)[3], int negbits, ACC* og,
+                                              const float* jsrc) {
+        constexpr int kBits = ((ACT & 1) ? 4 : 0) | ((ACT & 2) ? 2 : 0) | ((ACT & 4) ? 1 : 0);
+        axis_step_with<AX, ACT>(P, A, negbits, jsrc, [&]() {
+#pragma unroll
+            for (int u = 0; u < 2; ++u)
+#pragma unroll
+                for (int v = 0; v < 2; ++v) {
+                    if (slot<AX>(1, u, v) & ~kBits) continue;
+                    flush_slot(og, slot<AX>(0, u, v), A);
+                }
+        });
     }
 };
 
