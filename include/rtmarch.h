@@ -156,11 +156,12 @@ int rt_march_host(const float* j, const float* kappa, int nx, int ny, int nz,
 
 int rt_host_release(void);
 
-/* Bytes of device scratch one rt_march call needs: the ray-order and source-order tables and the fp64
- * accumulation grid (n_steps * nx*ny*nz*n_bins doubles: deposits are summed in fp64 and rounded to fp32 once,
- * DESIGN.md §7; where several copies of it fit 48 MiB the march spreads its reductions over up to 4 copies), plus
- * one fp32 grid of n_steps * nx*ny*nz*n_bins floats where the batched multi-bin path runs
- * (n_bins % 4 == 0 and that grid <= 128 MiB).  0 on invalid arguments. */
+/* Bytes of device scratch one rt_march call needs: the ray-order and source-order tables, the fp64 accumulation grid
+ * (n_steps * nx*ny*nz*n_bins doubles: deposits are summed in fp64 and rounded to fp32 once; the kernels
+ * of the non-default variants spread their reductions over up to 4 copies of it where they fit 48 MiB), one fp32 grid
+ * of n_steps * nx*ny*nz*n_bins floats where the batched multi-bin kernels of the variants run (n_bins % 4 == 0 and that
+ * grid <= 128 MiB), and for one-bin calls the fp32 window-brick scratch of the march (n_steps * nx*(ny+1)*(nz+1)*4
+ * floats, if <= 1 GiB).  0 on invalid arguments. */
 size_t rt_workspace_bytes(int nx, int ny, int nz, int n_src, int n_rays, int n_bins, int n_steps);
 
 /* N_s as the library computes it (D6): ceil(c dt / step_size), a ratio within 1e-6 (relative) of an
@@ -168,7 +169,8 @@ size_t rt_workspace_bytes(int nx, int ny, int nz, int n_src, int n_rays, int n_b
  * N_s >= 2^31. */
 int rt_substeps_per_step(float step_size, float c, float dt);
 
-/* Number of kernels of this library that one rt_march call with these arguments enqueues (memsets excluded). */
+/* Number of kernels of this library that one rt_march call with these arguments and a step_size below one cell
+ * enqueues (memsets excluded). */
 int rt_launch_count(int nx, int ny, int nz, int n_src, int n_rays, int n_bins, int n_steps);
 
 /* TEST HOOK.  Writes the library's direction lattice (D1) for i = 0..n_rays-1 into

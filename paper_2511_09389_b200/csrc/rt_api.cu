@@ -15,8 +15,8 @@
 #include "rt_march_direct.cuh"
 #include "rt_adjoint.cuh"
 #include "rt_brick.cuh"
+#include "rt_march_phased.cuh"
 #include "rt_march_sliding.cuh"
-#include "rt_march_table.cuh"
 #include "rt_setup_kernels.cuh"
 
 namespace {
@@ -87,19 +87,18 @@ struct Workspace {
     size_t src_order_at, flag_at, acc_at, scratch2_at, brick_at, brick_bytes, total;
     int acc_copies;
 };
-// march_table_kernel (one bin, >= 32 sources) deposits into an fp32 brick scratch (rt_brick.cuh): one 16-byte brick per
-// 2 x 2 (y, z) window of each time step's grid, ~4.1 x the fp32 grid; the table march is used while that stays below
-// kBrickScratchLimit
+// One-bin calls deposit into an fp32 brick scratch (rt_brick.cuh): one 16-byte brick per 2 x 2 (y, z) window of each
+// time step's grid, ~4.1 x the fp32 grid; the phased march is used while that stays below kBrickScratchLimit
 constexpr size_t kBrickScratchLimit = size_t(1) << 30;
-size_t brick_scratch_bytes(int nx, int ny, int nz, int n_src, int n_steps, int n_bins) {
-    if (n_bins != 1 || n_src < 32) return 0;
+size_t brick_scratch_bytes(int nx, int ny, int nz, int n_steps, int n_bins) {
+    if (n_bins != 1) return 0;
     const rt::BrickGeom g = rt::brick_geom(nx, ny, nz);
     const double bytes = double(g.step_stride) * double(n_steps) * sizeof(float);
     return bytes <= double(kBrickScratchLimit) ? size_t(g.step_stride) * size_t(n_steps) * sizeof(float) : 0;
 }
 bool use_batched_fp32(long long cells, int n_steps, int n_bins);
-// One-bin-per-thread marches with fp64 reductions spread them over up to 4 copies of the grid, 48 MiB in all (C2: 3
-// copies of 16 MiB; C4's 4 GiB grid: 1)
+// One-bin-per-thread marches with fp64 reductions (the kernels of the non-default variants and of substeps of a cell or
+// more) spread them over up to 4 copies of the grid, 48 MiB in all
 constexpr size_t kAccCopiesBytes = size_t(48) << 20;
 Workspace workspace_layout(int nx, int ny, int nz, int n_src, int n_rays, int n_steps, int n_bins) {
     Workspace w;
@@ -112,7 +111,7 @@ Workspace workspace_layout(int nx, int ny, int nz, int n_src, int n_rays, int n_
     w.scratch2_at = align_up(w.acc_at + grid * size_t(w.acc_copies), 256);
     // the batched fp32 path marches two batches at a time: `out` and this second fp32 grid are their scratch grids
     w.brick_at = align_up(w.scratch2_at + (use_batched_fp32(cells, n_steps, n_bins) ? size_t(cells) * size_t(n_steps) * sizeof(float) : 0), 256);
-    w.brick_bytes = brick_scratch_bytes(nx, ny, nz, n_src, n_steps, n_bins);
+    w.brick_bytes = brick_scratch_bytes(nx, ny, nz, n_steps, n_bins);
     w.total = w.brick_at + w.brick_bytes;
     return w;
 }
@@ -144,7 +143,7 @@ int launch_march(const rt::MarchParams& P, bool sliding, cudaStream_t st, bool o
         constexpr int kMinBlocks = (NB == 1) ? 8 : 4;
         if (P.kappa_trilinear) rt::march_sliding_kernel<NB, ACC, 1, false, true><<<g, rt::kThreads, 0, st>>>(P);
         else if (P.state_I) rt::march_sliding_kernel<NB, ACC, kMinBlocks, true><<<g, rt::kThreads, 0, st>>>(P);
-        else if (P.acc_copies > 1 || P.same_frac)
+        else if (P.acc_copies > 1)
             rt::march_sliding_kernel<NB, ACC, kMinBlocks, false, false, false, true><<<g, rt::kThreads, 0, st>>>(P);
         else rt::march_sliding_kernel<NB, ACC, kMinBlocks, false><<<g, rt::kThreads, 0, st>>>(P);
     } else {
@@ -204,10 +203,26 @@ bool make_plan(int variant, int n_src, Plan* pl) {
     return true;
 }
 
-// rt_march_table.cuh: in play for the default one-bin march with 32 sources per warp (whether the sources qualify is
-// decided on the device)
-bool use_table_march(int variant, const Plan& pl, int n_bins) {
-    return variant == RT_VARIANT_DEFAULT && pl.map_src && n_bins == 1;
+// march_phased_kernel (rt_march_phased.cuh) marches the calls of rt_march proper: the default variant with substeps
+// shorter than a cell (a substep crosses at most one plane per axis).  Where its deposits go:
+//   kPhasedOneBin    one bin, brick scratch affordable: fp32 window bricks in the workspace, one vector reduction per
+//                    stencil plane, drained into the fp64 grid during the march
+//   kPhasedFourBins  bins in groups of four and an fp32 grid of at most kBatchedScratchLimit (it then largely stays in
+//                    the L2): `out` is the fp32 scratch, a voxel's four bins are one red.v4.f32, drained likewise
+//   kPhasedDirect64  everything else (other bin counts; grids far larger than the L2, where a scratch and its drains
+//                    would only add HBM traffic: measured on C4, 42 -> 32 ms with a scratch in four forms against 26 ms
+//                    without): one bin per thread, bins in adjacent lanes, red.global.add.f64 straight into the fp64 grid
+constexpr int kPhasedNone = 0, kPhasedOneBin = 1, kPhasedFourBins = 4, kPhasedDirect64 = 3;
+int phased_kind(int variant, float step_size, long long cells, int n_steps, int n_bins, size_t brick_bytes, bool aligned16) {
+    if (variant != RT_VARIANT_DEFAULT || !(step_size < 1.0f)) return kPhasedNone;
+    if (n_bins == 1 && brick_bytes) return kPhasedOneBin;
+    if (n_bins % 4 == 0 && aligned16 && use_batched_fp32(cells, n_steps, n_bins)) return kPhasedFourBins;
+    return kPhasedDirect64;
+}
+// how often the scratch is drained during a march: an fp32 sum should not collect much more than 2^19 rays' deposits
+// (C2, 8.6 M rays: 16 rounds, relative L2 error 6e-6 against 2.5e-5 with 4 rounds and 1.2e-4 with none)
+int drain_rounds(long long n_rays_total) {
+    return int(std::min<long long>(std::max<long long>(n_rays_total >> 19, 1), rt::kDrainRounds));
 }
 
 // the plan of RT_VARIANT_DEFAULT (make_plan cannot fail for it)
@@ -308,6 +323,59 @@ int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const
     const bool vec4 = aligned4 && !pl.one_bin && (batched || !pl.acc64 || !pl.sliding);
     P.n_groups = vec4 ? n_bins / 4 : n_bins;
 
+    const int phased = step ? kPhasedNone : phased_kind(variant, step_size, ck.cells, n_steps, n_bins, wl.brick_bytes, aligned4);
+    if (phased != kPhasedNone) {
+        // rt_march proper: the phased march deposits into an fp32 scratch -- window bricks in the workspace (one bin), or
+        // `out` itself as the plain grid (four bins per thread) -- and drains it into the fp64 grid as it goes; what is
+        // left is drained after the march; or it reduces straight into the fp64 grid.  The snapshots are formed from
+        // the fp64 grid.
+        P.n_groups = phased == kPhasedFourBins ? n_bins / 4 : n_bins;
+        P.acc = master;
+        P.scratch = phased == kPhasedOneBin ? reinterpret_cast<float*>(ws + wl.brick_at) : out;
+        const size_t scratch_bytes = phased == kPhasedDirect64 ? 0 : (phased == kPhasedOneBin ? wl.brick_bytes : n_acc * sizeof(float));
+        P.n_drain_units = std::max<long long>(1, (long long)(scratch_bytes / 16));
+        RT_CUDA(cudaMemsetAsync(master, 0, n_acc * sizeof(double), st));
+        if (scratch_bytes) RT_CUDA(cudaMemsetAsync(P.scratch, 0, scratch_bytes, st));
+        const long long mb = rt::march_blocks(P.n_src, P.n_slots, P.n_groups, P.map_src);
+        if (mb > 2147483647LL) return RT_EINVAL;
+        const long long per = (P.n_drain_units * drain_rounds((long long)n_src * n_rays) + mb - 1) / mb;
+        P.drain_units_per_block = std::min<long long>(std::max<long long>(per, 1), rt::kDrainMaxUnits);
+        if (pl.map_src) {
+            // Sources that share their cell fractions (decided on the device) take the weight-table instantiation, others
+            // the plain one: both are launched, each returns at once when the flag says the call is the other's
+            int* flag = reinterpret_cast<int*>(ws + wl.flag_at);
+            rt::same_fraction_kernel<<<1, 256, 0, st>>>(flag, sources, n_src, step_size);
+            P.same_frac = flag;
+            if (phased == kPhasedOneBin) rt::march_phased_kernel<1, true><<<unsigned(mb), rt::kThreads, 0, st>>>(P);
+            else if (phased == kPhasedDirect64) rt::march_phased_kernel<1, true, false, double><<<unsigned(mb), rt::kThreads, 0, st>>>(P);
+            else rt::march_phased_kernel<4, true><<<unsigned(mb), rt::kThreads, 0, st>>>(P);
+            RT_CUDA(cudaGetLastError());
+        }
+        long long mb2 = mb;
+        if (phased == kPhasedDirect64 && pl.map_src) {
+            // sources in general position on a grid beyond the L2: warp = 32 (direction, bin) pairs of ONE source, so that the
+            // blocks in flight stay around a few sources (C4: 27.5 -> 26.3 ms; the brick path is faster by sorted sources)
+            P.map_src = 0;
+            P.src_order = nullptr;
+            mb2 = rt::march_blocks(P.n_src, P.n_slots, P.n_groups, 0);
+            if (mb2 > 2147483647LL) return RT_EINVAL;
+        }
+        if (phased == kPhasedOneBin) rt::march_phased_kernel<1, false><<<unsigned(mb2), rt::kThreads, 0, st>>>(P);
+        else if (phased == kPhasedDirect64) rt::march_phased_kernel<1, false, false, double><<<unsigned(mb2), rt::kThreads, 0, st>>>(P);
+        else rt::march_phased_kernel<4, false><<<unsigned(mb2), rt::kThreads, 0, st>>>(P);
+        RT_CUDA(cudaGetLastError());
+        long long db = (P.n_drain_units + 255) / 256;
+        if (db > 148 * 16) db = 148 * 16;
+        if (phased == kPhasedOneBin)
+            rt::drain_all_kernel<<<unsigned(db), 256, 0, st>>>(P.scratch, master, rt::brick_geom(nx, ny, nz), nx, ny, nz,
+                                                               P.n_drain_units);
+        else if (phased != kPhasedDirect64)
+            rt::drain_all_plain_kernel<<<unsigned(db), 256, 0, st>>>(P.scratch, master, P.n_drain_units);
+        RT_CUDA(cudaGetLastError());
+        rt::snapshot_finalize_kernel<double><<<unsigned(fin_blocks), fin_threads, 0, st>>>(master, out, ck.cells, n_steps);
+        RT_CUDA(cudaGetLastError());
+        return RT_OK;
+    }
     if (batched) {
         // `out` (rt_march_step: a grid behind the fp64 grid, it may be accumulating into out) is the fp32 scratch
         // grid of ONE batch: no fp32 sum ever holds more than 2^17 rays, which bounds the error of fp32
@@ -370,34 +438,10 @@ int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const
         P.acc_copy_stride = (long long)n_acc;
     }
     RT_CUDA(cudaMemsetAsync(P.acc, 0, n_acc * (pl.acc64 ? sizeof(double) * size_t(P.acc_copies) : sizeof(float)), st));   // D14: overwrite
-    const bool table = use_table_march(variant, pl, n_bins) && wl.brick_bytes;
-    if (table) {
-        // Sources that share their cell fractions (decided on the device) are marched by march_table_kernel, others by
-        // march_sliding_kernel<..., COPIES> below: each returns at once when the flag says it is the other's call.  The
-        // table march deposits into the fp32 brick scratch, which it drains into the fp64 grid as it goes (rt_brick.cuh).
-        int* flag = reinterpret_cast<int*>(ws + wl.flag_at);
-        rt::same_fraction_kernel<<<1, 256, 0, st>>>(flag, sources, n_src, step_size);
-        P.same_frac = flag;
-        P.scratch = reinterpret_cast<float*>(ws + wl.brick_at);
-        RT_CUDA(cudaMemsetAsync(P.scratch, 0, wl.brick_bytes, st));
-        const long long tb = rt::march_blocks(P.n_src, P.n_slots, 1, 1);
-        if (tb > 2147483647LL) return RT_EINVAL;
-        P.n_bricks = (long long)(wl.brick_bytes / (4 * sizeof(float)));
-        const long long per = (P.n_bricks * rt::kDrainRounds + tb - 1) / tb;
-        P.drain_bricks_per_block = int(std::min<long long>(std::max<long long>(per, 1), rt::kDrainMaxBricks));
-        rt::march_table_kernel<RT_TABLE_MINB><<<unsigned(tb), rt::kThreads, 0, st>>>(P);
-        RT_CUDA(cudaGetLastError());
-    }
     int rc3;
     if (vec4) rc3 = pl.acc64 ? launch_march<4, double>(P, pl.sliding, st) : launch_march<4, float>(P, pl.sliding, st);
     else rc3 = pl.acc64 ? launch_march<1, double>(P, pl.sliding, st) : launch_march<1, float>(P, pl.sliding, st);
     if (rc3 != RT_OK) return rc3;
-    if (table) {                       // what the table march left in the brick scratch
-        long long db = (P.n_bricks + 255) / 256;
-        if (db > 148 * 16) db = 148 * 16;
-        rt::drain_all_kernel<<<unsigned(db), 256, 0, st>>>(P.scratch, master, rt::brick_geom(nx, ny, nz), nx, ny, nz, P.n_bricks);
-        RT_CUDA(cudaGetLastError());
-    }
     if (pl.acc64) {
         rt::snapshot_finalize_kernel<double><<<unsigned(fin_blocks), fin_threads, 0, st>>>(master, out, ck.cells, n_steps,
                                                                                           P.acc_copies, P.acc_copy_stride);
@@ -711,17 +755,11 @@ int rt_launch_count(int nx, int ny, int nz, int n_src, int n_rays, int n_bins, i
     if (nx < 1 || ny < 1 || nz < 1 || n_src < 1 || n_rays < 1 || n_bins < 1 || n_steps < 1) return RT_EINVAL;
     const Plan pl = default_plan(n_src);
     const int setup = 1 + ((pl.map_src && n_src <= kMaxSortedSources) ? 1 : 0);     // ray order, (source order)
-    if (use_batched_fp32((long long)nx * ny * nz * n_bins, n_steps, n_bins)) {      // (march, drain) per batch
-        const int slots = ray_slots(n_rays);
-        const Batching bt = plan_batches(n_src, slots, pl.map_src);
-        const int batches = ((n_src + bt.src_per_batch - 1) / bt.src_per_batch) *
-                            ((slots + bt.slots_per_batch - 1) / bt.slots_per_batch);
-        return setup + batches + (batches + 1) / 2 + 1;         // batches march in pairs, one drain per pair
-    }
-    // march, snapshot finalisation; the one-bin march with >= 32 sources also launches the fraction test and
-    // march_table_kernel (one of the two march kernels returns at once)
-    // march_table_kernel and the final drain of its scratch (one of the two march kernels returns at once)
-    return setup + 2 + ((use_table_march(RT_VARIANT_DEFAULT, pl, n_bins) && brick_scratch_bytes(nx, ny, nz, n_src, n_steps, n_bins)) ? 3 : 0);
+    // the phased march (what rt_march runs when substeps are shorter than a cell): (fraction test, the weight-table
+    // instantiation,) the plain instantiation -- one of the two returns at once --, (the last drain of the scratch,) snapshots
+    const long long cells = (long long)nx * ny * nz * n_bins;
+    const int kind = phased_kind(RT_VARIANT_DEFAULT, 0.5f, cells, n_steps, n_bins, brick_scratch_bytes(nx, ny, nz, n_steps, n_bins), true);
+    return setup + (pl.map_src ? 2 : 0) + 1 + (kind == kPhasedDirect64 ? 0 : 1) + 1;
 }
 
 int rt_directions(int n_rays, double* nhat, void* stream) {
@@ -812,6 +850,6 @@ const char* rt_strerror(int code) {
     }
 }
 
-const char* rt_version(void) { return "rtmarch 0.6 (sm_100a; sliding-stencil RED march, 32 sources x 1 direction per warp, weight table per warp for sources sharing their cell fractions, fp64 accumulation grid in up to 4 copies)"; }
+const char* rt_version(void) { return "rtmarch 0.7 (sm_100a; sliding-stencil march in warp-uniform phases, weight table per warp for sources sharing their cell fractions, fp32 scratch (window bricks / bin vectors) with vector reductions, drained concurrently into an fp64 grid)"; }
 
 }  // extern "C"

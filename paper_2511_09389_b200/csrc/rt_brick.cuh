@@ -31,8 +31,11 @@
 
 namespace rt {
 
-constexpr int kDrainRounds = 32;          // the scratch is drained about this often per march launch
-constexpr int kDrainMaxBricks = 8192;     // bricks one block drains at most
+#ifndef RT_DRAIN_ROUNDS
+#define RT_DRAIN_ROUNDS 16
+#endif
+constexpr int kDrainRounds = RT_DRAIN_ROUNDS;          // the scratch is drained about this often per march launch
+constexpr long long kDrainMaxUnits = 1 << 16;   // 16-byte units (bricks) one block drains at most
 
 struct BrickGeom {
     int wy, wz;                   // windows per column / row: ny + 1, nz + 1
@@ -86,9 +89,30 @@ __device__ __forceinline__ void drain_bricks(float* scratch, double* master, con
     }
 }
 
+// The same for a scratch in the plain grid layout (four bins per thread: a voxel's bins are one red.v4.f32): units of 4
+// floats [u_begin, u_end), element e of the scratch belongs to element e of the fp64 grid.
+__device__ __forceinline__ void drain_plain(float* scratch, double* master, long long u_begin, long long u_end, int t,
+                                            int n_threads) {
+    for (long long u = u_begin + t; u < u_end; u += n_threads) {
+        float* e = scratch + 4 * u;
+        const float4 peek = __ldcg(reinterpret_cast<const float4*>(e));      // a hint only: all zero -> nothing to take
+        if (peek.x == 0.0f && peek.y == 0.0f && peek.z == 0.0f && peek.w == 0.0f) continue;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            uint32_t bits;
+            asm volatile("atom.global.exch.b32 %0, [%1], %2;" : "=r"(bits) : "l"(e + i), "r"(0u) : "memory");
+            const float v = __uint_as_float(bits);
+            if (v != 0.0f) asm volatile("red.global.add.f64 [%0], %1;" ::"l"(master + 4 * u + i), "d"(double(v)) : "memory");
+        }
+    }
+}
+
 // the pass after the march: everything that is left in the scratch goes to the fp64 grid
 __global__ void drain_all_kernel(float* scratch, double* master, BrickGeom G, int nx, int ny, int nz, long long n_bricks) {
     drain_bricks(scratch, master, G, nx, ny, nz, 0, n_bricks, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
+}
+__global__ void drain_all_plain_kernel(float* scratch, double* master, long long n_units) {
+    drain_plain(scratch, master, 0, n_units, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
 }
 
 }  // namespace rt

@@ -38,11 +38,12 @@ struct MarchParams {
     // march_sliding_kernel<..., COPIES = true> and march_table_kernel, else 1 / 0:
     int acc_copies;              // block b reduces into copy b % acc_copies of the accumulation grid ...
     long long acc_copy_stride;   // ... copies being acc_copy_stride elements apart (hot voxels meet fewer reductions)
-    // march_table_kernel (rt_brick.cuh): fp32 brick scratch [n_steps][4 copies][nx][nby][nbz][4], drained into the fp64
-    // grid `acc` while the march runs
+    // march_phased_kernel: the fp32 scratch its rays deposit into (rt_brick.cuh: window bricks [n_steps][nx][ny+1][nz+1][4]
+    // for one bin per thread, the plain grid [n_steps][nx][ny][nz][nb] for four), drained into the fp64 grid `acc`
+    // while the march runs
     float* scratch;
-    int drain_bricks_per_block;  // bricks one block drains when its rays are done
-    long long n_bricks;          // bricks of the whole scratch (all time steps and copies)
+    long long drain_units_per_block;   // 16-byte units of the scratch one block drains when its rays are done
+    long long n_drain_units;           // 16-byte units of the whole scratch
 };
 
 constexpr uint32_t kPad = 0xFFFFFFFFu;
