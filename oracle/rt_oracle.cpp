@@ -2,9 +2,15 @@
 //
 // This file is the plain, slow, obviously-correct restatement of what the hot path computes, written
 // from the paper (/root/reference/PAPER.md, cited below as P:<line>) and from nothing else.  It shares
-// no code, header, table or constant with the CUDA path under paper_2511_09389_b200/csrc/, and neither
-// side includes or links the other.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
-// `--impl reference` legs may build, load or call it.  The product path never routes through it.
+// no code, header or table with the CUDA path under paper_2511_09389_b200/csrc/, and neither side
+// includes or links the other.  What the two sides do share is a READING, D1/D3: positions live
+// on a 2^-64 cell grid and the azimuth is reduced with the golden turn as a 128-bit fixed-point fraction, so
+// the same mathematical constants ((3 - sqrt 5)/2 * 2^128, 2^-64) appear on both sides, each written out
+// separately; floor(x_k) on tie rays then agrees by construction of the reading, not by a shared routine.
+// The guards that are independent of both are the pins: the lattice against 50-digit arithmetic (P0) and the
+// positions against exact rationals (fractions.Fraction, D3) in tests/test_oracle_pins.py.
+// Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / `--impl reference` legs may build,
+// load or call it.  The product path never routes through it.
 //
 // What it computes (eq. (2) at P:23; readings D1..D16 are listed in DESIGN.md §4):
 //
