@@ -282,6 +282,16 @@ size_t step_scratch_bytes(long long cells, int n_bins) {
     return use_batched_fp32(cells, 1, n_bins) ? size_t(cells) * sizeof(float) : 0;
 }
 
+// the instantiation of march_phased_kernel for a deposit mode (phased_kind)
+template <bool TABLE, bool STEP>
+int launch_phased(const rt::MarchParams& P, int kind, unsigned blocks, cudaStream_t st) {
+    if (kind == kPhasedOneBin) rt::march_phased_kernel<1, TABLE, true, float, STEP><<<blocks, rt::kThreads, 0, st>>>(P);
+    else if (kind == kPhasedFourBins) rt::march_phased_kernel<4, TABLE, false, float, STEP><<<blocks, rt::kThreads, 0, st>>>(P);
+    else rt::march_phased_kernel<1, TABLE, false, double, STEP><<<blocks, rt::kThreads, 0, st>>>(P);
+    RT_CUDA(cudaGetLastError());
+    return RT_OK;
+}
+
 int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const float* sources, int n_src, int n_rays,
                int n_bins, float step_size, float c, float dt, int n_steps, float* out, void* workspace,
                size_t workspace_bytes, void* stream, int variant, const StepArgs* step = nullptr) {
@@ -323,15 +333,17 @@ int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const
     const bool vec4 = aligned4 && !pl.one_bin && (batched || !pl.acc64 || !pl.sliding);
     P.n_groups = vec4 ? n_bins / 4 : n_bins;
 
-    const int phased = step ? kPhasedNone : phased_kind(variant, step_size, ck.cells, n_steps, n_bins, wl.brick_bytes, aligned4);
+    const int phased = phased_kind(variant, step_size, ck.cells, n_steps, n_bins, wl.brick_bytes, aligned4);
     if (phased != kPhasedNone) {
-        // rt_march proper: the phased march deposits into an fp32 scratch -- window bricks in the workspace (one bin), or
-        // `out` itself as the plain grid (four bins per thread) -- and drains it into the fp64 grid as it goes; what is
-        // left is drained after the march; or it reduces straight into the fp64 grid.  The snapshots are formed from
-        // the fp64 grid.
+        // rt_march proper (and rt_march_step): the phased march deposits into an fp32 scratch -- window bricks in the
+        // workspace (one bin), or the plain grid (four bins per thread; `out` itself, or for rt_march_step, whose `out` may
+        // hold the running field, a grid behind the workspace) -- and drains it into the fp64 grid as it goes; what is
+        // left is drained after the march; or it reduces straight into the fp64 grid.  The snapshots (the step's
+        // increment) are formed from the fp64 grid.
         P.n_groups = phased == kPhasedFourBins ? n_bins / 4 : n_bins;
         P.acc = master;
-        P.scratch = phased == kPhasedOneBin ? reinterpret_cast<float*>(ws + wl.brick_at) : out;
+        P.scratch = phased == kPhasedOneBin ? reinterpret_cast<float*>(ws + wl.brick_at)
+                                            : (step ? reinterpret_cast<float*>(ws + wl.total) : out);
         const size_t scratch_bytes = phased == kPhasedDirect64 ? 0 : (phased == kPhasedOneBin ? wl.brick_bytes : n_acc * sizeof(float));
         P.n_drain_units = std::max<long long>(1, (long long)(scratch_bytes / 16));
         RT_CUDA(cudaMemsetAsync(master, 0, n_acc * sizeof(double), st));
@@ -346,10 +358,8 @@ int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const
             int* flag = reinterpret_cast<int*>(ws + wl.flag_at);
             rt::same_fraction_kernel<<<1, 256, 0, st>>>(flag, sources, n_src, step_size);
             P.same_frac = flag;
-            if (phased == kPhasedOneBin) rt::march_phased_kernel<1, true><<<unsigned(mb), rt::kThreads, 0, st>>>(P);
-            else if (phased == kPhasedDirect64) rt::march_phased_kernel<1, true, false, double><<<unsigned(mb), rt::kThreads, 0, st>>>(P);
-            else rt::march_phased_kernel<4, true><<<unsigned(mb), rt::kThreads, 0, st>>>(P);
-            RT_CUDA(cudaGetLastError());
+            const int rct = step ? launch_phased<true, true>(P, phased, unsigned(mb), st) : launch_phased<true, false>(P, phased, unsigned(mb), st);
+            if (rct != RT_OK) return rct;
         }
         long long mb2 = mb;
         if (phased == kPhasedDirect64 && pl.map_src) {
@@ -360,10 +370,8 @@ int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const
             mb2 = rt::march_blocks(P.n_src, P.n_slots, P.n_groups, 0);
             if (mb2 > 2147483647LL) return RT_EINVAL;
         }
-        if (phased == kPhasedOneBin) rt::march_phased_kernel<1, false><<<unsigned(mb2), rt::kThreads, 0, st>>>(P);
-        else if (phased == kPhasedDirect64) rt::march_phased_kernel<1, false, false, double><<<unsigned(mb2), rt::kThreads, 0, st>>>(P);
-        else rt::march_phased_kernel<4, false><<<unsigned(mb2), rt::kThreads, 0, st>>>(P);
-        RT_CUDA(cudaGetLastError());
+        const int rcp = step ? launch_phased<false, true>(P, phased, unsigned(mb2), st) : launch_phased<false, false>(P, phased, unsigned(mb2), st);
+        if (rcp != RT_OK) return rcp;
         long long db = (P.n_drain_units + 255) / 256;
         if (db > 148 * 16) db = 148 * 16;
         if (phased == kPhasedOneBin)
@@ -372,7 +380,10 @@ int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const
         else if (phased != kPhasedDirect64)
             rt::drain_all_plain_kernel<<<unsigned(db), 256, 0, st>>>(P.scratch, master, P.n_drain_units);
         RT_CUDA(cudaGetLastError());
-        rt::snapshot_finalize_kernel<double><<<unsigned(fin_blocks), fin_threads, 0, st>>>(master, out, ck.cells, n_steps);
+        if (step)
+            rt::step_finalize_kernel<<<unsigned(fin_blocks), fin_threads, 0, st>>>(master, out, ck.cells, step->accumulate);
+        else
+            rt::snapshot_finalize_kernel<double><<<unsigned(fin_blocks), fin_threads, 0, st>>>(master, out, ck.cells, n_steps);
         RT_CUDA(cudaGetLastError());
         return RT_OK;
     }

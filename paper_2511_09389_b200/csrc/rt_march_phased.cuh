@@ -172,7 +172,7 @@ template <int NB, typename ACC> __device__ __forceinline__ void phased_load_att(
 
 // The substep loop with the axes in ACT active; runs until the table runs out (TABLE), the time step ends or an
 // axis goes inactive, and returns the new set of active axes.
-template <int ACT, int NB, bool TABLE, bool BRICK, typename ACC>
+template <int ACT, int NB, bool TABLE, bool BRICK, typename ACC, bool STEP>
 __device__ __forceinline__ int phase(const MarchParams& P, const BrickGeom& G, PhasedLane<NB, ACC>& L, int negbits,
                                      uint32_t tbase) {
     constexpr int kBits = ((ACT & 1) ? 4 : 0) | ((ACT & 2) ? 2 : 0) | ((ACT & 4) ? 1 : 0);      // slot index bits in use
@@ -240,7 +240,8 @@ __device__ __forceinline__ int phase(const MarchParams& P, const BrickGeom& G, P
                         else jv = (r == 0) ? w[s] * jc : fmaf(w[s], jc, jv);
                     }
             }
-            L.I[b] = fmaf(L.I[b], L.att[b], (jv + ju) * L.T[b]);                   // eq. (2)
+            // eq. (2).  STEP: T is the carried exp(-tau) itself, else ds 4 pi/N_Omega rides on it
+            L.I[b] = fmaf(L.I[b], L.att[b], STEP ? (jv + ju) * L.T[b] * P.emis : (jv + ju) * L.T[b]);
             L.T[b] *= L.att[b];
 #pragma unroll
             for (int s = 0; s < 8; ++s)
@@ -297,7 +298,9 @@ __device__ __forceinline__ int phase(const MarchParams& P, const BrickGeom& G, P
 // BRICK: the scratch is the window-brick grid of rt_brick.cuh (one-bin calls); else the plain grid [x][y][z][bin].
 // ACC = double: no scratch -- the deposits are reduced straight into the fp64 grid (red.global.add.f64 per bin) and
 // nothing is drained: for grids far larger than the L2, where a scratch would only add HBM traffic.
-template <int NB, bool TABLE, bool BRICK = (NB == 1), typename ACC = float>
+// STEP: the rt_march_step form (D17) -- one time step from substep P.k0, (I, exp(-tau)) of every ray loaded
+// from and stored back to the ray state.
+template <int NB, bool TABLE, bool BRICK = (NB == 1), typename ACC = float, bool STEP = false>
 __global__ void __launch_bounds__(kThreads, NB == 1 ? RT_PHASED_MINB1 : RT_PHASED_MINB4)
 march_phased_kernel(const MarchParams P) {
     static_assert(!BRICK || (NB == 1 && sizeof(ACC) == 4), "the brick scratch holds one fp32 bin");
@@ -334,6 +337,7 @@ march_phased_kernel(const MarchParams P) {
                     ref[warp][a] = Fx96{0, L.A[a].p.fh, L.A[a].p.fl};
                     ref[warp][3 + a] = L.A[a].d;
                 }
+                if (STEP) fx_advance(L.A[a].p, L.A[a].d, P.k0);      // x_k0 = x_0 + k0 ds n
             }
         }
         asm volatile("" : "+r"(negbits));        // opaque: keeps ptxas from re-deriving the signs with fp64 compares
@@ -342,6 +346,12 @@ march_phased_kernel(const MarchParams P) {
         L.S.restart(P, L.A, negbits, id.group * NB, P.j);
 #pragma unroll
         for (int b = 0; b < NB; ++b) { L.I[b] = 0.0f; L.T[b] = live ? P.emis : 0.0f; }       // ds 4 pi/N_Omega rides on exp(-tau)
+        const size_t state_at = (size_t(id.src) * P.n_rays + id.index) * P.nb + size_t(id.group) * NB;
+        if (STEP && live) {                  // the ray's (I, exp(-tau)) carried from the previous call
+            const BinVec<NB> si = ld_bins<NB>(P.state_I + state_at), sT = ld_bins<NB>(P.state_T + state_at);
+#pragma unroll
+            for (int b = 0; b < NB; ++b) { L.I[b] = si.v[b]; L.T[b] = sT.v[b]; }
+        }
         phased_load_att<NB, ACC>(P, L, L.S.base + ((negbits & 1) ? L.A[0].dl : 0) + ((negbits & 2) ? L.A[1].dl : 0) +
                                       ((negbits & 4) ? L.A[2].dl : 0));
         L.g = 0;
@@ -378,7 +388,7 @@ march_phased_kernel(const MarchParams P) {
                     for (int a = 0; a < 3; ++a) {
                         Fx96 p = ref[warp][a];
                         const Fx96 d = ref[warp][3 + a];
-                        fx_advance(p, d, (long long)L.g + lane);
+                        fx_advance(p, d, (STEP ? P.k0 : 0) + (long long)L.g + lane);
                         const uint32_t h = p.fh;
                         const int c = p.c;
                         fx_add(p, d);
@@ -391,14 +401,14 @@ march_phased_kernel(const MarchParams P) {
                 }
             }
             switch (act) {
-                case 7: act = phase<7, NB, TABLE, BRICK, ACC>(P, G, L, negbits, tbase); break;
-                case 6: act = phase<6, NB, TABLE, BRICK, ACC>(P, G, L, negbits, tbase); break;
-                case 5: act = phase<5, NB, TABLE, BRICK, ACC>(P, G, L, negbits, tbase); break;
-                case 4: act = phase<4, NB, TABLE, BRICK, ACC>(P, G, L, negbits, tbase); break;
-                case 3: act = phase<3, NB, TABLE, BRICK, ACC>(P, G, L, negbits, tbase); break;
-                case 2: act = phase<2, NB, TABLE, BRICK, ACC>(P, G, L, negbits, tbase); break;
-                case 1: act = phase<1, NB, TABLE, BRICK, ACC>(P, G, L, negbits, tbase); break;
-                default: act = phase<0, NB, TABLE, BRICK, ACC>(P, G, L, negbits, tbase); break;
+                case 7: act = phase<7, NB, TABLE, BRICK, ACC, STEP>(P, G, L, negbits, tbase); break;
+                case 6: act = phase<6, NB, TABLE, BRICK, ACC, STEP>(P, G, L, negbits, tbase); break;
+                case 5: act = phase<5, NB, TABLE, BRICK, ACC, STEP>(P, G, L, negbits, tbase); break;
+                case 4: act = phase<4, NB, TABLE, BRICK, ACC, STEP>(P, G, L, negbits, tbase); break;
+                case 3: act = phase<3, NB, TABLE, BRICK, ACC, STEP>(P, G, L, negbits, tbase); break;
+                case 2: act = phase<2, NB, TABLE, BRICK, ACC, STEP>(P, G, L, negbits, tbase); break;
+                case 1: act = phase<1, NB, TABLE, BRICK, ACC, STEP>(P, G, L, negbits, tbase); break;
+                default: act = phase<0, NB, TABLE, BRICK, ACC, STEP>(P, G, L, negbits, tbase); break;
             }
             if (L.left == 0) {               // time-step boundary: the increments of this step are complete (rays continue, D7)
                 if constexpr (BRICK) {
@@ -411,6 +421,13 @@ march_phased_kernel(const MarchParams P) {
                     L.sg += P.snap_stride;
                 }
                 L.left = P.n_sub;
+            }
+        }
+        if (STEP && live) {
+#pragma unroll
+            for (int b = 0; b < NB; ++b) {
+                P.state_I[state_at + b] = L.I[b];
+                P.state_T[state_at + b] = L.T[b];
             }
         }
     }
