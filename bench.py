@@ -453,25 +453,9 @@ def run_native(args):
         if world == 1:
             red = roof if roof["bound"] == "l2_red" else roof["l2_red"]
             red["best_step_frac"] = red["frac"] * step_s / (min(step_ms) * 1e-3)
-        cnt = _ncu_counters(args.config, args.variant) if args.mode == "march" else None
-        if cnt and world == 1:
-            sm_hz = (clocks.get("sm_mhz") or 1965.0) * 1e6
-            substeps = n_src * w.n_rays * w.n_steps * w.substeps_per_step
-            roof["traffic"] = cnt["dram_bytes"]
-            roof["issued"] = {"red_sectors_per_launch": cnt["red_sectors"],
-                              "red_sectors_per_ray_substep": cnt["red_sectors"] / substeps,
-                              "achieved_Gsectors_per_s": cnt["red_sectors"] / step_s / 1e9,
-                              "frac_of_M3": cnt["red_sectors"] / step_s / 1e9 / ceil["M3_f64_stencil"]}
-            roof["alu"] = {"warp_instructions_per_launch": cnt["warp_instructions"],
-                           "warp_instructions_per_warp_substep": cnt["warp_instructions"] / (substeps / 32),
-                           "achieved_Ginst_per_s": cnt["warp_instructions"] / step_s / 1e9,
-                           "peak_Ginst_per_s": 148 * 4 * sm_hz / 1e9,
-                           "frac": cnt["warp_instructions"] / step_s / (148 * 4 * sm_hz),
-                           "peak_how": "148 SMs x 4 schedulers x 1 warp-instruction/clk x SM clock sampled in the run"}
-            roof["kernel"] = cnt["kernel"]
-            roof["counters_from"] = cnt["source"]
-            roof["how"] += ("; `traffic`, `issued` and `alu` are REPLAYED from the committed ncu capture named in "
-                            "`counters_from` (same library version string), divided by the step time measured here")
+        if args.mode == "march" and world == 1:
+            attach_counters(roof, args.config, args.variant, step_s, n_src * w.n_rays * w.n_steps * w.substeps_per_step,
+                            ceil.get("M3_f64_stencil") if nb == 1 else ceil["M3_stencil"], (clocks.get("sm_mhz") or 1965.0) * 1e6)
         line["roofline"] = roof
 
     # ---- the other large configs and the other entry points, a few steps each (single GPU, default run only)
@@ -507,6 +491,10 @@ def run_extras(rt, torch, w_c2, flush, steps):
                "ray_substeps_per_s": case.units / w.n_bins / mean_s, "checksum": case.checksum(),
                "gpu_launches_per_step": rt.rt_launch_count(*w.shape, n_src, w.n_rays, w.n_bins, w.n_steps) if mode == "march" else None,
                "roofline": roofline_of(rt, torch, w, n_src, mean_s, None, mode)}
+        if mode == "march" and label is None:
+            rf = row["roofline"]
+            attach_counters(rf, w.name, 0, mean_s, n_src * w.n_rays * w.n_steps * w.substeps_per_step,
+                            rf["peak"] if rf["bound"] == "l2_red" else rf["l2_red"]["peak"], 1965.0e6)
         del case
         torch.cuda.empty_cache()
         return row
@@ -526,17 +514,44 @@ def run_extras(rt, torch, w_c2, flush, steps):
 
 def _ncu_counters(config, variant):
     """Per-launch ncu counters of the march kernel (committed text under profiles/, one capture per kernel
-    revision): instruction count, L2 reduction sectors, DRAM bytes.  None if there is no capture for this case."""
+    revision).  None if there is no capture of this case for the loaded library."""
     import csv
     try:
         with open(os.path.join(ROOT, "profiles", "march_counters.csv"), newline="") as f:
             for row in csv.DictReader(f):
                 if row["case"] == f"{config}:v{variant}" and row["library"] == _lib_version():
-                    return {"warp_instructions": float(row["warp_instructions"]), "red_sectors": float(row["red_sectors"]),
-                            "dram_bytes": float(row["dram_bytes"]), "source": row["source"], "kernel": row["kernel"]}
+                    out = {k: float(row[k]) for k in ("warp_instructions", "red_sectors", "dram_bytes", "issue_active_pct",
+                                                      "l1_lsu_wavefronts_pct", "l2_hit_pct", "warps_active_pct", "registers")}
+                    out.update(source=row["source"], kernel=row["kernel"])
+                    return out
     except (OSError, KeyError, ValueError):
         pass
     return None
+
+
+def attach_counters(roof, config, variant, step_s, substeps, red_ceiling, sm_hz):
+    """`traffic`, `issued`, `alu`, `lsu`: ncu counters of the march kernel of this case REPLAYED from the committed capture
+    (profiles/march_counters.csv, same library version string), per launch, divided by the step time measured here."""
+    cnt = _ncu_counters(config, variant)
+    if not cnt:
+        return
+    roof["traffic"] = cnt["dram_bytes"]
+    roof["issued"] = {"red_sectors_per_launch": cnt["red_sectors"], "red_sectors_per_ray_substep": cnt["red_sectors"] / substeps,
+                      "achieved_Gsectors_per_s": cnt["red_sectors"] / step_s / 1e9,
+                      "frac_of_M3": cnt["red_sectors"] / step_s / 1e9 / red_ceiling if red_ceiling else None}
+    roof["alu"] = {"warp_instructions_per_launch": cnt["warp_instructions"],
+                   "warp_instructions_per_warp_substep": cnt["warp_instructions"] / (substeps / 32),
+                   "achieved_Ginst_per_s": cnt["warp_instructions"] / step_s / 1e9, "peak_Ginst_per_s": 148 * 4 * sm_hz / 1e9,
+                   "frac": cnt["warp_instructions"] / step_s / (148 * 4 * sm_hz), "issue_active_pct_under_ncu": cnt["issue_active_pct"],
+                   "peak_how": "148 SMs x 4 schedulers x 1 warp-instruction/clk x SM clock sampled in the run"}
+    roof["lsu"] = {"l1_lsu_data_pipe_wavefronts_pct_of_peak_under_ncu": cnt["l1_lsu_wavefronts_pct"], "l2_hit_pct": cnt["l2_hit_pct"],
+                   "warps_active_pct": cnt["warps_active_pct"], "registers_per_thread": cnt["registers"],
+                   "note": "the busiest unit of the one-bin march: one wavefront per 32-byte sector of a scattered load or "
+                           "reduction (DESIGN.md §7)"}
+    roof["kernel"] = cnt["kernel"]
+    roof["counters_from"] = cnt["source"]
+    roof["how"] += ("; `traffic`, `issued`, `alu` and `lsu` are REPLAYED from the committed ncu capture named in "
+                    "`counters_from` (same library version string), divided by the step time measured here")
 
 
 def _lib_version():
