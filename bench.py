@@ -227,6 +227,7 @@ class Case:
         self.units = n_src * w.n_rays * w.n_steps * w.substeps_per_step * nb
         u8 = torch.uint8
         if mode in ("adjoint_j", "adjoint_kappa"):
+            torch.manual_seed(939913)          # dL/d out of the adjoint modes: seeded, so the checksums repeat
             self.gbar = torch.rand((w.n_steps, nx, ny, nz, nb), dtype=torch.float32, device="cuda")
             self.result = torch.empty((nx, ny, nz, nb), dtype=torch.float32, device="cuda")
             nbytes = (rt.rt_adjoint_workspace_bytes(nx, ny, nz, n_src, w.n_rays, nb, w.n_steps) if mode == "adjoint_j" else
