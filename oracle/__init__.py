@@ -63,6 +63,10 @@ def lib() -> ctypes.CDLL:
             L.rt_adjoint_kappa_oracle.argtypes = [dp, fp, fp, ctypes.c_int, ctypes.c_int, ctypes.c_int, fp, ctypes.c_int,
                                                   ctypes.c_int, ctypes.c_int, ctypes.c_float, ctypes.c_float,
                                                   ctypes.c_float, ctypes.c_int, dp, ctypes.c_int]
+            L.rt_jvp_kappa_oracle.restype = ctypes.c_int
+            L.rt_jvp_kappa_oracle.argtypes = [fp, fp, fp, ctypes.c_int, ctypes.c_int, ctypes.c_int, fp, ctypes.c_int,
+                                              ctypes.c_int, ctypes.c_int, ctypes.c_float, ctypes.c_float, ctypes.c_float,
+                                              ctypes.c_int, dp, ctypes.c_int]
             L.rt_oracle_step.restype = ctypes.c_int
             L.rt_oracle_step.argtypes = [fp, fp, ctypes.c_int, ctypes.c_int, ctypes.c_int, fp, ctypes.c_int,
                                          ctypes.c_int, ctypes.c_int, ctypes.c_float, ctypes.c_float, ctypes.c_float,
@@ -164,6 +168,27 @@ def adjoint_kappa(gbar, j, kappa, sources, n_rays, step_size, c, dt, n_steps, n_
     if rc:
         raise ValueError("rt_adjoint_kappa_oracle: invalid arguments")
     return grad
+
+
+def jvp_kappa(j, kappa, dkappa, sources, n_rays, step_size, c, dt, n_steps, n_threads: int | None = None) -> np.ndarray:
+    """Tangent of the field for kappa -> kappa + eps * dkappa at eps = 0 (D21): float64
+    [n_steps, nx, ny, nz, n_bins], cumulative snapshots like ``march``."""
+    j = _f32(j, 4)
+    kappa = _f32(kappa, 4)
+    dkappa = _f32(dkappa, 4)
+    sources = _f32(sources, 2)
+    if kappa.shape != j.shape or dkappa.shape != j.shape or sources.shape[1] != 3:
+        raise ValueError("shape mismatch")
+    nx, ny, nz, nb = j.shape
+    if n_threads is None:
+        n_threads = host_threads()
+    n_threads = max(1, min(n_threads, (24 << 30) // max(1, j.size * 8 * n_steps)))
+    out = np.empty((n_steps, nx, ny, nz, nb), dtype=np.float64)
+    rc = lib().rt_jvp_kappa_oracle(_fp(j), _fp(kappa), _fp(dkappa), nx, ny, nz, _fp(sources), sources.shape[0], n_rays, nb,
+                                   step_size, c, dt, n_steps, _dp(out), n_threads)
+    if rc:
+        raise ValueError("rt_jvp_kappa_oracle: invalid arguments")
+    return out
 
 
 def new_state(n_src: int, n_rays: int, n_bins: int) -> np.ndarray:

@@ -510,6 +510,89 @@ int rt_adjoint_kappa_oracle(const double* gbar, const float* j, const float* kap
     return 0;
 }
 
+// FORWARD-MODE derivative of the march with respect to kappa (gradients "from jacfwd", extending to "a global
+// kappa scale"; reading D21): the tangent of the field for kappa -> kappa + eps dkappa at eps = 0 (a global
+// scale is dkappa = kappa).  kappa enters eq. (2) through exp(-kappa_k ds) and exp(-tau_k), read nearest
+// neighbour at the cell of x_k; the cells do not depend on kappa.  Differentiating eq. (2) term by term,
+// with dot = d/d eps:
+//   Idot_{k+1}   = Idot_k exp(-kappa_k ds) + I_k (-dkappa_k ds) exp(-kappa_k ds) + j(x_k) (-taudot_k) exp(-tau_k) ds
+//   taudot_{k+1} = taudot_k + dkappa_k ds
+// next to eq. (2) itself for (I, tau); the tangent field collects w_c Idot_{k+1} with the weights of x_k,
+// cumulative snapshots (D7), scaled by 4 pi / N_Omega (D8).  tangent: double [n_steps][nx][ny][nz][B], overwritten.
+int rt_jvp_kappa_oracle(const float* j, const float* kappa, const float* dkappa, int nx, int ny, int nz,
+                        const float* sources, int n_src, int n_rays, int n_bins, float step_size, float c, float dt,
+                        int n_steps, double* tangent, int n_threads) {
+    if (!j || !kappa || !dkappa || !sources || !tangent) return -1;
+    if (nx < 1 || ny < 1 || nz < 1 || n_src < 1 || n_rays < 1 || n_bins < 1 || n_steps < 1) return -1;
+    if (bad(step_size) || bad(c) || bad(dt)) return -1;
+    const long Ns = substeps(double(step_size), double(c), double(dt));
+    const double ds = double(step_size);
+    const long N[3] = {nx, ny, nz};
+    const Medium M{j, kappa, nx, ny, nz, n_bins};
+    const size_t grid = size_t(nx) * ny * nz * n_bins;
+    const double scale = double(4.0L * kPiL / (long double)n_rays);
+    const long total_rays = long(n_src) * n_rays;
+    const long T = std::min<long>(std::max(1, n_threads), total_rays);
+    std::vector<std::vector<double>> acc(T);                  // per thread: [n_steps][grid], per-step increments
+    for (auto& a : acc) a.assign(grid * size_t(n_steps), 0.0);
+    auto work = [&](long t) {
+        for (long r = total_rays * t / T; r < total_rays * (t + 1) / T; ++r) {
+            const long s = r / n_rays, i = r % n_rays;
+            double nhat[3];
+            fib_direction(i, n_rays, nhat);
+            fx_t X0[3], D[3];
+            for (int a = 0; a < 3; ++a) {
+                X0[a] = fx(double(sources[3 * s + a]));
+                volatile double step = ds * nhat[a];
+                D[a] = fx(step);
+            }
+            for (long b = 0; b < n_bins; ++b) {
+                double I = 0.0, tau = 0.0, Idot = 0.0, taudot = 0.0;
+                for (long k = 0; k < Ns * n_steps; ++k) {
+                    long lo[3], hi[3];
+                    double f[3];
+                    for (int a = 0; a < 3; ++a) {
+                        const fx_t X = X0[a] + fx_t(k) * D[a];
+                        const long i0 = long((long long)(X >> 64));
+                        f[a] = double((unsigned long long)X) * 5.42101086242752217e-20;
+                        lo[a] = clampl(i0, 0, N[a] - 1);
+                        hi[a] = clampl(i0 + 1, 0, N[a] - 1);
+                    }
+                    size_t corner[8];
+                    double w[8], jv = 0.0;
+                    for (int cc = 0; cc < 8; ++cc) {
+                        int dx = (cc >> 2) & 1, dy = (cc >> 1) & 1, dz = cc & 1;
+                        corner[cc] = M.cell(dx ? hi[0] : lo[0], dy ? hi[1] : lo[1], dz ? hi[2] : lo[2]);
+                        w[cc] = (dx ? f[0] : 1.0 - f[0]) * (dy ? f[1] : 1.0 - f[1]) * (dz ? f[2] : 1.0 - f[2]);
+                        jv += w[cc] * double(j[corner[cc] + b]);
+                    }
+                    const size_t base = M.cell(lo[0], lo[1], lo[2]);
+                    const double kap = double(kappa[base + b]), dkap = double(dkappa[base + b]);
+                    const double att = std::exp(-kap * ds), tr = std::exp(-tau);
+                    Idot = Idot * att + I * (-dkap * ds) * att + jv * (-taudot) * tr * ds;
+                    I = I * att + jv * tr * ds;                              // eq. (2)
+                    taudot += dkap * ds;
+                    tau += kap * ds;
+                    double* slice = acc[t].data() + size_t(k / Ns) * grid;
+                    for (int cc = 0; cc < 8; ++cc) slice[corner[cc] + b] += w[cc] * Idot;
+                }
+            }
+        }
+    };
+    std::vector<std::thread> pool;
+    for (long t = 1; t < T; ++t) pool.emplace_back(work, t);
+    work(0);
+    for (auto& th : pool) th.join();
+    for (size_t v = 0; v < grid; ++v) {
+        double run = 0.0;
+        for (long m = 0; m < n_steps; ++m) {
+            for (long u = 0; u < T; ++u) run += acc[u][size_t(m) * grid + v];
+            tangent[size_t(m) * grid + v] = scale * run;
+        }
+    }
+    return 0;
+}
+
 const char* rt_oracle_version(void) { return "rt_oracle 1 (fp64, PAPER.md eq. 2)"; }
 
 }  // extern "C"

@@ -291,6 +291,9 @@ __device__ __forceinline__ int phase(const MarchParams& P, const BrickGeom& G, P
 #ifndef RT_PHASED_MINB1
 #define RT_PHASED_MINB1 8
 #endif
+#ifndef RT_PHASED_MINB1P
+#define RT_PHASED_MINB1P 6
+#endif
 #ifndef RT_PHASED_MINB4
 #define RT_PHASED_MINB4 4
 #endif
@@ -301,7 +304,7 @@ __device__ __forceinline__ int phase(const MarchParams& P, const BrickGeom& G, P
 // STEP: the rt_march_step form (D17) -- one time step from substep P.k0, (I, exp(-tau)) of every ray loaded
 // from and stored back to the ray state.
 template <int NB, bool TABLE, bool BRICK = (NB == 1), typename ACC = float, bool STEP = false>
-__global__ void __launch_bounds__(kThreads, NB == 1 ? RT_PHASED_MINB1 : RT_PHASED_MINB4)
+__global__ void __launch_bounds__(kThreads, NB == 1 ? (TABLE ? RT_PHASED_MINB1 : RT_PHASED_MINB1P) : RT_PHASED_MINB4)
 march_phased_kernel(const MarchParams P) {
     static_assert(!BRICK || (NB == 1 && sizeof(ACC) == 4), "the brick scratch holds one fp32 bin");
     __shared__ __align__(16) TableRow table[TABLE ? kThreads / 32 : 1][32];

@@ -829,3 +829,49 @@ def test_d19_kappa_gradient_uniform_medium_closed_form(oracle_mod):
     a = math.exp(-k0 * ds)
     want = FOUR_PI * 2 * sum((k + 1) * j0 * ds * k * (-ds) * a ** k for k in range(N))
     assert abs(grad.sum() - want) <= 1e-12 * abs(want)
+
+
+# ------------------------------------------------------------------------------------------------------
+# D21  forward-mode derivative with respect to kappa: pinned by central differences of the (pinned) forward
+#      oracle, by its duality with the (pinned) kappa adjoint, and by a uniform-medium closed form
+# ------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("shape,nb,n_src,n_rays,ds,dt,n_steps", [
+    ((5, 4, 6), 1, 2, 9, 0.5, 4.0, 1),
+    ((4, 5, 3), 2, 1, 7, 0.37, 2.6, 3),          # several cumulative snapshots
+    ((4, 4, 4), 1, 1, 1, 0.5, 5.0, 2),           # axis ray leaving the box (clamped deposits go on)
+])
+def test_d21_jvp_kappa_matches_central_differences_and_the_adjoint(oracle_mod, shape, nb, n_src, n_rays, ds, dt, n_steps):
+    rng = np.random.default_rng(sum(shape) * 11 + nb)
+    kap = np.round(rng.uniform(0.05, 0.6, shape + (nb,)) * 1024) / 1024        # exactly representable with room for eps
+    j = rng.uniform(0.1, 1.0, shape + (nb,)).astype(np.float32)
+    src = rng.uniform(0.0, min(shape) - 1.0, (n_src, 3)).astype(np.float32)
+    args = (src, n_rays, ds, 1.0, dt, n_steps)
+    eps = 2.0 ** -12
+    for trial in range(3):
+        d = np.round(rng.uniform(-1.0, 1.0, kap.shape) * 16) / 16
+        tang = oracle_mod.jvp_kappa(j, kap.astype(np.float32), d.astype(np.float32), *args)
+        fd = (oracle_mod.march(j, (kap + eps * d).astype(np.float32), *args) -
+              oracle_mod.march(j, (kap - eps * d).astype(np.float32), *args)) / (2 * eps)
+        assert np.abs(tang - fd).max() <= 2e-6 * np.abs(fd).max(), np.abs(tang - fd).max() / np.abs(fd).max()
+        # duality: <g, J d> = <J^T g, d> with J^T g from the kappa adjoint (pinned on its own above)
+        g = rng.standard_normal(tang.shape)
+        lhs = float((g * tang).sum())
+        rhs = float((oracle_mod.adjoint_kappa(g, j, kap.astype(np.float32), *args) * d).sum())
+        assert abs(lhs - rhs) <= 1e-11 * max(abs(lhs), np.abs(g * tang).sum() * 1e-3), (lhs, rhs)
+
+
+def test_d21_global_kappa_scale_uniform_medium_closed_form(oracle_mod):
+    """The paper's example of a further parameter ("a global kappa scale"): kappa = theta kappa0, uniform j0.  Every
+    ray has I_k = k j0 ds a^(k-1), a = exp(-theta kappa0 ds) (pin P1), every substep deposits total weight 1 (P2), so
+    sum(out) = 4 pi n_src j0 ds sum_{k=1..N} k a^(k-1) and
+    d/dtheta sum(out) = 4 pi n_src j0 ds sum_k k (k-1) a^(k-2) (-kappa0 ds a); the tangent for dkappa = kappa sums to it."""
+    n, j0, k0, ds, N = 9, 0.3, 0.2, 0.5, 14
+    j = np.full((n, n, n, 1), j0, dtype=np.float32)
+    kap = np.full((n, n, n, 1), k0, dtype=np.float32)
+    src = np.array([[4.0, 4.0, 4.0], [1.5, 6.25, 3.0]], dtype=np.float32)
+    tang = oracle_mod.jvp_kappa(j, kap, kap, src, 24, ds, 1.0, N * ds, 1)
+    a = np.exp(-float(np.float32(k0)) * ds)
+    j0f, k0f = float(np.float32(j0)), float(np.float32(k0))
+    want = 4 * np.pi * len(src) * j0f * ds * sum(k * (k - 1) * a ** (k - 2) for k in range(1, N + 1)) * (-k0f * ds * a)
+    assert abs(tang.sum() - want) <= 1e-12 * abs(want), (tang.sum(), want)
+    assert (tang <= 0).all()                      # more absorption, less field, everywhere
