@@ -9,7 +9,7 @@ prefix) over the full workload.  Default workload = BASELINE.json configs[2] ("C
 One JSON line is printed by rank 0; see DESIGN.md §8 for every field.  Besides the headline (C2) the default
 single-GPU run also times, a few steps each, the other large configs (`per_config`: C3, C4, and C2 with its sources
 jittered off the cell nodes -- the general-position cost of the headline) and the other entry points on C2
-(`modes`: step, trilinear_kappa, adjoint_j, adjoint_kappa), each with its own roofline and a checksum
+(`modes`: step, trilinear_kappa, adjoint_j, adjoint_kappa, jvp_kappa), each with its own roofline and a checksum
 (--no-extras skips them).
 
 N > 1 (under torchrun): weak scaling — rank r marches sources [r*n_src, (r+1)*n_src) of the N*n_src
@@ -45,7 +45,7 @@ def parse():
     ap.add_argument("--config", default="C2", choices=["C0", "C1", "C2", "C3", "C4"])
     ap.add_argument("--impl", default="native", choices=["native", "reference"])
     ap.add_argument("--variant", type=int, default=0, help="RT_VARIANT_* (0 = the product path)")
-    ap.add_argument("--mode", default="march", choices=["march", "step", "trilinear_kappa", "adjoint_j", "adjoint_kappa"],
+    ap.add_argument("--mode", default="march", choices=["march", "step", "trilinear_kappa", "adjoint_j", "adjoint_kappa", "jvp_kappa"],
                     help="march: one rt_march call per bench step (the headline); step: the same workload as n_steps "
                          "rt_march_step calls with persistent ray state (DESIGN.md D17); trilinear_kappa: "
                          "rt_march_trilinear_kappa (DESIGN.md D18); adjoint_j: rt_march_adjoint_j, dL/dj for a "
@@ -232,6 +232,9 @@ class Case:
             self.result = torch.empty((nx, ny, nz, nb), dtype=torch.float32, device="cuda")
             nbytes = (rt.rt_adjoint_workspace_bytes(nx, ny, nz, n_src, w.n_rays, nb, w.n_steps) if mode == "adjoint_j" else
                       rt.rt_adjoint_kappa_workspace_bytes(nx, ny, nz, n_src, w.n_rays, nb, w.step_size, w.c, w.dt, w.n_steps))
+        elif mode == "jvp_kappa":          # the paper's "global kappa scale": dkappa = kappa
+            self.result = torch.empty((w.n_steps, nx, ny, nz, nb), dtype=torch.float32, device="cuda")
+            nbytes = rt.rt_workspace_bytes(nx, ny, nz, n_src, w.n_rays, nb, w.n_steps)
         elif mode == "step":
             self.state = rt.rt_state_reset(n_src, w.n_rays, nb)
             self.result = torch.empty((nx, ny, nz, nb), dtype=torch.float32, device="cuda")
@@ -254,6 +257,8 @@ class Case:
             for m in range(w.n_steps):
                 rt.rt_march_step(self.j, self.kappa, self.src, *a, m * w.substeps_per_step, self.state, out=self.result,
                                  accumulate=bool(m), workspace=self.ws)
+        elif self.mode == "jvp_kappa":
+            rt.rt_march_jvp_kappa(self.j, self.kappa, self.kappa, self.src, *a, w.n_steps, tangent=self.result, workspace=self.ws)
         elif self.mode == "trilinear_kappa":
             rt.rt_march_trilinear_kappa(self.j, self.kappa, self.src, *a, w.n_steps, out=self.result, workspace=self.ws)
         else:
@@ -500,7 +505,7 @@ def run_extras(rt, torch, w_c2, flush, steps):
         torch.cuda.empty_cache()
         return row
 
-    modes = {m: measure(w_c2, w_c2.sources, m) for m in ("step", "trilinear_kappa", "adjoint_j", "adjoint_kappa")}
+    modes = {m: measure(w_c2, w_c2.sources, m) for m in ("step", "trilinear_kappa", "adjoint_j", "adjoint_kappa", "jvp_kappa")}
     per_config = {}
     jit = (w_c2.sources.astype(np.float64) + np.random.default_rng(939912).uniform(-0.5, 0.5, w_c2.sources.shape))
     jit = np.clip(jit, 0.0, w_c2.shape[0] - 1.0).astype(np.float32)

@@ -135,6 +135,19 @@ int rt_march_adjoint_kappa(const float* gbar, const float* j, const float* kappa
                            float step_size, float c, float dt, int n_steps, float* grad_kappa,
                            void* workspace, size_t workspace_bytes, void* stream);
 
+/* FORWARD-MODE DERIVATIVE WITH RESPECT TO kappa (gradients "from jacfwd", "a global kappa scale"; DESIGN.md
+ * reading D21).  Writes tangent[n_steps][nx][ny][nz][n_bins] = d/d eps of rt_march(j, kappa + eps dkappa, ...) at eps = 0
+ * (device, fp32, OVERWRITTEN; cumulative snapshots like out).  dkappa has kappa's shape and layout; a global scale
+ * kappa -> theta kappa is dkappa = kappa.  The tangent of eq. (2) -- Idot_{k+1} = a_k (Idot_k - I_k dkappa_k ds) - j(x_k)
+ * taudot_k exp(-tau_k) ds, taudot_{k+1} = taudot_k + dkappa_k ds, kappa and dkappa read at the cell of x_k -- is marched
+ * next to eq. (2) and deposited with the weights of x_k.  <gbar, tangent> = <rt_march_adjoint_kappa(gbar), dkappa> up to
+ * rounding.  Argument rules, limits, error codes and workspace (rt_workspace_bytes) as rt_march, and step_size must be
+ * below one cell (RT_EINVAL otherwise). */
+int rt_march_jvp_kappa(const float* j, const float* kappa, const float* dkappa, int nx, int ny, int nz,
+                       const float* sources, int n_src, int n_rays, int n_bins,
+                       float step_size, float c, float dt, int n_steps, float* tangent,
+                       void* workspace, size_t workspace_bytes, void* stream);
+
 /* TEST HOOK.  rt_march_adjoint_kappa with the bound on the forward record of one source batch given explicitly
  * (record_limit bytes; 0 = the library's 2 GiB), so that tests can drive the source-batch loop on small cases.  A batch
  * never holds fewer than 32 sources (n_src >= 32) or 1 source (n_src < 32).  Same result for every limit. */

@@ -13,7 +13,7 @@ _BINDING_NAMES = (
     "RT_VARIANT_SLIDING_BY_SOURCE", "RT_VARIANT_SLIDING_LATTICE", "RtError", "alloc_workspace", "library_path",
     "rt_bench_red_ceiling", "rt_directions", "rt_host_release", "rt_launch_count", "rt_adjoint_kappa_workspace_bytes",
     "rt_adjoint_kappa_workspace_bytes_ex", "rt_adjoint_workspace_bytes", "rt_march", "rt_march_adjoint_j",
-    "rt_march_adjoint_kappa", "rt_march_adjoint_kappa_ex", "rt_march_ex", "rt_march_host", "rt_march_single",
+    "rt_march_adjoint_kappa", "rt_march_adjoint_kappa_ex", "rt_march_ex", "rt_march_jvp_kappa", "rt_march_host", "rt_march_single",
     "rt_march_step", "rt_march_trilinear_kappa", "rt_state_bytes", "rt_state_reset", "rt_step_workspace_bytes",
     "rt_ray_order", "rt_ray_slots", "rt_strerror", "rt_substeps_per_step", "rt_trace_ray", "rt_version",
     "rt_workspace_bytes")

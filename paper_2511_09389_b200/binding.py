@@ -27,7 +27,7 @@ EXPORTS = ("rt_march", "rt_march_single", "rt_march_ex", "rt_march_host", "rt_wo
            "rt_bench_red_ceiling", "rt_strerror", "rt_version", "rt_state_bytes", "rt_state_reset",
            "rt_step_workspace_bytes", "rt_march_step", "rt_march_trilinear_kappa", "rt_adjoint_workspace_bytes",
            "rt_march_adjoint_j", "rt_adjoint_kappa_workspace_bytes", "rt_march_adjoint_kappa",
-           "rt_adjoint_kappa_workspace_bytes_ex", "rt_march_adjoint_kappa_ex", "rt_host_release")
+           "rt_adjoint_kappa_workspace_bytes_ex", "rt_march_adjoint_kappa_ex", "rt_march_jvp_kappa", "rt_host_release")
 
 
 class RtError(RuntimeError):
@@ -60,6 +60,7 @@ def _load() -> ctypes.CDLL:
     L.rt_adjoint_kappa_workspace_bytes_ex.argtypes = [i] * 6 + [f, f, f, i, sz]
     L.rt_adjoint_kappa_workspace_bytes_ex.restype = sz
     L.rt_march_adjoint_kappa_ex.argtypes = [vp] + march_args + [vp, sz, vp, sz]
+    L.rt_march_jvp_kappa.argtypes = [vp, vp, vp, i, i, i, vp, i, i, i, f, f, f, i, vp, vp, sz, vp]
     L.rt_march_single.argtypes = [vp, vp, i, i, i, vp, i, i, f, f, f, i, vp, vp, sz, vp]
     L.rt_march_ex.argtypes = march_args + [vp, sz, vp, i]
     L.rt_march_host.argtypes = march_args
@@ -240,6 +241,29 @@ def rt_march_trilinear_kappa(j, kappa, sources, n_rays, step_size, c, dt, n_step
     """rt_march with kappa read trilinearly (D18)."""
     return rt_march_ex(j, kappa, sources, n_rays, step_size, c, dt, n_steps, out, workspace, stream,
                        _entry=_lib.rt_march_trilinear_kappa)
+
+
+def rt_march_jvp_kappa(j, kappa, dkappa, sources, n_rays, step_size, c, dt, n_steps, tangent=None, workspace=None,
+                       stream=None):
+    """tangent[n_steps,nx,ny,nz,n_bins] = d/d eps rt_march(j, kappa + eps dkappa) at eps = 0 (D21)."""
+    torch = _torch()
+    _check_dev(j, "j", torch.float32, 4)
+    _check_dev(kappa, "kappa", torch.float32, 4)
+    _check_dev(dkappa, "dkappa", torch.float32, 4)
+    _check_dev(sources, "sources", torch.float32, 2)
+    if kappa.shape != j.shape or dkappa.shape != j.shape or sources.shape[1] != 3:
+        raise ValueError("kappa and dkappa must have j's shape and sources must be [n_src, 3]")
+    nx, ny, nz, nb = j.shape
+    n_src = sources.shape[0]
+    with _Call(stream, j, kappa, dkappa, sources) as call:
+        tangent = _out_or_new(call, tangent, (n_steps, nx, ny, nz, nb), "tangent")
+        workspace = _workspace_or_new(call, workspace, rt_workspace_bytes(nx, ny, nz, n_src, n_rays, nb, n_steps))
+        rc = _lib.rt_march_jvp_kappa(j.data_ptr(), kappa.data_ptr(), dkappa.data_ptr(), nx, ny, nz, sources.data_ptr(), n_src,
+                                     n_rays, nb, step_size, c, dt, n_steps, tangent.data_ptr(), workspace.data_ptr(),
+                                     workspace.numel(), call.stream_ptr)
+    if rc != RT_OK:
+        raise RtError(rc, "rt_march_jvp_kappa")
+    return tangent
 
 
 def rt_adjoint_workspace_bytes(nx, ny, nz, n_src, n_rays, n_bins, n_steps) -> int:

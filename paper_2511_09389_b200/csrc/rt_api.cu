@@ -285,6 +285,13 @@ size_t step_scratch_bytes(long long cells, int n_bins) {
 // the instantiation of march_phased_kernel for a deposit mode (phased_kind)
 template <bool TABLE, bool STEP>
 int launch_phased(const rt::MarchParams& P, int kind, unsigned blocks, cudaStream_t st) {
+    if (P.dkappa) {                    // rt_march_jvp_kappa: one bin per thread in both deposit modes
+        if (STEP || kind == kPhasedFourBins) return RT_EINVAL;
+        if (kind == kPhasedOneBin) rt::march_phased_kernel<1, TABLE, true, float, false, true><<<blocks, rt::kThreads, 0, st>>>(P);
+        else rt::march_phased_kernel<1, TABLE, false, double, false, true><<<blocks, rt::kThreads, 0, st>>>(P);
+        RT_CUDA(cudaGetLastError());
+        return RT_OK;
+    }
     if (kind == kPhasedOneBin) rt::march_phased_kernel<1, TABLE, true, float, STEP><<<blocks, rt::kThreads, 0, st>>>(P);
     else if (kind == kPhasedFourBins) rt::march_phased_kernel<4, TABLE, false, float, STEP><<<blocks, rt::kThreads, 0, st>>>(P);
     else rt::march_phased_kernel<1, TABLE, false, double, STEP><<<blocks, rt::kThreads, 0, st>>>(P);
@@ -294,7 +301,8 @@ int launch_phased(const rt::MarchParams& P, int kind, unsigned blocks, cudaStrea
 
 int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const float* sources, int n_src, int n_rays,
                int n_bins, float step_size, float c, float dt, int n_steps, float* out, void* workspace,
-               size_t workspace_bytes, void* stream, int variant, const StepArgs* step = nullptr) {
+               size_t workspace_bytes, void* stream, int variant, const StepArgs* step = nullptr,
+               const float* dkappa = nullptr) {
     Checked ck;
     const int rc = check_args(j, kappa, nx, ny, nz, sources, n_src, n_rays, n_bins, step_size, c, dt, n_steps, out, &ck);
     if (rc != RT_OK) return rc;
@@ -333,7 +341,12 @@ int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const
     const bool vec4 = aligned4 && !pl.one_bin && (batched || !pl.acc64 || !pl.sliding);
     P.n_groups = vec4 ? n_bins / 4 : n_bins;
 
-    const int phased = phased_kind(variant, step_size, ck.cells, n_steps, n_bins, wl.brick_bytes, aligned4);
+    int phased = phased_kind(variant, step_size, ck.cells, n_steps, n_bins, wl.brick_bytes, aligned4);
+    if (dkappa) {                      // the tangent march exists in the phased kernel only, one bin per thread
+        if (phased == kPhasedNone || step) return RT_EINVAL;
+        if (phased == kPhasedFourBins) phased = kPhasedDirect64;
+        P.dkappa = dkappa;
+    }
     if (phased != kPhasedNone) {
         // rt_march proper (and rt_march_step): the phased march deposits into an fp32 scratch -- window bricks in the
         // workspace (one bin), or the plain grid (four bins per thread; `out` itself, or for rt_march_step, whose `out` may
@@ -480,6 +493,16 @@ int rt_march_trilinear_kappa(const float* j, const float* kappa, int nx, int ny,
                              void* workspace, size_t workspace_bytes, void* stream) {
     return march_impl(j, kappa, nx, ny, nz, sources, n_src, n_rays, n_bins, step_size, c, dt, n_steps, out, workspace,
                       workspace_bytes, stream, kVariantKappaTrilinear);
+}
+
+int rt_march_jvp_kappa(const float* j, const float* kappa, const float* dkappa, int nx, int ny, int nz, const float* sources,
+                       int n_src, int n_rays, int n_bins, float step_size, float c, float dt, int n_steps, float* tangent,
+                       void* workspace, size_t workspace_bytes, void* stream) {
+    if (!dkappa) return RT_EINVAL;
+    if (uintptr_t(dkappa) & 3u) return RT_EALIGN;
+    if (!(step_size < 1.0f)) return RT_EINVAL;         // (argument order: the other checks are march_impl's)
+    return march_impl(j, kappa, nx, ny, nz, sources, n_src, n_rays, n_bins, step_size, c, dt, n_steps, tangent, workspace,
+                      workspace_bytes, stream, RT_VARIANT_DEFAULT, nullptr, dkappa);
 }
 
 int rt_march_single(const float* j, const float* kappa, int nx, int ny, int nz, const float* source_pos, int n_rays,

@@ -13,6 +13,7 @@ namespace rt {
 struct MarchParams {
     const float* j;
     const float* kappa;
+    const float* dkappa;         // rt_march_jvp_kappa: the direction kappa is perturbed in (same layout), else nullptr
     const float* sources;        // [n_src][3]
     void* acc;                   // accumulation grid [n_steps][nx][ny][nz][nb], float or double: per-step INCREMENTS
     const uint32_t* ray_order;   // [n_slots] slot -> lattice index (0xFFFFFFFF = padding) or nullptr = identity

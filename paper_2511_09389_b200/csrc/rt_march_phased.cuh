@@ -74,10 +74,11 @@ __host__ __device__ constexpr int slot_rank(int s, int bits) {
 }
 
 // The state one lane carries through the march
-template <int NB, typename ACC = float> struct PhasedLane {
+template <int NB, typename ACC = float, bool JVP = false> struct PhasedLane {
     Stencil<NB, ACC, false> S;
     TravelAxis A[3];         // TABLE: only the cell word, dl and fmask are used
     float I[NB], T[NB], att[NB];   // I scaled by 4 pi/N_Omega; T = exp(-tau) ds 4 pi/N_Omega; att = exp(-kappa ds) of the kappa cell
+    float Id[JVP ? NB : 1], Td[JVP ? NB : 1], u[JVP ? NB : 1];     // JVP (D21): tangents of I and T, and dkappa ds of the kappa cell
     ACC* sg;                 // scratch (fp64 grid if ACC = double) of the current time step
     int woff;                // NB == 1: float offset in it of the window the trailing slots start (rt_brick.cuh)
     int g;                   // substep index since x_0
@@ -122,8 +123,8 @@ template <int ACT> struct BrickView {
 // L.woff is the window that starts at (lower y index, lower z index) of the trailing x slot; the leading x slot is one
 // x step on (if x is merged its sums are exact zeros and nothing is issued); a y-slide uses the window that starts at
 // the trailing row itself, a z-slide the one that starts at the trailing column.
-template <int AX, int ACT>
-__device__ __forceinline__ void brick_flush(const BrickGeom& G, PhasedLane<1>& L, int negbits) {
+template <int AX, int ACT, bool JVP>
+__device__ __forceinline__ void brick_flush(const BrickGeom& G, PhasedLane<1, float, JVP>& L, int negbits) {
     const BrickView<ACT> V{L.S, (negbits & 2) != 0, (negbits & 4) != 0};
     const int dx = (negbits & 1) ? -G.sx : G.sx;
     float* w0 = L.sg + L.woff;
@@ -156,24 +157,30 @@ __device__ __forceinline__ void brick_flush(const BrickGeom& G, PhasedLane<1>& L
 }
 
 // One stencil slide of the lane along axis AX, the trailing plane reduced into the scratch
-template <int AX, int ACT, int NB, bool BRICK, typename ACC>
-__device__ __forceinline__ void phased_axis_step(const MarchParams& P, const BrickGeom& G, PhasedLane<NB, ACC>& L, int negbits) {
+template <int AX, int ACT, int NB, bool BRICK, typename ACC, bool JVP>
+__device__ __forceinline__ void phased_axis_step(const MarchParams& P, const BrickGeom& G, PhasedLane<NB, ACC, JVP>& L, int negbits) {
     if constexpr (BRICK)
-        L.S.template axis_step_with<AX, ACT>(P, L.A, negbits, P.j, [&]() { brick_flush<AX, ACT>(G, L, negbits); });
+        L.S.template axis_step_with<AX, ACT>(P, L.A, negbits, P.j, [&]() { brick_flush<AX, ACT, JVP>(G, L, negbits); });
     else
         L.S.template axis_step<AX, ACT>(P, L.A, negbits, L.sg, P.j);        // per voxel: one red.v4.f32 (red.f32) of its bins
 }
 
-template <int NB, typename ACC> __device__ __forceinline__ void phased_load_att(const MarchParams& P, PhasedLane<NB, ACC>& L, int ko) {
+template <int NB, typename ACC, bool JVP>
+__device__ __forceinline__ void phased_load_att(const MarchParams& P, PhasedLane<NB, ACC, JVP>& L, int ko) {
     const BinVec<NB> kap = ld_bins<NB>(P.kappa + ko);
 #pragma unroll
     for (int b = 0; b < NB; ++b) L.att[b] = ex2_approx(kap.v[b] * P.att_scale);
+    if constexpr (JVP) {
+        const BinVec<NB> dk = ld_bins<NB>(P.dkappa + ko);
+#pragma unroll
+        for (int b = 0; b < NB; ++b) L.u[b] = dk.v[b] * P.ds_f;
+    }
 }
 
 // The substep loop with the axes in ACT active; runs until the table runs out (TABLE), the time step ends or an
 // axis goes inactive, and returns the new set of active axes.
-template <int ACT, int NB, bool TABLE, bool BRICK, typename ACC, bool STEP>
-__device__ __forceinline__ int phase(const MarchParams& P, const BrickGeom& G, PhasedLane<NB, ACC>& L, int negbits,
+template <int ACT, int NB, bool TABLE, bool BRICK, typename ACC, bool STEP, bool JVP>
+__device__ __forceinline__ int phase(const MarchParams& P, const BrickGeom& G, PhasedLane<NB, ACC, JVP>& L, int negbits,
                                      uint32_t tbase) {
     constexpr int kBits = ((ACT & 1) ? 4 : 0) | ((ACT & 2) ? 2 : 0) | ((ACT & 4) ? 1 : 0);      // slot index bits in use
     constexpr int kActive = ((ACT & 1) ? 1 : 0) + ((ACT & 2) ? 1 : 0) + ((ACT & 4) ? 1 : 0);
@@ -240,13 +247,20 @@ __device__ __forceinline__ int phase(const MarchParams& P, const BrickGeom& G, P
                         else jv = (r == 0) ? w[s] * jc : fmaf(w[s], jc, jv);
                     }
             }
+            if constexpr (JVP) {
+                // the tangent of eq. (2) for kappa -> kappa + eps dkappa (D21), u = dkappa_k ds:
+                //   Idot_{k+1} = a_k (Idot_k - I_k u) + J_k Tdot_k,   Tdot_{k+1} = a_k (Tdot_k - T_k u)      (old I, T on the right)
+                L.Id[b] = fmaf(L.att[b], fmaf(-L.I[b], L.u[b], L.Id[b]), (jv + ju) * L.Td[b]);
+                L.Td[b] = L.att[b] * fmaf(-L.T[b], L.u[b], L.Td[b]);
+            }
             // eq. (2).  STEP: T is the carried exp(-tau) itself, else ds 4 pi/N_Omega rides on it
             L.I[b] = fmaf(L.I[b], L.att[b], STEP ? (jv + ju) * L.T[b] * P.emis : (jv + ju) * L.T[b]);
             L.T[b] *= L.att[b];
+            const float dep = JVP ? L.Id[b] : L.I[b];           // what is deposited, with the weights of x_k
 #pragma unroll
             for (int s = 0; s < 8; ++s)
                 if ((s & ~kBits) == 0)
-                    L.S.acc[s].v[b] = (ACT == 0) ? L.S.acc[s].v[b] + L.I[b] : fmaf(w[s], L.I[b], L.S.acc[s].v[b]);
+                    L.S.acc[s].v[b] = (ACT == 0) ? L.S.acc[s].v[b] + dep : fmaf(w[s], dep, L.S.acc[s].v[b]);
         }
 
         if constexpr (ACT != 0) {
@@ -255,9 +269,9 @@ __device__ __forceinline__ int phase(const MarchParams& P, const BrickGeom& G, P
                 for (int a = 0; a < 3; ++a)
                     if ((ACT & (1 << a)) && cross[a]) {
                         if constexpr (TABLE) L.A[a].p.c += 1;
-                        if (a == 0) phased_axis_step<0, ACT, NB, BRICK, ACC>(P, G, L, negbits);
-                        if (a == 1) phased_axis_step<1, ACT, NB, BRICK, ACC>(P, G, L, negbits);
-                        if (a == 2) phased_axis_step<2, ACT, NB, BRICK, ACC>(P, G, L, negbits);
+                        if (a == 0) phased_axis_step<0, ACT, NB, BRICK, ACC, JVP>(P, G, L, negbits);
+                        if (a == 1) phased_axis_step<1, ACT, NB, BRICK, ACC, JVP>(P, G, L, negbits);
+                        if (a == 2) phased_axis_step<2, ACT, NB, BRICK, ACC, JVP>(P, G, L, negbits);
                         if constexpr (TABLE) {       // every lane crosses in the same substep: vote right here
                             const int lim = (a == 0 ? P.nx : (a == 1 ? P.ny : P.nz)) - 1;
                             const bool gone = L.A[a].p.c >= ((negbits & (1 << a)) ? 0 : lim);    // beyond the far face for good
@@ -268,7 +282,7 @@ __device__ __forceinline__ int phase(const MarchParams& P, const BrickGeom& G, P
                 if (ACT & 1) ko += (negbits & 1) ? L.A[0].dl : 0;
                 if (ACT & 2) ko += (negbits & 2) ? L.A[1].dl : 0;
                 if (ACT & 4) ko += (negbits & 4) ? L.A[2].dl : 0;
-                phased_load_att<NB, ACC>(P, L, ko);
+                phased_load_att<NB, ACC, JVP>(P, L, ko);
             }
             if constexpr (!TABLE) {
                 if ((L.g & 7) == 7) {        // lanes cross at different substeps: vote every 8th substep
@@ -303,7 +317,9 @@ __device__ __forceinline__ int phase(const MarchParams& P, const BrickGeom& G, P
 // nothing is drained: for grids far larger than the L2, where a scratch would only add HBM traffic.
 // STEP: the rt_march_step form (D17) -- one time step from substep P.k0, (I, exp(-tau)) of every ray loaded
 // from and stored back to the ray state.
-template <int NB, bool TABLE, bool BRICK = (NB == 1), typename ACC = float, bool STEP = false>
+// JVP: the rt_march_jvp_kappa form (D21) -- the tangent of I for kappa -> kappa + eps P.dkappa is carried
+// next to I and deposited instead of it.
+template <int NB, bool TABLE, bool BRICK = (NB == 1), typename ACC = float, bool STEP = false, bool JVP = false>
 __global__ void __launch_bounds__(kThreads, NB == 1 ? (TABLE ? RT_PHASED_MINB1 : RT_PHASED_MINB1P) : RT_PHASED_MINB4)
 march_phased_kernel(const MarchParams P) {
     static_assert(!BRICK || (NB == 1 && sizeof(ACC) == 4), "the brick scratch holds one fp32 bin");
@@ -324,7 +340,7 @@ march_phased_kernel(const MarchParams P) {
         const uint32_t lindex = __shfl_sync(0xFFFFFFFFu, id.index, leader);
         if (!live) { id.src = lsrc; id.group = lgroup; id.index = lindex; }
 
-        PhasedLane<NB, ACC> L;
+        PhasedLane<NB, ACC, JVP> L;
         L.sg = sizeof(ACC) == 4 ? reinterpret_cast<ACC*>(P.scratch) : static_cast<ACC*>(P.acc);
         int negbits = 0;
         {
@@ -349,13 +365,17 @@ march_phased_kernel(const MarchParams P) {
         L.S.restart(P, L.A, negbits, id.group * NB, P.j);
 #pragma unroll
         for (int b = 0; b < NB; ++b) { L.I[b] = 0.0f; L.T[b] = live ? P.emis : 0.0f; }       // ds 4 pi/N_Omega rides on exp(-tau)
+        if constexpr (JVP) {
+#pragma unroll
+            for (int b = 0; b < NB; ++b) { L.Id[b] = 0.0f; L.Td[b] = 0.0f; }
+        }
         const size_t state_at = (size_t(id.src) * P.n_rays + id.index) * P.nb + size_t(id.group) * NB;
         if (STEP && live) {                  // the ray's (I, exp(-tau)) carried from the previous call
             const BinVec<NB> si = ld_bins<NB>(P.state_I + state_at), sT = ld_bins<NB>(P.state_T + state_at);
 #pragma unroll
             for (int b = 0; b < NB; ++b) { L.I[b] = si.v[b]; L.T[b] = sT.v[b]; }
         }
-        phased_load_att<NB, ACC>(P, L, L.S.base + ((negbits & 1) ? L.A[0].dl : 0) + ((negbits & 2) ? L.A[1].dl : 0) +
+        phased_load_att<NB, ACC, JVP>(P, L, L.S.base + ((negbits & 1) ? L.A[0].dl : 0) + ((negbits & 2) ? L.A[1].dl : 0) +
                                       ((negbits & 4) ? L.A[2].dl : 0));
         L.g = 0;
         L.left = P.n_sub;
@@ -404,18 +424,18 @@ march_phased_kernel(const MarchParams P) {
                 }
             }
             switch (act) {
-                case 7: act = phase<7, NB, TABLE, BRICK, ACC, STEP>(P, G, L, negbits, tbase); break;
-                case 6: act = phase<6, NB, TABLE, BRICK, ACC, STEP>(P, G, L, negbits, tbase); break;
-                case 5: act = phase<5, NB, TABLE, BRICK, ACC, STEP>(P, G, L, negbits, tbase); break;
-                case 4: act = phase<4, NB, TABLE, BRICK, ACC, STEP>(P, G, L, negbits, tbase); break;
-                case 3: act = phase<3, NB, TABLE, BRICK, ACC, STEP>(P, G, L, negbits, tbase); break;
-                case 2: act = phase<2, NB, TABLE, BRICK, ACC, STEP>(P, G, L, negbits, tbase); break;
-                case 1: act = phase<1, NB, TABLE, BRICK, ACC, STEP>(P, G, L, negbits, tbase); break;
-                default: act = phase<0, NB, TABLE, BRICK, ACC, STEP>(P, G, L, negbits, tbase); break;
+                case 7: act = phase<7, NB, TABLE, BRICK, ACC, STEP, JVP>(P, G, L, negbits, tbase); break;
+                case 6: act = phase<6, NB, TABLE, BRICK, ACC, STEP, JVP>(P, G, L, negbits, tbase); break;
+                case 5: act = phase<5, NB, TABLE, BRICK, ACC, STEP, JVP>(P, G, L, negbits, tbase); break;
+                case 4: act = phase<4, NB, TABLE, BRICK, ACC, STEP, JVP>(P, G, L, negbits, tbase); break;
+                case 3: act = phase<3, NB, TABLE, BRICK, ACC, STEP, JVP>(P, G, L, negbits, tbase); break;
+                case 2: act = phase<2, NB, TABLE, BRICK, ACC, STEP, JVP>(P, G, L, negbits, tbase); break;
+                case 1: act = phase<1, NB, TABLE, BRICK, ACC, STEP, JVP>(P, G, L, negbits, tbase); break;
+                default: act = phase<0, NB, TABLE, BRICK, ACC, STEP, JVP>(P, G, L, negbits, tbase); break;
             }
             if (L.left == 0) {               // time-step boundary: the increments of this step are complete (rays continue, D7)
                 if constexpr (BRICK) {
-                    brick_flush<-1, 7>(G, L, negbits);           // slots of inactive axes hold exact zeros: skipped by value
+                    brick_flush<-1, 7, JVP>(G, L, negbits);      // slots of inactive axes hold exact zeros: skipped by value
 #pragma unroll
                     for (int s = 0; s < 8; ++s) L.S.zero_slot(s);
                     L.sg += G.step_stride;

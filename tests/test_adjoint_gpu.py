@@ -264,3 +264,89 @@ def test_relative_mse_amplitude_inversion_on_the_gpu(rt):
     assert abs(A - A_star) <= 2e-4 * abs(A_star), (A, A_star)
     plain = float((F * I_ref).sum() / (F * F).sum())
     assert abs(plain - A_star) > 1e-4 * abs(A_star)        # the weighting matters: another minimiser than the plain MSE's
+
+
+# ------------------------------------------------------------------------------------------------
+# forward mode: rt_march_jvp_kappa (D21)
+# ------------------------------------------------------------------------------------------------
+def _tangent_compare(got, ref, what):
+    """A tangent field has both signs (more absorption: less field; a negative dkappa: more): every snapshot against
+    the largest entry of the oracle's, like the kappa gradient."""
+    for m in range(ref.shape[0]):
+        scale = np.abs(ref[m]).max()
+        rel_l2 = np.linalg.norm(got[m] - ref[m]) / np.linalg.norm(ref[m])
+        worst = np.abs(got[m] - ref[m]).max() / scale
+        assert np.isfinite(got[m]).all(), what
+        assert rel_l2 <= parity.REL_L2_TOL and worst <= parity.REL_L2_TOL, (what, m, rel_l2, worst)
+    return rel_l2, worst
+
+
+@pytest.mark.parametrize("shape,nb,n_src,n_rays,ds,dt,n_steps,integer_sources", [
+    ((4, 4, 4), 1, 1, 1, 0.5, 4.0, 1, True),           # the axis ray through and out of a 4-cube
+    ((5, 4, 3), 3, 2, 7, 0.5, 5.0, 1, False),          # 3 bins: one bin per lane, fp64 reductions
+    ((6, 5, 7), 8, 1, 40, 0.5, 8.0, 3, False),         # source outside the box, three snapshots
+    ((9, 8, 7), 1, 40, 24, 0.25, 4.0, 2, True),        # warp = 32 sources x 1 direction, weight table, brick scratch
+    ((9, 8, 7), 1, 45, 24, 0.25, 4.0, 2, False),       # the same in general position (plain instantiation)
+    ((7, 6, 9), 4, 33, 11, 0.5, 4.0, 2, True),         # 4 bins
+])
+def test_jvp_kappa_matches_the_oracle(rt, oracle_mod, shape, nb, n_src, n_rays, ds, dt, n_steps, integer_sources):
+    rng = np.random.default_rng(sum(shape) + nb + n_src)
+    kap = rng.uniform(0.0, 0.6, shape + (nb,)).astype(np.float32)
+    j = rng.uniform(0.1, 1.0, shape + (nb,)).astype(np.float32)
+    dk = rng.uniform(-1.0, 1.0, shape + (nb,)).astype(np.float32)
+    src = rng.uniform(-2.0, max(shape) + 1.0, (n_src, 3))
+    if integer_sources:
+        src = np.round(src)
+    src = src.astype(np.float32)
+    if n_src == 1 and n_rays == 1:
+        src = np.array([[1.0, 2.0, 1.0]], dtype=np.float32)
+    ref = oracle_mod.jvp_kappa(j, kap, dk, src, n_rays, ds, 1.0, dt, n_steps)
+    got = rt.rt_march_jvp_kappa(_dev(j), _dev(kap), _dev(dk), _dev(src), n_rays, ds, 1.0, dt, n_steps)
+    torch.cuda.synchronize()
+    print(_tangent_compare(got.cpu().numpy().astype(np.float64), ref, f"jvp {shape} nb={nb} n_src={n_src}"))
+
+
+def test_jvp_kappa_on_c1_is_dual_to_the_kappa_adjoint_and_matches_a_difference_quotient(rt, oracle_mod):
+    """C1 in full against the oracle; <g, J dkappa> = <J^T g, dkappa> with J^T g from rt_march_adjoint_kappa; and the
+    paper's global kappa scale (dkappa = kappa) against a central difference of the CUDA march."""
+    w = workloads.make_config("C1")
+    rng = np.random.default_rng(17)
+    j, kap, src = _dev(w.j), _dev(w.kappa), _dev(w.sources)
+    args = (w.n_rays, w.step_size, w.c, w.dt, w.n_steps)
+    dk = (w.kappa * rng.uniform(0.5, 1.5, w.kappa.shape)).astype(np.float32)
+    tang = rt.rt_march_jvp_kappa(j, kap, _dev(dk), src, *args)
+    torch.cuda.synchronize()
+    ref = oracle_mod.jvp_kappa(w.j, w.kappa, dk, w.sources, *args)
+    print(_tangent_compare(tang.cpu().numpy().astype(np.float64), ref, "jvp C1"))
+    g = torch.from_numpy(rng.uniform(0.0, 1.0, tuple(tang.shape)).astype(np.float32)).cuda()
+    grad = rt.rt_march_adjoint_kappa(g, j, kap, src, *args)
+    lhs = float((g.double() * tang.double()).sum())
+    rhs = float((grad.double() * _dev(dk).double()).sum())
+    assert abs(lhs - rhs) <= 2e-5 * abs(lhs), (lhs, rhs)
+    scale = rt.rt_march_jvp_kappa(j, kap, kap, src, *args).double()            # d/d theta of rt_march(j, theta kappa) at 1
+    eps = 1e-2
+    fd = (rt.rt_march(j, (kap * (1 + eps)).contiguous(), src, *args).double() -
+          rt.rt_march(j, (kap * (1 - eps)).contiguous(), src, *args).double()) / (2 * eps)
+    assert float((scale - fd).abs().max()) <= 2e-3 * float(fd.abs().max())
+
+
+def test_jvp_kappa_on_a_c2_subset(rt, oracle_mod):
+    """C2's grid, rays and substeps, 40 of its cell-centred sources: the launch shape of the headline (weight table,
+    brick scratch, drains) carrying the tangent."""
+    w = workloads.make_config("C2")
+    src = np.ascontiguousarray(w.sources[_stratified(w.n_src, 40)])
+    got = rt.rt_march_jvp_kappa(_dev(w.j), _dev(w.kappa), _dev(w.kappa), _dev(src), w.n_rays, w.step_size, w.c, w.dt, w.n_steps)
+    torch.cuda.synchronize()
+    ref = oracle_mod.jvp_kappa(w.j, w.kappa, w.kappa, src, w.n_rays, w.step_size, w.c, w.dt, w.n_steps)
+    print(_tangent_compare(got.cpu().numpy().astype(np.float64), ref, "jvp C2 subset"))
+
+
+def test_jvp_argument_errors(rt):
+    n = 6
+    k = torch.zeros((n, n, n, 1), device="cuda")
+    s = torch.zeros((1, 3), device="cuda")
+    with pytest.raises(rt.RtError) as e:
+        rt.rt_march_jvp_kappa(k, k, k, s, 16, 1.5, 1.0, 3.0, 1)              # substeps of a cell or more: not offered
+    assert e.value.code == rt.RT_EINVAL
+    with pytest.raises(ValueError):
+        rt.rt_march_jvp_kappa(k, k, torch.zeros((n, n, n, 2), device="cuda"), s, 16, 0.5, 1.0, 2.0, 1)
