@@ -350,9 +350,9 @@ int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const
     if (phased != kPhasedNone) {
         // rt_march proper (and rt_march_step): the phased march deposits into an fp32 scratch -- window bricks in the
         // workspace (one bin), or the plain grid (four bins per thread; `out` itself, or for rt_march_step, whose `out` may
-        // hold the running field, a grid behind the workspace) -- and drains it into the fp64 grid as it goes; what is
-        // left is drained after the march; or it reduces straight into the fp64 grid.  The snapshots (the step's
-        // increment) are formed from the fp64 grid.
+        // hold the running field, a grid behind the workspace) -- and drains it into the fp64 grid as it goes; or it
+        // reduces straight into the fp64 grid.  The snapshots (the step's increment) are formed from the fp64 grid plus
+        // what the march left in the scratch.
         P.n_groups = phased == kPhasedFourBins ? n_bins / 4 : n_bins;
         P.acc = master;
         P.scratch = phased == kPhasedOneBin ? reinterpret_cast<float*>(ws + wl.brick_at)
@@ -385,18 +385,24 @@ int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const
         }
         const int rcp = step ? launch_phased<false, true>(P, phased, unsigned(mb2), st) : launch_phased<false, false>(P, phased, unsigned(mb2), st);
         if (rcp != RT_OK) return rcp;
-        long long db = (P.n_drain_units + 255) / 256;
-        if (db > 148 * 16) db = 148 * 16;
-        if (phased == kPhasedOneBin)
-            rt::drain_all_kernel<<<unsigned(db), 256, 0, st>>>(P.scratch, master, rt::brick_geom(nx, ny, nz), nx, ny, nz,
-                                                               P.n_drain_units);
-        else if (phased != kPhasedDirect64)
-            rt::drain_all_plain_kernel<<<unsigned(db), 256, 0, st>>>(P.scratch, master, P.n_drain_units);
-        RT_CUDA(cudaGetLastError());
-        if (step)
-            rt::step_finalize_kernel<<<unsigned(fin_blocks), fin_threads, 0, st>>>(master, out, ck.cells, step->accumulate);
-        else
-            rt::snapshot_finalize_kernel<double><<<unsigned(fin_blocks), fin_threads, 0, st>>>(master, out, ck.cells, n_steps);
+        // the snapshots (the step's increment): the fp64 grid plus what the march left in the scratch, rounded once
+        const rt::BrickGeom G = rt::brick_geom(nx, ny, nz);
+        const unsigned fb = unsigned(fin_blocks);
+        if (step) {
+            if (phased == kPhasedOneBin)
+                rt::step_finalize_scratch_kernel<true><<<fb, fin_threads, 0, st>>>(master, P.scratch, out, ck.cells, step->accumulate, G, ny, nz);
+            else if (phased == kPhasedFourBins)
+                rt::step_finalize_scratch_kernel<false><<<fb, fin_threads, 0, st>>>(master, P.scratch, out, ck.cells, step->accumulate, G, ny, nz);
+            else
+                rt::step_finalize_kernel<<<fb, fin_threads, 0, st>>>(master, out, ck.cells, step->accumulate);
+        } else {
+            if (phased == kPhasedOneBin)
+                rt::snapshot_finalize_scratch_kernel<true><<<fb, fin_threads, 0, st>>>(master, P.scratch, out, ck.cells, n_steps, G, ny, nz);
+            else if (phased == kPhasedFourBins)
+                rt::snapshot_finalize_scratch_kernel<false><<<fb, fin_threads, 0, st>>>(master, P.scratch, out, ck.cells, n_steps, G, ny, nz);
+            else
+                rt::snapshot_finalize_kernel<double><<<fb, fin_threads, 0, st>>>(master, out, ck.cells, n_steps);
+        }
         RT_CUDA(cudaGetLastError());
         return RT_OK;
     }
@@ -790,10 +796,8 @@ int rt_launch_count(int nx, int ny, int nz, int n_src, int n_rays, int n_bins, i
     const Plan pl = default_plan(n_src);
     const int setup = 1 + ((pl.map_src && n_src <= kMaxSortedSources) ? 1 : 0);     // ray order, (source order)
     // the phased march (what rt_march runs when substeps are shorter than a cell): (fraction test, the weight-table
-    // instantiation,) the plain instantiation -- one of the two returns at once --, (the last drain of the scratch,) snapshots
-    const long long cells = (long long)nx * ny * nz * n_bins;
-    const int kind = phased_kind(RT_VARIANT_DEFAULT, 0.5f, cells, n_steps, n_bins, brick_scratch_bytes(nx, ny, nz, n_steps, n_bins), true);
-    return setup + (pl.map_src ? 2 : 0) + 1 + (kind == kPhasedDirect64 ? 0 : 1) + 1;
+    // instantiation,) the plain instantiation -- one of the two returns at once --, snapshots
+    return setup + (pl.map_src ? 2 : 0) + 2;
 }
 
 int rt_directions(int n_rays, double* nhat, void* stream) {

@@ -107,12 +107,53 @@ __device__ __forceinline__ void drain_plain(float* scratch, double* master, long
     }
 }
 
-// the pass after the march: everything that is left in the scratch goes to the fp64 grid
-__global__ void drain_all_kernel(float* scratch, double* master, BrickGeom G, int nx, int ny, int nz, long long n_bricks) {
-    drain_bricks(scratch, master, G, nx, ny, nz, 0, n_bricks, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
+// What the march left in the scratch, read back voxel by voxel when the snapshots are formed (no pass of its own, no
+// atomics: the march is over).  Brick scratch: voxel (x, y, z) is element (a, b) of the four windows (Y0, Z0) =
+// (y + 1 - a, z + 1 - b).  `sm` = scratch of time step m.
+__device__ __forceinline__ double brick_residue(const float* sm, const BrickGeom& G, int x, int y, int z) {
+    const float* w = sm + (long long)x * G.sx + (long long)y * G.sy + 4ll * z;      // window (Y0, Z0) = (y, z)
+    return double(w[3]) + double(w[4 + 2]) + double(w[G.sy + 1]) + double(w[G.sy + 4]);
 }
-__global__ void drain_all_plain_kernel(float* scratch, double* master, long long n_units) {
-    drain_plain(scratch, master, 0, n_units, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
+
+// out[m] <- sum over m' <= m of (acc[m'] + what is left in the scratch of step m'): the per-step increments become
+// the cumulative snapshots (D7), summed in fp64 and rounded once.  BRICK: window-brick scratch (one bin),
+// else the plain grid, which may be `out` itself (an element is read before this thread overwrites it).
+template <bool BRICK>
+__global__ void snapshot_finalize_scratch_kernel(const double* acc, const float* scratch, float* out, long long stride,
+                                                 int n_steps, BrickGeom G, int ny, int nz) {
+    for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < stride;
+         e += (long long)gridDim.x * blockDim.x) {
+        int x = 0, y = 0, z = 0;
+        if (BRICK) {
+            const long long r = e / nz;
+            z = int(e - r * nz);
+            x = int(r / ny);
+            y = int(r - (long long)x * ny);
+        }
+        double run = 0.0;
+        for (int m = 0; m < n_steps; ++m) {
+            run += acc[m * stride + e];
+            run += BRICK ? brick_residue(scratch + m * G.step_stride, G, x, y, z) : double(scratch[m * stride + e]);
+            out[m * stride + e] = float(run);
+        }
+    }
+}
+
+// rt_march_step: out = (accumulate ? out : 0) + float(increment), increment = acc + what is left in the scratch
+template <bool BRICK>
+__global__ void step_finalize_scratch_kernel(const double* acc, const float* scratch, float* out, long long n, int accumulate,
+                                             BrickGeom G, int ny, int nz) {
+    for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < n; e += (long long)gridDim.x * blockDim.x) {
+        double inc = acc[e];
+        if (BRICK) {
+            const long long r = e / nz;
+            const int z = int(e - r * nz), x = int(r / ny), y = int(r - (long long)x * ny);
+            inc += brick_residue(scratch, G, x, y, z);
+        } else {
+            inc += double(scratch[e]);
+        }
+        out[e] = float((accumulate ? double(out[e]) : 0.0) + inc);
+    }
 }
 
 }  // namespace rt

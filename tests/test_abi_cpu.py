@@ -68,10 +68,9 @@ def test_host_side_helpers(rt):
     assert rt.rt_workspace_bytes(16, 16, 16, 1, 64, 1, 1) >= 64 * 4
     assert rt.rt_workspace_bytes(16, 16, 16, 1, 0, 1, 1) == 0
     assert rt.rt_ray_slots(4096) >= 4096 and rt.rt_ray_slots(0) == rt.RT_EINVAL
-    assert rt.rt_launch_count(16, 16, 16, 1, 64, 1, 1) == 4          # ray order, march, last drain of the scratch, snapshots
-    assert rt.rt_launch_count(16, 16, 16, 64, 64, 1, 4) == 7         # + source order, fraction test, the other march instantiation
-    assert rt.rt_launch_count(256, 256, 256, 64, 16384, 4, 8) == 6   # a grid beyond the L2: no scratch, no drain
-    assert rt.rt_launch_count(128, 128, 128, 256, 4096, 8, 2) == 7   # C3: bins in fours, `out` as the fp32 scratch: as the one-bin call
+    assert rt.rt_launch_count(16, 16, 16, 1, 64, 1, 1) == 3          # ray order, march, snapshots
+    assert rt.rt_launch_count(16, 16, 16, 64, 64, 1, 4) == 6         # + source order, fraction test, the other march instantiation
+    assert rt.rt_launch_count(256, 256, 256, 64, 16384, 4, 8) == 6 and rt.rt_launch_count(128, 128, 128, 256, 4096, 8, 2) == 6
     for code in (0, -1, -2, -3, -4, -99):
         assert isinstance(rt.rt_strerror(code), str) and rt.rt_strerror(code)
 
