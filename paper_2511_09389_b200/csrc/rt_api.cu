@@ -214,7 +214,7 @@ bool make_plan(int variant, int n_src, Plan* pl) {
 //                    without): one bin per thread, bins in adjacent lanes, red.global.add.f64 straight into the fp64 grid
 constexpr int kPhasedNone = 0, kPhasedOneBin = 1, kPhasedFourBins = 4, kPhasedDirect64 = 3;
 int phased_kind(int variant, float step_size, long long cells, int n_steps, int n_bins, size_t brick_bytes, bool aligned16) {
-    if (variant != RT_VARIANT_DEFAULT || !(step_size < 1.0f)) return kPhasedNone;
+    if ((variant != RT_VARIANT_DEFAULT && variant != kVariantKappaTrilinear) || !(step_size < 1.0f)) return kPhasedNone;
     if (n_bins == 1 && brick_bytes) return kPhasedOneBin;
     if (n_bins % 4 == 0 && aligned16 && use_batched_fp32(cells, n_steps, n_bins)) return kPhasedFourBins;
     return kPhasedDirect64;
@@ -285,6 +285,13 @@ size_t step_scratch_bytes(long long cells, int n_bins) {
 // the instantiation of march_phased_kernel for a deposit mode (phased_kind)
 template <bool TABLE, bool STEP>
 int launch_phased(const rt::MarchParams& P, int kind, unsigned blocks, cudaStream_t st) {
+    if (P.kappa_trilinear) {           // rt_march_trilinear_kappa: one bin per thread in both deposit modes
+        if (STEP || P.dkappa || kind == kPhasedFourBins) return RT_EINVAL;
+        if (kind == kPhasedOneBin) rt::march_phased_kernel<1, TABLE, true, float, false, false, true><<<blocks, rt::kThreads, 0, st>>>(P);
+        else rt::march_phased_kernel<1, TABLE, false, double, false, false, true><<<blocks, rt::kThreads, 0, st>>>(P);
+        RT_CUDA(cudaGetLastError());
+        return RT_OK;
+    }
     if (P.dkappa) {                    // rt_march_jvp_kappa: one bin per thread in both deposit modes
         if (STEP || kind == kPhasedFourBins) return RT_EINVAL;
         if (kind == kPhasedOneBin) rt::march_phased_kernel<1, TABLE, true, float, false, true><<<blocks, rt::kThreads, 0, st>>>(P);
@@ -343,10 +350,11 @@ int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const
 
     int phased = phased_kind(variant, step_size, ck.cells, n_steps, n_bins, wl.brick_bytes, aligned4);
     if (dkappa) {                      // the tangent march exists in the phased kernel only, one bin per thread
-        if (phased == kPhasedNone || step) return RT_EINVAL;
+        if (phased == kPhasedNone || step || pl.ktri) return RT_EINVAL;
         if (phased == kPhasedFourBins) phased = kPhasedDirect64;
         P.dkappa = dkappa;
     }
+    if (pl.ktri && phased == kPhasedFourBins) phased = kPhasedDirect64;      // the trilinear-kappa march: one bin per thread
     if (phased != kPhasedNone) {
         // rt_march proper (and rt_march_step): the phased march deposits into an fp32 scratch -- window bricks in the
         // workspace (one bin), or the plain grid (four bins per thread; `out` itself, or for rt_march_step, whose `out` may

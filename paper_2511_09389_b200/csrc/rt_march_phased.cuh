@@ -74,8 +74,8 @@ __host__ __device__ constexpr int slot_rank(int s, int bits) {
 }
 
 // The state one lane carries through the march
-template <int NB, typename ACC = float, bool JVP = false> struct PhasedLane {
-    Stencil<NB, ACC, false> S;
+template <int NB, typename ACC = float, bool JVP = false, bool KTRI = false> struct PhasedLane {
+    Stencil<NB, ACC, KTRI> S;
     TravelAxis A[3];         // TABLE: only the cell word, dl and fmask are used
     float I[NB], T[NB], att[NB];   // I scaled by 4 pi/N_Omega; T = exp(-tau) ds 4 pi/N_Omega; att = exp(-kappa ds) of the kappa cell
     float Id[JVP ? NB : 1], Td[JVP ? NB : 1], u[JVP ? NB : 1];     // JVP (D21): tangents of I and T, and dkappa ds of the kappa cell
@@ -97,8 +97,8 @@ template <int AX> __device__ __forceinline__ int aidx(const MarchParams& P, int 
 // slot is the lower element.  The lower index of an axis is (trailing index - 1 on a descending axis), also when the
 // axis is merged: the other element of the pair is then padding or a neighbour and carries the leading slot's exact
 // zero.  Slots on the leading side of an inactive axis (ACT) do not exist: zero.
-template <int ACT> struct BrickView {
-    const Stencil<1, float, false>& S;
+template <int ACT, class STENCIL> struct BrickView {
+    const STENCIL& S;
     bool ny, nz;             // the ray descends y / z
     __device__ __forceinline__ float val(int rx, int ry, int rz) const {
         if ((rx && !(ACT & 1)) || (ry && !(ACT & 2)) || (rz && !(ACT & 4))) return 0.0f;
@@ -123,9 +123,9 @@ template <int ACT> struct BrickView {
 // L.woff is the window that starts at (lower y index, lower z index) of the trailing x slot; the leading x slot is one
 // x step on (if x is merged its sums are exact zeros and nothing is issued); a y-slide uses the window that starts at
 // the trailing row itself, a z-slide the one that starts at the trailing column.
-template <int AX, int ACT, bool JVP>
-__device__ __forceinline__ void brick_flush(const BrickGeom& G, PhasedLane<1, float, JVP>& L, int negbits) {
-    const BrickView<ACT> V{L.S, (negbits & 2) != 0, (negbits & 4) != 0};
+template <int AX, int ACT, class LANE>
+__device__ __forceinline__ void brick_flush(const BrickGeom& G, LANE& L, int negbits) {
+    const BrickView<ACT, decltype(L.S)> V{L.S, (negbits & 2) != 0, (negbits & 4) != 0};
     const int dx = (negbits & 1) ? -G.sx : G.sx;
     float* w0 = L.sg + L.woff;
     float e[2][2];
@@ -157,16 +157,16 @@ __device__ __forceinline__ void brick_flush(const BrickGeom& G, PhasedLane<1, fl
 }
 
 // One stencil slide of the lane along axis AX, the trailing plane reduced into the scratch
-template <int AX, int ACT, int NB, bool BRICK, typename ACC, bool JVP>
-__device__ __forceinline__ void phased_axis_step(const MarchParams& P, const BrickGeom& G, PhasedLane<NB, ACC, JVP>& L, int negbits) {
+template <int AX, int ACT, bool BRICK, class LANE>
+__device__ __forceinline__ void phased_axis_step(const MarchParams& P, const BrickGeom& G, LANE& L, int negbits) {
     if constexpr (BRICK)
-        L.S.template axis_step_with<AX, ACT>(P, L.A, negbits, P.j, [&]() { brick_flush<AX, ACT, JVP>(G, L, negbits); });
+        L.S.template axis_step_with<AX, ACT>(P, L.A, negbits, P.j, [&]() { brick_flush<AX, ACT>(G, L, negbits); });
     else
         L.S.template axis_step<AX, ACT>(P, L.A, negbits, L.sg, P.j);        // per voxel: one red.v4.f32 (red.f32) of its bins
 }
 
-template <int NB, typename ACC, bool JVP>
-__device__ __forceinline__ void phased_load_att(const MarchParams& P, PhasedLane<NB, ACC, JVP>& L, int ko) {
+template <int NB, bool JVP, class LANE>
+__device__ __forceinline__ void phased_load_att(const MarchParams& P, LANE& L, int ko) {
     const BinVec<NB> kap = ld_bins<NB>(P.kappa + ko);
 #pragma unroll
     for (int b = 0; b < NB; ++b) L.att[b] = ex2_approx(kap.v[b] * P.att_scale);
@@ -179,9 +179,8 @@ __device__ __forceinline__ void phased_load_att(const MarchParams& P, PhasedLane
 
 // The substep loop with the axes in ACT active; runs until the table runs out (TABLE), the time step ends or an
 // axis goes inactive, and returns the new set of active axes.
-template <int ACT, int NB, bool TABLE, bool BRICK, typename ACC, bool STEP, bool JVP>
-__device__ __forceinline__ int phase(const MarchParams& P, const BrickGeom& G, PhasedLane<NB, ACC, JVP>& L, int negbits,
-                                     uint32_t tbase) {
+template <int ACT, int NB, bool TABLE, bool BRICK, bool STEP, bool JVP, bool KTRI, class LANE>
+__device__ __forceinline__ int phase(const MarchParams& P, const BrickGeom& G, LANE& L, int negbits, uint32_t tbase) {
     constexpr int kBits = ((ACT & 1) ? 4 : 0) | ((ACT & 2) ? 2 : 0) | ((ACT & 4) ? 1 : 0);      // slot index bits in use
     constexpr int kActive = ((ACT & 1) ? 1 : 0) + ((ACT & 2) ? 1 : 0) + ((ACT & 4) ? 1 : 0);
     constexpr int kLast = (ACT & 4) ? 2 : ((ACT & 2) ? 1 : 0);                                   // the last active axis
@@ -247,6 +246,17 @@ __device__ __forceinline__ int phase(const MarchParams& P, const BrickGeom& G, P
                         else jv = (r == 0) ? w[s] * jc : fmaf(w[s], jc, jv);
                     }
             }
+            if constexpr (KTRI) {            // D18: kappa(x_k) with the weights of j(x_k); one exponential per substep and bin
+                float kv = 0.0f;
+                if constexpr (ACT == 0) {
+                    kv = L.S.kc[0].v[b];
+                } else {
+#pragma unroll
+                    for (int s = 0; s < 8; ++s)
+                        if ((s & ~kBits) == 0) kv = (slot_rank(s, kBits) == 0) ? w[s] * L.S.kc[s].v[b] : fmaf(w[s], L.S.kc[s].v[b], kv);
+                }
+                L.att[b] = ex2_approx(kv * P.att_scale);
+            }
             if constexpr (JVP) {
                 // the tangent of eq. (2) for kappa -> kappa + eps dkappa (D21), u = dkappa_k ds:
                 //   Idot_{k+1} = a_k (Idot_k - I_k u) + J_k Tdot_k,   Tdot_{k+1} = a_k (Tdot_k - T_k u)      (old I, T on the right)
@@ -269,20 +279,22 @@ __device__ __forceinline__ int phase(const MarchParams& P, const BrickGeom& G, P
                 for (int a = 0; a < 3; ++a)
                     if ((ACT & (1 << a)) && cross[a]) {
                         if constexpr (TABLE) L.A[a].p.c += 1;
-                        if (a == 0) phased_axis_step<0, ACT, NB, BRICK, ACC, JVP>(P, G, L, negbits);
-                        if (a == 1) phased_axis_step<1, ACT, NB, BRICK, ACC, JVP>(P, G, L, negbits);
-                        if (a == 2) phased_axis_step<2, ACT, NB, BRICK, ACC, JVP>(P, G, L, negbits);
+                        if (a == 0) phased_axis_step<0, ACT, BRICK>(P, G, L, negbits);
+                        if (a == 1) phased_axis_step<1, ACT, BRICK>(P, G, L, negbits);
+                        if (a == 2) phased_axis_step<2, ACT, BRICK>(P, G, L, negbits);
                         if constexpr (TABLE) {       // every lane crosses in the same substep: vote right here
                             const int lim = (a == 0 ? P.nx : (a == 1 ? P.ny : P.nz)) - 1;
                             const bool gone = L.A[a].p.c >= ((negbits & (1 << a)) ? 0 : lim);    // beyond the far face for good
                             if (__all_sync(0xFFFFFFFFu, gone)) next &= ~(1 << a);
                         }
                     }
-                int ko = L.S.base;           // kappa: nearest neighbour at clamp(floor(x_k)) (D4)
-                if (ACT & 1) ko += (negbits & 1) ? L.A[0].dl : 0;
-                if (ACT & 2) ko += (negbits & 2) ? L.A[1].dl : 0;
-                if (ACT & 4) ko += (negbits & 4) ? L.A[2].dl : 0;
-                phased_load_att<NB, ACC, JVP>(P, L, ko);
+                if constexpr (!KTRI) {
+                    int ko = L.S.base;       // kappa: nearest neighbour at clamp(floor(x_k)) (D4)
+                    if (ACT & 1) ko += (negbits & 1) ? L.A[0].dl : 0;
+                    if (ACT & 2) ko += (negbits & 2) ? L.A[1].dl : 0;
+                    if (ACT & 4) ko += (negbits & 4) ? L.A[2].dl : 0;
+                    phased_load_att<NB, JVP>(P, L, ko);
+                }
             }
             if constexpr (!TABLE) {
                 if ((L.g & 7) == 7) {        // lanes cross at different substeps: vote every 8th substep
@@ -319,7 +331,9 @@ __device__ __forceinline__ int phase(const MarchParams& P, const BrickGeom& G, P
 // from and stored back to the ray state.
 // JVP: the rt_march_jvp_kappa form (D21) -- the tangent of I for kappa -> kappa + eps P.dkappa is carried
 // next to I and deposited instead of it.
-template <int NB, bool TABLE, bool BRICK = (NB == 1), typename ACC = float, bool STEP = false, bool JVP = false>
+// KTRI: the rt_march_trilinear_kappa form (D18) -- kappa cached at the stencil voxels like j and read with
+// the trilinear weights every substep.
+template <int NB, bool TABLE, bool BRICK = (NB == 1), typename ACC = float, bool STEP = false, bool JVP = false, bool KTRI = false>
 __global__ void __launch_bounds__(kThreads, NB == 1 ? (TABLE ? RT_PHASED_MINB1 : RT_PHASED_MINB1P) : RT_PHASED_MINB4)
 march_phased_kernel(const MarchParams P) {
     static_assert(!BRICK || (NB == 1 && sizeof(ACC) == 4), "the brick scratch holds one fp32 bin");
@@ -340,7 +354,7 @@ march_phased_kernel(const MarchParams P) {
         const uint32_t lindex = __shfl_sync(0xFFFFFFFFu, id.index, leader);
         if (!live) { id.src = lsrc; id.group = lgroup; id.index = lindex; }
 
-        PhasedLane<NB, ACC, JVP> L;
+        PhasedLane<NB, ACC, JVP, KTRI> L;
         L.sg = sizeof(ACC) == 4 ? reinterpret_cast<ACC*>(P.scratch) : static_cast<ACC*>(P.acc);
         int negbits = 0;
         {
@@ -375,8 +389,13 @@ march_phased_kernel(const MarchParams P) {
 #pragma unroll
             for (int b = 0; b < NB; ++b) { L.I[b] = si.v[b]; L.T[b] = sT.v[b]; }
         }
-        phased_load_att<NB, ACC, JVP>(P, L, L.S.base + ((negbits & 1) ? L.A[0].dl : 0) + ((negbits & 2) ? L.A[1].dl : 0) +
-                                      ((negbits & 4) ? L.A[2].dl : 0));
+        if constexpr (KTRI) {
+#pragma unroll
+            for (int b = 0; b < NB; ++b) L.att[b] = 1.0f;
+        } else {
+            phased_load_att<NB, JVP>(P, L, L.S.base + ((negbits & 1) ? L.A[0].dl : 0) + ((negbits & 2) ? L.A[1].dl : 0) +
+                                          ((negbits & 4) ? L.A[2].dl : 0));
+        }
         L.g = 0;
         L.left = P.n_sub;
         L.roff = 0;
@@ -424,18 +443,18 @@ march_phased_kernel(const MarchParams P) {
                 }
             }
             switch (act) {
-                case 7: act = phase<7, NB, TABLE, BRICK, ACC, STEP, JVP>(P, G, L, negbits, tbase); break;
-                case 6: act = phase<6, NB, TABLE, BRICK, ACC, STEP, JVP>(P, G, L, negbits, tbase); break;
-                case 5: act = phase<5, NB, TABLE, BRICK, ACC, STEP, JVP>(P, G, L, negbits, tbase); break;
-                case 4: act = phase<4, NB, TABLE, BRICK, ACC, STEP, JVP>(P, G, L, negbits, tbase); break;
-                case 3: act = phase<3, NB, TABLE, BRICK, ACC, STEP, JVP>(P, G, L, negbits, tbase); break;
-                case 2: act = phase<2, NB, TABLE, BRICK, ACC, STEP, JVP>(P, G, L, negbits, tbase); break;
-                case 1: act = phase<1, NB, TABLE, BRICK, ACC, STEP, JVP>(P, G, L, negbits, tbase); break;
-                default: act = phase<0, NB, TABLE, BRICK, ACC, STEP, JVP>(P, G, L, negbits, tbase); break;
+                case 7: act = phase<7, NB, TABLE, BRICK, STEP, JVP, KTRI>(P, G, L, negbits, tbase); break;
+                case 6: act = phase<6, NB, TABLE, BRICK, STEP, JVP, KTRI>(P, G, L, negbits, tbase); break;
+                case 5: act = phase<5, NB, TABLE, BRICK, STEP, JVP, KTRI>(P, G, L, negbits, tbase); break;
+                case 4: act = phase<4, NB, TABLE, BRICK, STEP, JVP, KTRI>(P, G, L, negbits, tbase); break;
+                case 3: act = phase<3, NB, TABLE, BRICK, STEP, JVP, KTRI>(P, G, L, negbits, tbase); break;
+                case 2: act = phase<2, NB, TABLE, BRICK, STEP, JVP, KTRI>(P, G, L, negbits, tbase); break;
+                case 1: act = phase<1, NB, TABLE, BRICK, STEP, JVP, KTRI>(P, G, L, negbits, tbase); break;
+                default: act = phase<0, NB, TABLE, BRICK, STEP, JVP, KTRI>(P, G, L, negbits, tbase); break;
             }
             if (L.left == 0) {               // time-step boundary: the increments of this step are complete (rays continue, D7)
                 if constexpr (BRICK) {
-                    brick_flush<-1, 7, JVP>(G, L, negbits);      // slots of inactive axes hold exact zeros: skipped by value
+                    brick_flush<-1, 7>(G, L, negbits);         // slots of inactive axes hold exact zeros: skipped by value
 #pragma unroll
                     for (int s = 0; s < 8; ++s) L.S.zero_slot(s);
                     L.sg += G.step_stride;
