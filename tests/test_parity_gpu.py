@@ -232,6 +232,24 @@ def test_sources_sharing_their_cell_fractions(rt, oracle_mod, case):
     assert np.abs(got - plain).max() <= 1e-6 * np.abs(plain).max()      # same arithmetic per ray, other summation order
 
 
+@pytest.mark.parametrize("nb,shape", [(3, (9, 7, 8)), (5, (6, 8, 7)), (4, (9, 7, 8)), (8, (7, 9, 6))])
+@pytest.mark.parametrize("shared_fractions", [True, False])
+def test_bins_with_many_sources(rt, oracle_mod, nb, shape, shared_fractions):
+    """>= 32 sources (warp = 32 (source, bin group) pairs x 1 direction) with several bins: bins in fours take the plain
+    fp32 scratch with one red.v4 per voxel, other bin counts one bin per lane with fp64 reductions; sources that share
+    their cell fractions take the weight-table instantiation, others the plain one.  Three time steps."""
+    n_src, n_rays, ds, dt, n_steps = 41, 13, 0.25, 3.0, 3
+    rng = np.random.default_rng(nb * 100 + shape[0])
+    src = rng.integers(-1, 10, (n_src, 3)).astype(np.float64) + (0.5, 0.25, 0.0)
+    if not shared_fractions:
+        src += rng.uniform(-0.2, 0.2, src.shape)
+    src = src.astype(np.float32)
+    j, k = _random_medium(shape, nb, seed=nb)
+    ref = oracle_mod.march(j, k, src, n_rays, ds, 1.0, dt, n_steps)
+    got = rt.rt_march(_dev(j), _dev(k), _dev(src), n_rays, ds, 1.0, dt, n_steps).cpu().numpy()
+    parity.assert_parity(got, ref, f"nb={nb} shared={shared_fractions}")
+
+
 def test_more_sources_than_the_sort_handles(rt, oracle_mod):
     """Above 65,536 sources the spatial source sort is skipped (identity order); same field."""
     shape, n_src = (4, 4, 4), 66000

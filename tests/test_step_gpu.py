@@ -41,6 +41,9 @@ def _media(n, nb, n_steps, seed):
     (16, 4, 36, 40, False),       # 4 bins per thread: batched fp32 path with the scratch grid in the workspace
     (16, 8, 2, 33, True),         # 8 bins = 2 bin groups in adjacent lanes
     (12, 3, 5, 20, False),        # bins not a multiple of 4
+    (14, 4, 40, 24, True),        # 4 bins per thread, >= 32 cell-centred sources: weight table + plain fp32 scratch
+    (12, 3, 33, 20, True),        # 3 bins, one per lane, fp64 reductions, weight table
+    (12, 5, 35, 20, False),       # 5 bins, sources in general position
 ])
 def test_steps_with_a_changing_medium_match_the_oracle(rt, oracle_mod, n, nb, n_src, n_rays, integer_sources):
     n_steps, ds, dt = 4, 0.5, 3.0
