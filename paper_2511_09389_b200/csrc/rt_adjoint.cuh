@@ -23,11 +23,169 @@ namespace rt {
 // substep i) dL/dkappa_i = ds [P_i lambda_{i+1} - R_i], R_i = sum_{k>=i} G_k I_{k+1}: the same backward march,
 // fed with (I_{k+1}, P_k) of every substep as recorded by march_sliding_kernel<..., RECORD = true>, summing into the kappa cell of x_i
 // (nearest neighbour: one voxel per substep, reduced when the cell changes).
+// The state one lane carries through the backward march
+struct AdjointLane {
+    Stencil<1, double, false> S;     // cached gsuf values (jc) and pending deposits (acc)
+    TravelAxis A[3];
+    float lambda, a_next, kap, att;
+    double tau, Rsum, kacc;          // WRT_KAPPA: R_i and the pending sum of the current kappa cell, in fp64 (P_i lambda_{i+1} - R_i cancels)
+    int ko;                          // element offset of the kappa cell
+    long long kk;                    // global substep index of the backward sweep
+    int left;                        // substeps left in the current time step
+};
+
+// PHASES of the backward march (cf. rt_march_phased.cuh).  The backward ray starts at x_{K-1}, for most rays far outside
+// the box, and comes in: an axis is INACTIVE for a warp while every lane is still short of the face it will enter
+// through (travel cell word below the near face, by a margin of kAdjMargin cells: the test runs every 4th substep and a
+// substep is shorter than a cell) -- merged, weights exactly (1, 0), leading slots never touched and exactly zero.
+// adjoint_phase<ACT> is the substep loop with those axes compiled out; it returns the new set of active axes (one more
+// axis: a warp vote), or ACT at a time-step boundary.  Activation needs no reload: no lane has entered yet, so the
+// axis is still merged in every lane and its first slide loads its leading slots.
+constexpr int kAdjMargin = 4;
+
+template <int ACT, bool WRT_KAPPA>
+__device__ __forceinline__ int adjoint_phase(const MarchParams& P, AdjointLane& L, int negbits, double* og, const float* gs,
+                                             const float2* fwd, long long fwd_stride, long long tid, int bin, bool live) {
+    constexpr int kBits = ((ACT & 1) ? 4 : 0) | ((ACT & 2) ? 2 : 0) | ((ACT & 4) ? 1 : 0);
+    constexpr int kActive = ((ACT & 1) ? 1 : 0) + ((ACT & 2) ? 1 : 0) + ((ACT & 4) ? 1 : 0);
+    constexpr int kLast = (ACT & 4) ? 2 : ((ACT & 2) ? 1 : 0);
+    auto load_kappa = [&]() {
+        int ko = L.S.base;
+        if (ACT & 1) ko += (negbits & 1) ? L.A[0].dl : 0;
+        if (ACT & 2) ko += (negbits & 2) ? L.A[1].dl : 0;
+        if (ACT & 4) ko += (negbits & 4) ? L.A[2].dl : 0;
+        L.ko = ko;
+        L.kap = __ldg(P.kappa + ko);
+        L.att = ex2_approx(L.kap * P.att_scale);
+    };
+    int next = ACT;
+    do {
+        float w[8];
+        bool cross[3] = {false, false, false};
+        {
+            float t[3] = {1.0f, 1.0f, 1.0f}, l[3] = {0.0f, 0.0f, 0.0f};
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                if (ACT & (1 << a)) {
+                    const uint32_t h = L.A[a].p.fh & L.A[a].fmask;
+                    const float sc = (a == kLast) ? (kActive == 3 ? 1.2621774483536189e-29f
+                                                                  : (kActive == 2 ? 5.421010862427522e-20f : 2.3283064365386963e-10f))
+                                                  : 1.0f;
+                    t[a] = __uint2float_rn(~h) * sc;
+                    l[a] = __uint2float_rn(h) * sc;
+                }
+                const int c = L.A[a].p.c;                  // every axis is advanced: an inactive one is watched for its entry
+                fx_add(L.A[a].p, L.A[a].d);
+                cross[a] = (ACT & (1 << a)) && L.A[a].p.c != c;
+            }
+            const float wx[2] = {t[0], l[0]}, wy[2] = {t[1], l[1]}, wz[2] = {t[2], l[2]};
+#pragma unroll
+            for (int s = 0; s < 8; ++s)
+                if ((s & ~kBits) == 0) {
+                    float v = 1.0f;
+                    bool first = true;
+                    if (ACT & 1) { v = wx[s >> 2]; first = false; }
+                    if (ACT & 2) { v = first ? wy[(s >> 1) & 1] : v * wy[(s >> 1) & 1]; first = false; }
+                    if (ACT & 4) { v = first ? wz[s & 1] : v * wz[s & 1]; }
+                    w[s] = v;
+                }
+        }
+        float gv = 0.0f, gu = 0.0f;
+#pragma unroll
+        for (int s = 0; s < 8; ++s)
+            if ((s & ~kBits) == 0) {
+                const int r = slot_rank(s, kBits);
+                const float g = L.S.jc[s].v[0];
+                if (r & 1) gu = (r == 1) ? w[s] * g : fmaf(w[s], g, gu);
+                else gv = (r == 0) ? w[s] * g : fmaf(w[s], g, gv);
+            }
+        if (!live) { gv = 0.0f; gu = 0.0f; }         // a dark lane: zero dL/d out, so lambda stays 0 and nothing is deposited
+        if (WRT_KAPPA) {
+            // (I_{k+1}, P_k), both x 4 pi/N_Omega (a dark lane has no record)
+            const float2 rec = live ? __ldg(fwd + L.kk * fwd_stride + tid) : make_float2(0.0f, 0.0f);
+            L.lambda = fmaf(L.a_next, L.lambda, gv + gu);
+            L.a_next = L.att;
+            L.Rsum = fma(double(gv + gu), double(rec.x), L.Rsum);
+            L.kacc = fma(fma(double(rec.y), double(L.lambda), -L.Rsum), P.ds, L.kacc);
+            --L.kk;
+        } else {
+            L.tau = fma(-double(L.kap), P.ds, L.tau);                             // tau_k = tau_{k+1} - kappa_k ds
+            const float T = ex2_approx(float(L.tau * -1.4426950408889634));       // exp(-tau_k)
+            L.lambda = fmaf(L.a_next, L.lambda, (gv + gu) * P.emis);              // lambda_{k+1} ds
+            L.a_next = L.att;
+            const float v = L.lambda * T;
+#pragma unroll
+            for (int s = 0; s < 8; ++s)
+                if ((s & ~kBits) == 0) L.S.acc[s].v[0] = (ACT == 0) ? L.S.acc[s].v[0] + v : fmaf(w[s], v, L.S.acc[s].v[0]);
+        }
+        if (cross[0] | cross[1] | cross[2]) {
+            bool jumped = false;
+            if constexpr (ACT == 7) {            // a substep of a cell or more (all axes active then) may cross two planes
+                if (P.ds_f >= 1.0f) {
+                    const int c0 = L.A[0].p.c, c1 = L.A[1].p.c, c2 = L.A[2].p.c;
+                    // cell words one substep ago: position minus increment (travel increments are >= 0)
+                    Fx96 q0 = L.A[0].p, q1 = L.A[1].p, q2 = L.A[2].p;
+                    fx_sub(q0, L.A[0].d); fx_sub(q1, L.A[1].d); fx_sub(q2, L.A[2].d);
+                    jumped = ((c0 - q0.c) | (c1 - q1.c) | (c2 - q2.c)) > 1;
+                    if (jumped) {
+                        L.S.flush_all(og, L.A);
+                        L.S.restart(P, L.A, negbits, bin, gs);
+                    }
+                }
+            }
+            if (!jumped) {
+                if (cross[0]) L.S.template axis_step<0, ACT>(P, L.A, negbits, og, gs);
+                if (cross[1]) L.S.template axis_step<1, ACT>(P, L.A, negbits, og, gs);
+                if (cross[2]) L.S.template axis_step<2, ACT>(P, L.A, negbits, og, gs);
+            }
+            if (WRT_KAPPA) {                     // the kappa cell may have changed: reduce the old one's sum
+                const int ko_old = L.ko;
+                load_kappa();
+                if (L.ko != ko_old) {
+                    if (L.kacc != 0.0)
+                        asm volatile("red.global.add.f64 [%0], %1;" ::"l"(og + ko_old), "d"(L.kacc) : "memory");
+                    L.kacc = 0.0;
+                }
+            } else {
+                load_kappa();
+            }
+        }
+        --L.left;
+        if constexpr (ACT != 7) {
+            if ((L.left & 3) == 0) {             // is a lane about to enter through an inactive axis?
+#pragma unroll
+                for (int a = 0; a < 3; ++a)
+                    if (!(ACT & (1 << a))) {
+                        const int lim = (a == 0 ? P.nx : (a == 1 ? P.ny : P.nz)) - 1;
+                        const bool near = L.A[a].p.c + kAdjMargin >= ((negbits & (1 << a)) ? -lim : 0);
+                        if (__any_sync(0xFFFFFFFFu, near)) next |= 1 << a;
+                    }
+            }
+        }
+    } while (L.left != 0 && next == ACT);
+    return next;
+}
+
+// WRT_KAPPA = false: dL/dj as described above.  WRT_KAPPA = true: dL/dkappa (D19).  Unrolling eq. (2),
+// I_{k+1} = T_{k+1} sum_{m<=k} ds J_m / a_m, so with G_k = w_k . gsuf and P_i = ds J_i T_i (the emission term of
+// substep i) dL/dkappa_i = ds [P_i lambda_{i+1} - R_i], R_i = sum_{k>=i} G_k I_{k+1}: the same backward march,
+// fed with (I_{k+1}, P_k) of every substep as recorded by march_sliding_kernel<..., RECORD = true>, summing into the kappa cell of x_i
+// (nearest neighbour: one voxel per substep, reduced when the cell changes).
 template <int MINB, bool WRT_KAPPA>
 __global__ void __launch_bounds__(kThreads, MINB) adjoint_kernel(const MarchParams P, const float* gsuf,
                                                                  const float2* fwd, long long fwd_stride) {
+    // a warp marches as a whole (its phases are warp votes): a lane without a ray of its own marches the ray of the
+    // warp's first live lane with gsuf read as zero weight -- lambda stays 0, nothing is deposited
     RayId id;
-    if (!ray_id(P, id)) return;
+    const bool live = ray_id(P, id);
+    const unsigned live_mask = __ballot_sync(0xFFFFFFFFu, live);
+    if (!live_mask) return;
+    {
+        const int leader = __ffs(live_mask) - 1;
+        const int lsrc = __shfl_sync(0xFFFFFFFFu, id.src, leader), lgroup = __shfl_sync(0xFFFFFFFFu, id.group, leader);
+        const uint32_t lindex = __shfl_sync(0xFFFFFFFFu, id.index, leader);
+        if (!live) { id.src = lsrc; id.group = lgroup; id.index = lindex; }
+    }
     const long long tid = (long long)blockIdx.x * kThreads + threadIdx.x;
     const int bin = id.group;                       // one bin per thread (n_groups = n_bins)
     double* og = static_cast<double*>(P.acc);
@@ -46,7 +204,8 @@ __global__ void __launch_bounds__(kThreads, MINB) adjoint_kernel(const MarchPara
     }
     // phase 1: tau_K = ds * sum_k kappa(cell of x_k), forwards (nearest neighbour, clamped: PAPER.md:29, D4)
     const int sx = P.ny * P.nz * P.nb, sy = P.nz * P.nb, sz = P.nb;
-    double tau = 0.0;
+    AdjointLane L;
+    L.tau = 0.0;
     const long long K = (long long)P.n_steps * P.n_sub;
     if (WRT_KAPPA) {                                 // tau is not needed: jump to x_K
 #pragma unroll
@@ -55,13 +214,12 @@ __global__ void __launch_bounds__(kThreads, MINB) adjoint_kernel(const MarchPara
         for (long long k = 0; k < K; ++k) {
             const int o = min(max(X[0].c, 0), P.nx - 1) * sx + min(max(X[1].c, 0), P.ny - 1) * sy +
                           min(max(X[2].c, 0), P.nz - 1) * sz;
-            tau = fma(double(__ldg(P.kappa + o + bin)), P.ds, tau);
+            L.tau = fma(double(__ldg(P.kappa + o + bin)), P.ds, L.tau);
 #pragma unroll
             for (int a = 0; a < 3; ++a) fx_add(X[a], D[a]);
         }
     }
     // phase 2: backwards from x_{K-1}
-    TravelAxis A[3];
     int negbits = 0;
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
@@ -71,103 +229,61 @@ __global__ void __launch_bounds__(kThreads, MINB) adjoint_kernel(const MarchPara
         nd.c = ~D[a].c + ((nd.fl == 0u && nd.fh == 0u) ? 1 : 0);
         fx_add(X[a], nd);                            // x_{K-1}
         if (fwd_neg[a]) {                            // the backward ray ascends this axis
-            A[a].p = X[a];
-            A[a].d = nd;
+            L.A[a].p = X[a];
+            L.A[a].d = nd;
         } else {                                     // it descends: complement coordinate, increment +D
-            A[a].p.c = ~X[a].c; A[a].p.fh = ~X[a].fh; A[a].p.fl = ~X[a].fl;
-            A[a].d = D[a];
+            L.A[a].p.c = ~X[a].c; L.A[a].p.fh = ~X[a].fh; L.A[a].p.fl = ~X[a].fl;
+            L.A[a].d = D[a];
             negbits |= 1 << a;
         }
     }
     asm volatile("" : "+r"(negbits));
-    Stencil<1, double, false> S;
 #pragma unroll
-    for (int s = 0; s < 8; ++s) S.zero_slot(s);
+    for (int s = 0; s < 8; ++s) L.S.zero_slot(s);
     const float* gs = gsuf + (long long)(P.n_steps - 1) * P.snap_stride;
-    S.restart(P, A, negbits, bin, gs);
-
-    float lambda = 0.0f, a_next = 0.0f, kap = 0.0f, att = 1.0f;
-    double Rsum = 0.0, kacc = 0.0;                   // WRT_KAPPA: R_i and the pending sum for the current kappa cell (fp64:
-                                                     // P_i lambda_{i+1} - R_i cancels)
-    int ko = 0;
-    auto load_kappa = [&]() {
-        ko = S.base + ((negbits & 1) ? A[0].dl : 0) + ((negbits & 2) ? A[1].dl : 0) + ((negbits & 4) ? A[2].dl : 0);
-        kap = __ldg(P.kappa + ko);
-        att = ex2_approx(kap * P.att_scale);
-    };
-    auto flush_kappa = [&]() {
-        if (kacc != 0.0) asm volatile("red.global.add.f64 [%0], %1;" ::"l"(og + ko), "d"(kacc) : "memory");
-        kacc = 0.0;
-    };
-    load_kappa();
-    long long kk = K - 1;                            // global substep index of the backward sweep
-
-    for (int m = P.n_steps - 1; m >= 0; --m) {
-        if (m != P.n_steps - 1) {                    // an earlier time step sees the suffix sum of one more snapshot
-            gs -= P.snap_stride;
-            S.reload(P, A, gs);
+    L.S.restart(P, L.A, negbits, bin, gs);
+    L.lambda = 0.0f; L.a_next = 0.0f;
+    L.Rsum = 0.0; L.kacc = 0.0;
+    L.ko = L.S.base + ((negbits & 1) ? L.A[0].dl : 0) + ((negbits & 2) ? L.A[1].dl : 0) + ((negbits & 4) ? L.A[2].dl : 0);
+    L.kap = __ldg(P.kappa + L.ko);
+    L.att = ex2_approx(L.kap * P.att_scale);
+    L.kk = K - 1;
+    L.left = P.n_sub;
+    // axes some lane is inside of, or about to enter, at x_{K-1}
+    int act = 0;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const int lim = (a == 0 ? P.nx : (a == 1 ? P.ny : P.nz)) - 1;
+        const bool near = L.A[a].p.c + kAdjMargin >= ((negbits & (1 << a)) ? -lim : 0);
+        if (__any_sync(0xFFFFFFFFu, near)) act |= 1 << a;
+    }
+    if (!(P.ds_f < 1.0f)) act = 7;                   // substeps of a cell or more: no phases (the margin assumes shorter ones)
+    int m = P.n_steps - 1;
+    while (true) {
+        {
+            switch (act) {
+                case 7: act = adjoint_phase<7, WRT_KAPPA>(P, L, negbits, og, gs, fwd, fwd_stride, tid, bin, live); break;
+                case 6: act = adjoint_phase<6, WRT_KAPPA>(P, L, negbits, og, gs, fwd, fwd_stride, tid, bin, live); break;
+                case 5: act = adjoint_phase<5, WRT_KAPPA>(P, L, negbits, og, gs, fwd, fwd_stride, tid, bin, live); break;
+                case 4: act = adjoint_phase<4, WRT_KAPPA>(P, L, negbits, og, gs, fwd, fwd_stride, tid, bin, live); break;
+                case 3: act = adjoint_phase<3, WRT_KAPPA>(P, L, negbits, og, gs, fwd, fwd_stride, tid, bin, live); break;
+                case 2: act = adjoint_phase<2, WRT_KAPPA>(P, L, negbits, og, gs, fwd, fwd_stride, tid, bin, live); break;
+                case 1: act = adjoint_phase<1, WRT_KAPPA>(P, L, negbits, og, gs, fwd, fwd_stride, tid, bin, live); break;
+                default: act = adjoint_phase<0, WRT_KAPPA>(P, L, negbits, og, gs, fwd, fwd_stride, tid, bin, live); break;
+            }
         }
-        for (int k = P.n_sub - 1; k >= 0; --k) {
-            const uint32_t hx = A[0].p.fh & A[0].fmask, hy = A[1].p.fh & A[1].fmask, hz = A[2].p.fh & A[2].fmask;
-            const float lx = __uint2float_rn(hx), tx = __uint2float_rn(~hx);
-            const float ly = __uint2float_rn(hy), ty = __uint2float_rn(~hy);
-            const float wz[2] = {__uint2float_rn(~hz) * 1.2621774483536189e-29f,      // 2^-96
-                                 __uint2float_rn(hz) * 1.2621774483536189e-29f};
-            const float wxy[4] = {tx * ty, tx * ly, lx * ty, lx * ly};
-            float w[8];
-#pragma unroll
-            for (int s = 0; s < 8; ++s) w[s] = wxy[s >> 1] * wz[s & 1];
-            float gv = w[0] * S.jc[0].v[0], gu = w[1] * S.jc[1].v[0];
-#pragma unroll
-            for (int s = 2; s < 8; s += 2) {
-                gv = fmaf(w[s], S.jc[s].v[0], gv);
-                gu = fmaf(w[s + 1], S.jc[s + 1].v[0], gu);
-            }
-            if (WRT_KAPPA) {
-                const float2 rec = __ldg(fwd + kk * fwd_stride + tid);            // (I_{k+1}, P_k), both x 4 pi/N_Omega
-                lambda = fmaf(a_next, lambda, gv + gu);
-                a_next = att;
-                Rsum = fma(double(gv + gu), double(rec.x), Rsum);
-                kacc = fma(fma(double(rec.y), double(lambda), -Rsum), P.ds, kacc);
-                --kk;
-            } else {
-                tau = fma(-double(kap), P.ds, tau);                               // tau_k = tau_{k+1} - kappa_k ds
-                const float T = ex2_approx(float(tau * -1.4426950408889634));     // exp(-tau_k)
-                lambda = fmaf(a_next, lambda, (gv + gu) * P.emis);                // lambda_{k+1} ds
-                a_next = att;
-                const float v = lambda * T;
-#pragma unroll
-                for (int s = 0; s < 8; ++s) S.acc[s].v[0] = fmaf(w[s], v, S.acc[s].v[0]);
-            }
-
-            const int c0 = A[0].p.c, c1 = A[1].p.c, c2 = A[2].p.c;
-#pragma unroll
-            for (int a = 0; a < 3; ++a) fx_add(A[a].p, A[a].d);
-            if ((c0 ^ A[0].p.c) | (c1 ^ A[1].p.c) | (c2 ^ A[2].p.c)) {
-                if (P.ds_f >= 1.0f && (((A[0].p.c - c0) | (A[1].p.c - c1) | (A[2].p.c - c2)) > 1)) {
-                    S.flush_all(og, A);
-                    S.restart(P, A, negbits, bin, gs);
-                } else {
-                    if (c0 != A[0].p.c) S.template axis_step<0>(P, A, negbits, og, gs);
-                    if (c1 != A[1].p.c) S.template axis_step<1>(P, A, negbits, og, gs);
-                    if (c2 != A[2].p.c) S.template axis_step<2>(P, A, negbits, og, gs);
-                }
-                if (WRT_KAPPA) {                     // the kappa cell may have changed: reduce the old one's sum
-                    const int ko_old = ko;
-                    load_kappa();
-                    if (ko != ko_old) {
-                        if (kacc != 0.0)
-                            asm volatile("red.global.add.f64 [%0], %1;" ::"l"(og + ko_old), "d"(kacc) : "memory");
-                        kacc = 0.0;
-                    }
-                } else {
-                    load_kappa();
-                }
-            }
+        if (L.left == 0) {                           // an earlier time step sees the suffix sum of one more snapshot
+            if (--m < 0) break;
+            gs -= P.snap_stride;
+            L.S.reload(P, L.A, gs);
+            L.left = P.n_sub;
         }
     }
-    if (WRT_KAPPA) flush_kappa();
-    else S.flush_all(og, A);
+    if (WRT_KAPPA) {
+        if (L.kacc != 0.0) asm volatile("red.global.add.f64 [%0], %1;" ::"l"(og + L.ko), "d"(L.kacc) : "memory");
+    } else {
+        L.S.flush_all(og, L.A);
+    }
 }
 
 // gsuf[m] = gbar[m] + gbar[m+1] + ... (the snapshots of the forward march are cumulative, D7)

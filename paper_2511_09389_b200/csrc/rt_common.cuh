@@ -120,6 +120,14 @@ __device__ __forceinline__ void fx_add(Fx96& p, const Fx96& d) {
         : "r"(d.fl), "r"(d.fh), "r"(d.c));
 }
 
+__device__ __forceinline__ void fx_sub(Fx96& p, const Fx96& d) {
+    asm("sub.cc.u32 %0, %0, %3;\n\t"
+        "subc.cc.u32 %1, %1, %4;\n\t"
+        "subc.s32 %2, %2, %5;"
+        : "+r"(p.fl), "+r"(p.fh), "+r"(p.c)
+        : "r"(d.fl), "r"(d.fh), "r"(d.c));
+}
+
 // p += k d, exact (k >= 0, the product stays far below 2^127: paths are limited to 2^28 cells)
 __device__ __forceinline__ void fx_advance(Fx96& p, const Fx96& d, long long k) {
     const __int128 pp = (__int128(p.c) << 64) | (__int128(p.fh) << 32) | __int128(p.fl);

@@ -66,13 +66,6 @@ __device__ __forceinline__ void mask_pair(float& t, float& l, uint32_t m) {
     l = __uint_as_float(__float_as_uint(l) & m);
 }
 
-// number of slots in use below s (slots in use: those with no bit outside `bits`)
-__host__ __device__ constexpr int slot_rank(int s, int bits) {
-    int r = 0;
-    for (int t = 0; t < s; ++t) r += ((t & ~bits) == 0) ? 1 : 0;
-    return r;
-}
-
 // The state one lane carries through the march
 template <int NB, typename ACC = float, bool JVP = false, bool KTRI = false> struct PhasedLane {
     Stencil<NB, ACC, KTRI> S;

@@ -32,6 +32,13 @@ template <int AX> __device__ __forceinline__ constexpr int slot(int p, int u, in
     return AX == 0 ? (p * 4 + u * 2 + v) : (AX == 1 ? (u * 4 + p * 2 + v) : (u * 4 + v * 2 + p));
 }
 
+// number of slots in use below s (slots in use: those with no bit outside `bits`)
+__host__ __device__ constexpr int slot_rank(int s, int bits) {
+    int r = 0;
+    for (int t = 0; t < s; ++t) r += ((t & ~bits) == 0) ? 1 : 0;
+    return r;
+}
+
 __device__ __forceinline__ float ex2_approx(float x) {
     float y;
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
