@@ -508,19 +508,40 @@ def test_full_size_oracle_parity(rt, oracle_mod, name):
 
 
 def test_overlapped_batches_never_lose_a_deposit(rt):
-    """C3 marches its ray batches in pairs, the second grid of a pair launched with programmatic stream serialization
-    over the tail of the first, and one drain kernel folds both scratch grids.  The drain must see every deposit of
-    BOTH grids whichever finishes first (the second grid waits for the first before it completes): 50 repetitions agree
-    with one another to the rounding of the reduction order; a drain that overtook a grid would drop whole batches
-    of deposits."""
+    """The batched multi-bin kernels (RT_VARIANT_SLIDING_BY_SOURCE on C3: what rt_march ran in round 1) march their ray
+    batches in pairs, the second grid of a pair launched with programmatic stream serialization over the tail of the
+    first, and one drain kernel folds both scratch grids.  The drain must see every deposit of BOTH grids whichever
+    finishes first (the second grid waits for the first before it completes): 50 repetitions agree with one another to
+    the rounding of the reduction order; a drain that overtook a grid would drop whole batches of deposits."""
     w = config("C3")
     j, k, s = _dev(w.j), _dev(w.kappa), _dev(w.sources)
     ws = rt.alloc_workspace(*w.shape, w.n_src, w.n_rays, w.n_bins, w.n_steps)
-    first = rt.rt_march(j, k, s, w.n_rays, w.step_size, w.c, w.dt, w.n_steps, workspace=ws).clone()
+    args = (w.n_rays, w.step_size, w.c, w.dt, w.n_steps)
+    first = rt.rt_march_ex(j, k, s, *args, workspace=ws, variant=rt.RT_VARIANT_SLIDING_BY_SOURCE).clone()
     scale = float(first.max())
     out = torch.empty_like(first)
     worst = 0.0
     for _ in range(50):
-        rt.rt_march(j, k, s, w.n_rays, w.step_size, w.c, w.dt, w.n_steps, out=out, workspace=ws)
+        rt.rt_march_ex(j, k, s, *args, out=out, workspace=ws, variant=rt.RT_VARIANT_SLIDING_BY_SOURCE)
         worst = max(worst, float((out - first).abs().max()) / scale)
     assert worst <= 2e-6, worst
+
+
+def test_concurrent_drains_never_lose_a_deposit(rt):
+    """The product path: every block drains a slice of the fp32 scratch into the fp64 grid (atom.exch) while other
+    blocks still reduce into it.  C2 (16 drain rounds over 67,584 blocks) and C3 repeated: the runs agree to the
+    rounding of the reduction order; a deposit lost between a read and a zeroing would show at the 1e-4 level of the
+    hot voxels."""
+    for name, reps in (("C2", 10), ("C3", 20)):
+        w = config(name)
+        j, k, s = _dev(w.j), _dev(w.kappa), _dev(w.sources)
+        ws = rt.alloc_workspace(*w.shape, w.n_src, w.n_rays, w.n_bins, w.n_steps)
+        args = (w.n_rays, w.step_size, w.c, w.dt, w.n_steps)
+        first = rt.rt_march(j, k, s, *args, workspace=ws).clone()
+        scale = float(first.max())
+        total = float(first.double().sum())
+        out = torch.empty_like(first)
+        for _ in range(reps):
+            rt.rt_march(j, k, s, *args, out=out, workspace=ws)
+            assert float((out - first).abs().max()) / scale <= 2e-6, name
+            assert abs(float(out.double().sum()) - total) <= 1e-6 * total, name       # deposit mass (pin P2) is conserved
