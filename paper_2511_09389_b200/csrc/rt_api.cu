@@ -82,7 +82,7 @@ int check_args(const void* j, const void* kappa, int nx, int ny, int nz, const v
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 // workspace layout: [ray order: slots u32][source order: n_src u32][flag][fp64 accumulation grid x copies][fp32 scratch]
-// [fp32 brick scratch of the table march]
+// [fp32 window-brick scratch of the one-bin phased march]
 struct Workspace {
     size_t src_order_at, flag_at, acc_at, scratch2_at, brick_at, brick_bytes, total;
     int acc_copies;
@@ -106,7 +106,7 @@ Workspace workspace_layout(int nx, int ny, int nz, int n_src, int n_rays, int n_
     const size_t grid = size_t(cells) * size_t(n_steps) * sizeof(double);
     w.acc_copies = use_batched_fp32(cells, n_steps, n_bins) ? 1 : int(std::min<size_t>(4, std::max<size_t>(1, kAccCopiesBytes / grid)));
     w.src_order_at = align_up(size_t(ray_slots(n_rays)) * sizeof(uint32_t), 16);
-    w.flag_at = align_up(w.src_order_at + size_t(n_src) * sizeof(uint32_t), 16);      // same-fraction flag (table march)
+    w.flag_at = align_up(w.src_order_at + size_t(n_src) * sizeof(uint32_t), 16);      // same-fraction flag (weight-table march)
     w.acc_at = align_up(w.flag_at + 16, 256);
     w.scratch2_at = align_up(w.acc_at + grid * size_t(w.acc_copies), 256);
     // the batched fp32 path marches two batches at a time: `out` and this second fp32 grid are their scratch grids

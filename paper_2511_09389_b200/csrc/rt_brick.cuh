@@ -1,4 +1,4 @@
-// rt_brick.cuh — the fp32 BRICK SCRATCH of the one-bin table march (sm_100a): vector reductions, concurrent drain.
+// rt_brick.cuh — the fp32 SCRATCH of march_phased_kernel (sm_100a): window bricks, vector reductions, concurrent drain.
 //
 // WHY.  ncu on C2 (profiles/r02b): the march is bound by the L1/LSU data pipe, and three quarters of its wavefronts
 // are the deposits -- every lane of a red.global.add is its own 32-byte sector on its way to the L2, whatever it

@@ -34,9 +34,9 @@ struct MarchParams {
     float* state_I;              // rt_march_step: carried I per (source, lattice index, bin), else nullptr
     float* state_T;              //                carried exp(-tau), same layout
     long long k0;                // substep index of the first substep of this launch (0 for rt_march)
-    const int* same_frac;        // device flag, or nullptr: all sources share their cell fractions -> march_table_kernel
-                                 // marches the call and march_sliding_kernel<..., COPIES> returns at once (and vice versa)
-    // march_sliding_kernel<..., COPIES = true> and march_table_kernel, else 1 / 0:
+    const int* same_frac;        // device flag, or nullptr: all sources share their cell fractions -> the TABLE instantiation
+                                 // of march_phased_kernel marches the call and the plain one returns at once (and vice versa)
+    // march_sliding_kernel<..., COPIES = true>, else 1 / 0:
     int acc_copies;              // block b reduces into copy b % acc_copies of the accumulation grid ...
     long long acc_copy_stride;   // ... copies being acc_copy_stride elements apart (hot voxels meet fewer reductions)
     // march_phased_kernel: the fp32 scratch its rays deposit into (rt_brick.cuh: window bricks [n_steps][nx][ny+1][nz+1][4]

@@ -79,7 +79,7 @@ template <int NB, typename ACC, bool KTRI> struct Stencil {
         for (int b = 0; b < NB; ++b) acc[s].v[b] = 0.0f;
     }
     // ACT (here and in axis_step): bit a set = axis a is ACTIVE.  An inactive axis is one every ray of the warp has
-    // left the box through for good (march_table_kernel's lower-dimensional phases): its leading slots hold exactly
+    // left the box through for good (march_phased_kernel's lower-dimensional phases): its leading slots hold exactly
     // zero and are skipped, i.e. only the slots whose index bit (4 >> a) is clear are touched.  ACT = 7: all 8 slots.
     template <int ACT = 7> __device__ __forceinline__ void flush_all(ACC* og, const TravelAxis (&A)[3]) {
         constexpr int kBits = ((ACT & 1) ? 4 : 0) | ((ACT & 2) ? 2 : 0) | ((ACT & 4) ? 1 : 0);
@@ -184,7 +184,7 @@ template <int NB, typename ACC, int MINB, bool STEP, bool KTRI = false, bool REC
 __global__ void __launch_bounds__(kThreads, MINB) march_sliding_kernel(const MarchParams P, float2* record = nullptr,
                                                                        long long record_stride = 0) {
     if constexpr (COPIES)
-        if (P.same_frac && *P.same_frac) return;     // march_table_kernel has marched this call (rt_march_table.cuh)
+        if (P.same_frac && *P.same_frac) return;     // (unused since the phased kernel took over the weight table)
     // the batched path launches the next batch (other scratch grid, no dependence on this one) with programmatic
     // stream serialization: it may start as soon as every block of this grid has started, filling this grid's tail
     // (and waits for this grid's completion at its own end: griddepcontrol.wait below)
