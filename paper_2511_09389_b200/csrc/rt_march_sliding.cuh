@@ -1,4 +1,6 @@
-// rt_march_sliding.cuh — the product march kernel (sm_100a): sliding-stencil register accumulation.
+// rt_march_sliding.cuh — the sliding stencil (sm_100a): register accumulation of the trilinear deposit, used by every
+// march kernel, and march_sliding_kernel, the march without phases, weight table and scratch (round 1's product kernel:
+// now the kernel of the rt_march_ex variants, of substeps of a cell or more and of the kappa adjoint's record pass).
 //
 // One thread marches one (source, direction, bin-group) ray for all n_steps * N_s substeps of eq. (2)
 // (PAPER.md:23).  The 8 voxels of the ray's clamped trilinear stencil live in registers: their j
