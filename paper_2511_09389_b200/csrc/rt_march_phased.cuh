@@ -303,7 +303,7 @@ __device__ __forceinline__ int phase(const MarchParams& P, const BrickGeom& G, L
         }
         ++L.g;
         --L.left;
-    } while ((TABLE ? L.roff != 0 : true) && L.left != 0 && next == ACT);
+    } while ((TABLE && ACT != 0 ? L.roff != 0 : true) && L.left != 0 && next == ACT);      // (no table without active axes)
     return next;
 }
 
