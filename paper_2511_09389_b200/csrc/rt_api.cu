@@ -306,6 +306,73 @@ int launch_phased(const rt::MarchParams& P, int kind, unsigned blocks, cudaStrea
     return RT_OK;
 }
 
+// rt_march proper (and rt_march_step, rt_march_trilinear_kappa, rt_march_jvp_kappa) through march_phased_kernel: memsets,
+// (fraction test, weight-table instantiation,) plain instantiation, snapshots.  P: base parameters with the orders built.
+int run_phased(rt::MarchParams P, int phased, const Plan& pl, const Workspace& wl, char* ws, double* master, float* out,
+               size_t n_acc, long long cells, const StepArgs* step, int nx, int ny, int nz, const float* sources, int n_src,
+               int n_rays, int n_bins, float step_size, int n_steps, cudaStream_t st) {
+    const int fin_threads = 256;
+    long long fin_blocks = (cells + fin_threads - 1) / fin_threads;
+    if (fin_blocks > 148 * 16) fin_blocks = 148 * 16;
+    // rt_march proper (and rt_march_step): the phased march deposits into an fp32 scratch -- window bricks in the
+    // workspace (one bin), or the plain grid (four bins per thread; `out` itself, or for rt_march_step, whose `out` may
+    // hold the running field, a grid behind the workspace) -- and drains it into the fp64 grid as it goes; or it
+    // reduces straight into the fp64 grid.  The snapshots (the step's increment) are formed from the fp64 grid plus
+    // what the march left in the scratch.
+    P.n_groups = phased == kPhasedFourBins ? n_bins / 4 : n_bins;
+    P.acc = master;
+    P.scratch = phased == kPhasedOneBin ? reinterpret_cast<float*>(ws + wl.brick_at)
+                                        : (step ? reinterpret_cast<float*>(ws + wl.total) : out);
+    const size_t scratch_bytes = phased == kPhasedDirect64 ? 0 : (phased == kPhasedOneBin ? wl.brick_bytes : n_acc * sizeof(float));
+    P.n_drain_units = std::max<long long>(1, (long long)(scratch_bytes / 16));
+    RT_CUDA(cudaMemsetAsync(master, 0, n_acc * sizeof(double), st));
+    if (scratch_bytes) RT_CUDA(cudaMemsetAsync(P.scratch, 0, scratch_bytes, st));
+    const long long mb = rt::march_blocks(P.n_src, P.n_slots, P.n_groups, P.map_src);
+    if (mb > 2147483647LL) return RT_EINVAL;
+    const long long per = (P.n_drain_units * drain_rounds((long long)n_src * n_rays) + mb - 1) / mb;
+    P.drain_units_per_block = std::min<long long>(std::max<long long>(per, 1), rt::kDrainMaxUnits);
+    if (pl.map_src) {
+        // Sources that share their cell fractions (decided on the device) take the weight-table instantiation, others
+        // the plain one: both are launched, each returns at once when the flag says the call is the other's
+        int* flag = reinterpret_cast<int*>(ws + wl.flag_at);
+        rt::same_fraction_kernel<<<1, 256, 0, st>>>(flag, sources, n_src, step_size);
+        P.same_frac = flag;
+        const int rct = step ? launch_phased<true, true>(P, phased, unsigned(mb), st) : launch_phased<true, false>(P, phased, unsigned(mb), st);
+        if (rct != RT_OK) return rct;
+    }
+    long long mb2 = mb;
+    if (phased == kPhasedDirect64 && pl.map_src) {
+        // sources in general position on a grid beyond the L2: warp = 32 (direction, bin) pairs of ONE source, so that the
+        // blocks in flight stay around a few sources (C4: 27.5 -> 26.3 ms; the brick path is faster by sorted sources)
+        P.map_src = 0;
+        P.src_order = nullptr;
+        mb2 = rt::march_blocks(P.n_src, P.n_slots, P.n_groups, 0);
+        if (mb2 > 2147483647LL) return RT_EINVAL;
+    }
+    const int rcp = step ? launch_phased<false, true>(P, phased, unsigned(mb2), st) : launch_phased<false, false>(P, phased, unsigned(mb2), st);
+    if (rcp != RT_OK) return rcp;
+    // the snapshots (the step's increment): the fp64 grid plus what the march left in the scratch, rounded once
+    const rt::BrickGeom G = rt::brick_geom(nx, ny, nz);
+    const unsigned fb = unsigned(fin_blocks);
+    if (step) {
+        if (phased == kPhasedOneBin)
+            rt::step_finalize_scratch_kernel<true><<<fb, fin_threads, 0, st>>>(master, P.scratch, out, cells, step->accumulate, G, ny, nz);
+        else if (phased == kPhasedFourBins)
+            rt::step_finalize_scratch_kernel<false><<<fb, fin_threads, 0, st>>>(master, P.scratch, out, cells, step->accumulate, G, ny, nz);
+        else
+            rt::step_finalize_kernel<<<fb, fin_threads, 0, st>>>(master, out, cells, step->accumulate);
+    } else {
+        if (phased == kPhasedOneBin)
+            rt::snapshot_finalize_scratch_kernel<true><<<fb, fin_threads, 0, st>>>(master, P.scratch, out, cells, n_steps, G, ny, nz);
+        else if (phased == kPhasedFourBins)
+            rt::snapshot_finalize_scratch_kernel<false><<<fb, fin_threads, 0, st>>>(master, P.scratch, out, cells, n_steps, G, ny, nz);
+        else
+            rt::snapshot_finalize_kernel<double><<<fb, fin_threads, 0, st>>>(master, out, cells, n_steps);
+    }
+    RT_CUDA(cudaGetLastError());
+    return RT_OK;
+}
+
 int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const float* sources, int n_src, int n_rays,
                int n_bins, float step_size, float c, float dt, int n_steps, float* out, void* workspace,
                size_t workspace_bytes, void* stream, int variant, const StepArgs* step = nullptr,
@@ -339,15 +406,7 @@ int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const
     long long fin_blocks = (ck.cells + fin_threads - 1) / fin_threads;
     if (fin_blocks > 148 * 16) fin_blocks = 148 * 16;
 
-    // 4 bins per thread (16-byte loads, 16-byte fp32 reductions) when the layout allows it -- and, with fp64
-    // accumulation, only on the batched path: there is no 16-byte fp64 reduction, and four scalar ones per voxel
-    // make the 4-bin kernel reduction bound, so larger grids march one bin per thread (bins in adjacent lanes
-    // share the sectors of their fp64 reductions)
     const bool aligned4 = (n_bins % 4 == 0) && !((uintptr_t(j) | uintptr_t(kappa) | uintptr_t(out)) & 15u);
-    const bool batched = aligned4 && !pl.one_bin && pl.acc64 && pl.sliding && use_batched_fp32(ck.cells, n_steps, n_bins);
-    const bool vec4 = aligned4 && !pl.one_bin && (batched || !pl.acc64 || !pl.sliding);
-    P.n_groups = vec4 ? n_bins / 4 : n_bins;
-
     int phased = phased_kind(variant, step_size, ck.cells, n_steps, n_bins, wl.brick_bytes, aligned4);
     if (dkappa) {                      // the tangent march exists in the phased kernel only, one bin per thread
         if (phased == kPhasedNone || step || pl.ktri) return RT_EINVAL;
@@ -355,65 +414,18 @@ int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const
         P.dkappa = dkappa;
     }
     if (pl.ktri && phased == kPhasedFourBins) phased = kPhasedDirect64;      // the trilinear-kappa march: one bin per thread
-    if (phased != kPhasedNone) {
-        // rt_march proper (and rt_march_step): the phased march deposits into an fp32 scratch -- window bricks in the
-        // workspace (one bin), or the plain grid (four bins per thread; `out` itself, or for rt_march_step, whose `out` may
-        // hold the running field, a grid behind the workspace) -- and drains it into the fp64 grid as it goes; or it
-        // reduces straight into the fp64 grid.  The snapshots (the step's increment) are formed from the fp64 grid plus
-        // what the march left in the scratch.
-        P.n_groups = phased == kPhasedFourBins ? n_bins / 4 : n_bins;
-        P.acc = master;
-        P.scratch = phased == kPhasedOneBin ? reinterpret_cast<float*>(ws + wl.brick_at)
-                                            : (step ? reinterpret_cast<float*>(ws + wl.total) : out);
-        const size_t scratch_bytes = phased == kPhasedDirect64 ? 0 : (phased == kPhasedOneBin ? wl.brick_bytes : n_acc * sizeof(float));
-        P.n_drain_units = std::max<long long>(1, (long long)(scratch_bytes / 16));
-        RT_CUDA(cudaMemsetAsync(master, 0, n_acc * sizeof(double), st));
-        if (scratch_bytes) RT_CUDA(cudaMemsetAsync(P.scratch, 0, scratch_bytes, st));
-        const long long mb = rt::march_blocks(P.n_src, P.n_slots, P.n_groups, P.map_src);
-        if (mb > 2147483647LL) return RT_EINVAL;
-        const long long per = (P.n_drain_units * drain_rounds((long long)n_src * n_rays) + mb - 1) / mb;
-        P.drain_units_per_block = std::min<long long>(std::max<long long>(per, 1), rt::kDrainMaxUnits);
-        if (pl.map_src) {
-            // Sources that share their cell fractions (decided on the device) take the weight-table instantiation, others
-            // the plain one: both are launched, each returns at once when the flag says the call is the other's
-            int* flag = reinterpret_cast<int*>(ws + wl.flag_at);
-            rt::same_fraction_kernel<<<1, 256, 0, st>>>(flag, sources, n_src, step_size);
-            P.same_frac = flag;
-            const int rct = step ? launch_phased<true, true>(P, phased, unsigned(mb), st) : launch_phased<true, false>(P, phased, unsigned(mb), st);
-            if (rct != RT_OK) return rct;
-        }
-        long long mb2 = mb;
-        if (phased == kPhasedDirect64 && pl.map_src) {
-            // sources in general position on a grid beyond the L2: warp = 32 (direction, bin) pairs of ONE source, so that the
-            // blocks in flight stay around a few sources (C4: 27.5 -> 26.3 ms; the brick path is faster by sorted sources)
-            P.map_src = 0;
-            P.src_order = nullptr;
-            mb2 = rt::march_blocks(P.n_src, P.n_slots, P.n_groups, 0);
-            if (mb2 > 2147483647LL) return RT_EINVAL;
-        }
-        const int rcp = step ? launch_phased<false, true>(P, phased, unsigned(mb2), st) : launch_phased<false, false>(P, phased, unsigned(mb2), st);
-        if (rcp != RT_OK) return rcp;
-        // the snapshots (the step's increment): the fp64 grid plus what the march left in the scratch, rounded once
-        const rt::BrickGeom G = rt::brick_geom(nx, ny, nz);
-        const unsigned fb = unsigned(fin_blocks);
-        if (step) {
-            if (phased == kPhasedOneBin)
-                rt::step_finalize_scratch_kernel<true><<<fb, fin_threads, 0, st>>>(master, P.scratch, out, ck.cells, step->accumulate, G, ny, nz);
-            else if (phased == kPhasedFourBins)
-                rt::step_finalize_scratch_kernel<false><<<fb, fin_threads, 0, st>>>(master, P.scratch, out, ck.cells, step->accumulate, G, ny, nz);
-            else
-                rt::step_finalize_kernel<<<fb, fin_threads, 0, st>>>(master, out, ck.cells, step->accumulate);
-        } else {
-            if (phased == kPhasedOneBin)
-                rt::snapshot_finalize_scratch_kernel<true><<<fb, fin_threads, 0, st>>>(master, P.scratch, out, ck.cells, n_steps, G, ny, nz);
-            else if (phased == kPhasedFourBins)
-                rt::snapshot_finalize_scratch_kernel<false><<<fb, fin_threads, 0, st>>>(master, P.scratch, out, ck.cells, n_steps, G, ny, nz);
-            else
-                rt::snapshot_finalize_kernel<double><<<fb, fin_threads, 0, st>>>(master, out, ck.cells, n_steps);
-        }
-        RT_CUDA(cudaGetLastError());
-        return RT_OK;
-    }
+    if (phased != kPhasedNone)
+        return run_phased(P, phased, pl, wl, ws, master, out, n_acc, ck.cells, step, nx, ny, nz, sources, n_src, n_rays, n_bins,
+                          step_size, n_steps, st);
+    // What is left: steps of a cell or more and the non-default variants, through march_sliding_kernel / march_kernel.
+    // 4 bins per thread (16-byte loads, 16-byte fp32 reductions) when the layout allows it -- and, with fp64
+    // accumulation, only on the batched path: there is no 16-byte fp64 reduction, and four scalar ones per voxel
+    // make the 4-bin kernel reduction bound, so larger grids march one bin per thread (bins in adjacent lanes
+    // share the sectors of their fp64 reductions)
+    const bool batched = aligned4 && !pl.one_bin && pl.acc64 && pl.sliding && use_batched_fp32(ck.cells, n_steps, n_bins);
+    const bool vec4 = aligned4 && !pl.one_bin && (batched || !pl.acc64 || !pl.sliding);
+    P.n_groups = vec4 ? n_bins / 4 : n_bins;
+
     if (batched) {
         // `out` (rt_march_step: a grid behind the fp64 grid, it may be accumulating into out) is the fp32 scratch
         // grid of ONE batch: no fp32 sum ever holds more than 2^17 rays, which bounds the error of fp32
