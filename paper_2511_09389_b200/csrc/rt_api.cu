@@ -15,6 +15,7 @@
 #include "rt_march_direct.cuh"
 #include "rt_adjoint.cuh"
 #include "rt_brick.cuh"
+#include "rt_chunk.cuh"
 #include "rt_march_phased.cuh"
 #include "rt_march_sliding.cuh"
 #include "rt_setup_kernels.cuh"
@@ -84,7 +85,7 @@ size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 // workspace layout: [ray order: slots u32][source order: n_src u32][flag][fp64 accumulation grid x copies][fp32 scratch]
 // [fp32 window-brick scratch of the one-bin phased march]
 struct Workspace {
-    size_t src_order_at, flag_at, acc_at, scratch2_at, brick_at, brick_bytes, total;
+    size_t src_order_at, flag_at, acc_at, scratch2_at, brick_at, brick_bytes, chunk_at, chunk_bytes, total;
     int acc_copies;
 };
 // One-bin calls deposit into an fp32 brick scratch (rt_brick.cuh): one 16-byte brick per 2 x 2 (y, z) window of each
@@ -97,6 +98,7 @@ size_t brick_scratch_bytes(int nx, int ny, int nz, int n_steps, int n_bins) {
     return bytes <= double(kBrickScratchLimit) ? size_t(g.step_stride) * size_t(n_steps) * sizeof(float) : 0;
 }
 bool use_batched_fp32(long long cells, int n_steps, int n_bins);
+size_t chunk_bytes(int nx, int ny, int nz, int n_src, int n_rays, int n_steps, int n_bins);
 // One-bin-per-thread marches with fp64 reductions (the kernels of the non-default variants and of substeps of a cell or
 // more) spread them over up to 4 copies of the grid, 48 MiB in all
 constexpr size_t kAccCopiesBytes = size_t(48) << 20;
@@ -112,7 +114,9 @@ Workspace workspace_layout(int nx, int ny, int nz, int n_src, int n_rays, int n_
     // the batched fp32 path marches two batches at a time: `out` and this second fp32 grid are their scratch grids
     w.brick_at = align_up(w.scratch2_at + (use_batched_fp32(cells, n_steps, n_bins) ? size_t(cells) * size_t(n_steps) * sizeof(float) : 0), 256);
     w.brick_bytes = brick_scratch_bytes(nx, ny, nz, n_steps, n_bins);
-    w.total = w.brick_at + w.brick_bytes;
+    w.chunk_at = align_up(w.brick_at + w.brick_bytes, 256);
+    w.chunk_bytes = chunk_bytes(nx, ny, nz, n_src, n_rays, n_steps, n_bins);
+    w.total = w.chunk_at + w.chunk_bytes;
     return w;
 }
 
@@ -282,6 +286,20 @@ size_t step_scratch_bytes(long long cells, int n_bins) {
     return use_batched_fp32(cells, 1, n_bins) ? size_t(cells) * sizeof(float) : 0;
 }
 
+// The chunked march (rt_chunk.cuh) of calls whose deposits go straight into an fp64 grid far larger than the L2.
+// Workspace behind the brick scratch: [I: rays x bins f32][exp(-tau): same][perm: rays u32][key: rays u32][hist][cursor]
+int chunk_substeps() {
+    const char* e = std::getenv("RT_CHUNK");
+    return e ? std::atoi(e) : 0;
+}
+size_t chunk_bytes(int nx, int ny, int nz, int n_src, int n_rays, int n_steps, int n_bins) {
+    const long long cells = (long long)nx * ny * nz * n_bins;
+    if ((n_bins == 1 && brick_scratch_bytes(nx, ny, nz, n_steps, n_bins)) || use_batched_fp32(cells, n_steps, n_bins)) return 0;
+    const long long rays = (long long)n_src * n_rays;
+    if (rays >= (1LL << 32)) return 0;
+    return size_t(rays) * (2 * size_t(n_bins) * sizeof(float) + 2 * sizeof(uint32_t)) + 2 * 32768 * sizeof(uint32_t);
+}
+
 // the instantiation of march_phased_kernel for a deposit mode (phased_kind)
 template <bool TABLE, bool STEP>
 int launch_phased(const rt::MarchParams& P, int kind, unsigned blocks, cudaStream_t st) {
@@ -306,6 +324,63 @@ int launch_phased(const rt::MarchParams& P, int kind, unsigned blocks, cudaStrea
     return RT_OK;
 }
 
+// rt_march in chunks of `chunk` substeps with the rays re-sorted by tile before every chunk (rt_chunk.cuh)
+int run_chunked(rt::MarchParams P, const Workspace& wl, char* ws, double* master, float* out, size_t n_acc, long long cells,
+                int nx, int ny, int nz, const float* sources, int n_src, int n_rays, int n_bins, int n_steps, int chunk,
+                int kind, cudaStream_t st) {
+    const long long rays = (long long)n_src * n_rays;
+    float* state_I = reinterpret_cast<float*>(ws + wl.chunk_at);
+    float* state_T = state_I + rays * n_bins;
+    uint32_t* perm = reinterpret_cast<uint32_t*>(state_T + rays * n_bins);
+    uint32_t* key = perm + rays;
+    uint32_t* hist = key + rays;
+    uint32_t* cursor = hist + 32768;
+    const rt::ChunkGeom g = rt::chunk_geom(nx, ny, nz);
+    RT_CUDA(cudaMemsetAsync(master, 0, n_acc * sizeof(double), st));
+    RT_CUDA(cudaMemsetAsync(hist, 0, 32768 * sizeof(uint32_t), st));
+    rt::state_reset_kernel<<<148 * 8, 256, 0, st>>>(state_I, state_T, rays * n_bins);
+    const int n_sub = P.n_sub;
+    P.n_groups = kind == kPhasedFourBins ? n_bins / 4 : n_bins;
+    if (kind == kPhasedFourBins) RT_CUDA(cudaMemsetAsync(out, 0, n_acc * sizeof(float), st));
+    P.map_src = 2;
+    P.perm = perm;
+    P.n_perm = rays;
+    P.src_order = nullptr;
+    P.ray_order = nullptr;
+    P.same_frac = nullptr;
+    P.state_I = state_I;
+    P.state_T = state_T;
+    P.n_steps = 1;
+    const long long mb = rt::perm_blocks(rays, P.n_groups);
+    if (mb > 2147483647LL) return RT_EINVAL;
+    P.n_drain_units = std::max<long long>(1, cells / 4);
+    P.drain_units_per_block = std::min<long long>(std::max<long long>((P.n_drain_units + mb - 1) / mb, 1), rt::kDrainMaxUnits);
+    const unsigned rb = unsigned((rays + 255) / 256);
+    for (int t = 0; t < n_steps; ++t)
+        for (int c0 = 0; c0 < n_sub; c0 += chunk) {
+            const int len = std::min(chunk, n_sub - c0);
+            P.k0 = (long long)t * n_sub + c0;
+            P.n_sub = len;
+            P.acc = master + size_t(t) * size_t(cells);
+            P.scratch = out + size_t(t) * size_t(cells);
+            rt::chunk_key_kernel<<<rb, 256, 0, st>>>(key, hist, sources, rays, n_rays, P.ds, P.k0 + len / 2, nx, ny, nz, g);
+            rt::chunk_scan_kernel<<<1, 1024, 0, st>>>(hist, cursor, g.n_tiles);
+            rt::chunk_scatter_kernel<<<rb, 256, 0, st>>>(perm, key, cursor, rays);
+            const int rcl = launch_phased<false, true>(P, kind, unsigned(mb), st);
+            if (rcl != RT_OK) return rcl;
+        }
+    const int fin_threads = 256;
+    long long fin_blocks = (cells + fin_threads - 1) / fin_threads;
+    if (fin_blocks > 148 * 16) fin_blocks = 148 * 16;
+    if (kind == kPhasedFourBins)
+        rt::snapshot_finalize_scratch_kernel<false><<<unsigned(fin_blocks), fin_threads, 0, st>>>(master, out, out, cells, n_steps,
+                                                                                                 rt::brick_geom(nx, ny, nz), ny, nz);
+    else
+        rt::snapshot_finalize_kernel<double><<<unsigned(fin_blocks), fin_threads, 0, st>>>(master, out, cells, n_steps);
+    RT_CUDA(cudaGetLastError());
+    return RT_OK;
+}
+
 // rt_march proper (and rt_march_step, rt_march_trilinear_kappa, rt_march_jvp_kappa) through march_phased_kernel: memsets,
 // (fraction test, weight-table instantiation,) plain instantiation, snapshots.  P: base parameters with the orders built.
 int run_phased(rt::MarchParams P, int phased, const Plan& pl, const Workspace& wl, char* ws, double* master, float* out,
@@ -319,6 +394,11 @@ int run_phased(rt::MarchParams P, int phased, const Plan& pl, const Workspace& w
     // hold the running field, a grid behind the workspace) -- and drains it into the fp64 grid as it goes; or it
     // reduces straight into the fp64 grid.  The snapshots (the step's increment) are formed from the fp64 grid plus
     // what the march left in the scratch.
+    if (phased == kPhasedDirect64 && !step && !P.dkappa && !P.kappa_trilinear && wl.chunk_bytes && chunk_substeps() > 0)
+        return run_chunked(P, wl, ws, master, out, n_acc, cells, nx, ny, nz, sources, n_src, n_rays, n_bins, n_steps,
+                           chunk_substeps(),
+                           (n_bins % 4 == 0 && !((uintptr_t(P.j) | uintptr_t(P.kappa) | uintptr_t(out)) & 15u) && !std::getenv("RT_CHUNK64"))
+                               ? kPhasedFourBins : kPhasedDirect64, st);
     P.n_groups = phased == kPhasedFourBins ? n_bins / 4 : n_bins;
     P.acc = master;
     P.scratch = phased == kPhasedOneBin ? reinterpret_cast<float*>(ws + wl.brick_at)

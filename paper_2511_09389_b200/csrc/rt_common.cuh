@@ -25,7 +25,10 @@ struct MarchParams {
     int n_groups;                // bin groups per ray (nb / NB)
     int n_steps, n_sub;          // time steps, substeps per step (N_s)
     int kappa_trilinear;         // reading D18 instead of D4 (rt_march_trilinear_kappa)
-    int map_src;                 // 0: the lanes of a warp are 32 directions of one source; 1: 32 sources, one direction
+    int map_src;                 // 0: the lanes of a warp are 32 directions of one source; 1: 32 sources, one direction;
+                                 // 2: consecutive entries of `perm` (rt_chunk.cuh: rays sorted by where they are)
+    const uint32_t* perm;        // map_src = 2: [n_perm] entry = source * n_rays + lattice index
+    long long n_perm;
     double ds;                   // step_size as double
     float ds_f;                  // step_size
     float emis;                  // ds * 4 pi / N_Omega: emission quadrature weight times solid-angle weight (D8)
@@ -200,6 +203,10 @@ struct RayId {
     uint32_t index;   // lattice index
 };
 
+__host__ __device__ inline long long perm_blocks(long long n_perm, int n_groups) {
+    return (n_perm * n_groups + kThreads - 1) / kThreads;
+}
+
 __host__ __device__ inline long long march_blocks(int n_src, int n_slots, int n_groups, int map_src) {
     if (map_src) return (long long)((n_slots + 3) / 4) * (((long long)n_src * n_groups + 31) / 32);
     return (((long long)n_slots * n_groups + kThreads - 1) / kThreads) * n_src;
@@ -208,6 +215,16 @@ __host__ __device__ inline long long march_blocks(int n_src, int n_slots, int n_
 __device__ __forceinline__ bool ray_id(const MarchParams& P, RayId& id) {
     const uint32_t G = uint32_t(P.n_groups);
     uint32_t b = blockIdx.x, slot, s;
+    if (P.map_src == 2) {
+        const long long f = (long long)b * kThreads + threadIdx.x;       // (entry, group), group fastest
+        const long long r = f / G;
+        id.group = int(f - r * G);
+        if (r >= P.n_perm) return false;
+        const uint32_t e = __ldg(P.perm + r);
+        id.src = int(e / uint32_t(P.n_rays));
+        id.index = e - uint32_t(id.src) * uint32_t(P.n_rays);
+        return true;
+    }
     if (P.map_src) {
         const uint32_t chunks = (uint32_t(P.n_slots) + 3u) / 4u;
         slot = (b % chunks) * 4u + (threadIdx.x >> 5);

@@ -149,13 +149,21 @@ __device__ __forceinline__ void brick_flush(const BrickGeom& G, LANE& L, int neg
     if (AX == 2) L.woff += V.nz ? -4 : 4;
 }
 
-// One stencil slide of the lane along axis AX, the trailing plane reduced into the scratch
+// One stencil slide of the lane along axis AX, the trailing plane reduced into the scratch; the loads of the new
+// leading plane are left to Stencil::load_stale (rt_march_sliding.cuh)
 template <int AX, int ACT, bool BRICK, class LANE>
-__device__ __forceinline__ void phased_axis_step(const MarchParams& P, const BrickGeom& G, LANE& L, int negbits) {
+__device__ __forceinline__ void phased_axis_step(const MarchParams& P, const BrickGeom& G, LANE& L, int negbits, uint32_t& stale) {
+#ifdef RT_NO_DEFER
     if constexpr (BRICK)
         L.S.template axis_step_with<AX, ACT>(P, L.A, negbits, P.j, [&]() { brick_flush<AX, ACT>(G, L, negbits); });
     else
         L.S.template axis_step<AX, ACT>(P, L.A, negbits, L.sg, P.j);        // per voxel: one red.v4.f32 (red.f32) of its bins
+#else
+    if constexpr (BRICK)
+        L.S.template axis_slide_deferred<AX, ACT>(P, L.A, negbits, stale, [&]() { brick_flush<AX, ACT>(G, L, negbits); });
+    else      // per voxel: one red.v4.f32 (red.f32, red.f64 per bin) of its bins
+        L.S.template axis_slide_deferred<AX, ACT>(P, L.A, negbits, stale, [&]() { L.S.template flush_trailing<AX, ACT>(L.sg, L.A); });
+#endif
 }
 
 template <int NB, bool JVP, class LANE>
@@ -268,19 +276,21 @@ __device__ __forceinline__ int phase(const MarchParams& P, const BrickGeom& G, L
 
         if constexpr (ACT != 0) {
             if (cross[0] | cross[1] | cross[2]) {     // TABLE: warp-uniform
+                uint32_t stale = 0;
 #pragma unroll
                 for (int a = 0; a < 3; ++a)
                     if ((ACT & (1 << a)) && cross[a]) {
                         if constexpr (TABLE) L.A[a].p.c += 1;
-                        if (a == 0) phased_axis_step<0, ACT, BRICK>(P, G, L, negbits);
-                        if (a == 1) phased_axis_step<1, ACT, BRICK>(P, G, L, negbits);
-                        if (a == 2) phased_axis_step<2, ACT, BRICK>(P, G, L, negbits);
+                        if (a == 0) phased_axis_step<0, ACT, BRICK>(P, G, L, negbits, stale);
+                        if (a == 1) phased_axis_step<1, ACT, BRICK>(P, G, L, negbits, stale);
+                        if (a == 2) phased_axis_step<2, ACT, BRICK>(P, G, L, negbits, stale);
                         if constexpr (TABLE) {       // every lane crosses in the same substep: vote right here
                             const int lim = (a == 0 ? P.nx : (a == 1 ? P.ny : P.nz)) - 1;
                             const bool gone = L.A[a].p.c >= ((negbits & (1 << a)) ? 0 : lim);    // beyond the far face for good
                             if (__all_sync(0xFFFFFFFFu, gone)) next &= ~(1 << a);
                         }
                     }
+                L.S.template load_stale<ACT>(P, L.A, P.j, stale);
                 if constexpr (!KTRI) {
                     int ko = L.S.base;       // kappa: nearest neighbour at clamp(floor(x_k)) (D4)
                     if (ACT & 1) ko += (negbits & 1) ? L.A[0].dl : 0;
