@@ -63,28 +63,55 @@ __device__ __forceinline__ void red_v2(float* p, float a, float b) {
 }
 
 // Drain bricks [b_begin, b_end) of the scratch (all time steps: brick b = ((m * nx + x) * wy + Y0) * wz + Z0) into the
-// fp64 grid master[m][x][y][z]; thread `t` of `n_threads` takes every n_threads-th brick.
-// CONCURRENT: safe while other blocks reduce into the same elements (see above).
+// fp64 grid master[m][x][y][z]; thread `t` of `n_threads` takes every n_threads-th brick, kDrainBatch at a time: the
+// peeks of a batch are in flight together, then its exchanges, then its reductions (a thread waits for three round
+// trips per batch instead of five per brick).
+// CONCURRENT: safe while other blocks reduce into the same elements (see above).  An element that reads zero at the
+// peek is left alone (whatever arrives later stays for the next drain or for the snapshots).
+constexpr int kDrainBatch = 4;
+
+__device__ __forceinline__ uint32_t drain_take(float* e, float seen) {
+    uint32_t bits = 0u;
+    if (seen != 0.0f) asm volatile("atom.global.exch.b32 %0, [%1], %2;" : "=r"(bits) : "l"(e), "r"(0u) : "memory");
+    return bits;
+}
+__device__ __forceinline__ void drain_give(double* m, uint32_t bits) {
+    if (bits != 0u) asm volatile("red.global.add.f64 [%0], %1;" ::"l"(m), "d"(double(__uint_as_float(bits))) : "memory");
+}
+
 __device__ __forceinline__ void drain_bricks(float* scratch, double* master, const BrickGeom& G, int nx, int ny, int nz,
                                              long long b_begin, long long b_end, int t, int n_threads) {
-    for (long long b = b_begin + t; b < b_end; b += n_threads) {
-        float* e = scratch + 4 * b;
-        const float4 peek = __ldcg(reinterpret_cast<const float4*>(e));      // a hint only: all zero -> nothing to take
-        if (peek.x == 0.0f && peek.y == 0.0f && peek.z == 0.0f && peek.w == 0.0f) continue;
-        const long long r = b / G.wz;
-        const int Z0 = int(b - r * G.wz);
-        const long long mx = r / G.wy;                      // m * nx + x
-        const int Y0 = int(r - mx * G.wy);
-        double* row = master + mx * ((long long)ny * nz);
+    for (long long b0 = b_begin + t; b0 < b_end; b0 += (long long)kDrainBatch * n_threads) {
+        float4 peek[kDrainBatch];
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            const int y = Y0 - 1 + (i >> 1), z = Z0 - 1 + (i & 1);
-            if (uint32_t(y) >= uint32_t(ny) || uint32_t(z) >= uint32_t(nz)) continue;      // padding: only zeros arrive
-            uint32_t bits;
-            asm volatile("atom.global.exch.b32 %0, [%1], %2;" : "=r"(bits) : "l"(e + i), "r"(0u) : "memory");
-            const float v = __uint_as_float(bits);
-            if (v != 0.0f)
-                asm volatile("red.global.add.f64 [%0], %1;" ::"l"(row + (long long)y * nz + z), "d"(double(v)) : "memory");
+        for (int q = 0; q < kDrainBatch; ++q) {
+            const long long b = b0 + (long long)q * n_threads;
+            peek[q] = b < b_end ? __ldcg(reinterpret_cast<const float4*>(scratch + 4 * b)) : make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+        }
+        uint32_t bits[kDrainBatch][4];
+#pragma unroll
+        for (int q = 0; q < kDrainBatch; ++q) {
+            float* e = scratch + 4 * (b0 + (long long)q * n_threads);
+            bits[q][0] = drain_take(e, peek[q].x);
+            bits[q][1] = drain_take(e + 1, peek[q].y);
+            bits[q][2] = drain_take(e + 2, peek[q].z);
+            bits[q][3] = drain_take(e + 3, peek[q].w);
+        }
+#pragma unroll
+        for (int q = 0; q < kDrainBatch; ++q) {
+            if ((bits[q][0] | bits[q][1] | bits[q][2] | bits[q][3]) == 0u) continue;
+            const long long b = b0 + (long long)q * n_threads;
+            const long long r = b / G.wz;
+            const int Z0 = int(b - r * G.wz);
+            const long long mx = r / G.wy;                      // m * nx + x
+            const int Y0 = int(r - mx * G.wy);
+            double* row = master + mx * ((long long)ny * nz);
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const int y = Y0 - 1 + (i >> 1), z = Z0 - 1 + (i & 1);
+                if (uint32_t(y) >= uint32_t(ny) || uint32_t(z) >= uint32_t(nz)) continue;      // padding: only zeros arrive
+                drain_give(row + (long long)y * nz + z, bits[q][i]);
+            }
         }
     }
 }
@@ -93,16 +120,27 @@ __device__ __forceinline__ void drain_bricks(float* scratch, double* master, con
 // floats [u_begin, u_end), element e of the scratch belongs to element e of the fp64 grid.
 __device__ __forceinline__ void drain_plain(float* scratch, double* master, long long u_begin, long long u_end, int t,
                                             int n_threads) {
-    for (long long u = u_begin + t; u < u_end; u += n_threads) {
-        float* e = scratch + 4 * u;
-        const float4 peek = __ldcg(reinterpret_cast<const float4*>(e));      // a hint only: all zero -> nothing to take
-        if (peek.x == 0.0f && peek.y == 0.0f && peek.z == 0.0f && peek.w == 0.0f) continue;
+    for (long long u0 = u_begin + t; u0 < u_end; u0 += (long long)kDrainBatch * n_threads) {
+        float4 peek[kDrainBatch];
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            uint32_t bits;
-            asm volatile("atom.global.exch.b32 %0, [%1], %2;" : "=r"(bits) : "l"(e + i), "r"(0u) : "memory");
-            const float v = __uint_as_float(bits);
-            if (v != 0.0f) asm volatile("red.global.add.f64 [%0], %1;" ::"l"(master + 4 * u + i), "d"(double(v)) : "memory");
+        for (int q = 0; q < kDrainBatch; ++q) {
+            const long long u = u0 + (long long)q * n_threads;
+            peek[q] = u < u_end ? __ldcg(reinterpret_cast<const float4*>(scratch + 4 * u)) : make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+        }
+        uint32_t bits[kDrainBatch][4];
+#pragma unroll
+        for (int q = 0; q < kDrainBatch; ++q) {
+            float* e = scratch + 4 * (u0 + (long long)q * n_threads);
+            bits[q][0] = drain_take(e, peek[q].x);
+            bits[q][1] = drain_take(e + 1, peek[q].y);
+            bits[q][2] = drain_take(e + 2, peek[q].z);
+            bits[q][3] = drain_take(e + 3, peek[q].w);
+        }
+#pragma unroll
+        for (int q = 0; q < kDrainBatch; ++q) {
+            double* m = master + 4 * (u0 + (long long)q * n_threads);
+#pragma unroll
+            for (int i = 0; i < 4; ++i) drain_give(m + i, bits[q][i]);
         }
     }
 }

@@ -71,6 +71,7 @@ template <int NB, typename ACC = float, bool JVP = false, bool KTRI = false> str
     Stencil<NB, ACC, KTRI> S;
     TravelAxis A[3];         // TABLE: only the cell word, dl and fmask are used
     float I[NB], T[NB], att[NB];   // I scaled by 4 pi/N_Omega; T = exp(-tau) ds 4 pi/N_Omega; att = exp(-kappa ds) of the kappa cell
+                                   // (kappa itself in the instantiations that convert per substep, phased_load_att)
     float Id[JVP ? NB : 1], Td[JVP ? NB : 1], u[JVP ? NB : 1];     // JVP (D21): tangents of I and T, and dkappa ds of the kappa cell
     ACC* sg;                 // scratch (fp64 grid if ACC = double) of the current time step
     int woff;                // NB == 1: float offset in it of the window the trailing slots start (rt_brick.cuh)
@@ -166,15 +167,18 @@ __device__ __forceinline__ void phased_axis_step(const MarchParams& P, const Bri
 #endif
 }
 
-template <int NB, bool JVP, class LANE>
+// kappa of the cell the lane is in (and dkappa of it, JVP).  RAW: the values are kept as loaded and turned into
+// exp(-kappa ds) (dkappa ds) where a substep uses them -- in the instantiations whose lanes cross cell planes on their
+// own the conversion right here would wait for the load in every substep (ncu: the top stall of the chunked march)
+template <int NB, bool JVP, bool RAW, class LANE>
 __device__ __forceinline__ void phased_load_att(const MarchParams& P, LANE& L, int ko) {
     const BinVec<NB> kap = ld_bins<NB>(P.kappa + ko);
 #pragma unroll
-    for (int b = 0; b < NB; ++b) L.att[b] = ex2_approx(kap.v[b] * P.att_scale);
+    for (int b = 0; b < NB; ++b) L.att[b] = RAW ? kap.v[b] : ex2_approx(kap.v[b] * P.att_scale);
     if constexpr (JVP) {
         const BinVec<NB> dk = ld_bins<NB>(P.dkappa + ko);
 #pragma unroll
-        for (int b = 0; b < NB; ++b) L.u[b] = dk.v[b] * P.ds_f;
+        for (int b = 0; b < NB; ++b) L.u[b] = RAW ? dk.v[b] : dk.v[b] * P.ds_f;
     }
 }
 
@@ -185,6 +189,7 @@ __device__ __forceinline__ int phase(const MarchParams& P, const BrickGeom& G, L
     constexpr int kBits = ((ACT & 1) ? 4 : 0) | ((ACT & 2) ? 2 : 0) | ((ACT & 4) ? 1 : 0);      // slot index bits in use
     constexpr int kActive = ((ACT & 1) ? 1 : 0) + ((ACT & 2) ? 1 : 0) + ((ACT & 4) ? 1 : 0);
     constexpr int kLast = (ACT & 4) ? 2 : ((ACT & 2) ? 1 : 0);                                   // the last active axis
+    constexpr bool RAW = !TABLE && !KTRI;      // L.att holds kappa itself (phased_load_att)
     int next = ACT;
     do {
         float w[8];
@@ -258,15 +263,17 @@ __device__ __forceinline__ int phase(const MarchParams& P, const BrickGeom& G, L
                 }
                 L.att[b] = ex2_approx(kv * P.att_scale);
             }
+            const float att = RAW ? ex2_approx(L.att[b] * P.att_scale) : L.att[b];
             if constexpr (JVP) {
                 // the tangent of eq. (2) for kappa -> kappa + eps dkappa (D21), u = dkappa_k ds:
                 //   Idot_{k+1} = a_k (Idot_k - I_k u) + J_k Tdot_k,   Tdot_{k+1} = a_k (Tdot_k - T_k u)      (old I, T on the right)
-                L.Id[b] = fmaf(L.att[b], fmaf(-L.I[b], L.u[b], L.Id[b]), (jv + ju) * L.Td[b]);
-                L.Td[b] = L.att[b] * fmaf(-L.T[b], L.u[b], L.Td[b]);
+                const float u = RAW ? L.u[b] * P.ds_f : L.u[b];
+                L.Id[b] = fmaf(att, fmaf(-L.I[b], u, L.Id[b]), (jv + ju) * L.Td[b]);
+                L.Td[b] = att * fmaf(-L.T[b], u, L.Td[b]);
             }
             // eq. (2).  STEP: T is the carried exp(-tau) itself, else ds 4 pi/N_Omega rides on it
-            L.I[b] = fmaf(L.I[b], L.att[b], STEP ? (jv + ju) * L.T[b] * P.emis : (jv + ju) * L.T[b]);
-            L.T[b] *= L.att[b];
+            L.I[b] = fmaf(L.I[b], att, STEP ? (jv + ju) * L.T[b] * P.emis : (jv + ju) * L.T[b]);
+            L.T[b] *= att;
             const float dep = JVP ? L.Id[b] : L.I[b];           // what is deposited, with the weights of x_k
 #pragma unroll
             for (int s = 0; s < 8; ++s)
@@ -296,7 +303,7 @@ __device__ __forceinline__ int phase(const MarchParams& P, const BrickGeom& G, L
                     if (ACT & 1) ko += (negbits & 1) ? L.A[0].dl : 0;
                     if (ACT & 2) ko += (negbits & 2) ? L.A[1].dl : 0;
                     if (ACT & 4) ko += (negbits & 4) ? L.A[2].dl : 0;
-                    phased_load_att<NB, JVP>(P, L, ko);
+                    phased_load_att<NB, JVP, RAW>(P, L, ko);
                 }
             }
             if constexpr (!TABLE) {
@@ -396,7 +403,7 @@ march_phased_kernel(const MarchParams P) {
 #pragma unroll
             for (int b = 0; b < NB; ++b) L.att[b] = 1.0f;
         } else {
-            phased_load_att<NB, JVP>(P, L, L.S.base + ((negbits & 1) ? L.A[0].dl : 0) + ((negbits & 2) ? L.A[1].dl : 0) +
+            phased_load_att<NB, JVP, !TABLE>(P, L, L.S.base + ((negbits & 1) ? L.A[0].dl : 0) + ((negbits & 2) ? L.A[1].dl : 0) +
                                           ((negbits & 4) ? L.A[2].dl : 0));
         }
         L.g = 0;
