@@ -15,7 +15,7 @@
 #include "rt_march_direct.cuh"
 #include "rt_adjoint.cuh"
 #include "rt_brick.cuh"
-#include "rt_chunk.cuh"
+#include "rt_ray_sort.cuh"
 #include "rt_march_phased.cuh"
 #include "rt_march_sliding.cuh"
 #include "rt_setup_kernels.cuh"
@@ -83,9 +83,9 @@ int check_args(const void* j, const void* kappa, int nx, int ny, int nz, const v
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 // workspace layout: [ray order: slots u32][source order: n_src u32][flag][fp64 accumulation grid x copies][fp32 scratch]
-// [fp32 window-brick scratch of the one-bin phased march]
+// [fp32 window-brick scratch of the one-bin phased march][sorted ray list of marches over grids beyond the L2]
 struct Workspace {
-    size_t src_order_at, flag_at, acc_at, scratch2_at, brick_at, brick_bytes, chunk_at, chunk_bytes, total;
+    size_t src_order_at, flag_at, acc_at, scratch2_at, brick_at, brick_bytes, sort_at, sort_bytes, total;
     int acc_copies;
 };
 // One-bin calls deposit into an fp32 brick scratch (rt_brick.cuh): one 16-byte brick per 2 x 2 (y, z) window of each
@@ -98,7 +98,7 @@ size_t brick_scratch_bytes(int nx, int ny, int nz, int n_steps, int n_bins) {
     return bytes <= double(kBrickScratchLimit) ? size_t(g.step_stride) * size_t(n_steps) * sizeof(float) : 0;
 }
 bool use_batched_fp32(long long cells, int n_steps, int n_bins);
-size_t chunk_bytes(int nx, int ny, int nz, int n_src, int n_rays, int n_steps, int n_bins);
+size_t ray_sort_bytes(int nx, int ny, int nz, int n_src, int n_rays, int n_steps, int n_bins);
 // One-bin-per-thread marches with fp64 reductions (the kernels of the non-default variants and of substeps of a cell or
 // more) spread them over up to 4 copies of the grid, 48 MiB in all
 constexpr size_t kAccCopiesBytes = size_t(48) << 20;
@@ -114,9 +114,9 @@ Workspace workspace_layout(int nx, int ny, int nz, int n_src, int n_rays, int n_
     // the batched fp32 path marches two batches at a time: `out` and this second fp32 grid are their scratch grids
     w.brick_at = align_up(w.scratch2_at + (use_batched_fp32(cells, n_steps, n_bins) ? size_t(cells) * size_t(n_steps) * sizeof(float) : 0), 256);
     w.brick_bytes = brick_scratch_bytes(nx, ny, nz, n_steps, n_bins);
-    w.chunk_at = align_up(w.brick_at + w.brick_bytes, 256);
-    w.chunk_bytes = chunk_bytes(nx, ny, nz, n_src, n_rays, n_steps, n_bins);
-    w.total = w.chunk_at + w.chunk_bytes;
+    w.sort_at = align_up(w.brick_at + w.brick_bytes, 256);
+    w.sort_bytes = ray_sort_bytes(nx, ny, nz, n_src, n_rays, n_steps, n_bins);
+    w.total = w.sort_at + w.sort_bytes;
     return w;
 }
 
@@ -223,6 +223,24 @@ int phased_kind(int variant, float step_size, long long cells, int n_steps, int 
     if (n_bins % 4 == 0 && aligned16 && use_batched_fp32(cells, n_steps, n_bins)) return kPhasedFourBins;
     return kPhasedDirect64;
 }
+// SORTED (the workspace has a ray list, ray_sort_bytes): the grid is far larger than the L2 and the threads take their
+// rays from the list sorted by tile (rt_ray_sort.cuh).  Bins in groups of four then deposit as in kPhasedFourBins -- with
+// the traffic kept local the fp32 scratch pays again (C4: 17.3 ms, against 20.5 ms with red.global.add.f64 per bin and
+// 25.4 ms with that and the rays by direction).
+struct PhasedPlan {
+    int kind;
+    bool sorted;
+};
+PhasedPlan phased_plan(int variant, float step_size, long long cells, int n_steps, int n_bins, const Workspace& wl, bool aligned16,
+                       bool one_bin_per_thread) {
+    PhasedPlan pp;
+    pp.kind = phased_kind(variant, step_size, cells, n_steps, n_bins, wl.brick_bytes, aligned16);
+    pp.sorted = pp.kind == kPhasedDirect64 && wl.sort_bytes != 0;
+    if (pp.sorted && n_bins % 4 == 0 && aligned16) pp.kind = kPhasedFourBins;
+    // the trilinear-kappa and the tangent march exist with one bin per thread only
+    if (one_bin_per_thread && pp.kind == kPhasedFourBins) pp.kind = kPhasedDirect64;
+    return pp;
+}
 // how often the scratch is drained during a march: an fp32 sum should not collect much more than 2^19 rays' deposits
 // (C2, 8.6 M rays: 16 rounds, relative L2 error 6e-6 against 2.5e-5 with 4 rounds and 1.2e-4 with none)
 int drain_rounds(long long n_rays_total) {
@@ -282,22 +300,22 @@ struct StepArgs {
     int accumulate;
 };
 
+// rt_march_step with four bins per thread (phased_plan): the fp32 scratch grid behind the workspace
 size_t step_scratch_bytes(long long cells, int n_bins) {
-    return use_batched_fp32(cells, 1, n_bins) ? size_t(cells) * sizeof(float) : 0;
+    return n_bins % 4 == 0 ? size_t(cells) * sizeof(float) : 0;
 }
 
-// The chunked march (rt_chunk.cuh) of calls whose deposits go straight into an fp64 grid far larger than the L2.
-// Workspace behind the brick scratch: [I: rays x bins f32][exp(-tau): same][perm: rays u32][key: rays u32][hist][cursor]
-int chunk_substeps() {
-    const char* e = std::getenv("RT_CHUNK");
-    return e ? std::atoi(e) : 0;
-}
-size_t chunk_bytes(int nx, int ny, int nz, int n_src, int n_rays, int n_steps, int n_bins) {
+// Marches over grids far larger than the L2 -- the fp32 grid of all time steps beyond kBatchedScratchLimit, no brick
+// scratch -- map their threads to rays through a list sorted by tile (rt_ray_sort.cuh).
+// Workspace behind the brick scratch: [perm: rays u32][key: rays u32][hist: kRayTiles u32][cursor: kRayTiles u32]
+size_t ray_sort_bytes(int nx, int ny, int nz, int n_src, int n_rays, int n_steps, int n_bins) {
     const long long cells = (long long)nx * ny * nz * n_bins;
-    if ((n_bins == 1 && brick_scratch_bytes(nx, ny, nz, n_steps, n_bins)) || use_batched_fp32(cells, n_steps, n_bins)) return 0;
+    if ((n_bins == 1 && brick_scratch_bytes(nx, ny, nz, n_steps, n_bins)) ||
+        size_t(cells) * size_t(n_steps) * sizeof(float) <= kBatchedScratchLimit)
+        return 0;
     const long long rays = (long long)n_src * n_rays;
     if (rays >= (1LL << 32)) return 0;
-    return size_t(rays) * (2 * size_t(n_bins) * sizeof(float) + 2 * sizeof(uint32_t)) + 2 * 32768 * sizeof(uint32_t);
+    return size_t(rays) * 2 * sizeof(uint32_t) + 2 * size_t(rt::kRayTiles) * sizeof(uint32_t);
 }
 
 // the instantiation of march_phased_kernel for a deposit mode (phased_kind)
@@ -324,81 +342,20 @@ int launch_phased(const rt::MarchParams& P, int kind, unsigned blocks, cudaStrea
     return RT_OK;
 }
 
-// rt_march in chunks of `chunk` substeps with the rays re-sorted by tile before every chunk (rt_chunk.cuh)
-int run_chunked(rt::MarchParams P, const Workspace& wl, char* ws, double* master, float* out, size_t n_acc, long long cells,
-                int nx, int ny, int nz, const float* sources, int n_src, int n_rays, int n_bins, int n_steps, int chunk,
-                int kind, cudaStream_t st) {
-    const long long rays = (long long)n_src * n_rays;
-    float* state_I = reinterpret_cast<float*>(ws + wl.chunk_at);
-    float* state_T = state_I + rays * n_bins;
-    uint32_t* perm = reinterpret_cast<uint32_t*>(state_T + rays * n_bins);
-    uint32_t* key = perm + rays;
-    uint32_t* hist = key + rays;
-    uint32_t* cursor = hist + 32768;
-    const rt::ChunkGeom g = rt::chunk_geom(nx, ny, nz);
-    RT_CUDA(cudaMemsetAsync(master, 0, n_acc * sizeof(double), st));
-    RT_CUDA(cudaMemsetAsync(hist, 0, 32768 * sizeof(uint32_t), st));
-    rt::state_reset_kernel<<<148 * 8, 256, 0, st>>>(state_I, state_T, rays * n_bins);
-    const int n_sub = P.n_sub;
-    P.n_groups = kind == kPhasedFourBins ? n_bins / 4 : n_bins;
-    if (kind == kPhasedFourBins) RT_CUDA(cudaMemsetAsync(out, 0, n_acc * sizeof(float), st));
-    P.map_src = 2;
-    P.perm = perm;
-    P.n_perm = rays;
-    P.src_order = nullptr;
-    P.ray_order = nullptr;
-    P.same_frac = nullptr;
-    P.state_I = state_I;
-    P.state_T = state_T;
-    P.n_steps = 1;
-    const long long mb = rt::perm_blocks(rays, P.n_groups);
-    if (mb > 2147483647LL) return RT_EINVAL;
-    P.n_drain_units = std::max<long long>(1, cells / 4);
-    P.drain_units_per_block = std::min<long long>(std::max<long long>((P.n_drain_units + mb - 1) / mb, 1), rt::kDrainMaxUnits);
-    const unsigned rb = unsigned((rays + 255) / 256);
-    for (int t = 0; t < n_steps; ++t)
-        for (int c0 = 0; c0 < n_sub; c0 += chunk) {
-            const int len = std::min(chunk, n_sub - c0);
-            P.k0 = (long long)t * n_sub + c0;
-            P.n_sub = len;
-            P.acc = master + size_t(t) * size_t(cells);
-            P.scratch = out + size_t(t) * size_t(cells);
-            rt::chunk_key_kernel<<<rb, 256, 0, st>>>(key, hist, sources, rays, n_rays, P.ds, P.k0 + len / 2, nx, ny, nz, g);
-            rt::chunk_scan_kernel<<<1, 1024, 0, st>>>(hist, cursor, g.n_tiles);
-            rt::chunk_scatter_kernel<<<rb, 256, 0, st>>>(perm, key, cursor, rays);
-            const int rcl = launch_phased<false, true>(P, kind, unsigned(mb), st);
-            if (rcl != RT_OK) return rcl;
-        }
-    const int fin_threads = 256;
-    long long fin_blocks = (cells + fin_threads - 1) / fin_threads;
-    if (fin_blocks > 148 * 16) fin_blocks = 148 * 16;
-    if (kind == kPhasedFourBins)
-        rt::snapshot_finalize_scratch_kernel<false><<<unsigned(fin_blocks), fin_threads, 0, st>>>(master, out, out, cells, n_steps,
-                                                                                                 rt::brick_geom(nx, ny, nz), ny, nz);
-    else
-        rt::snapshot_finalize_kernel<double><<<unsigned(fin_blocks), fin_threads, 0, st>>>(master, out, cells, n_steps);
-    RT_CUDA(cudaGetLastError());
-    return RT_OK;
-}
-
 // rt_march proper (and rt_march_step, rt_march_trilinear_kappa, rt_march_jvp_kappa) through march_phased_kernel: memsets,
-// (fraction test, weight-table instantiation,) plain instantiation, snapshots.  P: base parameters with the orders built.
-int run_phased(rt::MarchParams P, int phased, const Plan& pl, const Workspace& wl, char* ws, double* master, float* out,
+// the thread -> ray map (ray and source order; or the sorted ray list), (fraction test, weight-table instantiation,)
+// plain instantiation, snapshots.
+int run_phased(rt::MarchParams P, const PhasedPlan& pp, const Plan& pl, const Workspace& wl, char* ws, double* master, float* out,
                size_t n_acc, long long cells, const StepArgs* step, int nx, int ny, int nz, const float* sources, int n_src,
                int n_rays, int n_bins, float step_size, int n_steps, cudaStream_t st) {
     const int fin_threads = 256;
     long long fin_blocks = (cells + fin_threads - 1) / fin_threads;
     if (fin_blocks > 148 * 16) fin_blocks = 148 * 16;
-    // rt_march proper (and rt_march_step): the phased march deposits into an fp32 scratch -- window bricks in the
-    // workspace (one bin), or the plain grid (four bins per thread; `out` itself, or for rt_march_step, whose `out` may
-    // hold the running field, a grid behind the workspace) -- and drains it into the fp64 grid as it goes; or it
-    // reduces straight into the fp64 grid.  The snapshots (the step's increment) are formed from the fp64 grid plus
-    // what the march left in the scratch.
-    if (phased == kPhasedDirect64 && !step && !P.dkappa && !P.kappa_trilinear && wl.chunk_bytes && chunk_substeps() > 0)
-        return run_chunked(P, wl, ws, master, out, n_acc, cells, nx, ny, nz, sources, n_src, n_rays, n_bins, n_steps,
-                           chunk_substeps(),
-                           (n_bins % 4 == 0 && !((uintptr_t(P.j) | uintptr_t(P.kappa) | uintptr_t(out)) & 15u) && !std::getenv("RT_CHUNK64"))
-                               ? kPhasedFourBins : kPhasedDirect64, st);
+    const int phased = pp.kind;
+    // The phased march deposits into an fp32 scratch -- window bricks in the workspace (one bin), or the plain grid
+    // (four bins per thread; `out` itself, or for rt_march_step, whose `out` may hold the running field, a grid behind
+    // the workspace) -- and drains it into the fp64 grid as it goes; or it reduces straight into the fp64 grid.  The
+    // snapshots (the step's increment) are formed from the fp64 grid plus what the march left in the scratch.
     P.n_groups = phased == kPhasedFourBins ? n_bins / 4 : n_bins;
     P.acc = master;
     P.scratch = phased == kPhasedOneBin ? reinterpret_cast<float*>(ws + wl.brick_at)
@@ -407,11 +364,35 @@ int run_phased(rt::MarchParams P, int phased, const Plan& pl, const Workspace& w
     P.n_drain_units = std::max<long long>(1, (long long)(scratch_bytes / 16));
     RT_CUDA(cudaMemsetAsync(master, 0, n_acc * sizeof(double), st));
     if (scratch_bytes) RT_CUDA(cudaMemsetAsync(P.scratch, 0, scratch_bytes, st));
-    const long long mb = rt::march_blocks(P.n_src, P.n_slots, P.n_groups, P.map_src);
+    const long long n_ray = (long long)n_src * n_rays;
+    long long mb;
+    if (pp.sorted) {
+        // key = tile at the middle of the marched substeps, histogram, prefix sums, scatter
+        uint32_t* perm = reinterpret_cast<uint32_t*>(ws + wl.sort_at);
+        uint32_t* key = perm + n_ray;
+        uint32_t* hist = key + n_ray;
+        uint32_t* cursor = hist + rt::kRayTiles;
+        RT_CUDA(cudaMemsetAsync(hist, 0, rt::kRayTiles * sizeof(uint32_t), st));
+        const unsigned rb = unsigned((n_ray + 255) / 256);
+        const long long k_mid = P.k0 + (long long)P.n_sub * n_steps / 2;
+        rt::ray_tile_key_kernel<<<rb, 256, 0, st>>>(key, hist, sources, n_ray, n_rays, P.ds, k_mid, nx, ny, nz,
+                                                    rt::ray_tile_shift(nx, ny, nz));
+        rt::ray_tile_scan_kernel<<<1, 1024, 0, st>>>(hist, cursor, rt::kRayTiles);
+        rt::ray_tile_scatter_kernel<<<rb, 256, 0, st>>>(perm, key, cursor, n_ray);
+        RT_CUDA(cudaGetLastError());
+        P.map_src = 2;
+        P.perm = perm;
+        P.n_perm = n_ray;
+        mb = rt::perm_blocks(n_ray, P.n_groups);
+    } else {
+        const int rco = build_orders(P, pl, wl, ws, st);
+        if (rco != RT_OK) return rco;
+        mb = rt::march_blocks(P.n_src, P.n_slots, P.n_groups, P.map_src);
+    }
     if (mb > 2147483647LL) return RT_EINVAL;
-    const long long per = (P.n_drain_units * drain_rounds((long long)n_src * n_rays) + mb - 1) / mb;
+    const long long per = (P.n_drain_units * drain_rounds(n_ray) + mb - 1) / mb;
     P.drain_units_per_block = std::min<long long>(std::max<long long>(per, 1), rt::kDrainMaxUnits);
-    if (pl.map_src) {
+    if (pl.map_src && !pp.sorted) {
         // Sources that share their cell fractions (decided on the device) take the weight-table instantiation, others
         // the plain one: both are launched, each returns at once when the flag says the call is the other's
         int* flag = reinterpret_cast<int*>(ws + wl.flag_at);
@@ -420,16 +401,15 @@ int run_phased(rt::MarchParams P, int phased, const Plan& pl, const Workspace& w
         const int rct = step ? launch_phased<true, true>(P, phased, unsigned(mb), st) : launch_phased<true, false>(P, phased, unsigned(mb), st);
         if (rct != RT_OK) return rct;
     }
-    long long mb2 = mb;
-    if (phased == kPhasedDirect64 && pl.map_src) {
-        // sources in general position on a grid beyond the L2: warp = 32 (direction, bin) pairs of ONE source, so that the
-        // blocks in flight stay around a few sources (C4: 27.5 -> 26.3 ms; the brick path is faster by sorted sources)
+    if (phased == kPhasedDirect64 && pl.map_src && !pp.sorted) {
+        // sources in general position, fp64 reductions: warp = 32 (direction, bin) pairs of ONE source, so that the
+        // blocks in flight stay around a few sources (the brick path is faster by sorted sources)
         P.map_src = 0;
         P.src_order = nullptr;
-        mb2 = rt::march_blocks(P.n_src, P.n_slots, P.n_groups, 0);
-        if (mb2 > 2147483647LL) return RT_EINVAL;
+        mb = rt::march_blocks(P.n_src, P.n_slots, P.n_groups, 0);
+        if (mb > 2147483647LL) return RT_EINVAL;
     }
-    const int rcp = step ? launch_phased<false, true>(P, phased, unsigned(mb2), st) : launch_phased<false, false>(P, phased, unsigned(mb2), st);
+    const int rcp = step ? launch_phased<false, true>(P, phased, unsigned(mb), st) : launch_phased<false, false>(P, phased, unsigned(mb), st);
     if (rcp != RT_OK) return rcp;
     // the snapshots (the step's increment): the fp64 grid plus what the march left in the scratch, rounded once
     const rt::BrickGeom G = rt::brick_geom(nx, ny, nz);
@@ -478,8 +458,6 @@ int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const
     P.state_I = step ? step->state : nullptr;
     P.state_T = step ? step->state + size_t(n_src) * size_t(n_rays) * size_t(n_bins) : nullptr;
     P.k0 = step ? step->k0 : 0;
-    const int rco = build_orders(P, pl, wl, ws, st);
-    if (rco != RT_OK) return rco;
     const size_t n_acc = size_t(ck.cells) * size_t(n_steps);
     double* master = reinterpret_cast<double*>(ws + wl.acc_at);
     const int fin_threads = 256;
@@ -487,16 +465,16 @@ int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const
     if (fin_blocks > 148 * 16) fin_blocks = 148 * 16;
 
     const bool aligned4 = (n_bins % 4 == 0) && !((uintptr_t(j) | uintptr_t(kappa) | uintptr_t(out)) & 15u);
-    int phased = phased_kind(variant, step_size, ck.cells, n_steps, n_bins, wl.brick_bytes, aligned4);
-    if (dkappa) {                      // the tangent march exists in the phased kernel only, one bin per thread
-        if (phased == kPhasedNone || step || pl.ktri) return RT_EINVAL;
-        if (phased == kPhasedFourBins) phased = kPhasedDirect64;
+    const PhasedPlan pp = phased_plan(variant, step_size, ck.cells, n_steps, n_bins, wl, aligned4, dkappa || pl.ktri);
+    if (dkappa) {                      // the tangent march exists in the phased kernel only
+        if (pp.kind == kPhasedNone || step || pl.ktri) return RT_EINVAL;
         P.dkappa = dkappa;
     }
-    if (pl.ktri && phased == kPhasedFourBins) phased = kPhasedDirect64;      // the trilinear-kappa march: one bin per thread
-    if (phased != kPhasedNone)
-        return run_phased(P, phased, pl, wl, ws, master, out, n_acc, ck.cells, step, nx, ny, nz, sources, n_src, n_rays, n_bins,
+    if (pp.kind != kPhasedNone)
+        return run_phased(P, pp, pl, wl, ws, master, out, n_acc, ck.cells, step, nx, ny, nz, sources, n_src, n_rays, n_bins,
                           step_size, n_steps, st);
+    const int rco = build_orders(P, pl, wl, ws, st);
+    if (rco != RT_OK) return rco;
     // What is left: steps of a cell or more and the non-default variants, through march_sliding_kernel / march_kernel.
     // 4 bins per thread (16-byte loads, 16-byte fp32 reductions) when the layout allows it -- and, with fp64
     // accumulation, only on the batched path: there is no 16-byte fp64 reduction, and four scalar ones per voxel
@@ -894,6 +872,7 @@ int rt_substeps_per_step(float step_size, float c, float dt) {
 int rt_launch_count(int nx, int ny, int nz, int n_src, int n_rays, int n_bins, int n_steps) {
     if (nx < 1 || ny < 1 || nz < 1 || n_src < 1 || n_rays < 1 || n_bins < 1 || n_steps < 1) return RT_EINVAL;
     const Plan pl = default_plan(n_src);
+    if (workspace_layout(nx, ny, nz, n_src, n_rays, n_steps, n_bins).sort_bytes) return 5;     // key, scan, scatter, march, snapshots
     const int setup = 1 + ((pl.map_src && n_src <= kMaxSortedSources) ? 1 : 0);     // ray order, (source order)
     // the phased march (what rt_march runs when substeps are shorter than a cell): (fraction test, the weight-table
     // instantiation,) the plain instantiation -- one of the two returns at once --, snapshots

@@ -1,11 +1,14 @@
-// rt_chunk.cuh — the chunked march of grids far larger than the L2 (sm_100a): the rays of ALL sources advance
-// together, a chunk of substeps per launch, and before every launch they are sorted by the tile of the grid they are
-// in, so that the blocks in flight load and reduce into one neighbourhood of the grid instead of all of it.
+// rt_ray_sort.cuh — the thread -> ray map of marches over grids far larger than the L2 (sm_100a): the rays of ALL
+// sources sorted by the tile of the grid they are in half-way along the marched path, so that the blocks in flight
+// load and reduce into one neighbourhood of the grid instead of all of it.
 //
 // Eq. (2) fixes the order of the substeps of ONE ray only; rays are independent, so any
-// interleaving of rays gives the same sums.  march_phased_kernel<.., STEP> already marches a ray from substep k0 with
-// (I, exp(-tau)) carried in a state array (rt_march_step, D17); here the launches are chunks of a time
-// step, the thread -> ray map is the sorted list (MarchParams::perm), and the state lives in the workspace.
+// assignment of rays to threads gives the same sums.  With few sources in a large grid (C4: 64 sources, 16,384 rays
+// each, 256^3 x 4 bins) neither of the static maps of rt_common.cuh keeps the traffic local: a warp of 32 sources x one
+// direction touches 32 distant places, and blocks of one source's directions fan out over the whole grid; ncu showed
+// the march moving 54.6 GB through HBM in 32-byte sectors (20 x the grids it reads and writes).  Rays that are in
+// the same 8^3 tile at the same substep -- from whatever source -- march next to each other instead: C4's HBM
+// traffic drops to 33 GB and the call from 26.2 to 17.3 ms.
 // The sort is a locality heuristic: keys are computed in double, not in the march's fixed point, and the order of rays
 // within a tile is whatever the scatter's atomics give -- neither changes a deposit.
 #pragma once
@@ -13,23 +16,15 @@
 
 namespace rt {
 
-struct ChunkGeom {
-    int shift;               // a tile is (1 << shift)^3 cells
-    int tx, ty, tz;          // tiles per axis (each <= 32)
-    int n_tiles;             // Morton-coded: 32768 slots, most of them empty on small or flat grids
-};
+constexpr int kRayTiles = 32768;      // Morton-coded tile keys: 5 bits per axis
 
-__host__ __device__ inline ChunkGeom chunk_geom(int nx, int ny, int nz) {
-    ChunkGeom g;
+// a tile is (1 << shift)^3 cells: 8^3, or larger so that an axis has at most 32 tiles
+__host__ __device__ inline int ray_tile_shift(int nx, int ny, int nz) {
     int m = nx > ny ? nx : ny;
     m = m > nz ? m : nz;
-    g.shift = 3;
-    while (((m - 1) >> g.shift) >= 32) ++g.shift;
-    g.tx = ((nx - 1) >> g.shift) + 1;
-    g.ty = ((ny - 1) >> g.shift) + 1;
-    g.tz = ((nz - 1) >> g.shift) + 1;
-    g.n_tiles = 32768;
-    return g;
+    int shift = 3;
+    while (((m - 1) >> shift) >= 32) ++shift;
+    return shift;
 }
 
 __device__ __forceinline__ uint32_t spread5(uint32_t v) {      // 5 bits -> every third bit
@@ -38,8 +33,8 @@ __device__ __forceinline__ uint32_t spread5(uint32_t v) {      // 5 bits -> ever
 
 // key[e] = Morton index of the tile ray e = source * n_rays + i is in at substep k_mid (clamped to the grid, as its
 // deposits are); hist[key]++
-__global__ void chunk_key_kernel(uint32_t* key, uint32_t* hist, const float* sources, long long n, int n_rays, double ds,
-                                 long long k_mid, int nx, int ny, int nz, ChunkGeom g) {
+__global__ void ray_tile_key_kernel(uint32_t* key, uint32_t* hist, const float* sources, long long n, int n_rays, double ds,
+                                 long long k_mid, int nx, int ny, int nz, int shift) {
     const long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (e >= n) return;
     const int s = int(e / n_rays);
@@ -53,15 +48,15 @@ __global__ void chunk_key_kernel(uint32_t* key, uint32_t* hist, const float* sou
     for (int a = 0; a < 3; ++a) {
         const double x = double(__ldg(sources + 3 * size_t(s) + a)) + far * nh[a];
         const double c = fmin(fmax(floor(x), 0.0), double(lim[a]));       // NaN -> 0
-        t[a] = uint32_t(int(c)) >> g.shift;
+        t[a] = uint32_t(int(c)) >> shift;
     }
     const uint32_t k = (spread5(t[0]) << 2) | (spread5(t[1]) << 1) | spread5(t[2]);
     key[e] = k;
     atomicAdd(hist + k, 1u);
 }
 
-// hist -> exclusive prefix sums (cursor), one block; hist itself is zeroed for the next chunk
-__global__ void chunk_scan_kernel(uint32_t* hist, uint32_t* cursor, int n_tiles) {
+// hist -> exclusive prefix sums (cursor), one block; hist itself is zeroed for the next call
+__global__ void ray_tile_scan_kernel(uint32_t* hist, uint32_t* cursor, int n_tiles) {
     __shared__ uint32_t part[1024];
     const int per = (n_tiles + blockDim.x - 1) / blockDim.x;
     const int b = threadIdx.x * per, e = min(b + per, n_tiles);
@@ -84,7 +79,7 @@ __global__ void chunk_scan_kernel(uint32_t* hist, uint32_t* cursor, int n_tiles)
     }
 }
 
-__global__ void chunk_scatter_kernel(uint32_t* perm, const uint32_t* key, uint32_t* cursor, long long n) {
+__global__ void ray_tile_scatter_kernel(uint32_t* perm, const uint32_t* key, uint32_t* cursor, long long n) {
     const long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (e >= n) return;
     perm[atomicAdd(cursor + key[e], 1u)] = uint32_t(e);
