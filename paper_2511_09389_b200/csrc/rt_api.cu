@@ -227,18 +227,26 @@ int phased_kind(int variant, float step_size, long long cells, int n_steps, int 
 // rays from the list sorted by tile (rt_ray_sort.cuh).  Bins in groups of four then deposit as in kPhasedFourBins -- with
 // the traffic kept local the fp32 scratch pays again (C4: 17.3 ms, against 20.5 ms with red.global.add.f64 per bin and
 // 25.4 ms with that and the rays by direction).
+// FP32_ONLY: a sorted four-bin march whose elements collect few deposits -- on average at most kFp32OnlyDeposits per
+// element and time step (a ray-substep deposits into 8 voxels; C4: 32) -- sums them in the fp32 scratch alone: an fp32
+// sum of N non-negative terms is off by at most N 2^-24 relative (about sqrt(N) 2^-24 as a rule), below the 1e-3
+// per-voxel bound even for an element that collects 64 x the mean.  The fp64 grid and the drains, which on such a grid
+// are HBM traffic only (C4: 17 of the march's 33 GB), are left out: 17.3 -> 14.1 ms.
+constexpr double kFp32OnlyDeposits = 256.0;
 struct PhasedPlan {
     int kind;
-    bool sorted;
+    bool sorted, fp32_only;
 };
 PhasedPlan phased_plan(int variant, float step_size, long long cells, int n_steps, int n_bins, const Workspace& wl, bool aligned16,
-                       bool one_bin_per_thread) {
+                       bool one_bin_per_thread, double ray_substeps_per_step) {
     PhasedPlan pp;
     pp.kind = phased_kind(variant, step_size, cells, n_steps, n_bins, wl.brick_bytes, aligned16);
     pp.sorted = pp.kind == kPhasedDirect64 && wl.sort_bytes != 0;
     if (pp.sorted && n_bins % 4 == 0 && aligned16) pp.kind = kPhasedFourBins;
     // the trilinear-kappa and the tangent march exist with one bin per thread only
     if (one_bin_per_thread && pp.kind == kPhasedFourBins) pp.kind = kPhasedDirect64;
+    pp.fp32_only = pp.sorted && pp.kind == kPhasedFourBins &&
+                   ray_substeps_per_step * 8.0 <= kFp32OnlyDeposits * double(cells / n_bins);
     return pp;
 }
 // how often the scratch is drained during a march: an fp32 sum should not collect much more than 2^19 rays' deposits
@@ -362,7 +370,8 @@ int run_phased(rt::MarchParams P, const PhasedPlan& pp, const Plan& pl, const Wo
                                         : (step ? reinterpret_cast<float*>(ws + wl.total) : out);
     const size_t scratch_bytes = phased == kPhasedDirect64 ? 0 : (phased == kPhasedOneBin ? wl.brick_bytes : n_acc * sizeof(float));
     P.n_drain_units = std::max<long long>(1, (long long)(scratch_bytes / 16));
-    RT_CUDA(cudaMemsetAsync(master, 0, n_acc * sizeof(double), st));
+    const bool nodrain = pp.fp32_only;
+    if (!nodrain) RT_CUDA(cudaMemsetAsync(master, 0, n_acc * sizeof(double), st));
     if (scratch_bytes) RT_CUDA(cudaMemsetAsync(P.scratch, 0, scratch_bytes, st));
     const long long n_ray = (long long)n_src * n_rays;
     long long mb;
@@ -392,6 +401,7 @@ int run_phased(rt::MarchParams P, const PhasedPlan& pp, const Plan& pl, const Wo
     if (mb > 2147483647LL) return RT_EINVAL;
     const long long per = (P.n_drain_units * drain_rounds(n_ray) + mb - 1) / mb;
     P.drain_units_per_block = std::min<long long>(std::max<long long>(per, 1), rt::kDrainMaxUnits);
+    if (nodrain) P.drain_units_per_block = 0;        // and the fp64 grid stays untouched
     if (pl.map_src && !pp.sorted) {
         // Sources that share their cell fractions (decided on the device) take the weight-table instantiation, others
         // the plain one: both are launched, each returns at once when the flag says the call is the other's
@@ -418,9 +428,13 @@ int run_phased(rt::MarchParams P, const PhasedPlan& pp, const Plan& pl, const Wo
         if (phased == kPhasedOneBin)
             rt::step_finalize_scratch_kernel<true><<<fb, fin_threads, 0, st>>>(master, P.scratch, out, cells, step->accumulate, G, ny, nz);
         else if (phased == kPhasedFourBins)
-            rt::step_finalize_scratch_kernel<false><<<fb, fin_threads, 0, st>>>(master, P.scratch, out, cells, step->accumulate, G, ny, nz);
+            rt::step_finalize_scratch_kernel<false><<<fb, fin_threads, 0, st>>>(nodrain ? nullptr : master, P.scratch, out, cells,
+                                                                               step->accumulate, G, ny, nz);
         else
             rt::step_finalize_kernel<<<fb, fin_threads, 0, st>>>(master, out, cells, step->accumulate);
+    } else if (nodrain) {        // `out` holds the increments: cumulative sums in place (one step: nothing to do)
+        if (n_steps > 1)
+            rt::snapshot_finalize_scratch_kernel<false><<<fb, fin_threads, 0, st>>>(nullptr, out, out, cells, n_steps, G, ny, nz);
     } else {
         if (phased == kPhasedOneBin)
             rt::snapshot_finalize_scratch_kernel<true><<<fb, fin_threads, 0, st>>>(master, P.scratch, out, cells, n_steps, G, ny, nz);
@@ -465,7 +479,8 @@ int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const
     if (fin_blocks > 148 * 16) fin_blocks = 148 * 16;
 
     const bool aligned4 = (n_bins % 4 == 0) && !((uintptr_t(j) | uintptr_t(kappa) | uintptr_t(out)) & 15u);
-    const PhasedPlan pp = phased_plan(variant, step_size, ck.cells, n_steps, n_bins, wl, aligned4, dkappa || pl.ktri);
+    const PhasedPlan pp = phased_plan(variant, step_size, ck.cells, n_steps, n_bins, wl, aligned4, dkappa || pl.ktri,
+                                      double(n_src) * double(n_rays) * double(ck.n_sub));
     if (dkappa) {                      // the tangent march exists in the phased kernel only
         if (pp.kind == kPhasedNone || step || pl.ktri) return RT_EINVAL;
         P.dkappa = dkappa;

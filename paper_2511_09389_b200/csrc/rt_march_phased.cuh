@@ -486,6 +486,7 @@ march_phased_kernel(const MarchParams P) {
     if constexpr (sizeof(ACC) == 8) return;
     // this block's turn at the drain: one slice of the scratch goes to the fp64 grid (rt_brick.cuh)
     const long long per = P.drain_units_per_block;
+    if (per == 0) return;        // the scratch is the result grid itself: nothing to drain (rt_api.cu)
     const long long n_slices = (P.n_drain_units + per - 1) / per;
     const long long b0 = (blockIdx.x % n_slices) * per;
     if constexpr (BRICK)
