@@ -288,6 +288,7 @@ def _tangent_compare(got, ref, what):
     ((9, 8, 7), 1, 40, 24, 0.25, 4.0, 2, True),        # warp = 32 sources x 1 direction, weight table, brick scratch
     ((9, 8, 7), 1, 45, 24, 0.25, 4.0, 2, False),       # the same in general position (plain instantiation)
     ((7, 6, 9), 4, 33, 11, 0.5, 4.0, 2, True),         # 4 bins
+    ((64, 60, 72), 2, 3, 200, 0.5, 3.0, 61, False),    # 135 MB of fp32 snapshots: rays from the list sorted by tile
 ])
 def test_jvp_kappa_matches_the_oracle(rt, oracle_mod, shape, nb, n_src, n_rays, ds, dt, n_steps, integer_sources):
     rng = np.random.default_rng(sum(shape) + nb + n_src)

@@ -250,6 +250,29 @@ def test_bins_with_many_sources(rt, oracle_mod, nb, shape, shared_fractions):
     parity.assert_parity(got, ref, f"nb={nb} shared={shared_fractions}")
 
 
+@pytest.mark.parametrize("shape,nb,n_src,n_rays,dt,n_steps,what", [
+    ((48, 40, 44), 4, 5, 301, 4.0, 100, "four bins per thread, sums in the fp32 grid alone (1.1 deposits per element and step)"),
+    ((48, 40, 44), 4, 40, 1024, 34.0, 100, "four bins per thread, fp32 scratch drained into the fp64 grid (264 per element)"),
+    ((64, 60, 72), 2, 3, 200, 3.0, 61, "two bins: one bin per lane, fp64 reductions"),
+    ((64, 60, 72), 2, 1, 1, 3.0, 61, "one ray"),
+])
+def test_rays_from_the_list_sorted_by_tile(rt, oracle_mod, shape, nb, n_src, n_rays, dt, n_steps, what):
+    """Calls whose fp32 snapshots exceed 128 MiB (here through many time steps on a small grid; C4 through its 256^3
+    grid) take their rays from the list sorted by tile (rt_ray_sort.cuh), in every deposit mode of that path; the
+    launch count says so.  Sources in general position in and around the box, ragged ray counts."""
+    assert int(np.prod(shape)) * nb * n_steps * 4 > 128 << 20
+    assert rt.rt_launch_count(*shape, n_src, n_rays, nb, n_steps) == 5
+    rng = np.random.default_rng(n_src + n_rays)
+    src = rng.uniform(-2.0, max(shape) + 1.0, (n_src, 3)).astype(np.float32)
+    j, k = _random_medium(shape, nb, seed=nb + n_src)
+    ref = oracle_mod.march(j, k, src, n_rays, 0.5, 1.0, dt, n_steps)
+    got = rt.rt_march(_dev(j), _dev(k), _dev(src), n_rays, 0.5, 1.0, dt, n_steps).cpu().numpy()
+    parity.assert_parity(got, ref, what)
+    kt = rt.rt_march_trilinear_kappa(_dev(j), _dev(k), _dev(src), n_rays, 0.5, 1.0, dt, n_steps).cpu().numpy()
+    if n_src * n_rays <= 2000:
+        parity.assert_parity(kt, oracle_mod.march(j, k, src, n_rays, 0.5, 1.0, dt, n_steps, kappa_trilinear=True), what + ", trilinear kappa")
+
+
 def test_more_sources_than_the_sort_handles(rt, oracle_mod):
     """Above 65,536 sources the spatial source sort is skipped (identity order); same field."""
     shape, n_src = (4, 4, 4), 66000
