@@ -315,7 +315,7 @@ size_t step_scratch_bytes(long long cells, int n_bins) {
 
 // Marches over grids far larger than the L2 -- the fp32 grid of all time steps beyond kBatchedScratchLimit, no brick
 // scratch -- map their threads to rays through a list sorted by tile (rt_ray_sort.cuh).
-// Workspace behind the brick scratch: [perm: rays u32][key: rays u32][hist: kRayTiles u32][cursor: kRayTiles u32]
+// Workspace behind the brick scratch: [hist: kRayTiles u32][cursor: kRayTiles u32][perm: rays u32][key: rays u32]
 size_t ray_sort_bytes(int nx, int ny, int nz, int n_src, int n_rays, int n_steps, int n_bins) {
     const long long cells = (long long)nx * ny * nz * n_bins;
     if ((n_bins == 1 && brick_scratch_bytes(nx, ny, nz, n_steps, n_bins)) ||
@@ -377,16 +377,16 @@ int run_phased(rt::MarchParams P, const PhasedPlan& pp, const Plan& pl, const Wo
     long long mb;
     if (pp.sorted) {
         // key = tile at the middle of the marched substeps, histogram, prefix sums, scatter
-        uint32_t* perm = reinterpret_cast<uint32_t*>(ws + wl.sort_at);
-        uint32_t* key = perm + n_ray;
-        uint32_t* hist = key + n_ray;
+        uint32_t* hist = reinterpret_cast<uint32_t*>(ws + wl.sort_at);
         uint32_t* cursor = hist + rt::kRayTiles;
+        uint32_t* perm = cursor + rt::kRayTiles;
+        uint32_t* key = perm + n_ray;
         RT_CUDA(cudaMemsetAsync(hist, 0, rt::kRayTiles * sizeof(uint32_t), st));
         const unsigned rb = unsigned((n_ray + 255) / 256);
         const long long k_mid = P.k0 + (long long)P.n_sub * n_steps / 2;
         rt::ray_tile_key_kernel<<<rb, 256, 0, st>>>(key, hist, sources, n_ray, n_rays, P.ds, k_mid, nx, ny, nz,
                                                     rt::ray_tile_shift(nx, ny, nz));
-        rt::ray_tile_scan_kernel<<<1, 1024, 0, st>>>(hist, cursor, rt::kRayTiles);
+        rt::ray_tile_scan_kernel<<<1, 1024, 0, st>>>(hist, cursor);
         rt::ray_tile_scatter_kernel<<<rb, 256, 0, st>>>(perm, key, cursor, n_ray);
         RT_CUDA(cudaGetLastError());
         P.map_src = 2;

@@ -55,27 +55,48 @@ __global__ void ray_tile_key_kernel(uint32_t* key, uint32_t* hist, const float* 
     atomicAdd(hist + k, 1u);
 }
 
-// hist -> exclusive prefix sums (cursor), one block; hist itself is zeroed for the next call
-__global__ void ray_tile_scan_kernel(uint32_t* hist, uint32_t* cursor, int n_tiles) {
-    __shared__ uint32_t part[1024];
-    const int per = (n_tiles + blockDim.x - 1) / blockDim.x;
-    const int b = threadIdx.x * per, e = min(b + per, n_tiles);
+// hist -> exclusive prefix sums (cursor), one block of 1024 threads, 32 consecutive keys per thread (all 32 loads in
+// flight at once); hist itself is zeroed for the next call
+__global__ void __launch_bounds__(1024) ray_tile_scan_kernel(uint32_t* hist, uint32_t* cursor) {
+    constexpr int kPer = kRayTiles / 1024;
+    __shared__ uint32_t warp_sum[32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    uint4* h4 = reinterpret_cast<uint4*>(hist + threadIdx.x * kPer);
+    uint4 v[kPer / 4];
+#pragma unroll
+    for (int i = 0; i < kPer / 4; ++i) v[i] = h4[i];
     uint32_t sum = 0;
-    for (int t = b; t < e; ++t) sum += hist[t];
-    part[threadIdx.x] = sum;
-    __syncthreads();
-    for (int d = 1; d < int(blockDim.x); d <<= 1) {
-        const uint32_t v = (int(threadIdx.x) >= d) ? part[threadIdx.x - d] : 0u;
-        __syncthreads();
-        part[threadIdx.x] += v;
-        __syncthreads();
+#pragma unroll
+    for (int i = 0; i < kPer / 4; ++i) sum += v[i].x + v[i].y + v[i].z + v[i].w;
+    uint32_t incl = sum;                       // inclusive scan of the thread totals: within the warp ...
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const uint32_t up = __shfl_up_sync(0xFFFFFFFFu, incl, d);
+        if (lane >= d) incl += up;
     }
-    uint32_t run = part[threadIdx.x] - sum;
-    for (int t = b; t < e; ++t) {
-        const uint32_t h = hist[t];
-        cursor[t] = run;
-        run += h;
-        hist[t] = 0u;
+    if (lane == 31) warp_sum[warp] = incl;
+    __syncthreads();
+    if (warp == 0) {                           // ... and over the 32 warps
+        uint32_t w = warp_sum[lane];
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const uint32_t up = __shfl_up_sync(0xFFFFFFFFu, w, d);
+            if (lane >= d) w += up;
+        }
+        warp_sum[lane] = w;
+    }
+    __syncthreads();
+    uint32_t run = incl - sum + (warp ? warp_sum[warp - 1] : 0u);
+    uint4* c4 = reinterpret_cast<uint4*>(cursor + threadIdx.x * kPer);
+#pragma unroll
+    for (int i = 0; i < kPer / 4; ++i) {
+        uint4 c;
+        c.x = run; run += v[i].x;
+        c.y = run; run += v[i].y;
+        c.z = run; run += v[i].z;
+        c.w = run; run += v[i].w;
+        c4[i] = c;
+        h4[i] = make_uint4(0u, 0u, 0u, 0u);
     }
 }
 
