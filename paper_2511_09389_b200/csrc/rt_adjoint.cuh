@@ -133,10 +133,12 @@ __device__ __forceinline__ int adjoint_phase(const MarchParams& P, AdjointLane& 
                     }
                 }
             }
-            if (!jumped) {
-                if (cross[0]) L.S.template axis_step<0, ACT>(P, L.A, negbits, og, gs);
-                if (cross[1]) L.S.template axis_step<1, ACT>(P, L.A, negbits, og, gs);
-                if (cross[2]) L.S.template axis_step<2, ACT>(P, L.A, negbits, og, gs);
+            if (!jumped) {               // slides with the loads deferred (rt_march_sliding.cuh)
+                uint32_t stale = 0;
+                if (cross[0]) L.S.template axis_slide_deferred<0, ACT>(P, L.A, negbits, stale, [&]() { L.S.template flush_trailing<0, ACT>(og, L.A); });
+                if (cross[1]) L.S.template axis_slide_deferred<1, ACT>(P, L.A, negbits, stale, [&]() { L.S.template flush_trailing<1, ACT>(og, L.A); });
+                if (cross[2]) L.S.template axis_slide_deferred<2, ACT>(P, L.A, negbits, stale, [&]() { L.S.template flush_trailing<2, ACT>(og, L.A); });
+                L.S.template load_stale<ACT>(P, L.A, gs, stale);
             }
             if (WRT_KAPPA) {                     // the kappa cell may have changed: reduce the old one's sum
                 const int ko_old = L.ko;
