@@ -982,6 +982,6 @@ const char* rt_strerror(int code) {
     }
 }
 
-const char* rt_version(void) { return "rtmarch 0.7 (sm_100a; sliding-stencil march in warp-uniform phases, weight table per warp for sources sharing their cell fractions, fp32 scratch (window bricks / bin vectors) with vector reductions, drained concurrently into an fp64 grid)"; }
+const char* rt_version(void) { return "rtmarch 0.8 (sm_100a; sliding-stencil march in warp-uniform phases, weight table per warp for sources sharing their cell fractions, fp32 scratch (window bricks / bin vectors) with vector reductions drained concurrently into an fp64 grid, rays sorted by tile on grids beyond the L2)"; }
 
 }  // extern "C"
