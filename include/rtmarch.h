@@ -175,7 +175,8 @@ int rt_host_release(void);
  * of n_steps * nx*ny*nz*n_bins floats where the batched multi-bin kernels of the variants run (n_bins % 4 == 0 and that
  * grid <= 128 MiB), for one-bin calls the fp32 window-brick scratch of the march (n_steps * nx*(ny+1)*(nz+1)*4
  * floats, if <= 1 GiB), and for grids far larger than the L2 (that fp32 grid > 128 MiB, no brick scratch,
- * n_src * n_rays < 2^32) the sorted ray list (8 bytes per ray + 256 KiB).  0 on invalid arguments. */
+ * n_src * n_rays < 2^32) the sorted ray list (8 bytes per ray + 256 KiB, and with bins in fours a ray state of
+ * 8 bytes per ray and bin).  0 on invalid arguments. */
 size_t rt_workspace_bytes(int nx, int ny, int nz, int n_src, int n_rays, int n_bins, int n_steps);
 
 /* N_s as the library computes it (D6): ceil(c dt / step_size), a ratio within 1e-6 (relative) of an
@@ -185,8 +186,8 @@ int rt_substeps_per_step(float step_size, float c, float dt);
 
 /* Number of kernels of this library that one rt_march call with these arguments and a step_size below one cell
  * enqueues (memsets excluded).  Calls that march from the sorted ray list (rt_workspace_bytes) enqueue 5 -- key,
- * prefix sums, scatter, march, snapshots -- and one fewer if n_steps == 1 and the deposits are summed in `out` alone
- * (DESIGN.md §7); 5 is returned for them. */
+ * prefix sums, scatter, march, snapshots -- or, with bins in fours and few deposits per element, 7:
+ * + ray-state reset and a second march launch; 7 is returned whenever the bins come in fours. */
 int rt_launch_count(int nx, int ny, int nz, int n_src, int n_rays, int n_bins, int n_steps);
 
 /* TEST HOOK.  Writes the library's direction lattice (D1) for i = 0..n_rays-1 into

@@ -99,6 +99,7 @@ size_t brick_scratch_bytes(int nx, int ny, int nz, int n_steps, int n_bins) {
 }
 bool use_batched_fp32(long long cells, int n_steps, int n_bins);
 size_t ray_sort_bytes(int nx, int ny, int nz, int n_src, int n_rays, int n_steps, int n_bins);
+size_t near_state_bytes(long long rays, int n_bins);
 // One-bin-per-thread marches with fp64 reductions (the kernels of the non-default variants and of substeps of a cell or
 // more) spread them over up to 4 copies of the grid, 48 MiB in all
 constexpr size_t kAccCopiesBytes = size_t(48) << 20;
@@ -227,26 +228,36 @@ int phased_kind(int variant, float step_size, long long cells, int n_steps, int 
 // rays from the list sorted by tile (rt_ray_sort.cuh).  Bins in groups of four then deposit as in kPhasedFourBins -- with
 // the traffic kept local the fp32 scratch pays again (C4: 17.3 ms, against 20.5 ms with red.global.add.f64 per bin and
 // 25.4 ms with that and the rays by direction).
-// FP32_ONLY: a sorted four-bin march whose elements collect few deposits -- on average at most kFp32OnlyDeposits per
-// element and time step (a ray-substep deposits into 8 voxels; C4: 32) -- sums them in the fp32 scratch alone: an fp32
-// sum of N non-negative terms is off by at most N 2^-24 relative (about sqrt(N) 2^-24 as a rule), below the 1e-3
-// per-voxel bound even for an element that collects 64 x the mean.  The fp64 grid and the drains, which on such a grid
-// are HBM traffic only (C4: 17 of the march's 33 GB), are left out: 17.3 -> 14.1 ms.
-constexpr double kFp32OnlyDeposits = 256.0;
+// NO_DRAIN: a sorted four-bin march whose elements collect few deposits -- on average at most kNoDrainDeposits per
+// element and time step (a ray-substep deposits into 8 voxels; C4: 32) -- is not drained: on such a grid every drain
+// round streams the scratch and read-modify-writes the fp64 grid through HBM (C4: 17 of the march's 33 GB).  What fp32
+// sums cannot take are the voxels next to a SOURCE: all N_Omega rays of the source deposit there, with nearly the same
+// addend each, and the rounding errors of equal addends do not cancel (measured on C4: up to 3.9e-4 relative at the 8
+// voxels around each source with everything in fp32, everywhere else < 1e-5).  So the first near_substeps substeps of
+// every ray -- while it is within R = 2 + sqrt(N_Omega / (1024 pi)) cells of its source, beyond which fewer than 256
+// rays of the source meet in a voxel -- are a launch of their own that reduces into the fp64 grid (one bin per lane,
+// red.global.add.f64), (I, exp(-tau)) go through a ray state in the workspace as in rt_march_step, and the four-bin
+// launch marches the rest into the fp32 scratch.  Only the time steps those first substeps fall into have anything in
+// the fp64 grid: only they are zeroed, and read when the snapshots are formed.
+constexpr double kNoDrainDeposits = 256.0;
+long long near_substeps(int n_rays, float step_size) {
+    const double r = 2.0 + std::sqrt(double(n_rays) / (1024.0 * 3.14159265358979323846));
+    return (long long)std::ceil(r / double(step_size));
+}
 struct PhasedPlan {
     int kind;
-    bool sorted, fp32_only;
+    bool sorted, no_drain;
 };
 PhasedPlan phased_plan(int variant, float step_size, long long cells, int n_steps, int n_bins, const Workspace& wl, bool aligned16,
-                       bool one_bin_per_thread, double ray_substeps_per_step) {
+                       bool one_bin_per_thread, double ray_substeps_per_step, long long near_k, long long n_sub) {
     PhasedPlan pp;
     pp.kind = phased_kind(variant, step_size, cells, n_steps, n_bins, wl.brick_bytes, aligned16);
     pp.sorted = pp.kind == kPhasedDirect64 && wl.sort_bytes != 0;
     if (pp.sorted && n_bins % 4 == 0 && aligned16) pp.kind = kPhasedFourBins;
     // the trilinear-kappa and the tangent march exist with one bin per thread only
     if (one_bin_per_thread && pp.kind == kPhasedFourBins) pp.kind = kPhasedDirect64;
-    pp.fp32_only = pp.sorted && pp.kind == kPhasedFourBins &&
-                   ray_substeps_per_step * 8.0 <= kFp32OnlyDeposits * double(cells / n_bins);
+    pp.no_drain = pp.sorted && pp.kind == kPhasedFourBins && near_k <= n_sub &&
+                  ray_substeps_per_step * 8.0 <= kNoDrainDeposits * double(cells / n_bins);
     return pp;
 }
 // how often the scratch is drained during a march: an fp32 sum should not collect much more than 2^19 rays' deposits
@@ -315,7 +326,8 @@ size_t step_scratch_bytes(long long cells, int n_bins) {
 
 // Marches over grids far larger than the L2 -- the fp32 grid of all time steps beyond kBatchedScratchLimit, no brick
 // scratch -- map their threads to rays through a list sorted by tile (rt_ray_sort.cuh).
-// Workspace behind the brick scratch: [hist: kRayTiles u32][cursor: kRayTiles u32][perm: rays u32][key: rays u32]
+// Workspace behind the brick scratch: [hist: kRayTiles u32][cursor: kRayTiles u32][ray state: 2 x rays x bins f32, bins in
+// fours only][perm: rays u32][key: rays u32]
 size_t ray_sort_bytes(int nx, int ny, int nz, int n_src, int n_rays, int n_steps, int n_bins) {
     const long long cells = (long long)nx * ny * nz * n_bins;
     if ((n_bins == 1 && brick_scratch_bytes(nx, ny, nz, n_steps, n_bins)) ||
@@ -323,7 +335,11 @@ size_t ray_sort_bytes(int nx, int ny, int nz, int n_src, int n_rays, int n_steps
         return 0;
     const long long rays = (long long)n_src * n_rays;
     if (rays >= (1LL << 32)) return 0;
-    return size_t(rays) * 2 * sizeof(uint32_t) + 2 * size_t(rt::kRayTiles) * sizeof(uint32_t);
+    return 2 * size_t(rt::kRayTiles) * sizeof(uint32_t) + near_state_bytes(rays, n_bins) + size_t(rays) * 2 * sizeof(uint32_t);
+}
+// (I, exp(-tau)) of every ray and bin between the two launches of a march that is not drained (phased_plan)
+size_t near_state_bytes(long long rays, int n_bins) {
+    return n_bins % 4 == 0 ? 2 * size_t(rays) * size_t(n_bins) * sizeof(float) : 0;
 }
 
 // the instantiation of march_phased_kernel for a deposit mode (phased_kind)
@@ -350,6 +366,50 @@ int launch_phased(const rt::MarchParams& P, int kind, unsigned blocks, cudaStrea
     return RT_OK;
 }
 
+// The two launches of a sorted four-bin march that is not drained (phased_plan): substeps [k0, k_near) one bin per lane
+// into the fp64 grid, [k_near, k_end) four bins per thread into the fp32 scratch, (I, exp(-tau)) carried through a ray
+// state -- the caller's (rt_march_step) or one in the workspace.  P: the parameters of the whole call, the ray list set.
+int run_near_and_far(rt::MarchParams P, long long k_near, long long k_end, bool callers_state, char* state_ws, long long n_ray,
+                     int n_bins, cudaStream_t st) {
+    const int n_sub = P.n_sub;
+    const long long k0 = P.k0;
+    if (!callers_state) {
+        P.state_I = reinterpret_cast<float*>(state_ws);
+        P.state_T = P.state_I + n_ray * n_bins;
+        rt::state_reset_kernel<<<148 * 8, 256, 0, st>>>(P.state_I, P.state_T, n_ray * n_bins);
+    }
+    P.drain_units_per_block = 0;
+    if (k_near > k0) {                 // at most the first time steps of the call
+        rt::MarchParams N = P;
+        N.n_groups = n_bins;
+        N.n_steps = int((k_near - k0 + n_sub - 1) / n_sub);
+        N.first_left = 0;
+        if (k_near < k_end) {          // ends inside a time step: march it as (whole steps, then) a short last step
+            if (N.n_steps > 1) return RT_EINVAL;       // (near_substeps <= N_s is a condition of the plan)
+            N.n_sub = int(k_near - k0);
+        }
+        const long long nb_ = rt::perm_blocks(n_ray, N.n_groups);
+        if (nb_ > 2147483647LL) return RT_EINVAL;
+        const int rc = launch_phased<false, true>(N, kPhasedDirect64, unsigned(nb_), st);
+        if (rc != RT_OK) return rc;
+    }
+    if (k_near < k_end) {
+        rt::MarchParams F = P;
+        const long long into = (k_near - k0) % n_sub;            // substeps of its first time step already marched
+        F.k0 = k_near;
+        F.first_left = into ? int(n_sub - into) : 0;
+        const long long skipped = (k_near - k0) / n_sub;         // whole time steps marched by the first launch
+        F.n_steps = P.n_steps - int(skipped);
+        F.acc = static_cast<double*>(P.acc) + skipped * P.snap_stride;
+        F.scratch = P.scratch + skipped * P.snap_stride;
+        const long long fb_ = rt::perm_blocks(n_ray, F.n_groups);
+        if (fb_ > 2147483647LL) return RT_EINVAL;
+        const int rc = launch_phased<false, true>(F, kPhasedFourBins, unsigned(fb_), st);
+        if (rc != RT_OK) return rc;
+    }
+    return RT_OK;
+}
+
 // rt_march proper (and rt_march_step, rt_march_trilinear_kappa, rt_march_jvp_kappa) through march_phased_kernel: memsets,
 // the thread -> ray map (ray and source order; or the sorted ray list), (fraction test, weight-table instantiation,)
 // plain instantiation, snapshots.
@@ -370,8 +430,11 @@ int run_phased(rt::MarchParams P, const PhasedPlan& pp, const Plan& pl, const Wo
                                         : (step ? reinterpret_cast<float*>(ws + wl.total) : out);
     const size_t scratch_bytes = phased == kPhasedDirect64 ? 0 : (phased == kPhasedOneBin ? wl.brick_bytes : n_acc * sizeof(float));
     P.n_drain_units = std::max<long long>(1, (long long)(scratch_bytes / 16));
-    const bool nodrain = pp.fp32_only;
-    if (!nodrain) RT_CUDA(cudaMemsetAsync(master, 0, n_acc * sizeof(double), st));
+    // not drained (phased_plan): the substeps [k0, k_near) of this call go into the fp64 grid in a launch of their own
+    const long long k_end = P.k0 + (long long)P.n_sub * n_steps;
+    const long long k_near = pp.no_drain ? std::min(std::max(near_substeps(n_rays, step_size), P.k0), k_end) : P.k0;
+    const int acc_steps = pp.no_drain ? int((k_near - P.k0 + P.n_sub - 1) / P.n_sub) : n_steps;      // time steps with fp64 content
+    if (acc_steps) RT_CUDA(cudaMemsetAsync(master, 0, size_t(cells) * size_t(acc_steps) * sizeof(double), st));
     if (scratch_bytes) RT_CUDA(cudaMemsetAsync(P.scratch, 0, scratch_bytes, st));
     const long long n_ray = (long long)n_src * n_rays;
     long long mb;
@@ -379,7 +442,7 @@ int run_phased(rt::MarchParams P, const PhasedPlan& pp, const Plan& pl, const Wo
         // key = tile at the middle of the marched substeps, histogram, prefix sums, scatter
         uint32_t* hist = reinterpret_cast<uint32_t*>(ws + wl.sort_at);
         uint32_t* cursor = hist + rt::kRayTiles;
-        uint32_t* perm = cursor + rt::kRayTiles;
+        uint32_t* perm = reinterpret_cast<uint32_t*>(reinterpret_cast<char*>(cursor + rt::kRayTiles) + near_state_bytes(n_ray, n_bins));
         uint32_t* key = perm + n_ray;
         RT_CUDA(cudaMemsetAsync(hist, 0, rt::kRayTiles * sizeof(uint32_t), st));
         const unsigned rb = unsigned((n_ray + 255) / 256);
@@ -401,7 +464,11 @@ int run_phased(rt::MarchParams P, const PhasedPlan& pp, const Plan& pl, const Wo
     if (mb > 2147483647LL) return RT_EINVAL;
     const long long per = (P.n_drain_units * drain_rounds(n_ray) + mb - 1) / mb;
     P.drain_units_per_block = std::min<long long>(std::max<long long>(per, 1), rt::kDrainMaxUnits);
-    if (nodrain) P.drain_units_per_block = 0;        // and the fp64 grid stays untouched
+    if (pp.no_drain) {
+        const int rcn = run_near_and_far(P, k_near, k_end, step != nullptr, ws + wl.sort_at + 2 * rt::kRayTiles * sizeof(uint32_t), n_ray,
+                                         n_bins, st);
+        if (rcn != RT_OK) return rcn;
+    } else {
     if (pl.map_src && !pp.sorted) {
         // Sources that share their cell fractions (decided on the device) take the weight-table instantiation, others
         // the plain one: both are launched, each returns at once when the flag says the call is the other's
@@ -421,6 +488,7 @@ int run_phased(rt::MarchParams P, const PhasedPlan& pp, const Plan& pl, const Wo
     }
     const int rcp = step ? launch_phased<false, true>(P, phased, unsigned(mb), st) : launch_phased<false, false>(P, phased, unsigned(mb), st);
     if (rcp != RT_OK) return rcp;
+    }
     // the snapshots (the step's increment): the fp64 grid plus what the march left in the scratch, rounded once
     const rt::BrickGeom G = rt::brick_geom(nx, ny, nz);
     const unsigned fb = unsigned(fin_blocks);
@@ -428,18 +496,15 @@ int run_phased(rt::MarchParams P, const PhasedPlan& pp, const Plan& pl, const Wo
         if (phased == kPhasedOneBin)
             rt::step_finalize_scratch_kernel<true><<<fb, fin_threads, 0, st>>>(master, P.scratch, out, cells, step->accumulate, G, ny, nz);
         else if (phased == kPhasedFourBins)
-            rt::step_finalize_scratch_kernel<false><<<fb, fin_threads, 0, st>>>(nodrain ? nullptr : master, P.scratch, out, cells,
+            rt::step_finalize_scratch_kernel<false><<<fb, fin_threads, 0, st>>>(acc_steps ? master : nullptr, P.scratch, out, cells,
                                                                                step->accumulate, G, ny, nz);
         else
             rt::step_finalize_kernel<<<fb, fin_threads, 0, st>>>(master, out, cells, step->accumulate);
-    } else if (nodrain) {        // `out` holds the increments: cumulative sums in place (one step: nothing to do)
-        if (n_steps > 1)
-            rt::snapshot_finalize_scratch_kernel<false><<<fb, fin_threads, 0, st>>>(nullptr, out, out, cells, n_steps, G, ny, nz);
     } else {
         if (phased == kPhasedOneBin)
-            rt::snapshot_finalize_scratch_kernel<true><<<fb, fin_threads, 0, st>>>(master, P.scratch, out, cells, n_steps, G, ny, nz);
+            rt::snapshot_finalize_scratch_kernel<true><<<fb, fin_threads, 0, st>>>(master, P.scratch, out, cells, n_steps, G, ny, nz, acc_steps);
         else if (phased == kPhasedFourBins)
-            rt::snapshot_finalize_scratch_kernel<false><<<fb, fin_threads, 0, st>>>(master, P.scratch, out, cells, n_steps, G, ny, nz);
+            rt::snapshot_finalize_scratch_kernel<false><<<fb, fin_threads, 0, st>>>(master, P.scratch, out, cells, n_steps, G, ny, nz, acc_steps);
         else
             rt::snapshot_finalize_kernel<double><<<fb, fin_threads, 0, st>>>(master, out, cells, n_steps);
     }
@@ -480,7 +545,7 @@ int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const
 
     const bool aligned4 = (n_bins % 4 == 0) && !((uintptr_t(j) | uintptr_t(kappa) | uintptr_t(out)) & 15u);
     const PhasedPlan pp = phased_plan(variant, step_size, ck.cells, n_steps, n_bins, wl, aligned4, dkappa || pl.ktri,
-                                      double(n_src) * double(n_rays) * double(ck.n_sub));
+                                      double(n_src) * double(n_rays) * double(ck.n_sub), near_substeps(n_rays, step_size), ck.n_sub);
     if (dkappa) {                      // the tangent march exists in the phased kernel only
         if (pp.kind == kPhasedNone || step || pl.ktri) return RT_EINVAL;
         P.dkappa = dkappa;
@@ -887,7 +952,8 @@ int rt_substeps_per_step(float step_size, float c, float dt) {
 int rt_launch_count(int nx, int ny, int nz, int n_src, int n_rays, int n_bins, int n_steps) {
     if (nx < 1 || ny < 1 || nz < 1 || n_src < 1 || n_rays < 1 || n_bins < 1 || n_steps < 1) return RT_EINVAL;
     const Plan pl = default_plan(n_src);
-    if (workspace_layout(nx, ny, nz, n_src, n_rays, n_steps, n_bins).sort_bytes) return 5;     // key, scan, scatter, march, snapshots
+    // key, scan, scatter, march, snapshots; not drained (bins in fours, few deposits per element): + state reset, two marches
+    if (workspace_layout(nx, ny, nz, n_src, n_rays, n_steps, n_bins).sort_bytes) return n_bins % 4 == 0 ? 7 : 5;
     const int setup = 1 + ((pl.map_src && n_src <= kMaxSortedSources) ? 1 : 0);     // ray order, (source order)
     // the phased march (what rt_march runs when substeps are shorter than a cell): (fraction test, the weight-table
     // instantiation,) the plain instantiation -- one of the two returns at once --, snapshots

@@ -155,11 +155,11 @@ __device__ __forceinline__ double brick_residue(const float* sm, const BrickGeom
 
 // out[m] <- sum over m' <= m of (acc[m'] + what is left in the scratch of step m'): the per-step increments become
 // the cumulative snapshots (D7), summed in fp64 and rounded once.  BRICK: window-brick scratch (one bin),
-// else the plain grid, which may be `out` itself (an element is read before this thread overwrites it).  acc may be
-// nullptr: the scratch alone holds the increments (rt_api.cu, PhasedPlan::fp32_only).
+// else the plain grid, which may be `out` itself (an element is read before this thread overwrites it).  Only the
+// first acc_steps time steps have anything in the fp64 grid (all of them, but for PhasedPlan::no_drain of rt_api.cu).
 template <bool BRICK>
 __global__ void snapshot_finalize_scratch_kernel(const double* acc, const float* scratch, float* out, long long stride,
-                                                 int n_steps, BrickGeom G, int ny, int nz) {
+                                                 int n_steps, BrickGeom G, int ny, int nz, int acc_steps) {
     for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < stride;
          e += (long long)gridDim.x * blockDim.x) {
         int x = 0, y = 0, z = 0;
@@ -171,7 +171,7 @@ __global__ void snapshot_finalize_scratch_kernel(const double* acc, const float*
         }
         double run = 0.0;
         for (int m = 0; m < n_steps; ++m) {
-            if (acc) run += acc[m * stride + e];
+            if (m < acc_steps) run += acc[m * stride + e];
             run += BRICK ? brick_residue(scratch + m * G.step_stride, G, x, y, z) : double(scratch[m * stride + e]);
             out[m * stride + e] = float(run);
         }

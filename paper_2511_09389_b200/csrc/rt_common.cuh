@@ -37,6 +37,8 @@ struct MarchParams {
     float* state_I;              // rt_march_step: carried I per (source, lattice index, bin), else nullptr
     float* state_T;              //                carried exp(-tau), same layout
     long long k0;                // substep index of the first substep of this launch (0 for rt_march)
+    int first_left;              // state_I != nullptr: substeps left in the time step the launch starts in (0 = all n_sub); the
+                                 // launch marches first_left + (n_steps - 1) n_sub substeps
     const int* same_frac;        // device flag, or nullptr: all sources share their cell fractions -> the TABLE instantiation
                                  // of march_phased_kernel marches the call and the plain one returns at once (and vice versa)
     // march_sliding_kernel<..., COPIES = true>, else 1 / 0:

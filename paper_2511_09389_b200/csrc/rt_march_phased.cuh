@@ -407,7 +407,7 @@ march_phased_kernel(const MarchParams P) {
                                           ((negbits & 4) ? L.A[2].dl : 0));
         }
         L.g = 0;
-        L.left = P.n_sub;
+        L.left = (STEP && P.first_left) ? P.first_left : P.n_sub;
         L.roff = 0;
         L.woff = 0;
         if constexpr (BRICK)
@@ -429,7 +429,7 @@ march_phased_kernel(const MarchParams P) {
             const bool gone = L.A[a].p.c >= ((negbits & (1 << a)) ? 0 : lim);
             if (!__all_sync(0xFFFFFFFFu, gone)) act |= 1 << a;
         }
-        const int K = P.n_steps * P.n_sub;
+        const int K = P.n_steps * P.n_sub - ((STEP && P.first_left) ? P.n_sub - P.first_left : 0);
         while (L.g < K) {
             if constexpr (TABLE) {
                 if (L.roff == 0 && act != 0) {       // the table has run out: lane l writes the row of substep g + l

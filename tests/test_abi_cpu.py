@@ -71,7 +71,8 @@ def test_host_side_helpers(rt):
     assert rt.rt_launch_count(16, 16, 16, 1, 64, 1, 1) == 3          # ray order, march, snapshots
     assert rt.rt_launch_count(16, 16, 16, 64, 64, 1, 4) == 6         # + source order, fraction test, the other march instantiation
     assert rt.rt_launch_count(128, 128, 128, 256, 4096, 8, 2) == 6
-    assert rt.rt_launch_count(256, 256, 256, 64, 16384, 4, 8) == 5          # sorted ray list: key, scan, scatter, march, snapshots
+    assert rt.rt_launch_count(256, 256, 256, 64, 16384, 4, 8) == 7          # sorted ray list: key, scan, scatter, state, 2 marches, snapshots
+    assert rt.rt_launch_count(256, 256, 256, 64, 16384, 2, 8) == 5          # ... one march
     for code in (0, -1, -2, -3, -4, -99):
         assert isinstance(rt.rt_strerror(code), str) and rt.rt_strerror(code)
 
