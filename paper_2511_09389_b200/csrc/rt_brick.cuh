@@ -170,10 +170,23 @@ __global__ void snapshot_finalize_scratch_kernel(const double* acc, const float*
             y = int(r - (long long)x * ny);
         }
         double run = 0.0;
-        for (int m = 0; m < n_steps; ++m) {
-            if (m < acc_steps) run += acc[m * stride + e];
-            run += BRICK ? brick_residue(scratch + m * G.step_stride, G, x, y, z) : double(scratch[m * stride + e]);
-            out[m * stride + e] = float(run);
+        for (int m0 = 0; m0 < n_steps; m0 += 4) {      // four time steps' loads in flight (scratch may be out: the compiler
+            double inc[4];                             // cannot move a load above the previous step's store itself)
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const int m = m0 + i;
+                inc[i] = 0.0;
+                if (m < n_steps) {
+                    inc[i] = BRICK ? brick_residue(scratch + m * G.step_stride, G, x, y, z) : double(scratch[m * stride + e]);
+                    if (m < acc_steps) inc[i] += acc[m * stride + e];
+                }
+            }
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+                if (m0 + i < n_steps) {
+                    run += inc[i];
+                    out[(m0 + i) * stride + e] = float(run);
+                }
         }
     }
 }
