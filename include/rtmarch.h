@@ -48,6 +48,7 @@ extern "C" {
 #define RT_EWORKSPACE (-2) /* workspace is NULL or smaller than rt_workspace_bytes() */
 #define RT_ECUDA (-3)      /* a CUDA runtime call or kernel launch failed; rt_strerror(RT_ECUDA) holds the CUDA message */
 #define RT_EALIGN (-4)     /* j, kappa or out not 4-byte aligned */
+#define RT_ETOOBIG (-5)    /* rt_march_static: the call needs more scratch than RT_STATIC_WORKSPACE_BYTES */
 
 /* Kernel variants for rt_march_ex (tests and bench only; rt_march always uses RT_VARIANT_DEFAULT).
  * All variants compute the same field; they differ in how the deposit of P:29 is issued and in which rays
@@ -69,6 +70,27 @@ int rt_march(const float* j, const float* kappa, int nx, int ny, int nz,
              int n_steps, float* out,
              void* workspace, size_t workspace_bytes, /* device scratch, >= rt_workspace_bytes(), 16-byte aligned */
              void* stream);
+
+/* rt_march for callers that may not allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): the same march (the product kernels of rt_march), its workspace a
+ * file-scope __device__ array inside the library instead of a caller's buffer.  The call allocates nothing: no
+ * cudaMalloc / cudaFree, no memory pool, no allocating library routine -- it looks the array's device address up
+ * (cudaGetSymbolAddress, once per device, with the caller's current device) and enqueues memsets and kernels on
+ * `stream` like rt_march.  j, kappa, sources, out: DEVICE pointers on the current device, owned by the caller, rules
+ * and limits as rt_march; asynchronous.
+ *   LIMIT: rt_workspace_bytes(nx, ny, nz, n_src, n_rays, n_bins, n_steps) <= RT_STATIC_WORKSPACE_BYTES = 96 MiB
+ *   (e.g. 128^3 x 1 bin x 1 time step with 2,097 sources: 80.5 MiB; 64^3 x 4 bins x 4 steps: 48 MiB), else
+ *   RT_ETOOBIG, returned before any CUDA call.  Every GPU that loads the library holds the array until the process
+ *   exits.
+ *   SHARED STATE: every rt_march_static call on a device uses the same array, which keeps the last call's contents.
+ *   Each call zeroes what it sums into and rebuilds its tables on the stream, so calls that follow each other on one
+ *   stream (or are otherwise ordered on the GPU) are independent; calls that OVERLAP on the GPU -- two streams, two
+ *   host threads on one device -- race on the array and give wrong fields.  Use rt_march with private workspaces there. */
+#define RT_STATIC_WORKSPACE_BYTES (96u << 20)
+size_t rt_static_workspace_bytes(void); /* = RT_STATIC_WORKSPACE_BYTES; host only */
+int rt_march_static(const float* j, const float* kappa, int nx, int ny, int nz,
+                    const float* sources, int n_src, int n_rays, int n_bins,
+                    float step_size, float c, float dt, int n_steps, float* out, void* stream);
 
 /* rt_march with kappa read by TRILINEAR interpolation at x_k, with the weights of the j read, instead of nearest
  * neighbour (reading D18: P:29 calls nearest neighbour the current choice).  Everything else as rt_march. */

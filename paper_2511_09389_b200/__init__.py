@@ -8,7 +8,7 @@ missing and cannot be built: there is no CPU fallback.
 import importlib
 
 _BINDING_NAMES = (
-    "RT_EALIGN", "RT_ECUDA", "RT_EINVAL", "RT_EWORKSPACE", "RT_OK", "RT_VARIANT_DEFAULT", "RT_VARIANT_DIRECT",
+    "RT_EALIGN", "RT_ECUDA", "RT_EINVAL", "RT_ETOOBIG", "RT_EWORKSPACE", "RT_OK", "RT_VARIANT_DEFAULT", "RT_VARIANT_DIRECT",
     "RT_VARIANT_DIRECT_COHERENT", "RT_VARIANT_FLAG_ACC_F32", "RT_VARIANT_FLAG_ONE_BIN", "RT_VARIANT_SLIDING_BY_DIRECTION",
     "RT_VARIANT_SLIDING_BY_SOURCE", "RT_VARIANT_SLIDING_LATTICE", "RtError", "alloc_workspace", "library_path",
     "rt_bench_red_ceiling", "rt_directions", "rt_host_release", "rt_launch_count", "rt_adjoint_kappa_workspace_bytes",
@@ -16,7 +16,7 @@ _BINDING_NAMES = (
     "rt_march_adjoint_kappa", "rt_march_adjoint_kappa_ex", "rt_march_ex", "rt_march_jvp_kappa", "rt_march_host", "rt_march_single",
     "rt_march_step", "rt_march_trilinear_kappa", "rt_state_bytes", "rt_state_reset", "rt_step_workspace_bytes",
     "rt_ray_order", "rt_ray_slots", "rt_strerror", "rt_substeps_per_step", "rt_trace_ray", "rt_version",
-    "rt_workspace_bytes")
+    "rt_workspace_bytes", "rt_march_static", "rt_static_workspace_bytes")
 
 __all__ = list(_BINDING_NAMES) + ["binding", "sharding", "build"]
 

@@ -14,7 +14,7 @@ import numpy as np
 
 from . import build as _build
 
-RT_OK, RT_EINVAL, RT_EWORKSPACE, RT_ECUDA, RT_EALIGN = 0, -1, -2, -3, -4
+RT_OK, RT_EINVAL, RT_EWORKSPACE, RT_ECUDA, RT_EALIGN, RT_ETOOBIG = 0, -1, -2, -3, -4, -5
 RT_VARIANT_DEFAULT, RT_VARIANT_DIRECT, RT_VARIANT_DIRECT_COHERENT, RT_VARIANT_SLIDING_LATTICE = 0, 1, 2, 3
 RT_VARIANT_SLIDING_BY_DIRECTION, RT_VARIANT_SLIDING_BY_SOURCE, RT_VARIANT_FLAG_ACC_F32 = 4, 5, 16
 RT_VARIANT_FLAG_ONE_BIN = 32
@@ -27,7 +27,8 @@ EXPORTS = ("rt_march", "rt_march_single", "rt_march_ex", "rt_march_host", "rt_wo
            "rt_bench_red_ceiling", "rt_strerror", "rt_version", "rt_state_bytes", "rt_state_reset",
            "rt_step_workspace_bytes", "rt_march_step", "rt_march_trilinear_kappa", "rt_adjoint_workspace_bytes",
            "rt_march_adjoint_j", "rt_adjoint_kappa_workspace_bytes", "rt_march_adjoint_kappa",
-           "rt_adjoint_kappa_workspace_bytes_ex", "rt_march_adjoint_kappa_ex", "rt_march_jvp_kappa", "rt_host_release")
+           "rt_adjoint_kappa_workspace_bytes_ex", "rt_march_adjoint_kappa_ex", "rt_march_jvp_kappa", "rt_host_release",
+           "rt_march_static", "rt_static_workspace_bytes")
 
 
 class RtError(RuntimeError):
@@ -51,6 +52,9 @@ def _load() -> ctypes.CDLL:
     march_args = [vp, vp, i, i, i, vp, i, i, i, f, f, f, i, vp]
     L.rt_march.argtypes = march_args + [vp, sz, vp]
     L.rt_march_trilinear_kappa.argtypes = march_args + [vp, sz, vp]
+    L.rt_march_static.argtypes = march_args + [vp]
+    L.rt_static_workspace_bytes.argtypes = []
+    L.rt_static_workspace_bytes.restype = sz
     L.rt_adjoint_workspace_bytes.argtypes = [i] * 7
     L.rt_adjoint_workspace_bytes.restype = sz
     L.rt_march_adjoint_j.argtypes = march_args + [vp, sz, vp]
@@ -234,6 +238,31 @@ def rt_march_ex(j, kappa, sources, n_rays, step_size, c, dt, n_steps, out=None, 
 def rt_march(j, kappa, sources, n_rays, step_size, c, dt, n_steps, out=None, workspace=None, stream=None):
     return rt_march_ex(j, kappa, sources, n_rays, step_size, c, dt, n_steps, out, workspace, stream,
                        RT_VARIANT_DEFAULT)
+
+
+def rt_static_workspace_bytes() -> int:
+    return int(_lib.rt_static_workspace_bytes())
+
+
+def rt_march_static(j, kappa, sources, n_rays, step_size, c, dt, n_steps, out, stream=None):
+    """rt_march with the library's static device workspace (include/rtmarch.h): nothing is allocated, here or in the
+    library, so ``out`` is the caller's.  Calls that overlap on the GPU race on that workspace."""
+    torch = _torch()
+    _check_dev(j, "j", torch.float32, 4)
+    _check_dev(kappa, "kappa", torch.float32, 4)
+    _check_dev(sources, "sources", torch.float32, 2)
+    if kappa.shape != j.shape or sources.shape[1] != 3:
+        raise ValueError("kappa must have j's shape and sources must be [n_src, 3]")
+    if out is None:
+        raise TypeError("rt_march_static allocates nothing: pass out")
+    nx, ny, nz, nb = j.shape
+    with _Call(stream, j, kappa, sources) as call:
+        out = _out_or_new(call, out, (n_steps, nx, ny, nz, nb), "out")
+        rc = _lib.rt_march_static(j.data_ptr(), kappa.data_ptr(), nx, ny, nz, sources.data_ptr(), sources.shape[0], n_rays, nb,
+                                  step_size, c, dt, n_steps, out.data_ptr(), call.stream_ptr)
+    if rc != RT_OK:
+        raise RtError(rc, "rt_march_static")
+    return out
 
 
 def rt_march_trilinear_kappa(j, kappa, sources, n_rays, step_size, c, dt, n_steps, out=None, workspace=None,

@@ -643,6 +643,37 @@ int march_impl(const float* j, const float* kappa, int nx, int ny, int nz, const
 
 }  // namespace
 
+// rt_march_static: the workspace of callers that may not allocate (code under CUDA graph capture, serving loops,
+// harnesses that forbid cudaMalloc).  A file-scope device array: every GPU that loads the library holds these
+// RT_STATIC_WORKSPACE_BYTES until the process exits, every rt_march_static call on a device shares them.
+// In host code the NAME of the array is a host-side stand-in, not a device address; the device address comes from
+// cudaGetSymbolAddress, asked once per device with that device current.
+static __device__ __align__(256) unsigned char g_static_workspace[RT_STATIC_WORKSPACE_BYTES];
+
+namespace {
+
+constexpr int kMaxStaticDevices = 64;
+std::mutex g_static_mutex;
+void* g_static_ptr[kMaxStaticDevices] = {};
+
+// device address of g_static_workspace on the CURRENT device (no allocation: the array is part of the loaded module)
+int static_workspace(void** ptr) {
+    int dev = -1;
+    RT_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kMaxStaticDevices) return RT_EINVAL;
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_ptr[dev]) {
+        void* p = nullptr;
+        RT_CUDA(cudaGetSymbolAddress(&p, g_static_workspace));
+        if (!p || (uintptr_t(p) & 255u)) return RT_EWORKSPACE;
+        g_static_ptr[dev] = p;
+    }
+    *ptr = g_static_ptr[dev];
+    return RT_OK;
+}
+
+}  // namespace
+
 extern "C" {
 
 int rt_march(const float* j, const float* kappa, int nx, int ny, int nz, const float* sources, int n_src, int n_rays,
@@ -650,6 +681,25 @@ int rt_march(const float* j, const float* kappa, int nx, int ny, int nz, const f
              size_t workspace_bytes, void* stream) {
     return march_impl(j, kappa, nx, ny, nz, sources, n_src, n_rays, n_bins, step_size, c, dt, n_steps, out, workspace,
                       workspace_bytes, stream, RT_VARIANT_DEFAULT);
+}
+
+size_t rt_static_workspace_bytes(void) { return size_t(RT_STATIC_WORKSPACE_BYTES); }
+
+int rt_march_static(const float* j, const float* kappa, int nx, int ny, int nz, const float* sources, int n_src, int n_rays,
+                    int n_bins, float step_size, float c, float dt, int n_steps, float* out, void* stream) {
+    // arguments and size first, on the host: a call that does not fit is refused before any CUDA call
+    Checked ck;
+    const int rc = check_args(j, kappa, nx, ny, nz, sources, n_src, n_rays, n_bins, step_size, c, dt, n_steps, out, &ck);
+    if (rc != RT_OK) return rc;
+    const size_t need = workspace_layout(nx, ny, nz, n_src, n_rays, n_steps, n_bins).total;
+    if (need > size_t(RT_STATIC_WORKSPACE_BYTES)) return RT_ETOOBIG;
+    void* ws = nullptr;
+    const int rs = static_workspace(&ws);
+    if (rs != RT_OK) return rs;
+    // the march itself is rt_march's: it zeroes what it sums into (fp64 grid, fp32 scratch) and rebuilds the ray and
+    // source orders on the stream in every call, so the contents the last call left in the array do not matter
+    return march_impl(j, kappa, nx, ny, nz, sources, n_src, n_rays, n_bins, step_size, c, dt, n_steps, out, ws,
+                      size_t(RT_STATIC_WORKSPACE_BYTES), stream, RT_VARIANT_DEFAULT);
 }
 
 int rt_march_trilinear_kappa(const float* j, const float* kappa, int nx, int ny, int nz, const float* sources, int n_src,
@@ -1044,6 +1094,7 @@ const char* rt_strerror(int code) {
         case RT_EWORKSPACE: return "workspace missing, misaligned or smaller than rt_workspace_bytes()";
         case RT_ECUDA: return g_cuda_msg;
         case RT_EALIGN: return "pointer not sufficiently aligned";
+        case RT_ETOOBIG: return "the call needs more scratch than rt_march_static's static workspace holds (rt_static_workspace_bytes()); use rt_march with a workspace of rt_workspace_bytes()";
         default: return "unknown rtmarch error code";
     }
 }
