@@ -160,6 +160,13 @@ class ClockSampler:
         for line in self.proc.stdout:
             self.rows.append((time.perf_counter(), [c.strip() for c in line.split(",")]))
 
+    def wait_first(self, timeout=3.0):
+        """Block until nvidia-smi has printed its first row: its start-up holds driver locks for a few hundred ms, which
+        would land in a region timed by wall clock."""
+        t_end = time.perf_counter() + timeout
+        while self.proc and not self.rows and time.perf_counter() < t_end:
+            time.sleep(0.01)
+
     def stop(self):
         if self.proc:
             self.proc.terminate()
@@ -421,7 +428,10 @@ def run_native(args):
         e2e_sampler = ClockSampler(local)
         if rank == 0:
             e2e_sampler.start()
-            time.sleep(0.1)
+            e2e_sampler.wait_first()
+        for _ in range(2):             # untimed: the sampler's start-up is over, clocks are back up
+            e2e_call()
+        barrier()
         te0 = time.perf_counter()
         call_s = []
         for _ in range(n_e2e):
