@@ -23,6 +23,11 @@ namespace rt {
 // substep i) dL/dkappa_i = ds [P_i lambda_{i+1} - R_i], R_i = sum_{k>=i} G_k I_{k+1}: the same backward march,
 // fed with (I_{k+1}, P_k) of every substep as recorded by march_sliding_kernel<..., RECORD = true>, summing into the kappa cell of x_i
 // (nearest neighbour: one voxel per substep, reduced when the cell changes).
+#ifndef RT_REC_AHEAD
+#define RT_REC_AHEAD 2
+#endif
+constexpr int kRecAhead = RT_REC_AHEAD;      // how far ahead of its use the kappa adjoint loads the forward record
+
 // The state one lane carries through the backward march
 struct AdjointLane {
     Stencil<1, double, false> S;     // cached gsuf values (jc) and pending deposits (acc)
@@ -31,6 +36,7 @@ struct AdjointLane {
     double tau, Rsum, kacc;          // WRT_KAPPA: R_i and the pending sum of the current kappa cell, in fp64 (P_i lambda_{i+1} - R_i cancels)
     int ko;                          // element offset of the kappa cell
     long long kk;                    // global substep index of the backward sweep
+    float2 rec[kRecAhead];           // WRT_KAPPA: the records of substeps kk, kk - 1, ...: loaded kRecAhead substeps ahead of their use
     int left;                        // substeps left in the current time step
 };
 
@@ -102,7 +108,10 @@ __device__ __forceinline__ int adjoint_phase(const MarchParams& P, AdjointLane& 
         if (!live) { gv = 0.0f; gu = 0.0f; }         // a dark lane: zero dL/d out, so lambda stays 0 and nothing is deposited
         if (WRT_KAPPA) {
             // (I_{k+1}, P_k), both x 4 pi/N_Omega (a dark lane has no record)
-            const float2 rec = live ? __ldg(fwd + L.kk * fwd_stride + tid) : make_float2(0.0f, 0.0f);
+            const float2 rec = L.rec[0];
+#pragma unroll
+            for (int i = 0; i + 1 < kRecAhead; ++i) L.rec[i] = L.rec[i + 1];
+            L.rec[kRecAhead - 1] = (live && L.kk >= kRecAhead) ? __ldg(fwd + (L.kk - kRecAhead) * fwd_stride + tid) : make_float2(0.0f, 0.0f);
             L.lambda = fmaf(L.a_next, L.lambda, gv + gu);
             L.a_next = L.att;
             L.Rsum = fma(double(gv + gu), double(rec.x), L.Rsum);
@@ -250,6 +259,9 @@ __global__ void __launch_bounds__(kThreads, MINB) adjoint_kernel(const MarchPara
     L.kap = __ldg(P.kappa + L.ko);
     L.att = ex2_approx(L.kap * P.att_scale);
     L.kk = K - 1;
+#pragma unroll
+    for (int i = 0; i < kRecAhead; ++i)
+        L.rec[i] = (WRT_KAPPA && live && K - 1 - i >= 0) ? __ldg(fwd + (K - 1 - i) * fwd_stride + tid) : make_float2(0.0f, 0.0f);
     L.left = P.n_sub;
     // axes some lane is inside of, or about to enter, at x_{K-1}
     int act = 0;
