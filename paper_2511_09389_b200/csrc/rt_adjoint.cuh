@@ -24,19 +24,23 @@ namespace rt {
 // fed with (I_{k+1}, P_k) of every substep as recorded by march_sliding_kernel<..., RECORD = true>, summing into the kappa cell of x_i
 // (nearest neighbour: one voxel per substep, reduced when the cell changes).
 #ifndef RT_REC_AHEAD
-#define RT_REC_AHEAD 2
+#define RT_REC_AHEAD 8
 #endif
-constexpr int kRecAhead = RT_REC_AHEAD;      // how far ahead of its use the kappa adjoint loads the forward record
+// The kappa adjoint reads the forward record of substep kk - 1 into a register while it works on substep kk, and asks
+// the L2 for the record of substep kk - kRecAhead (a register queue deeper than one does not help: moving a value
+// along the queue waits for its load)
+constexpr int kRecAhead = RT_REC_AHEAD;
 
 // The state one lane carries through the backward march
 struct AdjointLane {
     Stencil<1, double, false> S;     // cached gsuf values (jc) and pending deposits (acc)
     TravelAxis A[3];
-    float lambda, a_next, kap, att;
+    float lambda, a_next, kap;       // kap: kappa of the cell of x_k as loaded; exp(-kappa ds) is formed where it is used, a
+                                     // substep after the load
     double tau, Rsum, kacc;          // WRT_KAPPA: R_i and the pending sum of the current kappa cell, in fp64 (P_i lambda_{i+1} - R_i cancels)
     int ko;                          // element offset of the kappa cell
     long long kk;                    // global substep index of the backward sweep
-    float2 rec[kRecAhead];           // WRT_KAPPA: the records of substeps kk, kk - 1, ...: loaded kRecAhead substeps ahead of their use
+    float2 rec;                      // WRT_KAPPA: the record of substep kk, loaded one substep ahead of its use
     int left;                        // substeps left in the current time step
 };
 
@@ -62,7 +66,6 @@ __device__ __forceinline__ int adjoint_phase(const MarchParams& P, AdjointLane& 
         if (ACT & 4) ko += (negbits & 4) ? L.A[2].dl : 0;
         L.ko = ko;
         L.kap = __ldg(P.kappa + ko);
-        L.att = ex2_approx(L.kap * P.att_scale);
     };
     int next = ACT;
     do {
@@ -108,12 +111,11 @@ __device__ __forceinline__ int adjoint_phase(const MarchParams& P, AdjointLane& 
         if (!live) { gv = 0.0f; gu = 0.0f; }         // a dark lane: zero dL/d out, so lambda stays 0 and nothing is deposited
         if (WRT_KAPPA) {
             // (I_{k+1}, P_k), both x 4 pi/N_Omega (a dark lane has no record)
-            const float2 rec = L.rec[0];
-#pragma unroll
-            for (int i = 0; i + 1 < kRecAhead; ++i) L.rec[i] = L.rec[i + 1];
-            L.rec[kRecAhead - 1] = (live && L.kk >= kRecAhead) ? __ldg(fwd + (L.kk - kRecAhead) * fwd_stride + tid) : make_float2(0.0f, 0.0f);
+            const float2 rec = L.rec;
+            if (live && L.kk >= 1) L.rec = __ldg(fwd + (L.kk - 1) * fwd_stride + tid);
+            if (live && L.kk >= kRecAhead) asm volatile("prefetch.global.L2 [%0];" ::"l"(fwd + (L.kk - kRecAhead) * fwd_stride + tid));
             L.lambda = fmaf(L.a_next, L.lambda, gv + gu);
-            L.a_next = L.att;
+            L.a_next = ex2_approx(L.kap * P.att_scale);
             L.Rsum = fma(double(gv + gu), double(rec.x), L.Rsum);
             L.kacc = fma(fma(double(rec.y), double(L.lambda), -L.Rsum), P.ds, L.kacc);
             --L.kk;
@@ -121,7 +123,7 @@ __device__ __forceinline__ int adjoint_phase(const MarchParams& P, AdjointLane& 
             L.tau = fma(-double(L.kap), P.ds, L.tau);                             // tau_k = tau_{k+1} - kappa_k ds
             const float T = ex2_approx(float(L.tau * -1.4426950408889634));       // exp(-tau_k)
             L.lambda = fmaf(L.a_next, L.lambda, (gv + gu) * P.emis);              // lambda_{k+1} ds
-            L.a_next = L.att;
+            L.a_next = ex2_approx(L.kap * P.att_scale);
             const float v = L.lambda * T;
 #pragma unroll
             for (int s = 0; s < 8; ++s)
@@ -257,11 +259,8 @@ __global__ void __launch_bounds__(kThreads, MINB) adjoint_kernel(const MarchPara
     L.Rsum = 0.0; L.kacc = 0.0;
     L.ko = L.S.base + ((negbits & 1) ? L.A[0].dl : 0) + ((negbits & 2) ? L.A[1].dl : 0) + ((negbits & 4) ? L.A[2].dl : 0);
     L.kap = __ldg(P.kappa + L.ko);
-    L.att = ex2_approx(L.kap * P.att_scale);
     L.kk = K - 1;
-#pragma unroll
-    for (int i = 0; i < kRecAhead; ++i)
-        L.rec[i] = (WRT_KAPPA && live && K - 1 - i >= 0) ? __ldg(fwd + (K - 1 - i) * fwd_stride + tid) : make_float2(0.0f, 0.0f);
+    L.rec = (WRT_KAPPA && live) ? __ldg(fwd + (K - 1) * fwd_stride + tid) : make_float2(0.0f, 0.0f);
     L.left = P.n_sub;
     // axes some lane is inside of, or about to enter, at x_{K-1}
     int act = 0;
