@@ -859,6 +859,12 @@ int rt_march_adjoint_kappa_ex(const float* gbar, const float* j, const float* ka
         RT_CUDA(cudaGetLastError());
         gsuf = gs;
     }
+    if (pl.map_src && step_size < 1.0f) {       // do the sources share their cell fractions? (rt_march_phased.cuh)
+        int* flag = reinterpret_cast<int*>(ws + wl.flag_at);
+        rt::same_fraction_kernel<<<1, 256, 0, st>>>(flag, sources, n_src, step_size);
+        RT_CUDA(cudaGetLastError());
+        P.same_frac = flag;
+    }
     const long long K = ck.n_sub * n_steps;
     const KappaBatch kb = plan_kappa_batches(n_src, P.n_slots, P.n_groups, pl.map_src, K, record_limit);
     float2* fwd = reinterpret_cast<float2*>(ws + align_up(base, 256));
@@ -868,7 +874,14 @@ int rt_march_adjoint_kappa_ex(const float* gbar, const float* j, const float* ka
         const long long mb = rt::march_blocks(P.n_src, P.n_slots, P.n_groups, P.map_src);
         if (mb > 2147483647LL) return RT_EINVAL;
         const long long stride = mb * rt::kThreads;
-        rt::march_sliding_kernel<1, double, 8, false, false, true><<<unsigned(mb), rt::kThreads, 0, st>>>(P, fwd, stride);
+        if (step_size < 1.0f) {        // the phased march, in its weight-table and its plain instantiation (one of them returns)
+            P.record = fwd;
+            P.record_stride = stride;
+            if (pl.map_src) rt::march_phased_kernel<1, true, false, float, false, false, false, true><<<unsigned(mb), rt::kThreads, 0, st>>>(P);
+            rt::march_phased_kernel<1, false, false, float, false, false, false, true><<<unsigned(mb), rt::kThreads, 0, st>>>(P);
+        } else {
+            rt::march_sliding_kernel<1, double, 8, false, false, true><<<unsigned(mb), rt::kThreads, 0, st>>>(P, fwd, stride);
+        }
         RT_CUDA(cudaGetLastError());
         rt::adjoint_kernel<4, true><<<unsigned(mb), rt::kThreads, 0, st>>>(P, gsuf, fwd, stride);
         RT_CUDA(cudaGetLastError());

@@ -78,6 +78,7 @@ template <int NB, typename ACC = float, bool JVP = false, bool KTRI = false> str
     int g;                   // substep index since x_0
     int left;                // substeps left in the current time step
     uint32_t roff;           // TABLE: byte offset of the row of substep g in the warp's table
+    long long rec_at;        // RECORD: the thread's column of the record, or -1 for a lane without a ray of its own
 };
 
 // array index of u-cell c of axis AX (c, or -c on a descending axis), clamped to the grid
@@ -152,7 +153,7 @@ __device__ __forceinline__ void brick_flush(const BrickGeom& G, LANE& L, int neg
 
 // One stencil slide of the lane along axis AX, the trailing plane reduced into the scratch; the loads of the new
 // leading plane are left to Stencil::load_stale (rt_march_sliding.cuh)
-template <int AX, int ACT, bool BRICK, class LANE>
+template <int AX, int ACT, bool BRICK, bool RECORD, class LANE>
 __device__ __forceinline__ void phased_axis_step(const MarchParams& P, const BrickGeom& G, LANE& L, int negbits, uint32_t& stale) {
 #ifdef RT_NO_DEFER
     if constexpr (BRICK)
@@ -160,7 +161,9 @@ __device__ __forceinline__ void phased_axis_step(const MarchParams& P, const Bri
     else
         L.S.template axis_step<AX, ACT>(P, L.A, negbits, L.sg, P.j);        // per voxel: one red.v4.f32 (red.f32) of its bins
 #else
-    if constexpr (BRICK)
+    if constexpr (RECORD)      // nothing is deposited, so nothing is flushed
+        L.S.template axis_slide_deferred<AX, ACT>(P, L.A, negbits, stale, []() {});
+    else if constexpr (BRICK)
         L.S.template axis_slide_deferred<AX, ACT>(P, L.A, negbits, stale, [&]() { brick_flush<AX, ACT>(G, L, negbits); });
     else      // per voxel: one red.v4.f32 (red.f32, red.f64 per bin) of its bins
         L.S.template axis_slide_deferred<AX, ACT>(P, L.A, negbits, stale, [&]() { L.S.template flush_trailing<AX, ACT>(L.sg, L.A); });
@@ -184,7 +187,7 @@ __device__ __forceinline__ void phased_load_att(const MarchParams& P, LANE& L, i
 
 // The substep loop with the axes in ACT active; runs until the table runs out (TABLE), the time step ends or an
 // axis goes inactive, and returns the new set of active axes.
-template <int ACT, int NB, bool TABLE, bool BRICK, bool STEP, bool JVP, bool KTRI, class LANE>
+template <int ACT, int NB, bool TABLE, bool BRICK, bool STEP, bool JVP, bool KTRI, bool RECORD, class LANE>
 __device__ __forceinline__ int phase(const MarchParams& P, const BrickGeom& G, LANE& L, int negbits, uint32_t tbase) {
     constexpr int kBits = ((ACT & 1) ? 4 : 0) | ((ACT & 2) ? 2 : 0) | ((ACT & 4) ? 1 : 0);      // slot index bits in use
     constexpr int kActive = ((ACT & 1) ? 1 : 0) + ((ACT & 2) ? 1 : 0) + ((ACT & 4) ? 1 : 0);
@@ -272,13 +275,18 @@ __device__ __forceinline__ int phase(const MarchParams& P, const BrickGeom& G, L
                 L.Td[b] = att * fmaf(-L.T[b], u, L.Td[b]);
             }
             // eq. (2).  STEP: T is the carried exp(-tau) itself, else ds 4 pi/N_Omega rides on it
-            L.I[b] = fmaf(L.I[b], att, STEP ? (jv + ju) * L.T[b] * P.emis : (jv + ju) * L.T[b]);
+            const float emitted = STEP ? (jv + ju) * L.T[b] * P.emis : (jv + ju) * L.T[b];
+            L.I[b] = fmaf(L.I[b], att, emitted);
             L.T[b] *= att;
-            const float dep = JVP ? L.Id[b] : L.I[b];           // what is deposited, with the weights of x_k
+            if constexpr (RECORD) {          // (I_{k+1}, P_k) of this substep; a warp writes one 256-byte run
+                if (b == 0 && L.rec_at >= 0) P.record[(long long)L.g * P.record_stride + L.rec_at] = make_float2(L.I[0], emitted);
+            } else {
+                const float dep = JVP ? L.Id[b] : L.I[b];       // what is deposited, with the weights of x_k
 #pragma unroll
-            for (int s = 0; s < 8; ++s)
-                if ((s & ~kBits) == 0)
-                    L.S.acc[s].v[b] = (ACT == 0) ? L.S.acc[s].v[b] + dep : fmaf(w[s], dep, L.S.acc[s].v[b]);
+                for (int s = 0; s < 8; ++s)
+                    if ((s & ~kBits) == 0)
+                        L.S.acc[s].v[b] = (ACT == 0) ? L.S.acc[s].v[b] + dep : fmaf(w[s], dep, L.S.acc[s].v[b]);
+            }
         }
 
         if constexpr (ACT != 0) {
@@ -288,9 +296,9 @@ __device__ __forceinline__ int phase(const MarchParams& P, const BrickGeom& G, L
                 for (int a = 0; a < 3; ++a)
                     if ((ACT & (1 << a)) && cross[a]) {
                         if constexpr (TABLE) L.A[a].p.c += 1;
-                        if (a == 0) phased_axis_step<0, ACT, BRICK>(P, G, L, negbits, stale);
-                        if (a == 1) phased_axis_step<1, ACT, BRICK>(P, G, L, negbits, stale);
-                        if (a == 2) phased_axis_step<2, ACT, BRICK>(P, G, L, negbits, stale);
+                        if (a == 0) phased_axis_step<0, ACT, BRICK, RECORD>(P, G, L, negbits, stale);
+                        if (a == 1) phased_axis_step<1, ACT, BRICK, RECORD>(P, G, L, negbits, stale);
+                        if (a == 2) phased_axis_step<2, ACT, BRICK, RECORD>(P, G, L, negbits, stale);
                         if constexpr (TABLE) {       // every lane crosses in the same substep: vote right here
                             const int lim = (a == 0 ? P.nx : (a == 1 ? P.ny : P.nz)) - 1;
                             const bool gone = L.A[a].p.c >= ((negbits & (1 << a)) ? 0 : lim);    // beyond the far face for good
@@ -343,10 +351,14 @@ __device__ __forceinline__ int phase(const MarchParams& P, const BrickGeom& G, L
 // next to I and deposited instead of it.
 // KTRI: the rt_march_trilinear_kappa form (D18) -- kappa cached at the stencil voxels like j and read with
 // the trilinear weights every substep.
-template <int NB, bool TABLE, bool BRICK = (NB == 1), typename ACC = float, bool STEP = false, bool JVP = false, bool KTRI = false>
+// RECORD: the first pass of rt_march_adjoint_kappa (D19) -- nothing is deposited; (I_{k+1}, P_k) of every
+// substep go to P.record for the backward march (rt_adjoint.cuh), which maps its threads to rays the same way.
+template <int NB, bool TABLE, bool BRICK = (NB == 1), typename ACC = float, bool STEP = false, bool JVP = false, bool KTRI = false,
+          bool RECORD = false>
 __global__ void __launch_bounds__(kThreads, NB == 1 ? (TABLE ? RT_PHASED_MINB1 : RT_PHASED_MINB1P) : RT_PHASED_MINB4)
 march_phased_kernel(const MarchParams P) {
     static_assert(!BRICK || (NB == 1 && sizeof(ACC) == 4), "the brick scratch holds one fp32 bin");
+    static_assert(!RECORD || (NB == 1 && !BRICK && !STEP && !JVP && !KTRI), "RECORD: the plain forward march, one bin per thread");
     __shared__ __align__(16) TableRow table[TABLE ? kThreads / 32 : 1][32];
     __shared__ Fx96 ref[TABLE ? kThreads / 32 : 1][6];      // per warp: fraction of x_0 (cell word 0) and increment, per axis
     if (P.same_frac && (*P.same_frac != 0) != TABLE) return;           // the other instantiation marches this call
@@ -407,6 +419,7 @@ march_phased_kernel(const MarchParams P) {
                                           ((negbits & 4) ? L.A[2].dl : 0));
         }
         L.g = 0;
+        L.rec_at = live ? (long long)blockIdx.x * kThreads + threadIdx.x : -1;
         L.left = (STEP && P.first_left) ? P.first_left : P.n_sub;
         L.roff = 0;
         L.woff = 0;
@@ -453,17 +466,19 @@ march_phased_kernel(const MarchParams P) {
                 }
             }
             switch (act) {
-                case 7: act = phase<7, NB, TABLE, BRICK, STEP, JVP, KTRI>(P, G, L, negbits, tbase); break;
-                case 6: act = phase<6, NB, TABLE, BRICK, STEP, JVP, KTRI>(P, G, L, negbits, tbase); break;
-                case 5: act = phase<5, NB, TABLE, BRICK, STEP, JVP, KTRI>(P, G, L, negbits, tbase); break;
-                case 4: act = phase<4, NB, TABLE, BRICK, STEP, JVP, KTRI>(P, G, L, negbits, tbase); break;
-                case 3: act = phase<3, NB, TABLE, BRICK, STEP, JVP, KTRI>(P, G, L, negbits, tbase); break;
-                case 2: act = phase<2, NB, TABLE, BRICK, STEP, JVP, KTRI>(P, G, L, negbits, tbase); break;
-                case 1: act = phase<1, NB, TABLE, BRICK, STEP, JVP, KTRI>(P, G, L, negbits, tbase); break;
-                default: act = phase<0, NB, TABLE, BRICK, STEP, JVP, KTRI>(P, G, L, negbits, tbase); break;
+                case 7: act = phase<7, NB, TABLE, BRICK, STEP, JVP, KTRI, RECORD>(P, G, L, negbits, tbase); break;
+                case 6: act = phase<6, NB, TABLE, BRICK, STEP, JVP, KTRI, RECORD>(P, G, L, negbits, tbase); break;
+                case 5: act = phase<5, NB, TABLE, BRICK, STEP, JVP, KTRI, RECORD>(P, G, L, negbits, tbase); break;
+                case 4: act = phase<4, NB, TABLE, BRICK, STEP, JVP, KTRI, RECORD>(P, G, L, negbits, tbase); break;
+                case 3: act = phase<3, NB, TABLE, BRICK, STEP, JVP, KTRI, RECORD>(P, G, L, negbits, tbase); break;
+                case 2: act = phase<2, NB, TABLE, BRICK, STEP, JVP, KTRI, RECORD>(P, G, L, negbits, tbase); break;
+                case 1: act = phase<1, NB, TABLE, BRICK, STEP, JVP, KTRI, RECORD>(P, G, L, negbits, tbase); break;
+                default: act = phase<0, NB, TABLE, BRICK, STEP, JVP, KTRI, RECORD>(P, G, L, negbits, tbase); break;
             }
             if (L.left == 0) {               // time-step boundary: the increments of this step are complete (rays continue, D7)
-                if constexpr (BRICK) {
+                if constexpr (RECORD) {
+                    // nothing was deposited
+                } else if constexpr (BRICK) {
                     brick_flush<-1, 7>(G, L, negbits);         // slots of inactive axes hold exact zeros: skipped by value
 #pragma unroll
                     for (int s = 0; s < 8; ++s) L.S.zero_slot(s);
@@ -483,7 +498,7 @@ march_phased_kernel(const MarchParams P) {
             }
         }
     }
-    if constexpr (sizeof(ACC) == 8) return;
+    if constexpr (RECORD || sizeof(ACC) == 8) return;
     // this block's turn at the drain: one slice of the scratch goes to the fp64 grid (rt_brick.cuh)
     const long long per = P.drain_units_per_block;
     if (per == 0) return;        // the scratch is the result grid itself: nothing to drain (rt_api.cu)
