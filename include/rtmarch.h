@@ -147,7 +147,7 @@ int rt_march_adjoint_j(const float* gbar, const float* kappa, int nx, int ny, in
  * grad_kappa[nx][ny][nz][n_bins] = dL/dkappa (device, fp32, OVERWRITTEN; summed in fp64) for gbar[m] = dL/d out[m] of
  * rt_march(j, kappa, ...): kappa enters eq. (2) through exp(-kappa ds) and exp(-tau), read nearest neighbour at the
  * cell of x_k, so dL/dkappa_i = ds [P_i lambda_{i+1} - sum_{k>=i} G_k I_{k+1}] summed into that cell.  The forward
- * intensities are recorded (8 bytes per ray-substep-bin, sources in batches so the record stays below 2 GiB) and the
+ * intensities are recorded (8 bytes per ray-substep-bin, sources in batches so the record stays below 8 GiB) and the
  * rays are then marched backwards.  Same argument rules, limits and error codes as rt_march; workspace:
  * rt_adjoint_kappa_workspace_bytes() bytes (0 on invalid arguments). */
 size_t rt_adjoint_kappa_workspace_bytes(int nx, int ny, int nz, int n_src, int n_rays, int n_bins,
@@ -171,7 +171,7 @@ int rt_march_jvp_kappa(const float* j, const float* kappa, const float* dkappa, 
                        void* workspace, size_t workspace_bytes, void* stream);
 
 /* TEST HOOK.  rt_march_adjoint_kappa with the bound on the forward record of one source batch given explicitly
- * (record_limit bytes; 0 = the library's 2 GiB), so that tests can drive the source-batch loop on small cases.  A batch
+ * (record_limit bytes; 0 = the library's 8 GiB), so that tests can drive the source-batch loop on small cases.  A batch
  * never holds fewer than 32 sources (n_src >= 32) or 1 source (n_src < 32).  Same result for every limit. */
 size_t rt_adjoint_kappa_workspace_bytes_ex(int nx, int ny, int nz, int n_src, int n_rays, int n_bins,
                                            float step_size, float c, float dt, int n_steps, size_t record_limit);

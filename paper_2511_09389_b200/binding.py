@@ -334,7 +334,7 @@ def rt_adjoint_kappa_workspace_bytes_ex(nx, ny, nz, n_src, n_rays, n_bins, step_
 def rt_march_adjoint_kappa_ex(gbar, j, kappa, sources, n_rays, step_size, c, dt, n_steps, grad_kappa=None,
                               workspace=None, stream=None, record_limit: int = 0):
     """rt_march_adjoint_kappa with the forward-record bound of one source batch given in bytes (0 = the library's
-    2 GiB): the test hook that drives the source-batch loop on small cases."""
+    8 GiB): the test hook that drives the source-batch loop on small cases."""
     torch = _torch()
     _check_dev(gbar, "gbar", torch.float32, 5)
     _check_dev(j, "j", torch.float32, 4)

@@ -227,7 +227,7 @@ def test_kappa_adjoint_source_batches_match_the_oracle(rt, oracle_mod, n_src, n_
 
 def test_kappa_adjoint_c2_subset_in_batches_matches_the_oracle(rt, oracle_mod):
     """C2's grid, rays and substeps with 72 of its sources: the record of all of them (72 x 4,096 x 444 x 8 B = 1 GB)
-    is cut into batches of 32 sources by the record limit, as the full config is cut by the 2 GiB default."""
+    is cut into batches of 32 sources by the record limit, as the full config is cut by the 8 GiB default."""
     w = workloads.make_config("C2")
     src = np.ascontiguousarray(w.sources[_stratified(w.n_src, 72)])
     rng = np.random.default_rng(13)
