@@ -197,7 +197,7 @@ int rt_host_release(void);
  * of n_steps * nx*ny*nz*n_bins floats where the batched multi-bin kernels of the variants run (n_bins % 4 == 0 and that
  * grid <= 128 MiB), for one-bin calls the fp32 window-brick scratch of the march (n_steps * nx*(ny+1)*(nz+1)*4
  * floats, if <= 1 GiB), and for grids far larger than the L2 (that fp32 grid > 128 MiB, no brick scratch,
- * n_src * n_rays < 2^32) the sorted ray list (8 bytes per ray + 256 KiB, and with bins in fours a ray state of
+ * n_src * n_rays < 2^32) the sorted ray list (8 bytes per ray + 4 MiB, and with bins in fours a ray state of
  * 8 bytes per ray and bin).  0 on invalid arguments. */
 size_t rt_workspace_bytes(int nx, int ny, int nz, int n_src, int n_rays, int n_bins, int n_steps);
 

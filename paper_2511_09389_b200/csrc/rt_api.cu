@@ -444,12 +444,12 @@ int run_phased(rt::MarchParams P, const PhasedPlan& pp, const Plan& pl, const Wo
         uint32_t* cursor = hist + rt::kRayTiles;
         uint32_t* perm = reinterpret_cast<uint32_t*>(reinterpret_cast<char*>(cursor + rt::kRayTiles) + near_state_bytes(n_ray, n_bins));
         uint32_t* key = perm + n_ray;
-        RT_CUDA(cudaMemsetAsync(hist, 0, rt::kRayTiles * sizeof(uint32_t), st));
+        const rt::RaySortGeom sg = rt::ray_sort_geom(nx, ny, nz);
+        RT_CUDA(cudaMemsetAsync(hist, 0, size_t(sg.n_keys) * sizeof(uint32_t), st));
         const unsigned rb = unsigned((n_ray + 255) / 256);
         const long long k_mid = P.k0 + (long long)P.n_sub * n_steps / 2;
-        rt::ray_tile_key_kernel<<<rb, 256, 0, st>>>(key, hist, sources, n_ray, n_rays, P.ds, k_mid, nx, ny, nz,
-                                                    rt::ray_tile_shift(nx, ny, nz));
-        rt::ray_tile_scan_kernel<<<1, 1024, 0, st>>>(hist, cursor);
+        rt::ray_tile_key_kernel<<<rb, 256, 0, st>>>(key, hist, sources, n_ray, n_rays, P.ds, k_mid, nx, ny, nz, sg);
+        rt::ray_tile_scan_kernel<<<1, 1024, 0, st>>>(hist, cursor, sg.n_keys);
         rt::ray_tile_scatter_kernel<<<rb, 256, 0, st>>>(perm, key, cursor, n_ray);
         RT_CUDA(cudaGetLastError());
         P.map_src = 2;
