@@ -239,7 +239,12 @@ int phased_kind(int variant, float step_size, long long cells, int n_steps, int 
 // red.global.add.f64), (I, exp(-tau)) go through a ray state in the workspace as in rt_march_step, and the four-bin
 // launch marches the rest into the fp32 scratch.  Only the time steps those first substeps fall into have anything in
 // the fp64 grid: only they are zeroed, and read when the snapshots are formed.
+// And no element may collect too many addends: a ray sums its deposits into a voxel in registers while the voxel is in
+// its stencil, so an element receives at most one addend per ray and time step -- also the corner and face voxels that
+// rays outside the box keep depositing into -- i.e. at most n_src N_Omega of them.  The bound is that of
+// two drain rounds (drain_rounds: one per 2^19 rays; on C2, sums of 2^21 rays' addends were off by 2e-4 at worst).
 constexpr double kNoDrainDeposits = 256.0;
+constexpr long long kNoDrainRays = 1LL << 21;
 long long near_substeps(int n_rays, float step_size) {
     const double r = 2.0 + std::sqrt(double(n_rays) / (1024.0 * 3.14159265358979323846));
     return (long long)std::ceil(r / double(step_size));
@@ -257,7 +262,8 @@ PhasedPlan phased_plan(int variant, float step_size, long long cells, int n_step
     // the trilinear-kappa and the tangent march exist with one bin per thread only
     if (one_bin_per_thread && pp.kind == kPhasedFourBins) pp.kind = kPhasedDirect64;
     pp.no_drain = pp.sorted && pp.kind == kPhasedFourBins && near_k <= n_sub &&
-                  ray_substeps_per_step * 8.0 <= kNoDrainDeposits * double(cells / n_bins);
+                  ray_substeps_per_step * 8.0 <= kNoDrainDeposits * double(cells / n_bins) &&
+                  ray_substeps_per_step <= double(kNoDrainRays) * double(n_sub);
     return pp;
 }
 // how often the scratch is drained during a march: an fp32 sum should not collect much more than 2^19 rays' deposits
