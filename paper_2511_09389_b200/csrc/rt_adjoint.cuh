@@ -14,6 +14,7 @@
 // the forward ray's, bit for bit, hence the same cells and the same weight bits.  tau_k is recovered by
 // subtracting kappa_k ds in fp64 (an fp32 running difference would lose 1e-3 of T over a few hundred substeps).
 #pragma once
+#include "rt_march_phased.cuh"
 #include "rt_march_sliding.cuh"
 
 namespace rt {
@@ -42,6 +43,8 @@ struct AdjointLane {
     long long kk;                    // global substep index of the backward sweep
     float2 rec;                      // WRT_KAPPA: the record of substep kk, loaded one substep ahead of its use
     int left;                        // substeps left in the current time step
+    float* sg;                       // BRICK: the fp32 window-brick scratch (rt_brick.cuh) the dL/dj deposits go to ...
+    int woff;                        // ... and the float offset in it of the window the trailing slots start
 };
 
 // PHASES of the backward march (cf. rt_march_phased.cuh).  The backward ray starts at x_{K-1}, for most rays far outside
@@ -53,8 +56,8 @@ struct AdjointLane {
 // axis is still merged in every lane and its first slide loads its leading slots.
 constexpr int kAdjMargin = 4;
 
-template <int ACT, bool WRT_KAPPA>
-__device__ __forceinline__ int adjoint_phase(const MarchParams& P, AdjointLane& L, int negbits, double* og, const float* gs,
+template <int ACT, bool WRT_KAPPA, bool BRICK>
+__device__ __forceinline__ int adjoint_phase(const MarchParams& P, const BrickGeom& G, AdjointLane& L, int negbits, double* og, const float* gs,
                                              const float2* fwd, long long fwd_stride, long long tid, int bin, bool live) {
     constexpr int kBits = ((ACT & 1) ? 4 : 0) | ((ACT & 2) ? 2 : 0) | ((ACT & 4) ? 1 : 0);
     constexpr int kActive = ((ACT & 1) ? 1 : 0) + ((ACT & 2) ? 1 : 0) + ((ACT & 4) ? 1 : 0);
@@ -146,9 +149,13 @@ __device__ __forceinline__ int adjoint_phase(const MarchParams& P, AdjointLane& 
             }
             if (!jumped) {               // slides with the loads deferred (rt_march_sliding.cuh)
                 uint32_t stale = 0;
-                if (cross[0]) L.S.template axis_slide_deferred<0, ACT>(P, L.A, negbits, stale, [&]() { L.S.template flush_trailing<0, ACT>(og, L.A); });
-                if (cross[1]) L.S.template axis_slide_deferred<1, ACT>(P, L.A, negbits, stale, [&]() { L.S.template flush_trailing<1, ACT>(og, L.A); });
-                if (cross[2]) L.S.template axis_slide_deferred<2, ACT>(P, L.A, negbits, stale, [&]() { L.S.template flush_trailing<2, ACT>(og, L.A); });
+                // the trailing plane goes slot by slot into the fp64 grid, or as one vector reduction into the brick scratch
+                if (cross[0]) L.S.template axis_slide_deferred<0, ACT>(P, L.A, negbits, stale, [&]() {
+                    if constexpr (BRICK) brick_flush<0, ACT>(G, L, negbits); else L.S.template flush_trailing<0, ACT>(og, L.A); });
+                if (cross[1]) L.S.template axis_slide_deferred<1, ACT>(P, L.A, negbits, stale, [&]() {
+                    if constexpr (BRICK) brick_flush<1, ACT>(G, L, negbits); else L.S.template flush_trailing<1, ACT>(og, L.A); });
+                if (cross[2]) L.S.template axis_slide_deferred<2, ACT>(P, L.A, negbits, stale, [&]() {
+                    if constexpr (BRICK) brick_flush<2, ACT>(G, L, negbits); else L.S.template flush_trailing<2, ACT>(og, L.A); });
                 L.S.template load_stale<ACT>(P, L.A, gs, stale);
             }
             if (WRT_KAPPA) {                     // the kappa cell may have changed: reduce the old one's sum
@@ -184,7 +191,19 @@ __device__ __forceinline__ int adjoint_phase(const MarchParams& P, AdjointLane& 
 // substep i) dL/dkappa_i = ds [P_i lambda_{i+1} - R_i], R_i = sum_{k>=i} G_k I_{k+1}: the same backward march,
 // fed with (I_{k+1}, P_k) of every substep as recorded by march_sliding_kernel<..., RECORD = true>, summing into the kappa cell of x_i
 // (nearest neighbour: one voxel per substep, reduced when the cell changes).
-template <int MINB, bool WRT_KAPPA>
+// this block's turn at the drain of the brick scratch (as at the end of march_phased_kernel)
+__device__ __forceinline__ void adjoint_drain_slice(const MarchParams& P, const BrickGeom& G) {
+    const long long per = P.drain_units_per_block;
+    if (per == 0) return;
+    const long long n_slices = (P.n_drain_units + per - 1) / per;
+    const long long b0 = (blockIdx.x % n_slices) * per;
+    drain_bricks(P.scratch, static_cast<double*>(P.acc), G, P.nx, P.ny, P.nz, b0, min(b0 + per, P.n_drain_units), threadIdx.x, kThreads);
+}
+
+// BRICK (dL/dj, one bin, substeps shorter than a cell): the deposits go to the fp32 window-brick scratch P.scratch with one
+// vector reduction per stencil plane and every block drains a slice of it into the fp64 grid when its rays are done, as
+// in the forward march (rt_brick.cuh, rt_march_phased.cuh).
+template <int MINB, bool WRT_KAPPA, bool BRICK = false>
 __global__ void __launch_bounds__(kThreads, MINB) adjoint_kernel(const MarchParams P, const float* gsuf,
                                                                  const float2* fwd, long long fwd_stride) {
     // a warp marches as a whole (its phases are warp votes): a lane without a ray of its own marches the ray of the
@@ -192,7 +211,11 @@ __global__ void __launch_bounds__(kThreads, MINB) adjoint_kernel(const MarchPara
     RayId id;
     const bool live = ray_id(P, id);
     const unsigned live_mask = __ballot_sync(0xFFFFFFFFu, live);
-    if (!live_mask) return;
+    const BrickGeom G = brick_geom(P.nx, P.ny, P.nz);
+    if (!live_mask) {
+        if constexpr (BRICK) adjoint_drain_slice(P, G);
+        return;
+    }
     {
         const int leader = __ffs(live_mask) - 1;
         const int lsrc = __shfl_sync(0xFFFFFFFFu, id.src, leader), lgroup = __shfl_sync(0xFFFFFFFFu, id.group, leader);
@@ -255,6 +278,11 @@ __global__ void __launch_bounds__(kThreads, MINB) adjoint_kernel(const MarchPara
     for (int s = 0; s < 8; ++s) L.S.zero_slot(s);
     const float* gs = gsuf + (long long)(P.n_steps - 1) * P.snap_stride;
     L.S.restart(P, L.A, negbits, bin, gs);
+    L.sg = P.scratch;
+    L.woff = 0;
+    if constexpr (BRICK)
+        L.woff = (aidx<0>(P, L.A[0].p.c, negbits) * G.wy + aidx<1>(P, L.A[1].p.c, negbits) + ((negbits & 2) ? 0 : 1)) * G.sy +
+                 (aidx<2>(P, L.A[2].p.c, negbits) + ((negbits & 4) ? 0 : 1)) * 4;
     L.lambda = 0.0f; L.a_next = 0.0f;
     L.Rsum = 0.0; L.kacc = 0.0;
     L.ko = L.S.base + ((negbits & 1) ? L.A[0].dl : 0) + ((negbits & 2) ? L.A[1].dl : 0) + ((negbits & 4) ? L.A[2].dl : 0);
@@ -275,14 +303,14 @@ __global__ void __launch_bounds__(kThreads, MINB) adjoint_kernel(const MarchPara
     while (true) {
         {
             switch (act) {
-                case 7: act = adjoint_phase<7, WRT_KAPPA>(P, L, negbits, og, gs, fwd, fwd_stride, tid, bin, live); break;
-                case 6: act = adjoint_phase<6, WRT_KAPPA>(P, L, negbits, og, gs, fwd, fwd_stride, tid, bin, live); break;
-                case 5: act = adjoint_phase<5, WRT_KAPPA>(P, L, negbits, og, gs, fwd, fwd_stride, tid, bin, live); break;
-                case 4: act = adjoint_phase<4, WRT_KAPPA>(P, L, negbits, og, gs, fwd, fwd_stride, tid, bin, live); break;
-                case 3: act = adjoint_phase<3, WRT_KAPPA>(P, L, negbits, og, gs, fwd, fwd_stride, tid, bin, live); break;
-                case 2: act = adjoint_phase<2, WRT_KAPPA>(P, L, negbits, og, gs, fwd, fwd_stride, tid, bin, live); break;
-                case 1: act = adjoint_phase<1, WRT_KAPPA>(P, L, negbits, og, gs, fwd, fwd_stride, tid, bin, live); break;
-                default: act = adjoint_phase<0, WRT_KAPPA>(P, L, negbits, og, gs, fwd, fwd_stride, tid, bin, live); break;
+                case 7: act = adjoint_phase<7, WRT_KAPPA, BRICK>(P, G, L, negbits, og, gs, fwd, fwd_stride, tid, bin, live); break;
+                case 6: act = adjoint_phase<6, WRT_KAPPA, BRICK>(P, G, L, negbits, og, gs, fwd, fwd_stride, tid, bin, live); break;
+                case 5: act = adjoint_phase<5, WRT_KAPPA, BRICK>(P, G, L, negbits, og, gs, fwd, fwd_stride, tid, bin, live); break;
+                case 4: act = adjoint_phase<4, WRT_KAPPA, BRICK>(P, G, L, negbits, og, gs, fwd, fwd_stride, tid, bin, live); break;
+                case 3: act = adjoint_phase<3, WRT_KAPPA, BRICK>(P, G, L, negbits, og, gs, fwd, fwd_stride, tid, bin, live); break;
+                case 2: act = adjoint_phase<2, WRT_KAPPA, BRICK>(P, G, L, negbits, og, gs, fwd, fwd_stride, tid, bin, live); break;
+                case 1: act = adjoint_phase<1, WRT_KAPPA, BRICK>(P, G, L, negbits, og, gs, fwd, fwd_stride, tid, bin, live); break;
+                default: act = adjoint_phase<0, WRT_KAPPA, BRICK>(P, G, L, negbits, og, gs, fwd, fwd_stride, tid, bin, live); break;
             }
         }
         if (L.left == 0) {                           // an earlier time step sees the suffix sum of one more snapshot
@@ -294,6 +322,9 @@ __global__ void __launch_bounds__(kThreads, MINB) adjoint_kernel(const MarchPara
     }
     if (WRT_KAPPA) {
         if (L.kacc != 0.0) asm volatile("red.global.add.f64 [%0], %1;" ::"l"(og + L.ko), "d"(L.kacc) : "memory");
+    } else if constexpr (BRICK) {
+        brick_flush<-1, 7>(G, L, negbits);
+        adjoint_drain_slice(P, G);
     } else {
         L.S.flush_all(og, L.A);
     }

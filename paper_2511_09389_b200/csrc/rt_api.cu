@@ -777,6 +777,20 @@ int rt_march_adjoint_j(const float* gbar, const float* kappa, int nx, int ny, in
     }
     const long long mb = rt::march_blocks(n_src, P.n_slots, P.n_groups, P.map_src);
     if (mb > 2147483647LL) return RT_EINVAL;
+    if (n_bins == 1 && wl.brick_bytes && step_size < 1.0f) {
+        // one bin: deposits as vector reductions into the fp32 brick scratch, drained into the fp64 grid during the march
+        P.scratch = reinterpret_cast<float*>(ws + wl.brick_at);
+        RT_CUDA(cudaMemsetAsync(P.scratch, 0, wl.brick_bytes, st));
+        P.n_drain_units = std::max<long long>(1, (long long)(wl.brick_bytes / 16));
+        const long long per = (P.n_drain_units * drain_rounds((long long)n_src * n_rays) + mb - 1) / mb;
+        P.drain_units_per_block = std::min<long long>(std::max<long long>(per, 1), rt::kDrainMaxUnits);
+        rt::adjoint_kernel<6, false, true><<<unsigned(mb), rt::kThreads, 0, st>>>(P, gsuf, nullptr, 0);
+        RT_CUDA(cudaGetLastError());
+        rt::snapshot_finalize_scratch_kernel<true><<<unsigned(blocks), threads, 0, st>>>(master, P.scratch, grad_j, ck.cells, 1,
+                                                                                        rt::brick_geom(nx, ny, nz), ny, nz, 1);
+        RT_CUDA(cudaGetLastError());
+        return RT_OK;
+    }
     rt::adjoint_kernel<6, false><<<unsigned(mb), rt::kThreads, 0, st>>>(P, gsuf, nullptr, 0);
     RT_CUDA(cudaGetLastError());
     rt::snapshot_finalize_kernel<double><<<unsigned(blocks), threads, 0, st>>>(master, grad_j, ck.cells, 1);
