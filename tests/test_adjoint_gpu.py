@@ -170,6 +170,26 @@ def _stratified(n_src, count):
     return np.unique(np.linspace(0, n_src - 1, count).round().astype(int))
 
 
+def test_adjoint_j_at_full_c2_size_is_the_transpose_and_adds_up_over_source_chunks(rt):
+    """The launch configuration of the headline (2,097 sources: brick scratch with 16 concurrent drain rounds): the
+    transpose identity against the CUDA march, and the gradient of all sources against the sum of the gradients of four
+    source chunks (other drain slices, other summation order), voxel by voxel at the parity tolerances."""
+    w = workloads.make_config("C2")
+    rng = np.random.default_rng(23)
+    j, kap, src = _dev(w.j), _dev(w.kappa), _dev(w.sources)
+    args = (w.n_rays, w.step_size, w.c, w.dt, w.n_steps)
+    out = rt.rt_march(j, kap, src, *args)
+    g = torch.from_numpy(rng.uniform(0.0, 1.0, tuple(out.shape)).astype(np.float32)).cuda()
+    grad = rt.rt_march_adjoint_j(g, kap, src, *args)
+    torch.cuda.synchronize()
+    lhs, rhs = float((out.double() * g.double()).sum()), float((j.double() * grad.double()).sum())
+    assert abs(lhs - rhs) <= 2e-5 * abs(lhs), (lhs, rhs)
+    parts = torch.zeros_like(grad, dtype=torch.float64)
+    for chunk in np.array_split(np.arange(w.n_src), 4):
+        parts += rt.rt_march_adjoint_j(g, kap, _dev(w.sources[chunk]), *args).double()
+    parity.assert_parity(grad.cpu().numpy()[None], parts.cpu().numpy()[None], "adjoint_j full C2 vs 4 source chunks")
+
+
 @pytest.mark.parametrize("name,count", [("C2", 40), ("C3", 36), ("C4", 2)])
 def test_adjoint_j_on_config_subsets_matches_the_oracle(rt, oracle_mod, name, count):
     """rt_march_adjoint_j with the config's own grid, rays, substeps, steps and bins on a stratified subset of its
