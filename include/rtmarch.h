@@ -132,7 +132,8 @@ int rt_march_step(const float* j, const float* kappa, int nx, int ny, int nz,
 
 /* ADJOINT WITH RESPECT TO j (P:62-64 differentiability; reading D19).  For fixed kappa the field of
  * rt_march is linear in j: out[m] = A_m j.  Given gbar[n_steps][nx][ny][nz][n_bins] = dL/d out[m] (device, fp32)
- * this writes grad_j[nx][ny][nz][n_bins] = sum_m A_m^T gbar[m] = dL/dj (device, fp32, OVERWRITTEN; summed in fp64):
+ * this writes grad_j[nx][ny][nz][n_bins] = sum_m A_m^T gbar[m] = dL/dj (device, fp32, OVERWRITTEN; summed in fp64 -- with
+ * one bin through the fp32 scratch of the forward march, drained into the fp64 grid during the march):
  * the backward recurrence of eq. (2), marched along every ray from its last substep to its first with the same
  * clamped trilinear stencils, gather and deposit exchanged.  <rt_march(j), gbar> = <j, grad_j> up to rounding.
  * kappa is read nearest neighbour (as rt_march).  Same argument rules, limits and error codes as rt_march;
