@@ -148,7 +148,7 @@ int rt_march_adjoint_j(const float* gbar, const float* kappa, int nx, int ny, in
  * grad_kappa[nx][ny][nz][n_bins] = dL/dkappa (device, fp32, OVERWRITTEN; summed in fp64) for gbar[m] = dL/d out[m] of
  * rt_march(j, kappa, ...): kappa enters eq. (2) through exp(-kappa ds) and exp(-tau), read nearest neighbour at the
  * cell of x_k, so dL/dkappa_i = ds [P_i lambda_{i+1} - sum_{k>=i} G_k I_{k+1}] summed into that cell.  The forward
- * intensities are recorded (8 bytes per ray-substep-bin, sources in batches so the record stays below 8 GiB) and the
+ * intensities I_{k+1} are recorded (4 bytes per ray-substep-bin; P_i = I_{i+1} - exp(-kappa_i ds) I_i is recovered from them; sources in batches so the record stays below 8 GiB) and the
  * rays are then marched backwards.  Same argument rules, limits and error codes as rt_march; workspace:
  * rt_adjoint_kappa_workspace_bytes() bytes (0 on invalid arguments). */
 size_t rt_adjoint_kappa_workspace_bytes(int nx, int ny, int nz, int n_src, int n_rays, int n_bins,

@@ -22,7 +22,7 @@ namespace rt {
 // WRT_KAPPA = false: dL/dj as described above.  WRT_KAPPA = true: dL/dkappa (D19).  Unrolling eq. (2),
 // I_{k+1} = T_{k+1} sum_{m<=k} ds J_m / a_m, so with G_k = w_k . gsuf and P_i = ds J_i T_i (the emission term of
 // substep i) dL/dkappa_i = ds [P_i lambda_{i+1} - R_i], R_i = sum_{k>=i} G_k I_{k+1}: the same backward march,
-// fed with (I_{k+1}, P_k) of every substep as recorded by march_sliding_kernel<..., RECORD = true>, summing into the kappa cell of x_i
+// fed with I_{k+1} of every substep as recorded by march_phased_kernel<..., RECORD = true> (P_k = I_{k+1} - a_k I_k), summing into the kappa cell of x_i
 // (nearest neighbour: one voxel per substep, reduced when the cell changes).
 #ifndef RT_REC_AHEAD
 #define RT_REC_AHEAD 8
@@ -41,7 +41,7 @@ struct AdjointLane {
     double tau, Rsum, kacc;          // WRT_KAPPA: R_i and the pending sum of the current kappa cell, in fp64 (P_i lambda_{i+1} - R_i cancels)
     int ko;                          // element offset of the kappa cell
     long long kk;                    // global substep index of the backward sweep
-    float2 rec;                      // WRT_KAPPA: the record of substep kk, loaded one substep ahead of its use
+    float rec, rec1;                 // WRT_KAPPA: the records I_{kk+1} and I_kk, loaded one and two substeps before this one
     int left;                        // substeps left in the current time step
     float* sg;                       // BRICK: the fp32 window-brick scratch (rt_brick.cuh) the dL/dj deposits go to ...
     int woff;                        // ... and the float offset in it of the window the trailing slots start
@@ -58,7 +58,7 @@ constexpr int kAdjMargin = 4;
 
 template <int ACT, bool WRT_KAPPA, bool BRICK>
 __device__ __forceinline__ int adjoint_phase(const MarchParams& P, const BrickGeom& G, AdjointLane& L, int negbits, double* og, const float* gs,
-                                             const float2* fwd, long long fwd_stride, long long tid, int bin, bool live) {
+                                             const float* fwd, long long fwd_stride, long long tid, int bin, bool live) {
     constexpr int kBits = ((ACT & 1) ? 4 : 0) | ((ACT & 2) ? 2 : 0) | ((ACT & 4) ? 1 : 0);
     constexpr int kActive = ((ACT & 1) ? 1 : 0) + ((ACT & 2) ? 1 : 0) + ((ACT & 4) ? 1 : 0);
     constexpr int kLast = (ACT & 4) ? 2 : ((ACT & 2) ? 1 : 0);
@@ -113,14 +113,18 @@ __device__ __forceinline__ int adjoint_phase(const MarchParams& P, const BrickGe
             }
         if (!live) { gv = 0.0f; gu = 0.0f; }         // a dark lane: zero dL/d out, so lambda stays 0 and nothing is deposited
         if (WRT_KAPPA) {
-            // (I_{k+1}, P_k), both x 4 pi/N_Omega (a dark lane has no record)
-            const float2 rec = L.rec;
-            if (live && L.kk >= 1) L.rec = __ldg(fwd + (L.kk - 1) * fwd_stride + tid);
+            // The record holds I_{k+1} (x 4 pi/N_Omega) of every substep; the emission term is recovered from two of them,
+            // P_k = I_{k+1} - a_k I_k (eq. (2) solved for it; off by the rounding of the forward fma, <= 2^-25 I_{k+1}).
+            // I_{k+1} and I_k were loaded one and two substeps ago; the load issued now is I_{k-1}.  (A dark lane: zeros.)
+            const float I_next = L.rec, I_cur = L.rec1;
+            L.rec = I_cur;
+            L.rec1 = (live && L.kk >= 2) ? __ldg(fwd + (L.kk - 2) * fwd_stride + tid) : 0.0f;
             if (live && L.kk >= kRecAhead) asm volatile("prefetch.global.L2 [%0];" ::"l"(fwd + (L.kk - kRecAhead) * fwd_stride + tid));
             L.lambda = fmaf(L.a_next, L.lambda, gv + gu);
-            L.a_next = ex2_approx(L.kap * P.att_scale);
-            L.Rsum = fma(double(gv + gu), double(rec.x), L.Rsum);
-            L.kacc = fma(fma(double(rec.y), double(L.lambda), -L.Rsum), P.ds, L.kacc);
+            L.a_next = ex2_approx(L.kap * P.att_scale);                          // a_k, the same bits as in the forward march
+            const float P_k = fmaf(-L.a_next, I_cur, I_next);
+            L.Rsum = fma(double(gv + gu), double(I_next), L.Rsum);
+            L.kacc = fma(fma(double(P_k), double(L.lambda), -L.Rsum), P.ds, L.kacc);
             --L.kk;
         } else {
             L.tau = fma(-double(L.kap), P.ds, L.tau);                             // tau_k = tau_{k+1} - kappa_k ds
@@ -189,7 +193,7 @@ __device__ __forceinline__ int adjoint_phase(const MarchParams& P, const BrickGe
 // WRT_KAPPA = false: dL/dj as described above.  WRT_KAPPA = true: dL/dkappa (D19).  Unrolling eq. (2),
 // I_{k+1} = T_{k+1} sum_{m<=k} ds J_m / a_m, so with G_k = w_k . gsuf and P_i = ds J_i T_i (the emission term of
 // substep i) dL/dkappa_i = ds [P_i lambda_{i+1} - R_i], R_i = sum_{k>=i} G_k I_{k+1}: the same backward march,
-// fed with (I_{k+1}, P_k) of every substep as recorded by march_sliding_kernel<..., RECORD = true>, summing into the kappa cell of x_i
+// fed with I_{k+1} of every substep as recorded by march_phased_kernel<..., RECORD = true> (P_k = I_{k+1} - a_k I_k), summing into the kappa cell of x_i
 // (nearest neighbour: one voxel per substep, reduced when the cell changes).
 // this block's turn at the drain of the brick scratch (as at the end of march_phased_kernel)
 __device__ __forceinline__ void adjoint_drain_slice(const MarchParams& P, const BrickGeom& G) {
@@ -205,7 +209,7 @@ __device__ __forceinline__ void adjoint_drain_slice(const MarchParams& P, const 
 // in the forward march (rt_brick.cuh, rt_march_phased.cuh).
 template <int MINB, bool WRT_KAPPA, bool BRICK = false>
 __global__ void __launch_bounds__(kThreads, MINB) adjoint_kernel(const MarchParams P, const float* gsuf,
-                                                                 const float2* fwd, long long fwd_stride) {
+                                                                 const float* fwd, long long fwd_stride) {
     // a warp marches as a whole (its phases are warp votes): a lane without a ray of its own marches the ray of the
     // warp's first live lane with gsuf read as zero weight -- lambda stays 0, nothing is deposited
     RayId id;
@@ -288,7 +292,8 @@ __global__ void __launch_bounds__(kThreads, MINB) adjoint_kernel(const MarchPara
     L.ko = L.S.base + ((negbits & 1) ? L.A[0].dl : 0) + ((negbits & 2) ? L.A[1].dl : 0) + ((negbits & 4) ? L.A[2].dl : 0);
     L.kap = __ldg(P.kappa + L.ko);
     L.kk = K - 1;
-    L.rec = (WRT_KAPPA && live) ? __ldg(fwd + (K - 1) * fwd_stride + tid) : make_float2(0.0f, 0.0f);
+    L.rec = (WRT_KAPPA && live) ? __ldg(fwd + (K - 1) * fwd_stride + tid) : 0.0f;
+    L.rec1 = (WRT_KAPPA && live && K >= 2) ? __ldg(fwd + (K - 2) * fwd_stride + tid) : 0.0f;
     L.left = P.n_sub;
     // axes some lane is inside of, or about to enter, at x_{K-1}
     int act = 0;

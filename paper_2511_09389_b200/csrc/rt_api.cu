@@ -140,7 +140,7 @@ int launch_march(const rt::MarchParams& P, bool sliding, cudaStream_t st, bool o
         cfg.attrs = attr;
         cfg.numAttrs = 1;
         RT_CUDA(cudaLaunchKernelEx(&cfg, rt::march_sliding_kernel<NB, ACC, 4, false, false, false>, P,
-                                   static_cast<float2*>(nullptr), 0LL));
+                                   static_cast<float*>(nullptr), 0LL));
         return RT_OK;
     }
     if (sliding) {
@@ -798,9 +798,9 @@ int rt_march_adjoint_j(const float* gbar, const float* kappa, int nx, int ny, in
     return RT_OK;
 }
 
-// rt_march_adjoint_kappa records (I_{k+1}, P_k) of every substep of every ray of a launch: 8 bytes per
+// rt_march_adjoint_kappa records I_{k+1} of every substep of every ray of a launch: 4 bytes per
 // ray-substep-bin.  Sources are marched in batches so that this record stays below kForwardRecordLimit.
-constexpr size_t kForwardRecordLimit = size_t(8) << 30;      // C2: 4 batches; 2 GiB (17 batches, 17 tails): 32.7 ms against 30.1
+constexpr size_t kForwardRecordLimit = size_t(8) << 30;      // C2: 2 batches, 27.3 ms; 2 GiB (8 batches, 8 tails): 28.4 ms
 struct KappaBatch {
     int src_per_batch;
     size_t record_bytes;
@@ -812,7 +812,7 @@ KappaBatch plan_kappa_batches(int n_src, int n_slots, int n_groups, bool map_src
     const int unit = map_src ? 32 : 1;                               // sources come in whole warps' worth
     const int n_units = (n_src + unit - 1) / unit;
     auto bytes_for = [&](int n) {
-        return size_t(rt::march_blocks(n, n_slots, n_groups, map_src ? 1 : 0)) * rt::kThreads * size_t(K) * sizeof(float2);
+        return size_t(rt::march_blocks(n, n_slots, n_groups, map_src ? 1 : 0)) * rt::kThreads * size_t(K) * sizeof(float);
     };
     int units = int(std::max<size_t>(1, record_limit / std::max<size_t>(1, bytes_for(unit))));
     units = std::min(units, n_units);
@@ -887,7 +887,7 @@ int rt_march_adjoint_kappa_ex(const float* gbar, const float* j, const float* ka
     }
     const long long K = ck.n_sub * n_steps;
     const KappaBatch kb = plan_kappa_batches(n_src, P.n_slots, P.n_groups, pl.map_src, K, record_limit);
-    float2* fwd = reinterpret_cast<float2*>(ws + align_up(base, 256));
+    float* fwd = reinterpret_cast<float*>(ws + align_up(base, 256));
     for (int s0 = 0; s0 < n_src; s0 += kb.src_per_batch) {
         P.src_begin = s0;
         P.n_src = std::min(kb.src_per_batch, n_src - s0);

@@ -48,9 +48,9 @@ struct MarchParams {
     // for one bin per thread, the plain grid [n_steps][nx][ny][nz][nb] for four), drained into the fp64 grid `acc`
     // while the march runs
     float* scratch;
-    // march_phased_kernel<..., RECORD> (rt_march_adjoint_kappa): nothing is deposited; (I_{k+1}, P_k = ds J_k T_k), both
-    // x 4 pi/N_Omega, of substep k go to record[k * record_stride + thread]
-    float2* record;
+    // march_phased_kernel<..., RECORD> (rt_march_adjoint_kappa): nothing is deposited; I_{k+1} (x 4 pi/N_Omega) of substep k
+    // goes to record[k * record_stride + thread]
+    float* record;
     long long record_stride;
     long long drain_units_per_block;   // 16-byte units of the scratch one block drains when its rays are done
     long long n_drain_units;           // 16-byte units of the whole scratch

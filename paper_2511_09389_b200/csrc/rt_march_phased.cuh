@@ -278,8 +278,8 @@ __device__ __forceinline__ int phase(const MarchParams& P, const BrickGeom& G, L
             const float emitted = STEP ? (jv + ju) * L.T[b] * P.emis : (jv + ju) * L.T[b];
             L.I[b] = fmaf(L.I[b], att, emitted);
             L.T[b] *= att;
-            if constexpr (RECORD) {          // (I_{k+1}, P_k) of this substep; a warp writes one 256-byte run
-                if (b == 0 && L.rec_at >= 0) P.record[(long long)L.g * P.record_stride + L.rec_at] = make_float2(L.I[0], emitted);
+            if constexpr (RECORD) {          // I_{k+1} of this substep; a warp writes one 128-byte run
+                if (b == 0 && L.rec_at >= 0) P.record[(long long)L.g * P.record_stride + L.rec_at] = L.I[0];
             } else {
                 const float dep = JVP ? L.Id[b] : L.I[b];       // what is deposited, with the weights of x_k
 #pragma unroll
@@ -351,7 +351,7 @@ __device__ __forceinline__ int phase(const MarchParams& P, const BrickGeom& G, L
 // next to I and deposited instead of it.
 // KTRI: the rt_march_trilinear_kappa form (D18) -- kappa cached at the stencil voxels like j and read with
 // the trilinear weights every substep.
-// RECORD: the first pass of rt_march_adjoint_kappa (D19) -- nothing is deposited; (I_{k+1}, P_k) of every
+// RECORD: the first pass of rt_march_adjoint_kappa (D19) -- nothing is deposited; I_{k+1} of every
 // substep go to P.record for the backward march (rt_adjoint.cuh), which maps its threads to rays the same way.
 template <int NB, bool TABLE, bool BRICK = (NB == 1), typename ACC = float, bool STEP = false, bool JVP = false, bool KTRI = false,
           bool RECORD = false>

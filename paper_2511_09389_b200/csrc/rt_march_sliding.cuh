@@ -236,14 +236,14 @@ template <int NB, typename ACC, bool KTRI> struct Stencil {
 };
 
 // STEP: the rt_march_step form -- start at substep P.k0 with (I, exp(-tau)) loaded from the ray state, store them back
-// RECORD (rt_march_adjoint_kappa): nothing is deposited; (I_{k+1}, P_k = ds J_k T_k), both scaled by 4 pi/N_Omega, of
-// every substep go to record[k * record_stride + thread], a warp writing one 256-byte run per substep.
+// RECORD (rt_march_adjoint_kappa): nothing is deposited; I_{k+1}, scaled by 4 pi/N_Omega, of every substep goes to
+// record[k * record_stride + thread], a warp writing one 128-byte run per substep.
 // COPIES: block b reduces into copy b % P.acc_copies of the accumulation grid.  ncu shows this march loading the L2
 // slices unevenly (atomic input 19-67 % busy across slices: the voxels next to the sources and on the faces are
 // hot); a few copies of a small grid spread a hot voxel over as many addresses, snapshot_finalize_kernel adds them
 // up (C2: 18.1 -> 17.2 ms with 3 copies).  A separate instantiation: the plain kernel's code stays as it is.
 template <int NB, typename ACC, int MINB, bool STEP, bool KTRI = false, bool RECORD = false, bool COPIES = false>
-__global__ void __launch_bounds__(kThreads, MINB) march_sliding_kernel(const MarchParams P, float2* record = nullptr,
+__global__ void __launch_bounds__(kThreads, MINB) march_sliding_kernel(const MarchParams P, float* record = nullptr,
                                                                        long long record_stride = 0) {
     if constexpr (COPIES)
         if (P.same_frac && *P.same_frac) return;     // (unused since the phased kernel took over the weight table)
@@ -338,7 +338,7 @@ __global__ void __launch_bounds__(kThreads, MINB) march_sliding_kernel(const Mar
                 T[b] *= att[b];
                 if (RECORD && b == 0)
                     record[((long long)m * P.n_sub + k) * record_stride + (long long)blockIdx.x * kThreads + threadIdx.x] =
-                        make_float2(I[0], emitted);
+                        I[0];
             }
             if (!RECORD) {
 #pragma unroll

@@ -226,11 +226,11 @@ def test_kappa_adjoint_source_batches_match_the_oracle(rt, oracle_mod, n_src, n_
     gbar = rng.standard_normal((n_steps,) + shape + (nb,)).astype(np.float32)
     K = rt.rt_substeps_per_step(ds, 1.0, dt) * n_steps
     slots = rt.rt_ray_slots(n_rays)
-    if n_src >= 32:     # record bytes of one batch = blocks(4 direction slots x 32 (source, bin) pairs) x 128 threads x K x 8
+    if n_src >= 32:     # record bytes of one batch = blocks(4 direction slots x 32 (source, bin) pairs) x 128 threads x K x 4
         blocks = ((slots + 3) // 4) * ((limit_sources * nb + 31) // 32)
     else:
         blocks = ((slots * nb + 127) // 128) * limit_sources
-    limit = blocks * 128 * K * 8
+    limit = blocks * 128 * K * 4
     args = (_dev(gbar), _dev(j), _dev(kap), _dev(src), n_rays, ds, 1.0, dt, n_steps)
     one = rt.rt_march_adjoint_kappa(*args)
     ws_one = rt.rt_adjoint_kappa_workspace_bytes(*shape, n_src, n_rays, nb, ds, 1.0, dt, n_steps)
@@ -253,7 +253,7 @@ def test_kappa_adjoint_c2_subset_in_batches_matches_the_oracle(rt, oracle_mod):
     rng = np.random.default_rng(13)
     gbar = rng.uniform(0.0, 1.0, (w.n_steps,) + w.j.shape).astype(np.float32)
     K = w.n_steps * w.substeps_per_step
-    limit = (rt.rt_ray_slots(w.n_rays) // 4) * 128 * K * 8               # one group of 32 sources
+    limit = (rt.rt_ray_slots(w.n_rays) // 4) * 128 * K * 4               # one group of 32 sources
     got = rt.rt_march_adjoint_kappa_ex(_dev(gbar), _dev(w.j), _dev(w.kappa), _dev(src), w.n_rays, w.step_size, w.c, w.dt,
                                        w.n_steps, record_limit=limit)
     torch.cuda.synchronize()
