@@ -475,25 +475,25 @@ int run_phased(rt::MarchParams P, const PhasedPlan& pp, const Plan& pl, const Wo
                                          n_bins, st);
         if (rcn != RT_OK) return rcn;
     } else {
-    if (pl.map_src && !pp.sorted) {
-        // Sources that share their cell fractions (decided on the device) take the weight-table instantiation, others
-        // the plain one: both are launched, each returns at once when the flag says the call is the other's
-        int* flag = reinterpret_cast<int*>(ws + wl.flag_at);
-        rt::same_fraction_kernel<<<1, 256, 0, st>>>(flag, sources, n_src, step_size);
-        P.same_frac = flag;
-        const int rct = step ? launch_phased<true, true>(P, phased, unsigned(mb), st) : launch_phased<true, false>(P, phased, unsigned(mb), st);
-        if (rct != RT_OK) return rct;
-    }
-    if (phased == kPhasedDirect64 && pl.map_src && !pp.sorted) {
-        // sources in general position, fp64 reductions: warp = 32 (direction, bin) pairs of ONE source, so that the
-        // blocks in flight stay around a few sources (the brick path is faster by sorted sources)
-        P.map_src = 0;
-        P.src_order = nullptr;
-        mb = rt::march_blocks(P.n_src, P.n_slots, P.n_groups, 0);
-        if (mb > 2147483647LL) return RT_EINVAL;
-    }
-    const int rcp = step ? launch_phased<false, true>(P, phased, unsigned(mb), st) : launch_phased<false, false>(P, phased, unsigned(mb), st);
-    if (rcp != RT_OK) return rcp;
+        if (pl.map_src && !pp.sorted) {
+            // Sources that share their cell fractions (decided on the device) take the weight-table instantiation, others
+            // the plain one: both are launched, each returns at once when the flag says the call is the other's
+            int* flag = reinterpret_cast<int*>(ws + wl.flag_at);
+            rt::same_fraction_kernel<<<1, 256, 0, st>>>(flag, sources, n_src, step_size);
+            P.same_frac = flag;
+            const int rct = step ? launch_phased<true, true>(P, phased, unsigned(mb), st) : launch_phased<true, false>(P, phased, unsigned(mb), st);
+            if (rct != RT_OK) return rct;
+        }
+        if (phased == kPhasedDirect64 && pl.map_src && !pp.sorted) {
+            // sources in general position, fp64 reductions: warp = 32 (direction, bin) pairs of ONE source, so that the
+            // blocks in flight stay around a few sources (the brick path is faster by sorted sources)
+            P.map_src = 0;
+            P.src_order = nullptr;
+            mb = rt::march_blocks(P.n_src, P.n_slots, P.n_groups, 0);
+            if (mb > 2147483647LL) return RT_EINVAL;
+        }
+        const int rcp = step ? launch_phased<false, true>(P, phased, unsigned(mb), st) : launch_phased<false, false>(P, phased, unsigned(mb), st);
+        if (rcp != RT_OK) return rcp;
     }
     // the snapshots (the step's increment): the fp64 grid plus what the march left in the scratch, rounded once
     const rt::BrickGeom G = rt::brick_geom(nx, ny, nz);
