@@ -351,6 +351,25 @@ def test_jvp_kappa_on_c1_is_dual_to_the_kappa_adjoint_and_matches_a_difference_q
     assert float((scale - fd).abs().max()) <= 2e-3 * float(fd.abs().max())
 
 
+def test_kappa_adjoint_and_tangent_are_dual_at_full_c2_size(rt):
+    """The launch configurations bench.py times: all 2,097 sources of C2 -- the kappa adjoint in the two source batches
+    its 8 GiB record limit gives (15 GB of 4-byte records), the tangent with 16 drain rounds.  <g, J dkappa> =
+    <J^T g, dkappa> for a random g and a random positive dkappa ties the two together at that size."""
+    w = workloads.make_config("C2")
+    rng = np.random.default_rng(29)
+    j, kap, src = _dev(w.j), _dev(w.kappa), _dev(w.sources)
+    args = (w.n_rays, w.step_size, w.c, w.dt, w.n_steps)
+    dk = _dev((w.kappa * rng.uniform(0.5, 1.5, w.kappa.shape)).astype(np.float32))
+    tang = rt.rt_march_jvp_kappa(j, kap, dk, src, *args)
+    g = torch.from_numpy(rng.uniform(0.0, 1.0, tuple(tang.shape)).astype(np.float32)).cuda()
+    grad = rt.rt_march_adjoint_kappa(g, j, kap, src, *args)
+    torch.cuda.synchronize()
+    assert torch.isfinite(grad).all() and torch.isfinite(tang).all()
+    lhs = float((g.double() * tang.double()).sum())
+    rhs = float((grad.double() * dk.double()).sum())
+    assert abs(lhs - rhs) <= 5e-6 * abs(lhs), (lhs, rhs)          # measured: 5.5e-7
+
+
 def test_jvp_kappa_on_a_c2_subset(rt, oracle_mod):
     """C2's grid, rays and substeps, 40 of its cell-centred sources: the launch shape of the headline (weight table,
     brick scratch, drains) carrying the tangent."""
