@@ -421,6 +421,12 @@ march_phased_kernel(const MarchParams P) {
             }
         }
         asm volatile("" : "+r"(negbits));        // opaque: keeps ptxas from re-deriving the signs with fp64 compares
+        // Weight table, one bin: one direction per warp, so the signs are the same in every lane.  Passing them through a vote
+        // says so: they live in uniform registers and what is derived from them runs on the uniform datapath (C2 11.84 ->
+        // 11.71 ms; with four bins per thread, C3, it makes no difference)
+        if constexpr (TABLE && NB == 1)
+            negbits = (__any_sync(0xFFFFFFFFu, (negbits & 1) != 0) ? 1 : 0) | (__any_sync(0xFFFFFFFFu, (negbits & 2) != 0) ? 2 : 0) |
+                      (__any_sync(0xFFFFFFFFu, (negbits & 4) != 0) ? 4 : 0);
 #pragma unroll
         for (int s = 0; s < 8; ++s) L.S.zero_slot(s);
         L.S.restart(P, L.A, negbits, id.group * NB, P.j);
