@@ -351,21 +351,26 @@ size_t near_state_bytes(long long rays, int n_bins) {
 // the instantiation of march_phased_kernel for a deposit mode (phased_kind)
 template <bool TABLE, bool STEP>
 int launch_phased(const rt::MarchParams& P, int kind, unsigned blocks, cudaStream_t st) {
+    // the plain one-bin march with 32 sources x ONE direction per warp (map_src = 1) has an instantiation of its own
+    const bool one_dir = !TABLE && kind == kPhasedOneBin && P.map_src == 1;
     if (P.kappa_trilinear) {           // rt_march_trilinear_kappa: one bin per thread in both deposit modes
         if (STEP || P.dkappa || kind == kPhasedFourBins) return RT_EINVAL;
-        if (kind == kPhasedOneBin) rt::march_phased_kernel<1, TABLE, true, float, false, false, true><<<blocks, rt::kThreads, 0, st>>>(P);
+        if (one_dir) rt::march_phased_kernel<1, false, true, float, false, false, true, false, true><<<blocks, rt::kThreads, 0, st>>>(P);
+        else if (kind == kPhasedOneBin) rt::march_phased_kernel<1, TABLE, true, float, false, false, true><<<blocks, rt::kThreads, 0, st>>>(P);
         else rt::march_phased_kernel<1, TABLE, false, double, false, false, true><<<blocks, rt::kThreads, 0, st>>>(P);
         RT_CUDA(cudaGetLastError());
         return RT_OK;
     }
     if (P.dkappa) {                    // rt_march_jvp_kappa: one bin per thread in both deposit modes
         if (STEP || kind == kPhasedFourBins) return RT_EINVAL;
-        if (kind == kPhasedOneBin) rt::march_phased_kernel<1, TABLE, true, float, false, true><<<blocks, rt::kThreads, 0, st>>>(P);
+        if (one_dir) rt::march_phased_kernel<1, false, true, float, false, true, false, false, true><<<blocks, rt::kThreads, 0, st>>>(P);
+        else if (kind == kPhasedOneBin) rt::march_phased_kernel<1, TABLE, true, float, false, true><<<blocks, rt::kThreads, 0, st>>>(P);
         else rt::march_phased_kernel<1, TABLE, false, double, false, true><<<blocks, rt::kThreads, 0, st>>>(P);
         RT_CUDA(cudaGetLastError());
         return RT_OK;
     }
-    if (kind == kPhasedOneBin) rt::march_phased_kernel<1, TABLE, true, float, STEP><<<blocks, rt::kThreads, 0, st>>>(P);
+    if (one_dir) rt::march_phased_kernel<1, false, true, float, STEP, false, false, false, true><<<blocks, rt::kThreads, 0, st>>>(P);
+    else if (kind == kPhasedOneBin) rt::march_phased_kernel<1, TABLE, true, float, STEP><<<blocks, rt::kThreads, 0, st>>>(P);
     else if (kind == kPhasedFourBins) rt::march_phased_kernel<4, TABLE, false, float, STEP><<<blocks, rt::kThreads, 0, st>>>(P);
     else rt::march_phased_kernel<1, TABLE, false, double, STEP><<<blocks, rt::kThreads, 0, st>>>(P);
     RT_CUDA(cudaGetLastError());

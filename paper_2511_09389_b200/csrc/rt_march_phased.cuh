@@ -376,13 +376,15 @@ __device__ __forceinline__ int phase(const MarchParams& P, const BrickGeom& G, L
 // next to I and deposited instead of it.
 // KTRI: the rt_march_trilinear_kappa form (D18) -- kappa cached at the stencil voxels like j and read with
 // the trilinear weights every substep.
+// ONE_DIR: every warp marches ONE direction (map_src = 1: 32 sources x 1 direction; always so with TABLE).
 // RECORD: the first pass of rt_march_adjoint_kappa (D19) -- nothing is deposited; I_{k+1} of every
 // substep go to P.record for the backward march (rt_adjoint.cuh), which maps its threads to rays the same way.
 template <int NB, bool TABLE, bool BRICK = (NB == 1), typename ACC = float, bool STEP = false, bool JVP = false, bool KTRI = false,
-          bool RECORD = false>
+          bool RECORD = false, bool ONE_DIR = TABLE>
 __global__ void __launch_bounds__(kThreads, NB == 1 ? (TABLE ? RT_PHASED_MINB1 : RT_PHASED_MINB1P) : RT_PHASED_MINB4)
 march_phased_kernel(const MarchParams P) {
     static_assert(!BRICK || (NB == 1 && sizeof(ACC) == 4), "the brick scratch holds one fp32 bin");
+    static_assert(ONE_DIR || !TABLE, "the weight table is one direction's");
     static_assert(!RECORD || (NB == 1 && !BRICK && !STEP && !JVP && !KTRI), "RECORD: the plain forward march, one bin per thread");
     __shared__ __align__(16) TableRow table[TABLE ? kThreads / 32 : 1][32];
     __shared__ Fx96 ref[TABLE ? kThreads / 32 : 1][6];      // per warp: fraction of x_0 (cell word 0) and increment, per axis
@@ -421,10 +423,10 @@ march_phased_kernel(const MarchParams P) {
             }
         }
         asm volatile("" : "+r"(negbits));        // opaque: keeps ptxas from re-deriving the signs with fp64 compares
-        // Weight table, one bin: one direction per warp, so the signs are the same in every lane.  Passing them through a vote
-        // says so: they live in uniform registers and what is derived from them runs on the uniform datapath (C2 11.84 ->
-        // 11.71 ms; with four bins per thread, C3, it makes no difference)
-        if constexpr (TABLE && NB == 1)
+        // One direction per warp, one bin: the signs are the same in every lane.  Passing them through a vote says so: they
+        // live in uniform registers and what is derived from them runs on the uniform datapath (C2 11.84 -> 11.71 ms,
+        // jittered C2 24.1 -> 22.7; with four bins per thread, C3, it makes no difference)
+        if constexpr (ONE_DIR && NB == 1)
             negbits = (__any_sync(0xFFFFFFFFu, (negbits & 1) != 0) ? 1 : 0) | (__any_sync(0xFFFFFFFFu, (negbits & 2) != 0) ? 2 : 0) |
                       (__any_sync(0xFFFFFFFFu, (negbits & 4) != 0) ? 4 : 0);
 #pragma unroll
