@@ -207,7 +207,9 @@ __device__ __forceinline__ void adjoint_drain_slice(const MarchParams& P, const 
 // BRICK (dL/dj, one bin, substeps shorter than a cell): the deposits go to the fp32 window-brick scratch P.scratch with one
 // vector reduction per stencil plane and every block drains a slice of it into the fp64 grid when its rays are done, as
 // in the forward march (rt_brick.cuh, rt_march_phased.cuh).
-template <int MINB, bool WRT_KAPPA, bool BRICK = false>
+// ONE_DIR: every warp marches one direction (map_src = 1): the direction signs pass through a vote and live in uniform
+// registers, as in march_phased_kernel (dL/dj 16.8 -> 16.5 ms, dL/dkappa 27.3 -> 26.9 on C2).
+template <int MINB, bool WRT_KAPPA, bool BRICK = false, bool ONE_DIR = false>
 __global__ void __launch_bounds__(kThreads, MINB) adjoint_kernel(const MarchParams P, const float* gsuf,
                                                                  const float* fwd, long long fwd_stride) {
     // a warp marches as a whole (its phases are warp votes): a lane without a ray of its own marches the ray of the
@@ -278,6 +280,9 @@ __global__ void __launch_bounds__(kThreads, MINB) adjoint_kernel(const MarchPara
         }
     }
     asm volatile("" : "+r"(negbits));
+    if constexpr (ONE_DIR)
+        negbits = (__any_sync(0xFFFFFFFFu, (negbits & 1) != 0) ? 1 : 0) | (__any_sync(0xFFFFFFFFu, (negbits & 2) != 0) ? 2 : 0) |
+                  (__any_sync(0xFFFFFFFFu, (negbits & 4) != 0) ? 4 : 0);
 #pragma unroll
     for (int s = 0; s < 8; ++s) L.S.zero_slot(s);
     const float* gs = gsuf + (long long)(P.n_steps - 1) * P.snap_stride;

@@ -789,14 +789,16 @@ int rt_march_adjoint_j(const float* gbar, const float* kappa, int nx, int ny, in
         P.n_drain_units = std::max<long long>(1, (long long)(wl.brick_bytes / 16));
         const long long per = (P.n_drain_units * drain_rounds((long long)n_src * n_rays) + mb - 1) / mb;
         P.drain_units_per_block = std::min<long long>(std::max<long long>(per, 1), rt::kDrainMaxUnits);
-        rt::adjoint_kernel<6, false, true><<<unsigned(mb), rt::kThreads, 0, st>>>(P, gsuf, nullptr, 0);
+        if (pl.map_src) rt::adjoint_kernel<6, false, true, true><<<unsigned(mb), rt::kThreads, 0, st>>>(P, gsuf, nullptr, 0);
+        else rt::adjoint_kernel<6, false, true><<<unsigned(mb), rt::kThreads, 0, st>>>(P, gsuf, nullptr, 0);
         RT_CUDA(cudaGetLastError());
         rt::snapshot_finalize_scratch_kernel<true><<<unsigned(blocks), threads, 0, st>>>(master, P.scratch, grad_j, ck.cells, 1,
                                                                                         rt::brick_geom(nx, ny, nz), ny, nz, 1);
         RT_CUDA(cudaGetLastError());
         return RT_OK;
     }
-    rt::adjoint_kernel<6, false><<<unsigned(mb), rt::kThreads, 0, st>>>(P, gsuf, nullptr, 0);
+    if (pl.map_src) rt::adjoint_kernel<6, false, false, true><<<unsigned(mb), rt::kThreads, 0, st>>>(P, gsuf, nullptr, 0);
+    else rt::adjoint_kernel<6, false><<<unsigned(mb), rt::kThreads, 0, st>>>(P, gsuf, nullptr, 0);
     RT_CUDA(cudaGetLastError());
     rt::snapshot_finalize_kernel<double><<<unsigned(blocks), threads, 0, st>>>(master, grad_j, ck.cells, 1);
     RT_CUDA(cudaGetLastError());
@@ -908,7 +910,8 @@ int rt_march_adjoint_kappa_ex(const float* gbar, const float* j, const float* ka
             rt::march_sliding_kernel<1, double, 8, false, false, true><<<unsigned(mb), rt::kThreads, 0, st>>>(P, fwd, stride);
         }
         RT_CUDA(cudaGetLastError());
-        rt::adjoint_kernel<4, true><<<unsigned(mb), rt::kThreads, 0, st>>>(P, gsuf, fwd, stride);
+        if (pl.map_src) rt::adjoint_kernel<4, true, false, true><<<unsigned(mb), rt::kThreads, 0, st>>>(P, gsuf, fwd, stride);
+        else rt::adjoint_kernel<4, true><<<unsigned(mb), rt::kThreads, 0, st>>>(P, gsuf, fwd, stride);
         RT_CUDA(cudaGetLastError());
     }
     rt::snapshot_finalize_kernel<double><<<unsigned(blocks), threads, 0, st>>>(master, grad_kappa, ck.cells, 1);
